@@ -1,0 +1,183 @@
+"""Independent checkers used to pin the oracle (and later the CUDA path).  None of this is
+imported by the oracle or by the product; each checker is a different formulation from the
+oracle's (brute force, exact rationals, dense matrices, BFS, the paper's sweeps)."""
+from __future__ import annotations
+
+from fractions import Fraction
+
+import numpy as np
+
+import datagen
+from datagen.configs import EtxConfig
+
+
+def toy_config(d=2, L=1, D=4, H=1, k=4, w=1, edge_enc_input=0, precision="fp32") -> EtxConfig:
+    return datagen.get_config("cfg0").replace(name="toy", emb_hidden=D, emb_n_hidden_layers=H, gnn_latent=d,
+                                              gnn_iters=L, k=k, window=w, edge_enc_input=edge_enc_input,
+                                              precision=precision)
+
+
+def zero_layers(cfg):
+    return [(n, np.zeros((o, i), np.float32), np.zeros(o, np.float32)) for (n, o, i) in datagen.layer_shapes(cfg)]
+
+
+def set_layer(layers, name, W=None, b=None):
+    for idx, (n, W0, b0) in enumerate(layers):
+        if n == name:
+            layers[idx] = (n, np.asarray(W if W is not None else W0, np.float32).reshape(W0.shape),
+                           np.asarray(b if b is not None else b0, np.float32).reshape(b0.shape))
+            return
+    raise KeyError(name)
+
+
+# ---- exact fp32 arithmetic by rationals -------------------------------------------------
+def round_f32(q: Fraction) -> np.float32:
+    """Round an exact rational to the nearest fp32, ties to even (normal range only)."""
+    if q == 0:
+        return np.float32(0.0)
+    s = -1 if q < 0 else 1
+    q = abs(q)
+    e = 0
+    while q >= 2:
+        q /= 2; e += 1
+    while q < 1:
+        q *= 2; e -= 1
+    m = q * (1 << 23)                      # in [2^23, 2^24)
+    fl = m.numerator // m.denominator
+    rem = m - fl
+    if rem > Fraction(1, 2) or (rem == Fraction(1, 2) and (fl & 1)):
+        fl += 1
+    assert -126 <= e <= 127, "subnormal/overflow not handled in this checker"
+    return np.float32(s * float(Fraction(fl) * Fraction(2) ** (e - 23)))
+
+
+def d2_exact_f32(a, b) -> np.float32:
+    """Eq.(1) in the pinned order: t0*t0, then fma(t_i, t_i, d2), each step one fp32 rounding."""
+    a = np.asarray(a, np.float32); b = np.asarray(b, np.float32)
+    t = np.float32(a[0] - b[0])
+    d2 = round_f32(Fraction(float(t)) * Fraction(float(t)))
+    for i in range(1, a.size):
+        t = np.float32(a[i] - b[i])
+        d2 = round_f32(Fraction(float(t)) * Fraction(float(t)) + Fraction(float(d2)))
+    return d2
+
+
+def knn_bruteforce(emb, plane, event_offsets, k, w, d2_max=np.inf, n_planes=26):
+    """All pairs of the event, filtered by plane window, full sort by (d2, index)."""
+    n = emb.shape[0]
+    nbr = np.full((n, k), -1, np.int32)
+    deg = np.zeros(n, np.int32)
+    for e in range(len(event_offsets) - 1):
+        lo, hi = int(event_offsets[e]), int(event_offsets[e + 1])
+        for q in range(lo, hi):
+            cand = []
+            for c in range(lo, hi):
+                dp = int(plane[c]) - int(plane[q])
+                if 1 <= dp <= w:
+                    d2 = d2_exact_f32(emb[q], emb[c])
+                    if d2 < d2_max:
+                        cand.append((float(d2), c))
+            cand.sort()
+            cand = cand[:k]
+            deg[q] = len(cand)
+            for s, (_, c) in enumerate(cand):
+                nbr[q, s] = c
+    return nbr, deg
+
+
+def knn_replace_the_max(emb, plane, event_offsets, k, w, d2_max=np.inf):
+    """The paper's own loop (sec. 7.2): scan candidates, fill k slots, then replace
+    the current maximum when a closer candidate comes.  Returns neighbour SETS per hit."""
+    out = []
+    for e in range(len(event_offsets) - 1):
+        lo, hi = int(event_offsets[e]), int(event_offsets[e + 1])
+        for q in range(lo, hi):
+            slots = []
+            for c in range(lo, hi):
+                dp = int(plane[c]) - int(plane[q])
+                if not (1 <= dp <= w):
+                    continue
+                d2 = float(d2_exact_f32(emb[q], emb[c]))
+                if not d2 < d2_max:
+                    continue
+                if len(slots) < k:
+                    slots.append((d2, c))
+                else:
+                    im = max(range(k), key=lambda s: slots[s][0])
+                    if d2 < slots[im][0]:
+                        slots[im] = (d2, c)
+            out.append(set(c for _, c in slots))
+    return out
+
+
+# ---- components ------------------------------------------------------------------------
+def components_bfs(src, dst, keep, n):
+    adj = [[] for _ in range(n)]
+    for s, t, kk in zip(src, dst, keep):
+        if kk:
+            adj[s].append(t); adj[t].append(s)
+    lab = np.full(n, -1, np.int32)
+    for r in range(n):                       # ascending: r is the min index of its component
+        if lab[r] >= 0:
+            continue
+        lab[r] = r
+        stack = [r]
+        while stack:
+            u = stack.pop()
+            for v in adj[u]:
+                if lab[v] < 0:
+                    lab[v] = r; stack.append(v)
+    return lab
+
+
+def components_paper_sweeps(src, dst, keep, plane, n, n_planes=26, max_rounds=1000):
+    """PAPER.md L261 sec. 7.3: label = own index; forward sweep over planes taking the lowest label
+    among left neighbours, then backward sweep over right neighbours; iterated to a fixed point.
+    Returns (labels, rounds)."""
+    lab = np.arange(n, dtype=np.int64)
+    left = [[] for _ in range(n)]; right = [[] for _ in range(n)]
+    for s, t, kk in zip(src, dst, keep):
+        if kk:
+            right[s].append(t); left[t].append(s)
+    by_plane = [np.nonzero(plane == p)[0] for p in range(n_planes)]
+    for rnd in range(1, max_rounds + 1):
+        changed = False
+        for p in range(n_planes):
+            for v in by_plane[p]:
+                for u in left[v]:
+                    if lab[u] < lab[v]:
+                        lab[v] = lab[u]; changed = True
+        for p in range(n_planes - 1, -1, -1):
+            for v in by_plane[p]:
+                for u in right[v]:
+                    if lab[u] < lab[v]:
+                        lab[v] = lab[u]; changed = True
+        if not changed:
+            return lab.astype(np.int32), rnd
+    raise RuntimeError("sweeps did not converge")
+
+
+def check_edge_invariants(src, dst, row_ptr, plane, event_offsets, k, w):
+    """PAPER.md L76/L101/L137: same event, plane[dst]-plane[src] in [1,w], out-degree <= k, no duplicates,
+    src ascending, row_ptr = prefix sums."""
+    n = plane.size
+    ev = np.repeat(np.arange(len(event_offsets) - 1), np.diff(event_offsets))
+    assert np.all(ev[src] == ev[dst])
+    dp = plane[dst].astype(np.int64) - plane[src]
+    assert np.all((dp >= 1) & (dp <= w))
+    deg = np.bincount(src, minlength=n)
+    assert deg.max(initial=0) <= k
+    assert np.all(np.diff(src) >= 0)
+    assert np.array_equal(row_ptr, np.concatenate([[0], np.cumsum(deg)]).astype(np.int32))
+    key = src.astype(np.int64) * n + dst
+    assert np.unique(key).size == key.size
+
+
+def check_track_invariants(tid, src, dst, keep, event_offsets):
+    n = tid.size
+    idx = np.arange(n)
+    assert np.all(tid <= idx)
+    assert np.array_equal(tid[tid], tid)
+    assert np.all(tid[src[keep]] == tid[dst[keep]])
+    ev = np.repeat(np.arange(len(event_offsets) - 1), np.diff(event_offsets))
+    assert np.all(ev[tid] == ev)
