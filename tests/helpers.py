@@ -181,3 +181,18 @@ def check_track_invariants(tid, src, dst, keep, event_offsets):
     assert np.all(tid[src[keep]] == tid[dst[keep]])
     ev = np.repeat(np.arange(len(event_offsets) - 1), np.diff(event_offsets))
     assert np.all(ev[tid] == ev)
+
+
+def centred_parity_weights(cfg, batch, seed=None):
+    """"parity" preset weights with the head bias moved to -median(logit) of `batch` (computed with the
+    fp32 oracle), so that scores spread around 0.5 and the threshold keeps about half of the edges
+    (SURVEY.md sec. 8(c) A24).  Test utility: the product never sees how the bias was chosen."""
+    import oracle
+    layers = datagen.make_weights(cfg, "parity", seed=seed)
+    o = oracle.Oracle(datagen.pack_blob(cfg, layers), "fp32")
+    r = o.run(batch.xyz, batch.plane, batch.event_offsets, cfg.k, cfg.window, cfg.d2_max, cfg.threshold)
+    med = float(np.median(r["logit"])) if r["logit"].size else 0.0
+    name, W, b = layers[-1]
+    assert name == "head"
+    layers[-1] = (name, W, (b - np.float32(med)).astype(np.float32))
+    return layers

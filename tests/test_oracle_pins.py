@@ -10,7 +10,7 @@ import torch
 
 import datagen
 import oracle
-from helpers import (check_edge_invariants, check_track_invariants, components_bfs,
+from helpers import (centred_parity_weights, check_edge_invariants, check_track_invariants, components_bfs,
                      components_paper_sweeps, d2_exact_f32, knn_bruteforce, knn_replace_the_max,
                      set_layer, toy_config, zero_layers)
 
@@ -178,3 +178,340 @@ def _fma_chain(x, W):
     for j in range(W.shape[1]):
         acc = (x[:, j:j + 1].astype(np.float64) * W[None, :, j].astype(np.float64) + acc.astype(np.float64)).astype(F)
     return acc
+
+
+# ------------------------------------------------------------------ distance (L98 Eq.(1); R4)
+def test_distance_integer_embeddings_and_self_distance():
+    # integer-valued embeddings: Eq.(1) is exact in fp32, so the k-NN order is fixed by integers
+    emb = np.array([[0, 0, 0, 0], [1, 2, 2, 0], [3, 0, 0, 0], [0, 0, 0, 0], [1, 1, 1, 1]], F)
+    plane = np.array([0, 1, 1, 1, 1], np.int32)
+    off = np.array([0, 5], np.int32)
+    nbr, deg = oracle.knn(emb, plane, off, k=4, window=1)
+    # d2 from hit 0: (9, 9, 0, 4) -> order: 3 (0), 4 (4), 1 (9, lower index first), 2 (9)
+    assert deg[0] == 4 and nbr[0].tolist() == [3, 4, 1, 2]
+    assert deg[1:].tolist() == [0, 0, 0, 0]
+    assert float(d2_exact_f32(emb[1], emb[1])) == 0.0
+
+
+def test_distance_pinned_fma_order_detects_plain_sum():
+    # t = (2^-12+..) values where mul-then-add and fma differ: check the oracle orders by the fma chain
+    rng = np.random.default_rng(5)
+    emb = rng.normal(0, 1, (40, 4)).astype(F)
+    plane = np.repeat(np.arange(2), 20).astype(np.int32)
+    off = np.array([0, 40], np.int32)
+    nbr, deg = oracle.knn(emb, plane, off, k=20, window=1)
+    for q in range(20):
+        d = [float(d2_exact_f32(emb[q], emb[c])) for c in nbr[q]]
+        assert d == sorted(d) and sorted(nbr[q].tolist()) == list(range(20, 40))
+
+
+# ------------------------------------------------------------------ k-NN (L101, L257; R5-R8)
+def _small_events(seed, n_events=3, n_hits=40, n_dim=4, ties=False):
+    rng = np.random.default_rng(seed)
+    planes, embs, off = [], [], [0]
+    for _ in range(n_events):
+        n = int(rng.integers(0, n_hits))
+        p = np.sort(rng.integers(0, 26, n)).astype(np.int32)
+        e = rng.normal(0, 1, (n, n_dim)).astype(F)
+        if ties:
+            e = np.round(e)            # many exact ties and duplicates
+        planes.append(p); embs.append(e); off.append(off[-1] + n)
+    return (np.concatenate(embs).reshape(-1, n_dim), np.concatenate(planes).astype(np.int32),
+            np.asarray(off, np.int32))
+
+
+@pytest.mark.parametrize("k,w,ties", [(3, 1, False), (4, 2, False), (10, 2, True), (2, 3, True), (50, 25, False)])
+def test_knn_equals_bruteforce(k, w, ties):
+    emb, plane, off = _small_events(11 + k + w, ties=ties)
+    nbr, deg = oracle.knn(emb, plane, off, k, w)
+    bn, bd = knn_bruteforce(emb, plane, off, k, w)
+    assert np.array_equal(deg, bd) and np.array_equal(nbr, bn)
+
+
+def test_knn_equals_papers_replace_the_max_scan_when_no_ties():
+    emb, plane, off = _small_events(3, ties=False)
+    nbr, deg = oracle.knn(emb, plane, off, 3, 2)
+    sets = knn_replace_the_max(emb, plane, off, 3, 2)
+    for q in range(emb.shape[0]):
+        assert set(nbr[q, :deg[q]].tolist()) == sets[q]
+
+
+def test_knn_radius_cut_strict_and_special_cases():
+    emb = np.array([[0, 0, 0, 0], [1, 0, 0, 0], [2, 0, 0, 0], [0.5, 0, 0, 0]], F)
+    plane = np.array([3, 4, 4, 25], np.int32)
+    off = np.array([0, 4], np.int32)
+    nbr, deg = oracle.knn(emb, plane, off, 4, 1, d2_max=1.0)      # d2 = 1 is NOT < 1 (R6 strict)
+    assert deg.tolist() == [0, 0, 0, 0]
+    nbr, deg = oracle.knn(emb, plane, off, 4, 1, d2_max=np.nextafter(F(1), F(2)))
+    assert deg[0] == 1 and nbr[0, 0] == 1
+    nbr, deg = oracle.knn(emb, plane, off, 4, 30)                 # window past the last plane (R7)
+    assert nbr[0, :deg[0]].tolist() == [3, 1, 2] and deg[3] == 0  # plane-25 hit has no out-edges
+    nbr, deg = oracle.knn(emb, plane, off, 1, 30)
+    assert nbr[0].tolist() == [3]
+    # duplicates: lower index first (R5)
+    emb2 = np.array([[0, 0, 0, 0], [1, 1, 1, 1], [1, 1, 1, 1], [1, 1, 1, 1]], F)
+    nbr, deg = oracle.knn(emb2, np.array([0, 1, 1, 1], np.int32), off, 2, 1)
+    assert nbr[0].tolist() == [1, 2]
+
+
+def test_knn_never_crosses_events_and_handles_empty_events():
+    emb, plane, off = _small_events(21, n_events=6)
+    off = np.concatenate([[0], off, [off[-1]]]).astype(np.int32)   # empty first and last events
+    nbr, deg = oracle.knn(emb, plane, off, 5, 2)
+    src, dst, row_ptr = oracle.build_edges(nbr, deg)
+    check_edge_invariants(src, dst, row_ptr, plane, off, 5, 2)
+    po = oracle.plane_offsets(plane, off)
+    for e in range(off.size - 1):
+        for p in range(27):
+            lo, hi = off[e], off[e + 1]
+            assert po[e, p] == lo + np.searchsorted(plane[lo:hi], p, side="left")
+    # no hits at all
+    nbr, deg = oracle.knn(np.zeros((0, 4), F), np.zeros(0, np.int32), np.array([0, 0, 0], np.int32), 4, 2)
+    assert nbr.shape == (0, 4) and deg.size == 0
+
+
+# ------------------------------------------------------------------ edge list + CSC (L74-76; R9)
+def test_edge_list_order_and_csc_invariants():
+    cfg = datagen.get_config("cfg1")
+    b = datagen.generate_batch(cfg, n_events=2)
+    o = oracle.Oracle(datagen.pack_blob(cfg, datagen.make_weights(cfg, "parity")))
+    nbr, deg = oracle.knn(o.embed(b.xyz), b.plane, b.event_offsets, cfg.k, cfg.window)
+    src, dst, row_ptr = oracle.build_edges(nbr, deg)
+    check_edge_invariants(src, dst, row_ptr, b.plane, b.event_offsets, cfg.k, cfg.window)
+    E, n = src.size, b.n_hits
+    assert E == deg.sum() and E > 5 * n
+    for q in (0, n // 2, n - 1):
+        assert dst[row_ptr[q]:row_ptr[q + 1]].tolist() == nbr[q, :deg[q]].tolist()
+    col_ptr, in_edge = oracle.csc(dst, n)
+    assert np.array_equal(np.sort(in_edge), np.arange(E))
+    assert np.array_equal(col_ptr, np.concatenate([[0], np.cumsum(np.bincount(dst, minlength=n))]))
+    grp = np.repeat(np.arange(n), np.diff(col_ptr))
+    assert np.array_equal(dst[in_edge], grp)
+    same = grp[1:] == grp[:-1]
+    assert np.all(np.diff(in_edge)[same] > 0)
+
+
+# ------------------------------------------------------------------ GNN (L133-142, Eq.(4); R10-R16)
+def _tiny_graph(seed=0, n=12, E=30):
+    rng = np.random.default_rng(seed)
+    xyz = rng.uniform(-30, 30, (n, 3)).astype(F)
+    src = np.sort(rng.integers(0, n, E)).astype(np.int32)
+    dst = rng.integers(0, n, E).astype(np.int32)
+    return xyz, src, dst
+
+
+def test_scatter_sum_equals_dense_incidence_product():
+    # Eq.(4): m = [A_out e, A_in e].  Integer-valued e makes the sums exact in any order.
+    d = 4
+    cfg = toy_config(d=d, L=1)
+    L = zero_layers(cfg)
+    # edge encoder: e0 = round-ish integer features: eenc0 = 64*I on |df| then eenc1 = selector
+    W = np.zeros((d, 3)); W[0, 0] = W[1, 1] = W[2, 2] = 1; W[3, :] = 1
+    set_layer(L, "eenc0", W)
+    set_layer(L, "eenc1", np.eye(d) * 40 * 8)               # |dx|/40 * 320 = 8*|dx| mm
+    o = oracle.Oracle(datagen.pack_blob(cfg, L))
+    xyz, src, dst = _tiny_graph()
+    xyz = np.round(xyz)                                      # integer mm -> e0 multiples of 1/..; use double check
+    xyz[:, 2] = 0
+    out = o.gnn(xyz, src, dst, want_states=True, m_iter=0)
+    e0 = out["e"]                                            # node/edge nets are zero: e stays e0 (residual, L140)
+    n, E = xyz.shape[0], src.size
+    A_out = np.zeros((n, E)); A_out[src, np.arange(E)] = 1
+    A_in = np.zeros((n, E)); A_in[dst, np.arange(E)] = 1
+    want = np.concatenate([A_out @ e0.astype(np.float64), A_in @ e0.astype(np.float64)], axis=1)
+    assert np.abs(out["m"] - want).max() <= 1e-4 * max(1.0, np.abs(want).max())
+    assert np.allclose(out["m"][:, :d].sum(0), e0.sum(0), rtol=1e-5)
+    assert np.allclose(out["m"][:, d:].sum(0), e0.sum(0), rtol=1e-5)
+    assert np.abs(e0).max() > 1
+
+
+def test_scatter_sum_exact_on_integer_messages():
+    d = 2
+    cfg = toy_config(d=d, L=1)
+    L = zero_layers(cfg)
+    set_layer(L, "eenc1", np.zeros((d, d)), [3, -5])         # e0 = (3, -5) for every edge
+    o = oracle.Oracle(datagen.pack_blob(cfg, L))
+    xyz, src, dst = _tiny_graph(1, n=9, E=40)
+    out = o.gnn(xyz, src, dst, m_iter=0)
+    n = xyz.shape[0]
+    od, idg = np.bincount(src, minlength=n), np.bincount(dst, minlength=n)
+    want = np.stack([3 * od, -5 * od, 3 * idg, -5 * idg], axis=1).astype(F)
+    assert np.array_equal(out["m"], want)
+
+
+def test_residual_zero_branches_leave_encodings_unchanged():
+    cfg = toy_config(d=4, L=3)
+    rng = np.random.default_rng(2)
+    L = zero_layers(cfg)
+    for name in ("nenc0", "nenc1", "eenc0", "eenc1", "head"):
+        shp = [s for s in datagen.layer_shapes(cfg) if s[0] == name][0]
+        set_layer(L, name, rng.normal(0, 1, (shp[1], shp[2])), rng.normal(0, 1, shp[1]))
+    o = oracle.Oracle(datagen.pack_blob(cfg, L))
+    xyz, src, dst = _tiny_graph(3)
+    out = o.gnn(xyz, src, dst, want_states=True)
+    f = o.features(xyz).astype(np.float64)
+    lay = {n: (W.astype(np.float64), b.astype(np.float64)) for n, W, b in L}
+    h0 = np.maximum(f @ lay["nenc0"][0].T + lay["nenc0"][1], 0) @ lay["nenc1"][0].T + lay["nenc1"][1]
+    x = np.abs(f[dst] - f[src])                                   # R11: |f_dst - f_src|
+    e0 = np.maximum(x @ lay["eenc0"][0].T + lay["eenc0"][1], 0) @ lay["eenc1"][0].T + lay["eenc1"][1]
+    assert np.allclose(out["h"], h0, atol=1e-5) and np.allclose(out["e"], e0, atol=1e-5)
+    z = e0 @ lay["head"][0].T[:, 0] + lay["head"][1][0]
+    assert np.allclose(out["logit"], z, atol=1e-5)
+    assert np.allclose(out["score"], 1 / (1 + np.exp(-z)), atol=1e-6)
+
+
+def test_gnn_full_forward_matches_float64_numpy_in_papers_order():
+    # independent restatement of L133-142 with numpy float64 matmuls: messages from e^k, node
+    # update, then edge update with the UPDATED h (R13), concat orders [h, m_out, m_in] / [h_s, h_d, e]
+    for eei in (0, 1):
+        cfg = toy_config(d=8, L=3, edge_enc_input=eei)
+        W = datagen.make_weights(cfg, "parity", seed=5)
+        o = oracle.Oracle(datagen.pack_blob(cfg, W))
+        xyz, src, dst = _tiny_graph(4, n=15, E=50)
+        out = o.gnn(xyz, src, dst, want_states=True)
+        lay = {n: (w.astype(np.float64), b.astype(np.float64)) for n, w, b in W}
+        mlp = lambda x, a, b_: np.maximum(x @ lay[a][0].T + lay[a][1], 0) @ lay[b_][0].T + lay[b_][1]
+        f = o.features(xyz).astype(np.float64)
+        h = mlp(f, "nenc0", "nenc1")
+        e = mlp(np.abs(f[dst] - f[src]) if eei == 0 else np.concatenate([h[src], h[dst]], 1), "eenc0", "eenc1")
+        n, E = xyz.shape[0], src.size
+        for it in range(cfg.gnn_iters):
+            mo = np.zeros((n, 8)); mi = np.zeros((n, 8))
+            np.add.at(mo, src, e); np.add.at(mi, dst, e)
+            h = h + mlp(np.concatenate([h, mo, mi], 1), f"node{it}_0", f"node{it}_1")
+            e = e + mlp(np.concatenate([h[src], h[dst], e], 1), f"edge{it}_0", f"edge{it}_1")
+        z = e @ lay["head"][0][0] + lay["head"][1][0]
+        scale = max(1.0, np.abs(e).max())
+        assert np.abs(out["e"] - e).max() < 1e-4 * scale and np.abs(out["h"] - h).max() < 1e-4 * scale
+        assert np.abs(out["logit"] - z).max() < 1e-4 * max(1.0, np.abs(z).max())
+        assert np.abs(z).max() > 1e-2
+
+
+def test_bf16_and_int8_modes_stay_close_to_fp32_on_parity_weights():
+    cfg = datagen.get_config("cfg0")
+    W = datagen.make_weights(cfg, "parity")
+    b = datagen.generate_batch(cfg)
+    blob = datagen.pack_blob(cfg, W)
+    r32 = oracle.Oracle(blob, "fp32").run(b.xyz, b.plane, b.event_offsets, cfg.k, cfg.window)
+    g16 = oracle.Oracle(blob, "bf16").gnn(b.xyz, r32["src"], r32["dst"])
+    assert 0 < np.abs(g16["logit"] - r32["logit"]).max() < 0.25
+    sc = oracle.calibrate_int8(blob, b.xyz, b.plane, b.event_offsets, cfg.k, cfg.window)
+    g8 = oracle.Oracle(datagen.pack_blob(cfg, W, sc), "int8").gnn(b.xyz, r32["src"], r32["dst"])
+    assert 0 < np.abs(g8["logit"] - r32["logit"]).max() < 0.5
+    frac_mid = np.mean((r32["score"] > 0.01) & (r32["score"] < 0.99))
+    assert frac_mid > 0.9                                   # the parity preset keeps scores informative (R24)
+
+
+# ------------------------------------------------------------------ head + threshold (L80; R16, R17)
+def test_sigmoid_closed_forms_and_threshold_boundary():
+    cfg = toy_config(d=2, L=0)
+    L = zero_layers(cfg)
+    set_layer(L, "eenc1", np.zeros((2, 2)), [1, 0])
+    set_layer(L, "head", [[1, 0]], [-1])                    # z = 1*1 - 1 = 0 -> score exactly 0.5
+    o = oracle.Oracle(datagen.pack_blob(cfg, L))
+    xyz, src, dst = _tiny_graph(6, n=5, E=6)
+    out = o.gnn(xyz, src, dst)
+    assert np.all(out["logit"] == 0) and np.all(out["score"] == 0.5)
+    assert oracle.logit_threshold(0.5) == 0.0
+    assert abs(oracle.logit_threshold(0.9) - math.log(9)) < 1e-6
+    # score == thr is kept (L80: scores BELOW the threshold are discarded)
+    tid = oracle.components(src, dst, out["logit"], oracle.logit_threshold(0.5), 5)
+    keep = np.ones(6, bool)
+    assert np.array_equal(tid, components_bfs(src, dst, keep, 5))
+    tid = oracle.components(src, dst, out["logit"], np.nextafter(F(0), F(1)), 5)
+    assert np.array_equal(tid, np.arange(5))
+    # huge logits do not make NaNs
+    set_layer(L, "head", [[1e30, 0]], [0])
+    out = oracle.Oracle(datagen.pack_blob(cfg, L)).gnn(xyz, src, dst)
+    assert np.all(out["score"] == 1.0)
+    set_layer(L, "head", [[-1e30, 0]], [0])
+    out = oracle.Oracle(datagen.pack_blob(cfg, L)).gnn(xyz, src, dst)
+    assert np.all(out["score"] == 0.0)
+
+
+# ------------------------------------------------------------------ components (L82, L261; R18)
+def test_components_equal_bfs_scipy_and_iterated_paper_sweeps():
+    from scipy.sparse import coo_matrix
+    from scipy.sparse.csgraph import connected_components
+    rng = np.random.default_rng(8)
+    for trial in range(6):
+        n = int(rng.integers(5, 120))
+        plane = np.sort(rng.integers(0, 26, n)).astype(np.int32)
+        src, dst = [], []
+        for _ in range(int(rng.integers(0, 3 * n))):
+            a, b = rng.integers(0, n, 2)
+            if plane[a] < plane[b]:
+                src.append(a); dst.append(b)
+        src, dst = np.asarray(src, np.int32), np.asarray(dst, np.int32)
+        logit = rng.normal(0, 1, src.size).astype(F)
+        keep = logit >= 0
+        tid = oracle.components(src, dst, logit, 0.0, n)
+        assert np.array_equal(tid, components_bfs(src, dst, keep, n))
+        sw, rounds = components_paper_sweeps(src, dst, keep, plane, n)
+        assert np.array_equal(tid, sw)
+        ncomp, lab = connected_components(coo_matrix((np.ones(keep.sum()), (src[keep], dst[keep])), shape=(n, n)),
+                                          directed=False)
+        assert ncomp == np.unique(tid).size
+        for c in range(ncomp):
+            assert np.unique(tid[lab == c]).size == 1
+        check_track_invariants(tid, src, dst, keep, np.array([0, n], np.int32))
+
+
+def test_zigzag_component_needs_more_than_two_sweeps_but_oracle_is_exact():
+    # kept edges a->c, b->c, b->d with a<b on plane 0 and c<d on plane 1, plus d->f, g->f with g a
+    # low-plane, high-index... build a chain that two sweeps under-merge (documented in R18)
+    plane = np.array([0, 0, 1, 1], np.int32)
+    src = np.array([0, 1, 1], np.int32); dst = np.array([2, 2, 3], np.int32)
+    keep = np.ones(3, bool)
+    tid = oracle.components(src, dst, np.ones(3, F), 0.0, 4)
+    assert tid.tolist() == [0, 0, 0, 0]
+    sw, rounds = components_paper_sweeps(src, dst, keep, plane, 4)
+    assert sw.tolist() == [0, 0, 0, 0]
+
+
+def test_truth_edges_on_noise_free_event_give_one_component_per_particle():
+    cfg = datagen.get_config("cfg0")
+    b = datagen.generate_batch(cfg, n_events=3)
+    src, dst = [], []
+    for e in range(b.n_events):
+        lo, hi = b.event_offsets[e], b.event_offsets[e + 1]
+        for pid in np.unique(b.particle[lo:hi]):
+            idx = lo + np.nonzero(b.particle[lo:hi] == pid)[0]
+            idx = idx[np.argsort(b.plane[idx], kind="stable")]
+            src += idx[:-1].tolist(); dst += idx[1:].tolist()
+    src, dst = np.asarray(src, np.int32), np.asarray(dst, np.int32)
+    assert np.all(b.plane[src] < b.plane[dst])
+    tid = oracle.components(src, dst, np.ones(src.size, F), 0.0, b.n_hits)
+    ev = np.repeat(np.arange(b.n_events), np.diff(b.event_offsets))
+    key = ev * 100000 + b.particle
+    assert np.unique(tid).size == np.unique(key).size
+    for t in np.unique(tid):
+        assert np.unique(key[tid == t]).size == 1
+    check_track_invariants(tid, src, dst, np.ones(src.size, bool), b.event_offsets)
+
+
+def test_full_run_invariants_every_hit_gets_one_track_id():
+    cfg = datagen.get_config("cfg0")
+    b = datagen.generate_batch(cfg)
+    o = oracle.Oracle(datagen.pack_blob(cfg, centred_parity_weights(cfg, b)))
+    r = o.run(b.xyz, b.plane, b.event_offsets, cfg.k, cfg.window)
+    check_edge_invariants(r["src"], r["dst"], r["row_ptr"], b.plane, b.event_offsets, cfg.k, cfg.window)
+    assert r["track_id"].shape == (b.n_hits,)
+    keep = r["logit"] >= 0
+    check_track_invariants(r["track_id"], r["src"], r["dst"], keep, b.event_offsets)
+    assert 0 < keep.mean() < 1
+
+
+# ------------------------------------------------------------------ generator shapes
+def test_generator_shapes_follow_baseline_configs():
+    b0 = datagen.generate_batch(datagen.get_config("cfg0"))
+    assert b0.n_events == 1 and 150 < b0.n_hits < 260 and np.all(b0.particle >= 0)
+    b1 = datagen.generate_batch(datagen.get_config("cfg1"), n_events=24)
+    per = np.diff(b1.event_offsets)
+    assert 1500 < per.mean() < 2800
+    assert np.all(np.diff(b1.plane)[np.diff(np.repeat(np.arange(24), per)) == 0] >= 0)
+    r = np.hypot(b1.xyz[:, 0], b1.xyz[:, 1])
+    assert r.min() > 5.0 and r.max() < 42.2
+    assert 0.01 < np.mean(b1.particle < 0) < 0.035
+    again = datagen.generate_batch(datagen.get_config("cfg1"), n_events=2, first_event=3)
+    assert np.array_equal(again.xyz, b1.slice_events(3, 5).xyz)
