@@ -1,0 +1,294 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the ETX4VELO hot path (S0..S5) on synthetic VELO-shaped events.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config cfg2] [--engine auto|simt]
+    python bench.py --impl reference ...        # the CPU oracle on a bounded sample of the same workload
+
+One "step" = one pass of the whole hot path over one batch (BASELINE.json configs[2]: 500 events at
+pile-up 5, bf16 MLPs).  `value` is events/s with inputs resident in HBM; `e2e` is the same metric through
+etx_run_host with pinned HOST buffers (H2D + D2H inside the timed region).  `roofline` describes the
+dominant kernel (the edge network, S4e), timed live with CUDA events on the launching stream.  N > 1:
+one process per GPU (torchrun), each rank runs its own batch, no collective on the data path (events are
+independent) -- weak scaling.  DESIGN.md sec. 7 states every formula used here.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import datagen  # noqa: E402
+
+METRIC = "events_per_s"
+UNIT = "events/s"
+DTYPE = {"fp32": "f32", "bf16": "bf16", "int8": "int8"}
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm=float(d["hbm_gbs"]), bf16=float(d["bf16_tflops"]), bf16_sustained=float(d["bf16_tflops_sustained"]),
+                    source="measured")
+    return dict(hbm=6650.0, bf16=1590.0, bf16_sustained=1400.0, source="fallback")
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks + throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.index, self.samples, self._stop_evt = index, [], threading.Event()
+
+    def run(self):
+        while not self._stop_evt.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-i", str(self.index)],
+                                     capture_output=True, text=True, timeout=5).stdout.strip()
+                if out:
+                    self.samples.append([x.strip() for x in out.split(",")])
+            except Exception:
+                pass
+            self._stop_evt.wait(0.2)
+
+    def stop(self):
+        self._stop_evt.set()
+        self.join(timeout=6)
+        sm = [float(s[0]) for s in self.samples if s[0].replace(".", "").isdigit()]
+        mx = [float(s[1]) for s in self.samples if s[1].replace(".", "").isdigit()]
+        reasons = set()
+        for s in self.samples:
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), s[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(self.samples)}
+
+
+def workload(cfg, rank: int):
+    batch = datagen.generate_batch(cfg, first_event=rank * cfg.n_events)
+    layers = datagen.make_weights(cfg, "he")                      # BASELINE.json: He-uniform, zero bias
+    return batch, layers
+
+
+def int8_scales(cfg, layers):
+    import oracle  # calibration is part of producing the blob, not of the timed path (R21)
+    cal = datagen.generate_batch(datagen.get_config("cfg1"), n_events=datagen.configs.CALIBRATION_EVENTS,
+                                 seed=datagen.configs.CALIBRATION_SEED)
+    return oracle.calibrate_int8(datagen.pack_blob(cfg, layers), cal.xyz, cal.plane, cal.event_offsets, cfg.k, cfg.window)
+
+
+def stage_model(cfg, N, E, pairs, peaks):
+    """Algorithmic bytes / flops per step for every stage -> {stage: (bound, work, peak, unit)}."""
+    D, H, d, L, k = cfg.emb_hidden, cfg.emb_n_hidden_layers, cfg.gnn_latent, cfg.gnn_iters, cfg.k
+    b = 2 if cfg.precision == "bf16" else 4
+    tens = peaks["bf16_sustained"] * (2.0 if cfg.precision == "int8" else 1.0)      # int8 nominal = 2x bf16
+    ffma = 148 * 128 * 2 * 1.965e9 / 1e12                                           # TFLOP/s at max clock
+    mlp_peak, mlp_bound = (ffma, "alu") if cfg.precision == "fp32" else (tens, "tensor")
+    alu_lane = 148 * 128 * 1.965e9                                                  # lane-instructions / s
+    return {
+        "S0_plane_offsets": ("hbm", 16.0 * N + 4.0 * N, peaks["hbm"], "GB/s"),
+        "S1_embedding": (mlp_bound, N * 2.0 * (3 * D + (H - 1) * D * D + 4 * D), mlp_peak, "TFLOP/s"),
+        "S2_knn": ("alu", pairs * 12.0, alu_lane, "lane-instr/s"),
+        "S3_compaction_csc": ("hbm", 4.0 * k * N + 12.0 * E + 12.0 * E + 16.0 * N, peaks["hbm"], "GB/s"),
+        "S4_encoders": (mlp_bound, 2.0 * (3 * d + d * d) * (N + E), mlp_peak, "TFLOP/s"),
+        "S4c_scatter": ("hbm", L * (2.0 * E * d * b + 2.0 * N * d * b + 4.0 * E + 8.0 * N), peaks["hbm"], "GB/s"),
+        "S4d_node_net": ("hbm", L * (5.0 * N * d * b), peaks["hbm"], "GB/s"),
+        "S4e_edge_net_head": ("hbm", L * ((2.0 * d * b + 8.0) * E + N * d * b) + 8.0 * E, peaks["hbm"], "GB/s"),
+        "S5_components": ("hbm", 12.0 * E + 8.0 * N, peaks["hbm"], "GB/s"),
+    }
+
+
+def run_oracle_sample(cfg, batch, layers, n_events, scales=None):
+    import oracle
+    sub = batch.slice_events(0, min(n_events, batch.n_events))
+    o = oracle.Oracle(datagen.pack_blob(cfg, layers, scales), cfg.precision)
+    t0 = time.perf_counter()
+    o.run(sub.xyz, sub.plane, sub.event_offsets, cfg.k, cfg.window, cfg.d2_max, cfg.threshold)
+    dt = time.perf_counter() - t0
+    return sub.n_events / dt, dt, sub.n_events, oracle.threads()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="etx", choices=["etx", "reference"])
+    ap.add_argument("--config", default="cfg2")
+    ap.add_argument("--events", type=int, default=None, help="override the batch size (debugging only)")
+    ap.add_argument("--engine", default="auto", choices=["auto", "simt"])
+    ap.add_argument("--cpu-events", type=int, default=32, help="oracle sample size for cpu_baseline")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    cfg = datagen.get_config(args.config)
+    if args.events:
+        cfg = cfg.replace(n_events=args.events)
+    config = {"workload": f"{cfg.name}: {cfg.n_events} synthetic VELO events/GPU, pile-up {cfg.mu_pv:g}, "
+                          f"emb 3->{'->'.join([str(cfg.emb_hidden)] * cfg.emb_n_hidden_layers)}->4, k={cfg.k}, w={cfg.window}, "
+                          f"d={cfg.gnn_latent}, L={cfg.gnn_iters}, {cfg.precision}",
+              "events_per_gpu": cfg.n_events, "weights": "He-uniform seed 7, zero bias",
+              "l2": "per-step working set (edge state alone > 1 GB) exceeds the 126 MB L2; no explicit flush"}
+
+    # ------------------------------------------------------------------ reference arm = the CPU oracle
+    if args.impl == "reference":
+        if rank != 0:
+            return 0
+        batch, layers = workload(cfg, 0)
+        scales = int8_scales(cfg, layers) if cfg.precision == "int8" else None
+        n_ev = max(1, min(args.cpu_events // 4, batch.n_events))
+        for _ in range(min(args.warmup, 1)):
+            run_oracle_sample(cfg, batch, layers, 1, scales)
+        t_tot, ev_tot, cores = 0.0, 0, 1
+        for _ in range(args.steps):
+            _, dt, n, cores = run_oracle_sample(cfg, batch, layers, n_ev, scales)
+            t_tot += dt; ev_tot += n
+        value = ev_tot / t_tot
+        hits = float(batch.event_offsets[n_ev]) / n_ev
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "impl": "reference", "n_gpus": args.gpus, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": 1e3 * t_tot / args.steps, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": DTYPE[cfg.precision], "data": "synthetic", "config": config,
+                "hits_per_s": value * hits,
+                "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                 "sample": f"each step = the first {n_ev} events of the {cfg.n_events}-event batch, whole path S0..S5"},
+                "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
+        print(json.dumps(line))
+        return 0
+
+    # ------------------------------------------------------------------ the CUDA path
+    import torch
+    import paper_2407_12119_b200 as etx
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    batch, layers = workload(cfg, rank)
+    scales = int8_scales(cfg, layers) if cfg.precision == "int8" else None
+    blob = datagen.pack_blob(cfg, layers, scales)
+    hp = etx.hyperparams_from_config(cfg, batch.n_events, batch.n_hits, engine=args.engine)
+    ctx = etx.Etx(blob, hp)
+    d_xyz = torch.from_numpy(batch.xyz).cuda()
+    d_plane = torch.from_numpy(batch.plane).cuda()
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        out = ctx.run(d_xyz, d_plane, batch.event_offsets)
+    torch.cuda.synchronize()
+    E = int(out.h_n_edges[0]); N = batch.n_hits
+    ctx.enable_timing(True)
+    sampler = ClockSampler(local_rank); sampler.start()
+    launches0 = ctx.launch_count()
+    barrier()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record(stream)
+    for _ in range(args.steps):
+        out = ctx.run(d_xyz, d_plane, batch.event_offsets)
+    ev1.record(stream)
+    barrier()
+    ms = ev0.elapsed_time(ev1)
+    clocks = sampler.stop()
+    launches = ctx.launch_count() - launches0
+    stage_ms = ctx.stage_times()                      # CUDA events of the last timed step, on the launching stream
+    ctx.enable_timing(False)
+    if dist is not None:
+        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+        cnt = torch.tensor([batch.n_events, N, E], device="cuda", dtype=torch.float64)
+        dist.all_reduce(cnt)
+        tot_events, tot_hits, _ = [float(x) for x in cnt.tolist()]
+    else:
+        tot_events, tot_hits = float(batch.n_events), float(N)
+    value = tot_events * args.steps / (ms * 1e-3)
+
+    # ---- end to end through etx_run_host: pinned host buffers, H2D + D2H inside the timed region
+    cap = cfg.k * N
+    h_xyz = torch.from_numpy(batch.xyz).pin_memory(); h_plane = torch.from_numpy(batch.plane).pin_memory()
+    h_score = torch.empty(max(cap, 1), dtype=torch.float32).pin_memory()
+    h_src = torch.empty(max(cap, 1), dtype=torch.int32).pin_memory(); h_dst = torch.empty(max(cap, 1), dtype=torch.int32).pin_memory()
+    h_tid = torch.empty(max(N, 1), dtype=torch.int32).pin_memory()
+    ctx.run_host(h_xyz, h_plane, batch.event_offsets, h_score, h_src, h_dst, h_tid)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        E2 = ctx.run_host(h_xyz, h_plane, batch.event_offsets, h_score, h_src, h_dst, h_tid)
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    if dist is not None:
+        t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    e2e = {"value": tot_events * args.steps / e2e_s, "unit": UNIT,
+           "h2d_bytes_per_step": int(16 * N + 4 * (batch.n_events + 1)), "d2h_bytes_per_step": int(12 * E2 + 4 * N + 4)}
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return 0
+
+    # ---- per-stage roofline fractions + the dominant kernel
+    peaks = measured_peaks()
+    po = batch.plane.astype(np.int64)
+    pairs = 0
+    for e in range(batch.n_events):
+        cnt = np.bincount(po[batch.event_offsets[e]:batch.event_offsets[e + 1]], minlength=27)
+        for w in range(1, cfg.window + 1):
+            pairs += int((cnt[:26 - w] * cnt[w:26]).sum())
+    model = stage_model(cfg, N, E, pairs, peaks)
+    stages = {}
+    for name, (bound, work, peak, unit) in model.items():
+        t = stage_ms.get(name, 0.0) * 1e-3
+        ach = (work / t / (1e12 if unit == "TFLOP/s" else 1e9 if unit == "GB/s" else 1.0)) if t > 0 else None
+        stages[name] = {"ms": stage_ms.get(name, 0.0), "bound": bound, "achieved": ach, "peak": peak, "unit": unit,
+                        "frac": (ach / peak) if ach else None}
+    dom = "S4e_edge_net_head"
+    L = max(cfg.gnn_iters, 1)
+    dom_ms = stage_ms[dom] / L
+    dom_bytes = model[dom][1] / L
+    roofline = {"kernel": "edge network MLP (S4e), one launch per message-passing step", "bound": "hbm",
+                "achieved": dom_bytes / (dom_ms * 1e-3) / 1e9 if dom_ms > 0 else None, "peak": peaks["hbm"], "unit": "GB/s",
+                "frac": (dom_bytes / (dom_ms * 1e-3) / 1e9 / peaks["hbm"]) if dom_ms > 0 else None, "traffic": None,
+                "peak_source": peaks["source"], "avg_launch_ms": dom_ms, "algorithmic_bytes_per_launch": dom_bytes,
+                "share_of_step": stage_ms[dom] / (ms / args.steps) if ms > 0 else None}
+    cpu_baseline = None
+    if not args.no_cpu_baseline:
+        v, dt, n, cores = run_oracle_sample(cfg, batch, layers, args.cpu_events, scales)
+        cpu_baseline = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+                        "sample": f"first {n} events of the same batch, whole path S0..S5, {dt:.1f} s"}
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": DTYPE[cfg.precision], "data": "synthetic", "config": dict(config, engine=args.engine),
+            "hits_per_s": tot_hits * args.steps / (ms * 1e-3), "n_hits": N, "n_edges": E, "clocks": clocks, "e2e": e2e,
+            "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu_baseline, "stages": stages}
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -1,0 +1,161 @@
+/* ============================================================================
+ * etx.h -- C-ABI boundary of the B200-native ETX4VELO hot path.
+ *
+ * The path (sec. 7: "embedding inference, k-NN, GNN up to the edge
+ * classifier, WCC"; triplet steps excluded exactly as in the paper's CUDA code,
+ * L20 / L238), batched over many events (L12 abstract, L38 sec. 2, L223 sec. 7:
+ * 500 events per stream):
+ *
+ *   S0 plane offsets      hits arrive per (event, plane)              L26, L223, L257
+ *   S1 embedding MLP      e_h = MLP(norm(x,y,z))                      L96 sec. 5.1, L107 fn.5
+ *   S2 k-NN               k nearest hits on planes p+1..p+w, d2<d2max L98 Eq.(1), L101, L257 sec. 7.2
+ *   S3 edge list          G_rough^hit, directed i->j, i on lower plane L74-76, L137
+ *   S4 interaction net    encoders, L x (Eq.(4) messages, node net,
+ *                         edge net, residual), edge classifier        L133-148 sec. 5.2
+ *   S5 threshold + WCC    discard score < s_edge,min; components      L80, L82, L206, L261 sec. 7.3
+ *
+ * Readings of every point where the paper is silent are in DESIGN.md sec. 4
+ * (R1..R26).  All pointers are plain pointers; "d_" = device memory on the
+ * current CUDA device, "h_" = host memory.  No C++ or torch types cross this
+ * boundary.  Every function returns an etx_status; nothing throws or aborts.
+ * ==========================================================================*/
+#ifndef ETX_H_
+#define ETX_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct etx_ctx* etx_handle;
+typedef void* etx_stream;            /* a cudaStream_t, passed as an opaque pointer (NULL = default stream) */
+
+typedef enum {
+  ETX_OK = 0,
+  ETX_ERR_ARG = -1,          /* null pointer, negative size, inconsistent offsets            */
+  ETX_ERR_BLOB = -2,         /* weights blob: bad magic / version / shapes / size / scales   */
+  ETX_ERR_CAPACITY = -3,     /* n_events > max_events or n_hits > max_hits                   */
+  ETX_ERR_INPUT_ORDER = -4,  /* device-side validation found hits not sorted by (event,plane)*/
+  ETX_ERR_CUDA = -5,         /* a CUDA runtime call failed; see etx_last_error               */
+  ETX_ERR_UNSUPPORTED = -6   /* shape / precision not built into this library                */
+} etx_status;
+
+typedef enum { ETX_FP32 = 0, ETX_BF16 = 1, ETX_INT8 = 2 } etx_precision;
+
+/* How the MLP layers with K >= 16 are executed (the K = 3 input layers and the d->1 head are
+ * always fp32 FFMA in a pinned order, R4/R20/R21). */
+typedef enum {
+  ETX_ENGINE_AUTO = 0,       /* fp32: FFMA kernels; bf16 / int8: tcgen05 tensor-core kernels  */
+  ETX_ENGINE_SIMT = 1        /* FFMA kernels in every precision (bf16 / int8 rounding points
+                                reproduced exactly; the deterministic debugging path)         */
+} etx_engine;
+
+typedef struct {
+  uint32_t struct_size;              /* sizeof(etx_hyperparams); ABI check                              */
+  int32_t  n_planes;                 /* 26 (L26)                                                        */
+  float    norm_offset[3];           /* f = (x + offset) / div, true IEEE division (L107 fn.5, R1)      */
+  float    norm_div[3];
+  int32_t  emb_hidden;               /* width D of the embedding MLP's hidden layers (64 | 128)         */
+  int32_t  emb_n_hidden_layers;      /* H hidden layers: 3 -> D -> ... -> D -> emb_dim                  */
+  int32_t  emb_dim;                  /* 4                                                               */
+  int32_t  k;                        /* k_max neighbours per hit (L101)                                 */
+  int32_t  window;                   /* w: candidates on planes p+1..p+w (L101: 2)                      */
+  float    d2_max;                   /* keep candidate iff d2 < d2_max; +inf = no cut (L101, R6)        */
+  int32_t  gnn_latent;               /* d = n_h = n_e (L148)                                            */
+  int32_t  gnn_iters;                /* L message-passing steps with distinct weights (L148)            */
+  int32_t  edge_enc_input;           /* 0: |f_dst - f_src| (BASELINE configs)  1: [h0_src,h0_dst] (L133)*/
+  float    threshold;                /* s_edge,min: keep edge iff score >= threshold (L80, R17)         */
+  int32_t  precision;                /* etx_precision of the MLP layers with K >= 16                    */
+  int32_t  engine;                   /* etx_engine                                                      */
+  int32_t  max_events;               /* workspace capacity (L223: fixed memory per stream)              */
+  int32_t  max_hits;                 /* max_edges = k * max_hits                                        */
+  int32_t  validate_input;           /* 1: device-side check that hits are sorted by (event, plane)     */
+} etx_hyperparams;
+
+typedef struct {                     /* device pointers into the handle's workspace (library-owned);   */
+  const int32_t* d_edge_src;         /* [n_edges]  valid until the next call on the handle             */
+  const int32_t* d_edge_dst;         /* [n_edges]  edges ordered by (src asc, neighbour rank asc) (R9)  */
+  const float*   d_edge_score;       /* [n_edges]  sigmoid of the edge classifier output (L80)          */
+  const float*   d_edge_logit;       /* [n_edges]  pre-sigmoid value; the threshold is applied here     */
+  const int32_t* d_track_id;         /* [n_hits]   smallest global hit index of the hit's component     */
+  const int32_t* d_n_edges;          /* device scalar                                                   */
+  const int32_t* h_n_edges;          /* pinned host mirror; valid once the stream has been synchronised */
+  int32_t        n_hits;
+} etx_output;
+
+/* Create a context: parse + validate the weights blob (layout: datagen/weights.py header; fp32
+ * tensors W[out][in], b[out] in the order emb 0..H, node enc (2), edge enc (2), per step node net (2)
+ * + edge net (2), head; INT8 additionally one activation scale per Linear with K >= 16), convert the
+ * weights to the precision's operand format, allocate the workspace for (max_events, max_hits, k).
+ * The blob is copied; the caller may free it on return.  *out is set only on ETX_OK. */
+etx_status etx_create(const void* h_weights_blob, size_t blob_bytes, const etx_hyperparams* hp,
+                      etx_handle* out);
+
+/* Enqueue the whole path S0..S5 for one packed batch on `stream` and return without synchronising.
+ *   d_xyz             [n_hits][3] fp32, millimetres, device; borrowed until the enqueued work is done
+ *   d_plane           [n_hits] int32 in [0, n_planes), device; hits sorted by (event, plane)
+ *   h_event_offsets   [n_events+1] int32, host; [0] = 0, non-decreasing, [n_events] = n_hits
+ * Empty events / planes are legal; n_events = 0 is a no-op that reports 0 edges.
+ * One handle serves one stream at a time; calls on one handle are not thread-safe. */
+etx_status etx_run(etx_handle h, const float* d_xyz, const int32_t* d_plane,
+                   const int32_t* h_event_offsets, int32_t n_events, etx_stream stream,
+                   etx_output* out);
+
+/* The same call with HOST buffers (the end-to-end measurement of bench.py): copies xyz / plane to the
+ * device, runs S0..S5, copies edge_score [n_edges], edge_src/dst (if non-NULL) and track_id [n_hits]
+ * back, and synchronises `stream`.  h_* output buffers must hold k*n_hits (edges) / n_hits entries.
+ * Pinned host memory makes the copies asynchronous; pageable memory works too.  *n_edges_out = E. */
+etx_status etx_run_host(etx_handle h, const float* h_xyz, const int32_t* h_plane,
+                        const int32_t* h_event_offsets, int32_t n_events, etx_stream stream,
+                        float* h_edge_score, int32_t* h_edge_src, int32_t* h_edge_dst,
+                        int32_t* h_track_id, int32_t* n_edges_out);
+
+etx_status etx_destroy(etx_handle h);
+
+const char* etx_status_string(etx_status s);
+const char* etx_last_error(etx_handle h);         /* message of the last failing call on this handle */
+
+/* ---------------------------------------------------------------------------
+ * Debug / measurement entry points (not part of the three-call contract).  They exist for the
+ * stage-isolated parity protocol: a stage is bit-exact only for identical inputs
+ * to that stage, so the tests inject the oracle's embedding / edge list / logits.
+ * -------------------------------------------------------------------------*/
+typedef struct {
+  const float*   d_emb;        /* non-NULL: skip S1 and use this [n_hits][emb_dim] embedding           */
+  const int32_t* d_src;        /* non-NULL (with d_dst): skip S2 + pack and use this edge list; it must */
+  const int32_t* d_dst;        /*   be sorted by src; row_ptr / CSC are rebuilt from it                 */
+  int32_t        n_edges;
+  const float*   d_logit;      /* non-NULL: skip S4 and use these [n_edges] logits                      */
+  int32_t        last_stage;   /* stop after stage 1..5 (5 = run everything)                            */
+} etx_inject;
+
+etx_status etx_dbg_run(etx_handle h, const float* d_xyz, const int32_t* d_plane,
+                       const int32_t* h_event_offsets, int32_t n_events, etx_stream stream,
+                       const etx_inject* inj, etx_output* out);
+
+/* Device pointer + byte size of an internal buffer of the last run: "plane_off", "emb", "nbr", "deg",
+ * "row_ptr", "col_ptr", "in_edge", "h", "e", "m", "logit", "tap".  h / e / m are in the state dtype
+ * (fp32 for ETX_FP32 and ETX_INT8, bf16 for ETX_BF16). */
+etx_status etx_dbg_buffer(etx_handle h, const char* name, const void** d_ptr, size_t* bytes);
+
+/* INT8 only: record the int32 accumulators of Linear `layer_index` (blob order) of the next run into
+ * the "tap" buffer ([rows][out] int32); -1 switches it off. */
+etx_status etx_dbg_tap_layer(etx_handle h, int32_t layer_index);
+
+/* Per-stage device times of the last etx_run / etx_dbg_run in milliseconds (CUDA events recorded on
+ * the run's stream; valid after the stream is synchronised).  Order: S0, S1, S2, S3, S4 encoders,
+ * S4 scatter (sum over steps), S4 node nets, S4 edge nets (+ head), S5.  Recording is enabled by
+ * etx_dbg_enable_timing(h, 1). */
+#define ETX_N_STAGE_TIMES 9
+etx_status etx_dbg_enable_timing(etx_handle h, int32_t on);
+etx_status etx_dbg_stage_times(etx_handle h, float* ms_out /* [ETX_N_STAGE_TIMES] */);
+
+/* Number of kernels this library launched since the handle was created (bench.py's gpu_launches). */
+int64_t etx_dbg_launch_count(etx_handle h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif  /* ETX_H_ */

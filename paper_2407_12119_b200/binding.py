@@ -1,0 +1,254 @@
+"""ctypes binding of include/etx.h.  Marshalling only."""
+from __future__ import annotations
+
+import ctypes as C
+import math
+import os
+import re
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(HERE, "libetx.so")
+_HEADER = os.path.join(HERE, "..", "include", "etx.h")
+
+PRECISION = {"fp32": 0, "bf16": 1, "int8": 2}
+ENGINE = {"auto": 0, "simt": 1}
+STAGE_NAMES = ["S0_plane_offsets", "S1_embedding", "S2_knn", "S3_compaction_csc", "S4_encoders",
+               "S4c_scatter", "S4d_node_net", "S4e_edge_net_head", "S5_components"]
+STATUS = {0: "ETX_OK", -1: "ETX_ERR_ARG", -2: "ETX_ERR_BLOB", -3: "ETX_ERR_CAPACITY", -4: "ETX_ERR_INPUT_ORDER",
+          -5: "ETX_ERR_CUDA", -6: "ETX_ERR_UNSUPPORTED"}
+
+
+class EtxError(RuntimeError):
+    def __init__(self, status: int, msg: str = ""):
+        self.status = status
+        super().__init__(f"{STATUS.get(status, status)}: {msg}")
+
+
+class Hyperparams(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("n_planes", C.c_int32), ("norm_offset", C.c_float * 3),
+                ("norm_div", C.c_float * 3), ("emb_hidden", C.c_int32), ("emb_n_hidden_layers", C.c_int32),
+                ("emb_dim", C.c_int32), ("k", C.c_int32), ("window", C.c_int32), ("d2_max", C.c_float),
+                ("gnn_latent", C.c_int32), ("gnn_iters", C.c_int32), ("edge_enc_input", C.c_int32),
+                ("threshold", C.c_float), ("precision", C.c_int32), ("engine", C.c_int32),
+                ("max_events", C.c_int32), ("max_hits", C.c_int32), ("validate_input", C.c_int32)]
+
+
+class EtxOutput(C.Structure):
+    _fields_ = [("d_edge_src", C.c_void_p), ("d_edge_dst", C.c_void_p), ("d_edge_score", C.c_void_p),
+                ("d_edge_logit", C.c_void_p), ("d_track_id", C.c_void_p), ("d_n_edges", C.c_void_p),
+                ("h_n_edges", C.POINTER(C.c_int32)), ("n_hits", C.c_int32)]
+
+
+class Inject(C.Structure):
+    _fields_ = [("d_emb", C.c_void_p), ("d_src", C.c_void_p), ("d_dst", C.c_void_p), ("n_edges", C.c_int32),
+                ("d_logit", C.c_void_p), ("last_stage", C.c_int32)]
+
+
+def lib_path() -> str:
+    return _LIB_PATH
+
+
+def declared_symbols() -> list[str]:
+    """Every function include/etx.h declares (used by the CPU test that checks the exports)."""
+    text = open(_HEADER).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(etx_[a-z_0-9]+)\s*\(", text)))
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen libetx.so and declare the signatures.  Raises if the library has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        raise ImportError(f"{_LIB_PATH} is missing: run `python -m paper_2407_12119_b200._build` "
+                          "(there is no CPU fallback)")
+    L = C.CDLL(_LIB_PATH)
+    vp, i32p, f32p = C.c_void_p, C.POINTER(C.c_int32), C.POINTER(C.c_float)
+    L.etx_create.restype = C.c_int
+    L.etx_create.argtypes = [vp, C.c_size_t, C.POINTER(Hyperparams), C.POINTER(vp)]
+    L.etx_run.restype = C.c_int
+    L.etx_run.argtypes = [vp, vp, vp, i32p, C.c_int32, vp, C.POINTER(EtxOutput)]
+    L.etx_run_host.restype = C.c_int
+    L.etx_run_host.argtypes = [vp, vp, vp, i32p, C.c_int32, vp, vp, vp, vp, vp, i32p]
+    L.etx_destroy.restype = C.c_int
+    L.etx_destroy.argtypes = [vp]
+    L.etx_status_string.restype = C.c_char_p
+    L.etx_status_string.argtypes = [C.c_int]
+    L.etx_last_error.restype = C.c_char_p
+    L.etx_last_error.argtypes = [vp]
+    L.etx_dbg_run.restype = C.c_int
+    L.etx_dbg_run.argtypes = [vp, vp, vp, i32p, C.c_int32, vp, C.POINTER(Inject), C.POINTER(EtxOutput)]
+    L.etx_dbg_buffer.restype = C.c_int
+    L.etx_dbg_buffer.argtypes = [vp, C.c_char_p, C.POINTER(vp), C.POINTER(C.c_size_t)]
+    L.etx_dbg_tap_layer.restype = C.c_int
+    L.etx_dbg_tap_layer.argtypes = [vp, C.c_int32]
+    L.etx_dbg_enable_timing.restype = C.c_int
+    L.etx_dbg_enable_timing.argtypes = [vp, C.c_int32]
+    L.etx_dbg_stage_times.restype = C.c_int
+    L.etx_dbg_stage_times.argtypes = [vp, f32p]
+    L.etx_dbg_launch_count.restype = C.c_int64
+    L.etx_dbg_launch_count.argtypes = [vp]
+    _lib = L
+    return L
+
+
+def lib():
+    return load_library()
+
+
+def hyperparams_from_config(cfg, max_events: int, max_hits: int, precision: str | None = None,
+                            engine: str = "auto", validate_input: bool = False, n_planes: int = 26,
+                            norm_offset=(0.0, 0.0, 300.0), norm_div=(40.0, 40.0, 1050.0)) -> Hyperparams:
+    """etx_hyperparams from a datagen.EtxConfig-like object (attribute access only)."""
+    hp = Hyperparams()
+    hp.struct_size = C.sizeof(Hyperparams)
+    hp.n_planes = n_planes
+    hp.norm_offset = (C.c_float * 3)(*norm_offset)
+    hp.norm_div = (C.c_float * 3)(*norm_div)
+    hp.emb_hidden, hp.emb_n_hidden_layers, hp.emb_dim = cfg.emb_hidden, cfg.emb_n_hidden_layers, cfg.emb_dim
+    hp.k, hp.window = cfg.k, cfg.window
+    hp.d2_max = cfg.d2_max if math.isfinite(cfg.d2_max) else float("inf")
+    hp.gnn_latent, hp.gnn_iters, hp.edge_enc_input = cfg.gnn_latent, cfg.gnn_iters, cfg.edge_enc_input
+    hp.threshold = cfg.threshold
+    hp.precision = PRECISION[precision or cfg.precision]
+    hp.engine = ENGINE[engine]
+    hp.max_events, hp.max_hits = max_events, max_hits
+    hp.validate_input = int(validate_input)
+    return hp
+
+
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("paper_2407_12119_b200 needs a CUDA device (no CPU fallback)")
+    return torch
+
+
+class Etx:
+    """One etx_handle.  Methods mirror the C entry points; tensors are torch CUDA tensors used as plain
+    device buffers, the stream is torch's current stream."""
+
+    def __init__(self, blob: bytes, hp: Hyperparams):
+        self._L = load_library()
+        _torch()
+        self._h = C.c_void_p()
+        self.hp = hp
+        self._blob = bytes(blob)
+        st = self._L.etx_create(self._blob, len(self._blob), C.byref(hp), C.byref(self._h))
+        if st != 0:
+            self._h = C.c_void_p()
+            raise EtxError(st, "etx_create")
+        self._keep = None
+
+    # -- lifetime -------------------------------------------------------------------------------
+    def destroy(self):
+        if getattr(self, "_h", None) and self._h.value:
+            self._L.etx_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    def _check(self, st: int, what: str):
+        if st != 0:
+            raise EtxError(st, f"{what}: {self._L.etx_last_error(self._h).decode()}")
+
+    @staticmethod
+    def _stream():
+        import torch
+        return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+    @staticmethod
+    def _offsets(event_offsets):
+        import numpy as np
+        eo = np.ascontiguousarray(event_offsets, dtype=np.int32)
+        return eo, eo.ctypes.data_as(C.POINTER(C.c_int32)), int(eo.size - 1)
+
+    # -- the three-call contract ----------------------------------------------------------------
+    def run(self, d_xyz, d_plane, event_offsets) -> EtxOutput:
+        """etx_run: enqueue on the current stream; returns the raw output struct (device pointers)."""
+        eo, eop, B = self._offsets(event_offsets)
+        out = EtxOutput()
+        self._keep = (d_xyz, d_plane, eo)
+        st = self._L.etx_run(self._h, C.c_void_p(d_xyz.data_ptr()), C.c_void_p(d_plane.data_ptr()), eop, B,
+                             self._stream(), C.byref(out))
+        self._check(st, "etx_run")
+        return out
+
+    def run_host(self, h_xyz, h_plane, event_offsets, h_score, h_src, h_dst, h_track_id) -> int:
+        """etx_run_host: host (ideally pinned) tensors in and out; synchronises; returns E."""
+        eo, eop, B = self._offsets(event_offsets)
+        E = C.c_int32(0)
+        ptr = lambda t: C.c_void_p(t.data_ptr()) if t is not None else C.c_void_p()
+        st = self._L.etx_run_host(self._h, ptr(h_xyz), ptr(h_plane), eop, B, self._stream(), ptr(h_score),
+                                  ptr(h_src), ptr(h_dst), ptr(h_track_id), C.byref(E))
+        self._check(st, "etx_run_host")
+        return int(E.value)
+
+    # -- debug entry points ----------------------------------------------------------------------
+    def dbg_run(self, d_xyz, d_plane, event_offsets, emb=None, src=None, dst=None, logit=None,
+                last_stage: int = 5) -> EtxOutput:
+        eo, eop, B = self._offsets(event_offsets)
+        inj = Inject()
+        ptr = lambda t: C.c_void_p(t.data_ptr()) if t is not None else C.c_void_p()
+        inj.d_emb, inj.d_src, inj.d_dst, inj.d_logit = ptr(emb), ptr(src), ptr(dst), ptr(logit)
+        inj.n_edges = int(src.numel()) if src is not None else 0
+        inj.last_stage = last_stage
+        out = EtxOutput()
+        self._keep = (d_xyz, d_plane, eo, emb, src, dst, logit)
+        st = self._L.etx_dbg_run(self._h, ptr(d_xyz), ptr(d_plane), eop, B, self._stream(), C.byref(inj), C.byref(out))
+        self._check(st, "etx_dbg_run")
+        return out
+
+    def tap_layer(self, index: int):
+        self._check(self._L.etx_dbg_tap_layer(self._h, index), "etx_dbg_tap_layer")
+
+    def enable_timing(self, on: bool = True):
+        self._check(self._L.etx_dbg_enable_timing(self._h, int(on)), "etx_dbg_enable_timing")
+
+    def stage_times(self) -> dict:
+        arr = (C.c_float * len(STAGE_NAMES))()
+        self._check(self._L.etx_dbg_stage_times(self._h, arr), "etx_dbg_stage_times")
+        return {n: float(v) for n, v in zip(STAGE_NAMES, arr)}
+
+    def launch_count(self) -> int:
+        return int(self._L.etx_dbg_launch_count(self._h))
+
+    def buffer(self, name: str, dtype, shape=None):
+        """A torch copy of an internal device buffer of the last run; synchronises."""
+        import torch
+        torch.cuda.current_stream().synchronize()
+        p, n = C.c_void_p(), C.c_size_t()
+        self._check(self._L.etx_dbg_buffer(self._h, name.encode(), C.byref(p), C.byref(n)), "etx_dbg_buffer")
+        return self._copy_out(p.value, n.value, dtype, shape)
+
+    @staticmethod
+    def _copy_out(ptr, nbytes: int, dtype, shape=None):
+        import torch
+        esz = torch.empty(0, dtype=dtype).element_size()
+        out = torch.empty(nbytes // esz, dtype=dtype, device="cuda")
+        if nbytes:
+            err = torch.cuda.cudart().cudaMemcpy(out.data_ptr(), int(ptr), nbytes, 3)   # device -> device
+            code = err[0] if isinstance(err, tuple) else err
+            if int(code) != 0:
+                raise RuntimeError(f"cudaMemcpy failed: {err}")
+        return out.view(shape) if shape is not None else out
+
+    def results(self, out: EtxOutput) -> dict:
+        """Synchronise and copy the outputs of a run into torch tensors."""
+        import torch
+        torch.cuda.current_stream().synchronize()
+        E, N = int(out.h_n_edges[0]), int(out.n_hits)
+        return dict(n_edges=E,
+                    src=self._copy_out(out.d_edge_src, 4 * E, torch.int32),
+                    dst=self._copy_out(out.d_edge_dst, 4 * E, torch.int32),
+                    score=self._copy_out(out.d_edge_score, 4 * E, torch.float32),
+                    logit=self._copy_out(out.d_edge_logit, 4 * E, torch.float32),
+                    track_id=self._copy_out(out.d_track_id, 4 * N, torch.int32))

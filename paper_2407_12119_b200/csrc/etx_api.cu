@@ -1,0 +1,469 @@
+// C-ABI entry points (include/etx.h): blob parsing, weight conversion, workspace, the stream-ordered launch
+// sequence S0..S5.  No host synchronisation inside etx_run; E lives on the device (n_edges) and every
+// E-sized kernel reads it there.
+#include <math.h>
+#include <string.h>
+
+#include <new>
+
+#include "etx_internal.h"
+
+using namespace etx;
+
+namespace {
+
+constexpr uint32_t kBlobMagic = 0x57585445u;   // 'ETXW'
+
+struct CudaFail { cudaError_t err; const char* what; };
+
+#define ETX_CUDA(call)                                                                  \
+  do {                                                                                  \
+    cudaError_t err__ = (call);                                                         \
+    if (err__ != cudaSuccess) throw CudaFail{err__, #call};                             \
+  } while (0)
+
+template <typename T>
+T* dev_alloc(etx_ctx* c, size_t n) {
+  void* p = nullptr;
+  ETX_CUDA(cudaMalloc(&p, (n ? n : 1) * sizeof(T)));
+  c->allocs.push_back(p);
+  return static_cast<T*>(p);
+}
+
+float* upload(etx_ctx* c, const std::vector<float>& v) {
+  float* p = dev_alloc<float>(c, v.size());
+  ETX_CUDA(cudaMemcpy(p, v.data(), v.size() * sizeof(float), cudaMemcpyHostToDevice));
+  return p;
+}
+
+float host_bf16_round(float x) { return __bfloat162float(__float2bfloat16_rn(x)); }
+
+etx_status fail(etx_ctx* c, etx_status st, const std::string& msg) {
+  if (c) c->error = msg;
+  return st;
+}
+
+// Blob layout: datagen/weights.py header comment (and include/etx.h, etx_create).
+etx_status parse_blob(etx_ctx* c, const uint8_t* blob, size_t bytes) {
+  const etx_hyperparams& hp = c->hp;
+  if (bytes < 64) return fail(c, ETX_ERR_BLOB, "blob smaller than its header");
+  uint32_t h[16];
+  memcpy(h, blob, 64);
+  if (h[0] != kBlobMagic || h[1] != 1u) return fail(c, ETX_ERR_BLOB, "bad blob magic / version");
+  if ((int)h[2] != hp.emb_hidden || (int)h[3] != hp.emb_n_hidden_layers || (int)h[4] != hp.emb_dim ||
+      (int)h[5] != hp.gnn_latent || (int)h[6] != hp.gnn_iters || (int)h[7] != hp.edge_enc_input)
+    return fail(c, ETX_ERR_BLOB, "blob shapes differ from the hyper-parameters");
+  const int D = hp.emb_hidden, H = hp.emb_n_hidden_layers, d = hp.gnn_latent, L = hp.gnn_iters;
+  auto add = [&](int out, int in, bool head = false) {
+    HostLayer l;
+    l.out = out; l.in = in; l.index = (int)c->layers.size();
+    l.tensor = (in >= 16) && !head;
+    c->layers.push_back(l);
+  };
+  c->i_emb0 = 0;
+  add(D, 3);
+  for (int i = 1; i < H; ++i) add(D, D);
+  add(hp.emb_dim, D);
+  c->i_nenc = (int)c->layers.size();
+  add(d, 3); add(d, d);
+  c->i_eenc = (int)c->layers.size();
+  add(d, hp.edge_enc_input ? 2 * d : 3); add(d, d);
+  c->i_iter0 = (int)c->layers.size();
+  for (int it = 0; it < L; ++it) { add(d, 3 * d); add(d, d); add(d, 3 * d); add(d, d); }
+  c->i_head = (int)c->layers.size();
+  add(1, d, true);
+  size_t need = 0; int nq = 0;
+  for (auto& l : c->layers) { need += (size_t)l.out * l.in + l.out; nq += l.tensor; }
+  if (h[8] != need) return fail(c, ETX_ERR_BLOB, "blob weight count differs from the shapes");
+  const size_t n_scales = h[9];
+  if (bytes != 64 + 4 * (need + n_scales)) return fail(c, ETX_ERR_BLOB, "blob size mismatch");
+  if (c->precision == ETX_INT8 && (int)n_scales != nq)
+    return fail(c, ETX_ERR_BLOB, "INT8 needs one activation scale per Linear with K >= 16");
+  const float* p = reinterpret_cast<const float*>(blob + 64);
+  const float* scales = p + need;
+  int qi = 0;
+  for (auto& l : c->layers) {
+    l.W.assign(p, p + (size_t)l.out * l.in); p += (size_t)l.out * l.in;
+    l.b.assign(p, p + l.out); p += l.out;
+    if (c->precision == ETX_INT8 && l.tensor) {
+      l.sx = scales[qi++];
+      if (!(l.sx > 0.0f) || !isfinite(l.sx)) return fail(c, ETX_ERR_BLOB, "activation scale must be finite and > 0");
+    }
+  }
+  return ETX_OK;
+}
+
+// fp32 -> the operand set of the precision mode (R20 bf16 RNE; R21 symmetric per-channel int8)
+void convert_layer(etx_ctx* c, HostLayer& l) {
+  const int K = l.in, N = l.out;
+  std::vector<float> Wt((size_t)K * N), scale(N, 1.0f);
+  std::vector<float> Wop((size_t)N * K);               // operand values, [N][K]
+  float inv_sx = 1.0f;
+  if (c->precision == ETX_INT8 && l.tensor) {
+    inv_sx = 1.0f / l.sx;
+    for (int n = 0; n < N; ++n) {
+      float m = 0.0f;
+      for (int k = 0; k < K; ++k) m = fmaxf(m, fabsf(l.W[(size_t)n * K + k]));
+      const float sw = m > 0.0f ? m / 127.0f : 1.0f;
+      scale[n] = l.sx * sw;
+      for (int k = 0; k < K; ++k) {
+        float r = nearbyintf(l.W[(size_t)n * K + k] / sw);
+        r = fminf(127.0f, fmaxf(-127.0f, r));
+        Wop[(size_t)n * K + k] = r;
+      }
+    }
+  } else if (c->precision == ETX_BF16 && l.tensor) {
+    for (size_t i = 0; i < Wop.size(); ++i) Wop[i] = host_bf16_round(l.W[i]);
+  } else {
+    Wop = l.W;
+  }
+  for (int n = 0; n < N; ++n)
+    for (int k = 0; k < K; ++k) Wt[(size_t)k * N + n] = Wop[(size_t)n * K + k];
+  l.dev.Wt = upload(c, Wt);
+  l.dev.scale = upload(c, scale);
+  l.dev.bias = upload(c, l.b);
+  l.dev.Wtc = nullptr;
+  l.dev.inv_sx = inv_sx;
+  l.dev.K = K; l.dev.N = N; l.dev.tensor = l.tensor ? 1 : 0; l.dev.index = l.index;
+  l.W.swap(Wop);   // keep the operand values for the tensor-core packer (umma_configure)
+}
+
+__global__ void set_scalar_kernel(int32_t* p, int32_t v) { *p = v; }
+__global__ void sigmoid_kernel(const float* __restrict__ z, const int32_t* __restrict__ n, float* __restrict__ s) {
+  const int E = *n;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < E; i += gridDim.x * blockDim.x) s[i] = 1.0f / (1.0f + expf(-z[i]));
+}
+
+struct StageTimer {
+  etx_ctx* c; cudaStream_t s;
+  void begin(int stage) {
+    if (!c->timing || c->n_ev + 2 > 256) return;
+    cudaEventRecord(c->ev[c->n_ev], s);
+    c->spans.push_back({c->n_ev, -1, stage});
+    c->n_ev++;
+  }
+  void end() {
+    if (!c->timing || c->spans.empty() || c->spans.back().b >= 0 || c->n_ev + 1 > 256) return;
+    cudaEventRecord(c->ev[c->n_ev], s);
+    c->spans.back().b = c->n_ev++;
+  }
+};
+
+etx_status run_impl(etx_ctx* c, const float* d_xyz, const int32_t* d_plane, const int32_t* h_eo, int n_events,
+                    cudaStream_t s, const etx_inject* inj, etx_output* out) {
+  if (!c) return ETX_ERR_ARG;
+  if (!h_eo || n_events < 0 || !out) return fail(c, ETX_ERR_ARG, "null event offsets / output, or n_events < 0");
+  if (n_events > c->hp.max_events) return fail(c, ETX_ERR_CAPACITY, "n_events exceeds max_events");
+  if (h_eo[0] != 0) return fail(c, ETX_ERR_ARG, "event_offsets[0] must be 0");
+  for (int e = 0; e < n_events; ++e)
+    if (h_eo[e + 1] < h_eo[e]) return fail(c, ETX_ERR_ARG, "event_offsets must be non-decreasing");
+  const int n_hits = h_eo[n_events];
+  if (n_hits > c->hp.max_hits) return fail(c, ETX_ERR_CAPACITY, "n_hits exceeds max_hits");
+  if (n_hits > 0 && (!d_xyz || !d_plane)) return fail(c, ETX_ERR_ARG, "null hit arrays");
+  if (c->h_flags[0] & 1) { c->h_flags[0] = 0; return fail(c, ETX_ERR_INPUT_ORDER, "previous batch: hits not sorted by (event, plane) or plane out of range"); }
+  const int last = inj ? (inj->last_stage > 0 ? inj->last_stage : 5) : 5;
+  if (inj && ((inj->d_src == nullptr) != (inj->d_dst == nullptr))) return fail(c, ETX_ERR_ARG, "inject: src and dst go together");
+  if (inj && inj->d_logit && !inj->d_src) return fail(c, ETX_ERR_ARG, "inject: logits need the edge list they belong to");
+  if (inj && inj->d_src && (inj->n_edges < 0 || inj->n_edges > c->max_edges)) return fail(c, ETX_ERR_CAPACITY, "inject: n_edges exceeds k * max_hits");
+  try {
+    // event offsets: pinned staging -> device (the only H2D of the call)
+    ETX_CUDA(cudaEventSynchronize(c->staging_free));
+    memcpy(c->h_event_off, h_eo, sizeof(int32_t) * ((size_t)n_events + 1));
+    ETX_CUDA(cudaMemcpyAsync(c->event_off, c->h_event_off, sizeof(int32_t) * ((size_t)n_events + 1), cudaMemcpyHostToDevice, s));
+    ETX_CUDA(cudaEventRecord(c->staging_free, s));
+    ETX_CUDA(cudaMemsetAsync(c->n_edges, 0, sizeof(int32_t), s));
+    c->n_ev = 0; c->spans.clear();
+    c->last_n_hits = n_hits;
+    StageTimer tm{c, s};
+    const bool tensor_engine = (c->precision != ETX_FP32) && c->engine == ETX_ENGINE_AUTO;
+    if (n_hits > 0) {
+      // ---- S0
+      tm.begin(0);
+      launch_features(c, d_xyz, n_hits, s);
+      launch_plane_offsets(c, d_plane, n_events, s);
+      if (c->hp.validate_input) launch_validate(c, d_plane, n_events, n_hits, s);
+      tm.end();
+      // ---- S1
+      tm.begin(1);
+      if (inj && inj->d_emb) ETX_CUDA(cudaMemcpyAsync(c->emb, inj->d_emb, sizeof(float4) * (size_t)n_hits, cudaMemcpyDeviceToDevice, s));
+      else if (tensor_engine) launch_embed_umma(c, n_hits, s);
+      else launch_embed_simt(c, n_hits, s);
+      tm.end();
+      if (last >= 2) {
+        // ---- S2, S3
+        if (inj && inj->d_src) {
+          tm.begin(3);
+          if (inj->n_edges > 0) {
+            ETX_CUDA(cudaMemcpyAsync(c->src, inj->d_src, sizeof(int32_t) * (size_t)inj->n_edges, cudaMemcpyDeviceToDevice, s));
+            ETX_CUDA(cudaMemcpyAsync(c->dst, inj->d_dst, sizeof(int32_t) * (size_t)inj->n_edges, cudaMemcpyDeviceToDevice, s));
+          }
+          set_scalar_kernel<<<1, 1, 0, s>>>(c->n_edges, inj->n_edges); c->launches++;
+          launch_rows_from_src(c, n_hits, inj->n_edges, s);
+        } else {
+          tm.begin(2);
+          launch_knn(c, d_plane, n_events, n_hits, s);
+          tm.end();
+          tm.begin(3);
+          launch_pack_edges(c, n_hits, s);
+        }
+        if (last >= 3) launch_csc(c, n_hits, s);
+        tm.end();
+      }
+      if (last >= 4) {
+        // ---- S4
+        if (inj && inj->d_logit) {
+          tm.begin(7);
+          if (inj->n_edges > 0) ETX_CUDA(cudaMemcpyAsync(c->logit, inj->d_logit, sizeof(float) * (size_t)inj->n_edges, cudaMemcpyDeviceToDevice, s));
+          sigmoid_kernel<<<c->sm_count * 4, 256, 0, s>>>(c->logit, c->n_edges, c->score); c->launches++;
+          tm.end();
+        } else {
+          const int L = c->hp.gnn_iters;
+          auto mlp = [&](int kind, int it, bool head) {
+            if (tensor_engine) launch_gnn_mlp_umma(c, kind, it, n_hits, head, s);
+            else launch_gnn_mlp_simt(c, kind, it, n_hits, head, s);
+          };
+          tm.begin(4);
+          mlp(kNodeEnc, 0, false);
+          mlp(kEdgeEnc, 0, L == 0);
+          tm.end();
+          for (int it = 0; it < L; ++it) {
+            tm.begin(5); launch_scatter(c, n_hits, s); tm.end();
+            tm.begin(6); mlp(kNodeNet, it, false); tm.end();
+            tm.begin(7); mlp(kEdgeNet, it, it == L - 1); tm.end();
+          }
+        }
+      }
+      if (last >= 5) {
+        tm.begin(8);
+        launch_components(c, c->logit, n_hits, s);
+        tm.end();
+      }
+    }
+    ETX_CUDA(cudaMemcpyAsync(c->h_n_edges, c->n_edges, sizeof(int32_t), cudaMemcpyDeviceToHost, s));
+    if (c->hp.validate_input) {
+      ETX_CUDA(cudaMemcpyAsync(c->h_flags, c->flags, sizeof(int32_t), cudaMemcpyDeviceToHost, s));
+      ETX_CUDA(cudaMemsetAsync(c->flags, 0, sizeof(int32_t), s));
+    }
+    ETX_CUDA(cudaGetLastError());
+  } catch (const CudaFail& f) {
+    return fail(c, ETX_ERR_CUDA, std::string(f.what) + ": " + cudaGetErrorString(f.err));
+  }
+  out->d_edge_src = c->src; out->d_edge_dst = c->dst; out->d_edge_score = c->score; out->d_edge_logit = c->logit;
+  out->d_track_id = c->track_id; out->d_n_edges = c->n_edges; out->h_n_edges = c->h_n_edges; out->n_hits = n_hits;
+  return ETX_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+etx_status etx_create(const void* blob, size_t blob_bytes, const etx_hyperparams* hp, etx_handle* out) {
+  if (!blob || !hp || !out) return ETX_ERR_ARG;
+  if (hp->struct_size != sizeof(etx_hyperparams)) return ETX_ERR_ARG;
+  etx_ctx* c = new (std::nothrow) etx_ctx();
+  if (!c) return ETX_ERR_CUDA;
+  c->hp = *hp;
+  c->precision = hp->precision; c->engine = hp->engine;
+  auto bail = [&](etx_status st) { etx_destroy(c); return st; };
+  if (hp->precision < 0 || hp->precision > 2 || hp->engine < 0 || hp->engine > 1) return bail(ETX_ERR_ARG);
+  if (hp->n_planes < 1 || hp->n_planes > 1024 || hp->k < 1 || hp->window < 1 || hp->max_events < 0 || hp->max_hits < 0 ||
+      hp->gnn_iters < 0 || hp->gnn_iters > 64 || hp->emb_n_hidden_layers < 1 || hp->emb_n_hidden_layers > 8 ||
+      !(hp->threshold >= 0.0f && hp->threshold <= 1.0f) || isnan(hp->d2_max))
+    return bail(ETX_ERR_ARG);
+  for (int i = 0; i < 3; ++i) if (!(hp->norm_div[i] != 0.0f)) return bail(ETX_ERR_ARG);
+  // shapes built into the kernels
+  if (!(hp->emb_hidden == 64 || hp->emb_hidden == 128) || hp->emb_dim != 4 || !(hp->gnn_latent == 32 || hp->gnn_latent == 64) ||
+      hp->k > 64 || (hp->edge_enc_input != 0 && hp->edge_enc_input != 1))
+    return bail(ETX_ERR_UNSUPPORTED);
+  if ((long long)hp->k * hp->max_hits > 0x7fffffffLL) return bail(ETX_ERR_CAPACITY);
+  c->max_edges = hp->k * hp->max_hits;
+  c->state_bf16 = (hp->precision == ETX_BF16);
+  if (hp->threshold <= 0.0f) c->tau = -INFINITY;
+  else if (hp->threshold >= 1.0f) c->tau = INFINITY;
+  else c->tau = (float)log((double)hp->threshold / (1.0 - (double)hp->threshold));      // R17
+  etx_status st = parse_blob(c, static_cast<const uint8_t*>(blob), blob_bytes);
+  if (st != ETX_OK) return bail(st);
+  try {
+    int dev = 0;
+    ETX_CUDA(cudaGetDevice(&dev));
+    ETX_CUDA(cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev));
+    for (auto& l : c->layers) convert_layer(c, l);
+    const size_t N = (size_t)hp->max_hits, E = (size_t)c->max_edges, B = (size_t)hp->max_events, d = hp->gnn_latent;
+    const size_t sb = c->state_bf16 ? 2 : 4;
+    c->event_off = dev_alloc<int32_t>(c, B + 1);
+    c->plane_off = dev_alloc<int32_t>(c, B * (hp->n_planes + 1));
+    c->feat = dev_alloc<float4>(c, N);
+    c->emb = dev_alloc<float4>(c, N);
+    c->nbr = dev_alloc<int32_t>(c, N * hp->k);
+    c->deg = dev_alloc<int32_t>(c, N);
+    c->row_ptr = dev_alloc<int32_t>(c, N + 1);
+    c->col_ptr = dev_alloc<int32_t>(c, N + 1);
+    c->cursor = dev_alloc<int32_t>(c, N + 1);
+    c->src = dev_alloc<int32_t>(c, E);
+    c->dst = dev_alloc<int32_t>(c, E);
+    c->in_edge = dev_alloc<int32_t>(c, E);
+    c->scan_tmp = dev_alloc<int32_t>(c, N / 2048 + 2);
+    c->n_edges = dev_alloc<int32_t>(c, 1);
+    c->flags = dev_alloc<int32_t>(c, 1);
+    c->h = dev_alloc<uint8_t>(c, N * d * sb + 256);
+    c->m = dev_alloc<uint8_t>(c, N * 2 * d * sb + 256);
+    c->e = dev_alloc<uint8_t>(c, E * d * sb + 256);
+    c->logit = dev_alloc<float>(c, E);
+    c->score = dev_alloc<float>(c, E);
+    c->track_id = dev_alloc<int32_t>(c, N);
+    c->d_xyz_in = dev_alloc<float>(c, N * 3);
+    c->d_plane_in = dev_alloc<int32_t>(c, N);
+    ETX_CUDA(cudaMemset(c->n_edges, 0, sizeof(int32_t)));
+    ETX_CUDA(cudaMemset(c->flags, 0, sizeof(int32_t)));
+    ETX_CUDA(cudaMallocHost(&c->h_event_off, sizeof(int32_t) * (B + 1)));
+    ETX_CUDA(cudaMallocHost(&c->h_n_edges, sizeof(int32_t)));
+    ETX_CUDA(cudaMallocHost(&c->h_flags, sizeof(int32_t)));
+    c->h_n_edges[0] = 0; c->h_flags[0] = 0;
+    ETX_CUDA(cudaEventCreateWithFlags(&c->staging_free, cudaEventDisableTiming));
+    for (int i = 0; i < 256; ++i) ETX_CUDA(cudaEventCreate(&c->ev[i]));
+    simt_configure(c);
+    if (c->precision != ETX_FP32 && c->engine == ETX_ENGINE_AUTO) {
+      if (!umma_supported(c)) { c->error = "tensor-core engine not available for these shapes"; return bail(ETX_ERR_UNSUPPORTED); }
+      umma_configure(c);
+    }
+    ETX_CUDA(cudaDeviceSynchronize());
+  } catch (const CudaFail& f) {
+    (void)f;
+    return bail(ETX_ERR_CUDA);
+  }
+  *out = c;
+  return ETX_OK;
+}
+
+etx_status etx_destroy(etx_handle c) {
+  if (!c) return ETX_OK;
+  cudaDeviceSynchronize();
+  for (void* p : c->allocs) cudaFree(p);
+  if (c->tap) cudaFree(c->tap);
+  if (c->h_event_off) cudaFreeHost(c->h_event_off);
+  if (c->h_n_edges) cudaFreeHost(c->h_n_edges);
+  if (c->h_flags) cudaFreeHost(c->h_flags);
+  if (c->staging_free) cudaEventDestroy(c->staging_free);
+  for (int i = 0; i < 256; ++i) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
+  delete c;
+  return ETX_OK;
+}
+
+etx_status etx_run(etx_handle c, const float* d_xyz, const int32_t* d_plane, const int32_t* h_event_offsets,
+                   int32_t n_events, etx_stream stream, etx_output* out) {
+  return run_impl(c, d_xyz, d_plane, h_event_offsets, n_events, static_cast<cudaStream_t>(stream), nullptr, out);
+}
+
+etx_status etx_dbg_run(etx_handle c, const float* d_xyz, const int32_t* d_plane, const int32_t* h_event_offsets,
+                       int32_t n_events, etx_stream stream, const etx_inject* inj, etx_output* out) {
+  return run_impl(c, d_xyz, d_plane, h_event_offsets, n_events, static_cast<cudaStream_t>(stream), inj, out);
+}
+
+etx_status etx_run_host(etx_handle c, const float* h_xyz, const int32_t* h_plane, const int32_t* h_event_offsets,
+                        int32_t n_events, etx_stream stream, float* h_edge_score, int32_t* h_edge_src,
+                        int32_t* h_edge_dst, int32_t* h_track_id, int32_t* n_edges_out) {
+  if (!c) return ETX_ERR_ARG;
+  if (!h_event_offsets || n_events < 0 || !n_edges_out) return fail(c, ETX_ERR_ARG, "null argument");
+  if (n_events > c->hp.max_events) return fail(c, ETX_ERR_CAPACITY, "n_events exceeds max_events");
+  const int n_hits = h_event_offsets[n_events];
+  if (n_hits < 0 || n_hits > c->hp.max_hits) return fail(c, ETX_ERR_CAPACITY, "n_hits exceeds max_hits");
+  if (n_hits > 0 && (!h_xyz || !h_plane)) return fail(c, ETX_ERR_ARG, "null hit arrays");
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  try {
+    if (n_hits > 0) {
+      ETX_CUDA(cudaMemcpyAsync(c->d_xyz_in, h_xyz, sizeof(float) * 3 * (size_t)n_hits, cudaMemcpyHostToDevice, s));
+      ETX_CUDA(cudaMemcpyAsync(c->d_plane_in, h_plane, sizeof(int32_t) * (size_t)n_hits, cudaMemcpyHostToDevice, s));
+    }
+    etx_output o;
+    etx_status st = run_impl(c, c->d_xyz_in, c->d_plane_in, h_event_offsets, n_events, s, nullptr, &o);
+    if (st != ETX_OK) return st;
+    if (h_track_id && n_hits > 0)
+      ETX_CUDA(cudaMemcpyAsync(h_track_id, c->track_id, sizeof(int32_t) * (size_t)n_hits, cudaMemcpyDeviceToHost, s));
+    ETX_CUDA(cudaStreamSynchronize(s));            // E is needed on the host to size the edge copies
+    const int E = c->h_n_edges[0];
+    *n_edges_out = E;
+    if (E > 0) {
+      if (h_edge_score) ETX_CUDA(cudaMemcpyAsync(h_edge_score, c->score, sizeof(float) * (size_t)E, cudaMemcpyDeviceToHost, s));
+      if (h_edge_src) ETX_CUDA(cudaMemcpyAsync(h_edge_src, c->src, sizeof(int32_t) * (size_t)E, cudaMemcpyDeviceToHost, s));
+      if (h_edge_dst) ETX_CUDA(cudaMemcpyAsync(h_edge_dst, c->dst, sizeof(int32_t) * (size_t)E, cudaMemcpyDeviceToHost, s));
+      ETX_CUDA(cudaStreamSynchronize(s));
+    }
+  } catch (const CudaFail& f) {
+    return fail(c, ETX_ERR_CUDA, std::string(f.what) + ": " + cudaGetErrorString(f.err));
+  }
+  return ETX_OK;
+}
+
+const char* etx_status_string(etx_status s) {
+  switch (s) {
+    case ETX_OK: return "ETX_OK";
+    case ETX_ERR_ARG: return "ETX_ERR_ARG";
+    case ETX_ERR_BLOB: return "ETX_ERR_BLOB";
+    case ETX_ERR_CAPACITY: return "ETX_ERR_CAPACITY";
+    case ETX_ERR_INPUT_ORDER: return "ETX_ERR_INPUT_ORDER";
+    case ETX_ERR_CUDA: return "ETX_ERR_CUDA";
+    case ETX_ERR_UNSUPPORTED: return "ETX_ERR_UNSUPPORTED";
+  }
+  return "ETX_ERR_UNKNOWN";
+}
+
+const char* etx_last_error(etx_handle c) { return c ? c->error.c_str() : "null handle"; }
+
+etx_status etx_dbg_buffer(etx_handle c, const char* name, const void** d_ptr, size_t* bytes) {
+  if (!c || !name || !d_ptr || !bytes) return ETX_ERR_ARG;
+  const size_t N = (size_t)c->last_n_hits, E = (size_t)c->h_n_edges[0], d = c->hp.gnn_latent, sb = c->state_bf16 ? 2 : 4;
+  const std::string n(name);
+  if (n == "plane_off") { *d_ptr = c->plane_off; *bytes = 0; return ETX_OK; }
+  if (n == "emb") { *d_ptr = c->emb; *bytes = N * 16; return ETX_OK; }
+  if (n == "feat") { *d_ptr = c->feat; *bytes = N * 16; return ETX_OK; }
+  if (n == "nbr") { *d_ptr = c->nbr; *bytes = N * c->hp.k * 4; return ETX_OK; }
+  if (n == "deg") { *d_ptr = c->deg; *bytes = N * 4; return ETX_OK; }
+  if (n == "row_ptr") { *d_ptr = c->row_ptr; *bytes = (N + 1) * 4; return ETX_OK; }
+  if (n == "col_ptr") { *d_ptr = c->col_ptr; *bytes = (N + 1) * 4; return ETX_OK; }
+  if (n == "in_edge") { *d_ptr = c->in_edge; *bytes = E * 4; return ETX_OK; }
+  if (n == "h") { *d_ptr = c->h; *bytes = N * d * sb; return ETX_OK; }
+  if (n == "m") { *d_ptr = c->m; *bytes = N * 2 * d * sb; return ETX_OK; }
+  if (n == "e") { *d_ptr = c->e; *bytes = E * d * sb; return ETX_OK; }
+  if (n == "logit") { *d_ptr = c->logit; *bytes = E * 4; return ETX_OK; }
+  if (n == "tap") { *d_ptr = c->tap; *bytes = c->tap_bytes; return ETX_OK; }
+  return fail(c, ETX_ERR_ARG, "unknown buffer name");
+}
+
+etx_status etx_dbg_tap_layer(etx_handle c, int32_t layer_index) {
+  if (!c) return ETX_ERR_ARG;
+  if (layer_index < 0) { c->tap_layer = -1; return ETX_OK; }
+  if (c->precision != ETX_INT8 || layer_index >= (int)c->layers.size() || !c->layers[layer_index].tensor)
+    return fail(c, ETX_ERR_ARG, "tap: INT8 mode and a quantised layer index are required");
+  if (!c->tap) {
+    const size_t rows = (size_t)(c->max_edges > c->hp.max_hits ? c->max_edges : c->hp.max_hits);
+    const size_t width = (size_t)(c->hp.emb_hidden > c->hp.gnn_latent ? c->hp.emb_hidden : c->hp.gnn_latent);
+    const size_t bytes = rows * width * 4;
+    if (bytes > (size_t)4 << 30) return fail(c, ETX_ERR_CAPACITY, "tap buffer would exceed 4 GiB; use a smaller max_hits");
+    if (cudaMalloc(&c->tap, bytes ? bytes : 4) != cudaSuccess) return fail(c, ETX_ERR_CUDA, "cudaMalloc(tap)");
+    c->tap_bytes = bytes;
+  }
+  c->tap_layer = layer_index;
+  return ETX_OK;
+}
+
+etx_status etx_dbg_enable_timing(etx_handle c, int32_t on) {
+  if (!c) return ETX_ERR_ARG;
+  c->timing = on != 0;
+  return ETX_OK;
+}
+
+etx_status etx_dbg_stage_times(etx_handle c, float* ms_out) {
+  if (!c || !ms_out) return ETX_ERR_ARG;
+  for (int i = 0; i < ETX_N_STAGE_TIMES; ++i) ms_out[i] = 0.0f;
+  for (auto& sp : c->spans) {
+    if (sp.b < 0) continue;
+    float ms = 0.0f;
+    if (cudaEventElapsedTime(&ms, c->ev[sp.a], c->ev[sp.b]) != cudaSuccess) return fail(c, ETX_ERR_CUDA, "cudaEventElapsedTime");
+    ms_out[sp.stage] += ms;
+  }
+  return ETX_OK;
+}
+
+int64_t etx_dbg_launch_count(etx_handle c) { return c ? c->launches : 0; }
+
+}  // extern "C"

@@ -1,0 +1,143 @@
+// Internal declarations of the ETX4VELO B200 library (not part of the C-ABI; see include/etx.h).
+// Shares nothing with oracle/ (the CPU oracle is test infrastructure and has its own code).
+#pragma once
+
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/etx.h"
+
+namespace etx {
+
+constexpr int kMaxEmbLayers = 9;     // H + 1, H <= 8
+constexpr int kTileRows = 64;        // rows (hits / edges) per CTA tile of the FFMA MLP kernels
+constexpr int kMlpThreads = 256;
+
+// One Linear, as the kernels see it.  W is stored transposed ([K][N], N contiguous) in fp32 holding the
+// values the precision mode multiplies with: the fp32 weights, their bf16 roundings, or the int8 codes.
+struct LayerP {
+  const float* Wt;        // [K][N]
+  const float* scale;     // [N]  y = fmaf(acc, scale, bias); 1.0 except INT8 tensor layers (s_x * s_w[c])
+  const float* bias;      // [N]
+  const void* Wtc;        // tensor-core operand: W[N][K] K-major, bf16 or int8, swizzled per K-block
+  float inv_sx;           // INT8 tensor layers: 1 / s_x of the layer's input tensor
+  int K, N;
+  int tensor;             // K >= 16 and not the head (R20 / R21)
+  int index;              // position in blob order
+};
+
+enum MlpKind { kNodeEnc = 0, kEdgeEnc = 1, kNodeNet = 2, kEdgeNet = 3 };
+
+struct GnnArgs {
+  LayerP l0, l1, head;
+  const float4* feat;        // [n_hits] normalised (fx, fy, fz, 0)
+  const int32_t* src;        // [E]
+  const int32_t* dst;        // [E]
+  const int32_t* n_rows_ptr; // device scalar: number of rows (E for edge kernels), or nullptr -> n_rows
+  int n_rows;
+  void* h;                   // [n_hits][d]  state dtype
+  void* e;                   // [E][d]
+  const void* m;             // [n_hits][2d]
+  float* logit;              // [E]  (do_head)
+  float* score;              // [E]
+  int do_head;
+  int edge_enc_input;
+  int32_t* tap;              // int32 accumulators of layer tap_layer, or nullptr
+  int tap_layer;
+};
+
+struct EmbArgs {
+  LayerP layers[kMaxEmbLayers];
+  int n_layers;              // H + 1
+  const float4* feat;
+  float4* emb;               // [n_hits] (emb_dim == 4)
+  int n_rows;
+  int32_t* tap;
+  int tap_layer;
+};
+
+struct HostLayer {
+  int out = 0, in = 0, index = 0;
+  bool tensor = false;
+  std::vector<float> W, b;       // blob values
+  float sx = 1.0f;
+  LayerP dev{};
+};
+
+}  // namespace etx
+
+struct etx_ctx {
+  etx_hyperparams hp{};
+  int precision = 0, engine = 0;
+  bool state_bf16 = false;
+  int max_edges = 0;
+  int sm_count = 148;
+  std::string error;
+  std::vector<etx::HostLayer> layers;     // blob order
+  int i_emb0 = 0, i_nenc = 0, i_eenc = 0, i_iter0 = 0, i_head = 0;
+  std::vector<void*> allocs;              // every cudaMalloc of this handle
+  // workspace
+  int32_t* event_off = nullptr;           // [max_events + 1]
+  int32_t* plane_off = nullptr;           // [max_events][P + 1]
+  float4* feat = nullptr;                 // [max_hits]
+  float4* emb = nullptr;                  // [max_hits]
+  int32_t *nbr = nullptr, *deg = nullptr; // [max_hits][k], [max_hits]
+  int32_t *row_ptr = nullptr, *col_ptr = nullptr, *cursor = nullptr;   // [max_hits + 1]
+  int32_t *src = nullptr, *dst = nullptr, *in_edge = nullptr;          // [max_edges]
+  int32_t* scan_tmp = nullptr;            // block sums
+  int32_t* n_edges = nullptr;             // device scalar
+  int32_t* flags = nullptr;               // device: [0] input-order violation
+  void *h = nullptr, *e = nullptr, *m = nullptr;
+  float *logit = nullptr, *score = nullptr;
+  int32_t *track_id = nullptr;
+  int32_t* tap = nullptr;
+  size_t tap_bytes = 0;
+  int tap_layer = -1;
+  // host side
+  int32_t* h_event_off = nullptr;         // pinned staging [max_events + 1]
+  int32_t* h_n_edges = nullptr;           // pinned mirror
+  int32_t* h_flags = nullptr;             // pinned mirror
+  cudaEvent_t staging_free = nullptr;
+  // staging for etx_run_host
+  float* d_xyz_in = nullptr;
+  int32_t* d_plane_in = nullptr;
+  // timing
+  bool timing = false;
+  cudaEvent_t ev[256] = {};
+  int n_ev = 0;
+  struct Span { int a, b, stage; };
+  std::vector<Span> spans;
+  int64_t launches = 0;
+  int last_n_hits = 0;
+  float tau = 0.0f;
+};
+
+namespace etx {
+
+// ---- launchers (each file owns its kernels) -------------------------------------------------------------
+// k_graph.cu
+void launch_features(etx_ctx* c, const float* xyz, int n_hits, cudaStream_t s);
+void launch_plane_offsets(etx_ctx* c, const int32_t* plane, int n_events, cudaStream_t s);
+void launch_validate(etx_ctx* c, const int32_t* plane, int n_events, int n_hits, cudaStream_t s);
+void launch_knn(etx_ctx* c, const int32_t* plane, int n_events, int n_hits, cudaStream_t s);
+void launch_pack_edges(etx_ctx* c, int n_hits, cudaStream_t s);                 // deg, nbr -> row_ptr, src, dst, n_edges
+void launch_rows_from_src(etx_ctx* c, int n_hits, int n_edges, cudaStream_t s); // injected edge list -> row_ptr
+void launch_csc(etx_ctx* c, int n_hits, cudaStream_t s);                        // dst -> col_ptr, in_edge
+void launch_components(etx_ctx* c, const float* logit, int n_hits, cudaStream_t s);
+// k_mlp_simt.cu
+void launch_embed_simt(etx_ctx* c, int n_hits, cudaStream_t s);
+void launch_gnn_mlp_simt(etx_ctx* c, int kind, int iter, int n_hits, bool do_head, cudaStream_t s);
+void launch_scatter(etx_ctx* c, int n_hits, cudaStream_t s);
+void simt_configure(etx_ctx* c);
+void fill_gnn_args(etx_ctx* c, int kind, int iter, int n_hits, bool do_head, GnnArgs& a);
+// k_mlp_umma.cu
+bool umma_supported(const etx_ctx* c);
+void umma_configure(etx_ctx* c);
+void launch_embed_umma(etx_ctx* c, int n_hits, cudaStream_t s);
+void launch_gnn_mlp_umma(etx_ctx* c, int kind, int iter, int n_hits, bool do_head, cudaStream_t s);
+
+}  // namespace etx

@@ -1,0 +1,411 @@
+// Graph stages of the ETX4VELO hot path on sm_100a: S0 plane offsets, S2 plane-restricted k-NN,
+// S3 edge compaction + CSC, S5 threshold + connected components.  All integer / index work here is
+// bit-exact by construction; the only floating point is Eq.(1) in a pinned operation order.
+#include "etx_internal.h"
+
+namespace etx {
+
+// --------------------------------------------------------------------------------------------------------
+// C1 (PAPER.md L107 fn.5; R1): f = ((x,y,z) + offset) / div, one IEEE add and one correctly
+// rounded division.  Stored once as float4 so every later stage gathers 16 B per hit.
+__global__ void features_kernel(const float* __restrict__ xyz, float4* __restrict__ feat, int n,
+                                float ox, float oy, float oz, float dx, float dy, float dz) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  float x = xyz[3 * (size_t)i], y = xyz[3 * (size_t)i + 1], z = xyz[3 * (size_t)i + 2];
+  feat[i] = make_float4(__fdiv_rn(__fadd_rn(x, ox), dx), __fdiv_rn(__fadd_rn(y, oy), dy),
+                        __fdiv_rn(__fadd_rn(z, oz), dz), 0.0f);
+}
+
+void launch_features(etx_ctx* c, const float* xyz, int n_hits, cudaStream_t s) {
+  if (n_hits == 0) return;
+  const etx_hyperparams& hp = c->hp;
+  features_kernel<<<(n_hits + 255) / 256, 256, 0, s>>>(xyz, c->feat, n_hits, hp.norm_offset[0], hp.norm_offset[1],
+                                                       hp.norm_offset[2], hp.norm_div[0], hp.norm_div[1],
+                                                       hp.norm_div[2]);
+  c->launches++;
+}
+
+// --------------------------------------------------------------------------------------------------------
+// S0 (L26, L223, L257): plane_off[e][p] = first hit of event e with plane >= p (lower bound in the sorted
+// plane array); entry P is the event's end.  One thread per (event, p).
+__global__ void plane_offsets_kernel(const int32_t* __restrict__ plane, const int32_t* __restrict__ event_off,
+                                     int n_events, int P, int32_t* __restrict__ plane_off) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n_events * (P + 1)) return;
+  int e = i / (P + 1), p = i % (P + 1);
+  int lo = event_off[e], hi = event_off[e + 1];
+  while (lo < hi) {
+    int mid = (lo + hi) >> 1;
+    if (plane[mid] < p) lo = mid + 1; else hi = mid;
+  }
+  plane_off[i] = lo;
+}
+
+void launch_plane_offsets(etx_ctx* c, const int32_t* plane, int n_events, cudaStream_t s) {
+  int n = n_events * (c->hp.n_planes + 1);
+  if (n == 0) return;
+  plane_offsets_kernel<<<(n + 255) / 256, 256, 0, s>>>(plane, c->event_off, n_events, c->hp.n_planes, c->plane_off);
+  c->launches++;
+}
+
+// Input contract check (include/etx.h): plane in range, and non-decreasing except across an event boundary.
+__global__ void validate_kernel(const int32_t* __restrict__ plane, const int32_t* __restrict__ event_off,
+                                int n_events, int n_hits, int P, int32_t* __restrict__ flags) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n_hits) return;
+  int p = plane[i];
+  bool bad = p < 0 || p >= P;
+  if (!bad && i + 1 < n_hits && plane[i + 1] < p) {
+    int lo = 0, hi = n_events + 1;               // is i + 1 the start of some event?
+    while (lo < hi) { int mid = (lo + hi) >> 1; if (event_off[mid] < i + 1) lo = mid + 1; else hi = mid; }
+    bad = !(lo <= n_events && event_off[lo] == i + 1);
+  }
+  if (bad) atomicOr(&flags[0], 1);
+}
+
+void launch_validate(etx_ctx* c, const int32_t* plane, int n_events, int n_hits, cudaStream_t s) {
+  if (n_hits == 0) return;
+  validate_kernel<<<(n_hits + 255) / 256, 256, 0, s>>>(plane, c->event_off, n_events, n_hits, c->hp.n_planes, c->flags);
+  c->launches++;
+}
+
+// --------------------------------------------------------------------------------------------------------
+// S2 (L98 Eq.(1), L101, L257 sec. 7.2; R4-R8).  For hit q on plane p the candidates are the hits of the same
+// event on planes p+1 .. min(p+w, P-1): one contiguous index range given by the plane offsets.  The result
+// is the first min(k, #kept) candidates in ascending (d2, index) order, d2 < d2_max strict.
+//
+// The paper's kernel is one thread per query with a sequential scan ("lacks parallelisation over the
+// neighbours", L286).  Here a CTA owns one (event, plane) bucket: the candidate range is staged through
+// shared memory in tiles (so capacity never depends on the window size), and every query is scanned by
+// LANES cooperating lanes (lane j takes candidates j, j+LANES, ...), each keeping a sorted top-k of 64-bit
+// keys (d2 bits << 32 | index) in registers; the LANES partial lists are merged with warp shuffles.
+// Keys are unique, so the merged list does not depend on how candidates were split.
+template <int KCAP>
+struct TopK {
+  unsigned long long key[KCAP];
+  __device__ __forceinline__ void init() {
+#pragma unroll
+    for (int s = 0; s < KCAP; ++s) key[s] = ~0ull;
+  }
+  // insert into the ascending list of the first k slots
+  __device__ __forceinline__ void insert(unsigned long long cur, int k) {
+#pragma unroll
+    for (int s = 0; s < KCAP; ++s) {
+      if (s < k) {
+        unsigned long long old = key[s];
+        bool lt = cur < old;
+        key[s] = lt ? cur : old;
+        cur = lt ? old : cur;
+      }
+    }
+  }
+};
+
+constexpr int kKnnThreads = 128;
+constexpr int kKnnTile = 1024;       // candidates per shared-memory tile (16 KB)
+
+template <int KCAP, int LANES>
+__global__ void __launch_bounds__(kKnnThreads)
+knn_kernel(const float4* __restrict__ emb, const int32_t* __restrict__ plane_off, int P, int k, int w,
+           float d2_max, int32_t* __restrict__ nbr, int32_t* __restrict__ deg) {
+  __shared__ float4 cand[kKnnTile];
+  const int bucket = blockIdx.x;                 // e * P + p
+  const int e = bucket / P, p = bucket % P;
+  const int32_t* po = plane_off + (size_t)e * (P + 1);
+  const int q_lo = po[p], q_hi = po[p + 1];
+  if (q_lo == q_hi) return;
+  const int p_hi = min(p + w, P - 1);
+  const int c_lo = po[p + 1], c_hi = (p + 1 <= p_hi) ? po[p_hi + 1] : po[p + 1];
+  constexpr int QPB = kKnnThreads / LANES;       // queries per pass
+  const int sub = threadIdx.x % LANES, qslot = threadIdx.x / LANES;
+
+  for (int q0 = q_lo; q0 < q_hi; q0 += QPB) {
+    const int q = q0 + qslot;
+    const bool active = q < q_hi;
+    float4 a = active ? emb[q] : make_float4(0.f, 0.f, 0.f, 0.f);
+    TopK<KCAP> top;
+    top.init();
+    unsigned long long worst = ~0ull;
+    for (int t0 = c_lo; t0 < c_hi; t0 += kKnnTile) {
+      const int nt = min(kKnnTile, c_hi - t0);
+      __syncthreads();
+      for (int i = threadIdx.x; i < nt; i += kKnnThreads) cand[i] = emb[t0 + i];
+      __syncthreads();
+      if (active) {
+        for (int i = sub; i < nt; i += LANES) {
+          const float4 b = cand[i];
+          // Eq.(1) in the pinned order: t0*t0, then fma(t_i, t_i, d2)   (R4)
+          float t = __fsub_rn(a.x, b.x);
+          float d2 = __fmul_rn(t, t);
+          t = __fsub_rn(a.y, b.y); d2 = __fmaf_rn(t, t, d2);
+          t = __fsub_rn(a.z, b.z); d2 = __fmaf_rn(t, t, d2);
+          t = __fsub_rn(a.w, b.w); d2 = __fmaf_rn(t, t, d2);
+          if (d2 < d2_max) {
+            unsigned long long key = ((unsigned long long)__float_as_uint(d2) << 32) | (unsigned)(t0 + i);
+            if (key < worst) {
+              top.insert(key, k);
+#pragma unroll
+              for (int s = 0; s < KCAP; ++s) if (s == k - 1) worst = top.key[s];
+            }
+          }
+        }
+      }
+    }
+    // merge the LANES partial lists: round r folds lane (sub ^ r)'s list into ours
+    if (LANES > 1) {
+#pragma unroll
+      for (int r = 1; r < LANES; r <<= 1) {
+        unsigned long long other[KCAP];
+#pragma unroll
+        for (int s = 0; s < KCAP; ++s) other[s] = __shfl_xor_sync(0xffffffffu, top.key[s], r);
+#pragma unroll
+        for (int s = 0; s < KCAP; ++s) if (s < k && other[s] != ~0ull) top.insert(other[s], k);
+      }
+    }
+    if (active && sub == 0) {
+      int cnt = 0;
+#pragma unroll
+      for (int s = 0; s < KCAP; ++s) {
+        if (s < k) {
+          const bool valid = top.key[s] != ~0ull;
+          nbr[(size_t)q * k + s] = valid ? (int32_t)(unsigned)(top.key[s] & 0xffffffffull) : -1;
+          cnt += valid;
+        }
+      }
+      deg[q] = cnt;
+    }
+  }
+}
+
+template <int KCAP>
+static void knn_dispatch(etx_ctx* c, int n_buckets, cudaStream_t s) {
+  const etx_hyperparams& hp = c->hp;
+  knn_kernel<KCAP, 4><<<n_buckets, kKnnThreads, 0, s>>>(c->emb, c->plane_off, hp.n_planes, hp.k, hp.window,
+                                                       hp.d2_max, c->nbr, c->deg);
+}
+
+void launch_knn(etx_ctx* c, const int32_t* plane, int n_events, int n_hits, cudaStream_t s) {
+  (void)plane;
+  if (n_hits == 0 || n_events == 0) return;
+  const int nb = n_events * c->hp.n_planes;
+  const int k = c->hp.k;
+  if (k <= 4) knn_dispatch<4>(c, nb, s);
+  else if (k <= 10) knn_dispatch<10>(c, nb, s);
+  else if (k <= 16) knn_dispatch<16>(c, nb, s);
+  else if (k <= 32) knn_dispatch<32>(c, nb, s);
+  else knn_dispatch<64>(c, nb, s);
+  c->launches++;
+}
+
+// --------------------------------------------------------------------------------------------------------
+// S3 (L74-76, L137; R9): exclusive scan of the out-degrees -> row_ptr, E; pack (src, dst) in (src asc, rank asc)
+// order; in-degree histogram -> col_ptr; in_edge = edge ids grouped by dst, ascending inside a group.
+constexpr int kScanThreads = 256;
+constexpr int kScanItems = 8;                       // per thread
+constexpr int kScanChunk = kScanThreads * kScanItems;
+
+__device__ __forceinline__ int block_exclusive_scan(int v, int* total) {   // blockDim = kScanThreads
+  __shared__ int warp_sums[kScanThreads / 32];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  int x = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+  if (lane == 31) warp_sums[wid] = x;
+  __syncthreads();
+  if (wid == 0) {
+    int s = lane < kScanThreads / 32 ? warp_sums[lane] : 0;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, s, o); if (lane >= o) s += y; }
+    if (lane < kScanThreads / 32) warp_sums[lane] = s;
+  }
+  __syncthreads();
+  const int base = wid ? warp_sums[wid - 1] : 0;
+  *total = warp_sums[kScanThreads / 32 - 1];
+  __syncthreads();
+  return base + x - v;
+}
+
+__global__ void __launch_bounds__(kScanThreads) scan_reduce_kernel(const int32_t* __restrict__ in, int n,
+                                                                  int32_t* __restrict__ bsum) {
+  const int base = blockIdx.x * kScanChunk;
+  int v = 0;
+#pragma unroll
+  for (int j = 0; j < kScanItems; ++j) { int i = base + threadIdx.x * kScanItems + j; if (i < n) v += in[i]; }
+  int tot; block_exclusive_scan(v, &tot);
+  if (threadIdx.x == 0) bsum[blockIdx.x] = tot;
+}
+
+__global__ void __launch_bounds__(kScanThreads) scan_bsum_kernel(int32_t* __restrict__ bsum, int nb) {
+  int carry = 0;                                   // single block, sequential over chunks of 256
+  for (int b0 = 0; b0 < nb; b0 += kScanThreads) {
+    int i = b0 + threadIdx.x;
+    int v = i < nb ? bsum[i] : 0, tot;
+    int ex = block_exclusive_scan(v, &tot);
+    if (i < nb) bsum[i] = carry + ex;
+    carry += tot;
+  }
+}
+
+__global__ void __launch_bounds__(kScanThreads) scan_write_kernel(const int32_t* __restrict__ in, int n,
+                                                                 const int32_t* __restrict__ bsum,
+                                                                 int32_t* __restrict__ out, int32_t* __restrict__ total) {
+  const int base = blockIdx.x * kScanChunk;
+  int vals[kScanItems], v = 0;
+#pragma unroll
+  for (int j = 0; j < kScanItems; ++j) {
+    int i = base + threadIdx.x * kScanItems + j;
+    vals[j] = i < n ? in[i] : 0;
+    v += vals[j];
+  }
+  int tot;
+  int ex = block_exclusive_scan(v, &tot) + bsum[blockIdx.x];
+#pragma unroll
+  for (int j = 0; j < kScanItems; ++j) {
+    int i = base + threadIdx.x * kScanItems + j;
+    if (i < n) out[i] = ex;
+    ex += vals[j];
+    if (i == n - 1) { out[n] = ex; if (total) *total = ex; }
+  }
+}
+
+__global__ void scan_empty_kernel(int32_t* out, int32_t* total) { out[0] = 0; if (total) *total = 0; }
+
+// out[0..n] = exclusive prefix sums of in[0..n); *total = out[n]
+static void exclusive_scan(etx_ctx* c, const int32_t* in, int n, int32_t* out, int32_t* total, cudaStream_t s) {
+  if (n == 0) { scan_empty_kernel<<<1, 1, 0, s>>>(out, total); c->launches++; return; }
+  const int nb = (n + kScanChunk - 1) / kScanChunk;
+  scan_reduce_kernel<<<nb, kScanThreads, 0, s>>>(in, n, c->scan_tmp);
+  scan_bsum_kernel<<<1, kScanThreads, 0, s>>>(c->scan_tmp, nb);
+  scan_write_kernel<<<nb, kScanThreads, 0, s>>>(in, n, c->scan_tmp, out, total);
+  c->launches += 3;
+}
+
+__global__ void pack_edges_kernel(const int32_t* __restrict__ nbr, const int32_t* __restrict__ deg,
+                                  const int32_t* __restrict__ row_ptr, int n_hits, int k,
+                                  int32_t* __restrict__ src, int32_t* __restrict__ dst) {
+  size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= (size_t)n_hits * k) return;
+  int q = (int)(i / k), sidx = (int)(i % k);
+  if (sidx < deg[q]) {
+    int pos = row_ptr[q] + sidx;
+    src[pos] = q;
+    dst[pos] = nbr[i];
+  }
+}
+
+void launch_pack_edges(etx_ctx* c, int n_hits, cudaStream_t s) {
+  exclusive_scan(c, c->deg, n_hits, c->row_ptr, c->n_edges, s);
+  if (n_hits == 0) return;
+  size_t n = (size_t)n_hits * c->hp.k;
+  pack_edges_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(c->nbr, c->deg, c->row_ptr, n_hits, c->hp.k, c->src, c->dst);
+  c->launches++;
+}
+
+// injected, src-sorted edge list: row_ptr[q] = lower bound of q in src
+__global__ void rows_from_src_kernel(const int32_t* __restrict__ src, int n_edges, int n_hits, int32_t* __restrict__ row_ptr) {
+  int q = blockIdx.x * blockDim.x + threadIdx.x;
+  if (q > n_hits) return;
+  int lo = 0, hi = n_edges;
+  while (lo < hi) { int mid = (lo + hi) >> 1; if (src[mid] < q) lo = mid + 1; else hi = mid; }
+  row_ptr[q] = lo;
+}
+
+void launch_rows_from_src(etx_ctx* c, int n_hits, int n_edges, cudaStream_t s) {
+  rows_from_src_kernel<<<(n_hits + 1 + 255) / 256, 256, 0, s>>>(c->src, n_edges, n_hits, c->row_ptr);
+  c->launches++;
+}
+
+__global__ void indegree_kernel(const int32_t* __restrict__ dst, const int32_t* __restrict__ n_edges, int32_t* __restrict__ indeg) {
+  const int E = *n_edges;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < E; i += gridDim.x * blockDim.x) atomicAdd(&indeg[dst[i]], 1);
+}
+
+__global__ void csc_fill_kernel(const int32_t* __restrict__ dst, const int32_t* __restrict__ n_edges,
+                                int32_t* __restrict__ cursor, int32_t* __restrict__ in_edge) {
+  const int E = *n_edges;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < E; i += gridDim.x * blockDim.x)
+    in_edge[atomicAdd(&cursor[dst[i]], 1)] = i;
+}
+
+// ascending edge id inside every dst group (R9 / R22): groups are short (in-degree ~ k), insertion sort
+__global__ void csc_sort_kernel(const int32_t* __restrict__ col_ptr, int n_hits, int32_t* __restrict__ in_edge) {
+  int l = blockIdx.x * blockDim.x + threadIdx.x;
+  if (l >= n_hits) return;
+  const int a = col_ptr[l], b = col_ptr[l + 1];
+  for (int i = a + 1; i < b; ++i) {
+    int v = in_edge[i], j = i - 1;
+    while (j >= a && in_edge[j] > v) { in_edge[j + 1] = in_edge[j]; --j; }
+    in_edge[j + 1] = v;
+  }
+}
+
+void launch_csc(etx_ctx* c, int n_hits, cudaStream_t s) {
+  if (n_hits == 0) { exclusive_scan(c, c->cursor, 0, c->col_ptr, nullptr, s); return; }
+  cudaMemsetAsync(c->cursor, 0, sizeof(int32_t) * ((size_t)n_hits + 1), s);
+  const int grid = c->sm_count * 8;
+  indegree_kernel<<<grid, 256, 0, s>>>(c->dst, c->n_edges, c->cursor);
+  exclusive_scan(c, c->cursor, n_hits, c->col_ptr, nullptr, s);
+  cudaMemcpyAsync(c->cursor, c->col_ptr, sizeof(int32_t) * (size_t)n_hits, cudaMemcpyDeviceToDevice, s);
+  csc_fill_kernel<<<grid, 256, 0, s>>>(c->dst, c->n_edges, c->cursor, c->in_edge);
+  csc_sort_kernel<<<(n_hits + 255) / 256, 256, 0, s>>>(c->col_ptr, n_hits, c->in_edge);
+  c->launches += 3;
+}
+
+// --------------------------------------------------------------------------------------------------------
+// S5 (L80, L82, L206, L261 sec. 7.3; R17, R18): an edge is kept iff logit >= tau; track_id[h] = smallest hit
+// index in h's component of the kept-edge graph.  The paper's kernel propagates the lowest label with one
+// forward and one backward plane sweep (a heuristic that can under-merge); here exact components by a
+// lock-free union-find: a root is only ever re-pointed to a SMALLER index, so the final root of a set is
+// its minimum and the result does not depend on the interleaving.  Pointer jumping compresses paths.
+__device__ __forceinline__ int uf_find(int32_t* parent_, int x) {
+  volatile int32_t* parent = parent_;  // other threads re-point entries concurrently: always re-read
+  int p = parent[x];
+  while (p != x) {
+    int gp = parent[p];
+    if (gp != p) parent[x] = gp;       // path halving (benign race: only ever stores an ancestor)
+    x = p; p = gp;
+  }
+  return x;
+}
+
+__global__ void uf_init_kernel(int32_t* __restrict__ parent, int n) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) parent[i] = i;
+}
+
+__global__ void uf_union_kernel(const int32_t* __restrict__ src, const int32_t* __restrict__ dst,
+                                const float* __restrict__ logit, const int32_t* __restrict__ n_edges, float tau,
+                                int32_t* parent) {
+  const int E = *n_edges;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < E; i += gridDim.x * blockDim.x) {
+    if (!(logit[i] >= tau)) continue;
+    int a = uf_find(parent, src[i]), b = uf_find(parent, dst[i]);
+    while (a != b) {
+      if (a > b) { int t = a; a = b; b = t; }       // a < b : hang root b under a
+      int old = atomicCAS(&parent[b], b, a);
+      if (old == b) break;
+      b = uf_find(parent, old);                     // b was no longer a root: retry from its new root
+      a = uf_find(parent, a);
+    }
+  }
+}
+
+__global__ void uf_flatten_kernel(int32_t* parent, int n) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  volatile int32_t* vp = parent;
+  int r = i;
+  while (true) { int p = vp[r]; if (p == r) break; r = p; }
+  vp[i] = r;     // racing readers still see an ancestor of i
+}
+
+void launch_components(etx_ctx* c, const float* logit, int n_hits, cudaStream_t s) {
+  if (n_hits == 0) return;
+  uf_init_kernel<<<(n_hits + 255) / 256, 256, 0, s>>>(c->track_id, n_hits);
+  uf_union_kernel<<<c->sm_count * 8, 256, 0, s>>>(c->src, c->dst, logit, c->n_edges, c->tau, c->track_id);
+  uf_flatten_kernel<<<(n_hits + 255) / 256, 256, 0, s>>>(c->track_id, n_hits);
+  c->launches += 3;
+}
+
+}  // namespace etx

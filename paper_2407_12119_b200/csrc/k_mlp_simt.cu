@@ -1,0 +1,429 @@
+// FFMA ("SIMT") kernels of the MLP stages S1 and S4 and the Eq.(4) scatter-sum.
+//
+// These run the fp32 precision mode (configs 0 and 1), and in every precision they are the deterministic
+// debugging path (etx_engine = ETX_ENGINE_SIMT): each output is ONE sequential chain
+//     acc = 0; for j ascending: acc = fmaf(x_j, w_j, acc);  y = fmaf(acc, scale, b)
+// (scale = 1 outside INT8, where it is s_x*s_w[c]; R3/R4/R21), so results do not depend on the
+// tiling.  INT8 is emulated exactly on the FFMA pipe: int8 codes are small integers, every partial sum is an
+// integer below 2^24, so the fp32 chain reproduces the int32 accumulator bit for bit.
+#include "etx_internal.h"
+
+namespace etx {
+
+enum { kModeF32 = 0, kModeBf16 = 1, kModeInt8 = 2 };
+
+__device__ __forceinline__ float bf16r(float x) { return __bfloat162float(__float2bfloat16_rn(x)); }
+
+// q = clamp(rne(x * inv_s), -127, 127) as a float (R21)
+__device__ __forceinline__ float quant_i8(float x, float inv_s) {
+  float r = rintf(__fmul_rn(x, inv_s));
+  r = fmaxf(r, -127.0f);
+  return fminf(r, 127.0f);
+}
+
+// ---- state access: fp32 or bf16 rows of d values, 4 at a time ---------------------------------------------
+template <typename ST> struct State;
+template <> struct State<float> {
+  static __device__ __forceinline__ float4 ld4(const void* base, size_t elem) {
+    return *reinterpret_cast<const float4*>(static_cast<const float*>(base) + elem);
+  }
+  static __device__ __forceinline__ void st4(void* base, size_t elem, float4 v) {
+    *reinterpret_cast<float4*>(static_cast<float*>(base) + elem) = v;
+  }
+  static __device__ __forceinline__ float round(float x) { return x; }
+};
+template <> struct State<__nv_bfloat16> {
+  static __device__ __forceinline__ float4 ld4(const void* base, size_t elem) {
+    uint2 u = *reinterpret_cast<const uint2*>(static_cast<const __nv_bfloat16*>(base) + elem);
+    return make_float4(__uint_as_float(u.x << 16), __uint_as_float(u.x & 0xffff0000u),
+                       __uint_as_float(u.y << 16), __uint_as_float(u.y & 0xffff0000u));
+  }
+  static __device__ __forceinline__ void st4(void* base, size_t elem, float4 v) {   // values already rounded
+    uint2 u;
+    u.x = (__float_as_uint(v.x) >> 16) | (__float_as_uint(v.y) & 0xffff0000u);
+    u.y = (__float_as_uint(v.z) >> 16) | (__float_as_uint(v.w) & 0xffff0000u);
+    *reinterpret_cast<uint2*>(static_cast<__nv_bfloat16*>(base) + elem) = u;
+  }
+  static __device__ __forceinline__ float round(float x) { return bf16r(x); }
+};
+
+// hidden activation -> operand of the next (tensor) layer: bf16 rounding / int8 quantisation (R20, R21)
+template <int MODE>
+__device__ __forceinline__ float to_operand(float v, float inv_sx_next) {
+  if (MODE == kModeBf16) return bf16r(v);
+  if (MODE == kModeInt8) return quant_i8(v, inv_sx_next);
+  return v;
+}
+
+// ---- one dense layer over a tile of R rows held in shared memory -----------------------------------------
+// 256 threads; thread (rg, cg) owns TM consecutive rows x 4 consecutive output columns.  X: [R][ldx] fp32 in
+// shared memory (ldx % 4 == 0), Wt: [K][N] in global memory (L1-resident).  epi(row_in_tile, col, acc[4]).
+template <int N, int R, typename Epi>
+__device__ __forceinline__ void dense_tile(const float* __restrict__ X, int ldx, int K,
+                                           const float* __restrict__ Wt, Epi epi) {
+  constexpr int CG = N / 4, RG = kMlpThreads / CG, TM = R / RG;
+  static_assert(TM >= 1 && RG * TM == R, "tile shape");
+  const int cg = threadIdx.x % CG, rg = threadIdx.x / CG;
+  float acc[TM][4];
+#pragma unroll
+  for (int i = 0; i < TM; ++i) acc[i][0] = acc[i][1] = acc[i][2] = acc[i][3] = 0.0f;
+  const float* xr = X + (size_t)(rg * TM) * ldx;
+  const float4* w4 = reinterpret_cast<const float4*>(Wt) + cg;
+  int k = 0;
+  for (; k + 4 <= K; k += 4) {
+    const float4 w0 = __ldg(w4 + (size_t)(k + 0) * CG), w1 = __ldg(w4 + (size_t)(k + 1) * CG),
+                 w2 = __ldg(w4 + (size_t)(k + 2) * CG), w3 = __ldg(w4 + (size_t)(k + 3) * CG);
+#pragma unroll
+    for (int i = 0; i < TM; ++i) {
+      const float4 x = *reinterpret_cast<const float4*>(xr + i * ldx + k);
+      acc[i][0] = __fmaf_rn(x.x, w0.x, acc[i][0]); acc[i][1] = __fmaf_rn(x.x, w0.y, acc[i][1]);
+      acc[i][2] = __fmaf_rn(x.x, w0.z, acc[i][2]); acc[i][3] = __fmaf_rn(x.x, w0.w, acc[i][3]);
+      acc[i][0] = __fmaf_rn(x.y, w1.x, acc[i][0]); acc[i][1] = __fmaf_rn(x.y, w1.y, acc[i][1]);
+      acc[i][2] = __fmaf_rn(x.y, w1.z, acc[i][2]); acc[i][3] = __fmaf_rn(x.y, w1.w, acc[i][3]);
+      acc[i][0] = __fmaf_rn(x.z, w2.x, acc[i][0]); acc[i][1] = __fmaf_rn(x.z, w2.y, acc[i][1]);
+      acc[i][2] = __fmaf_rn(x.z, w2.z, acc[i][2]); acc[i][3] = __fmaf_rn(x.z, w2.w, acc[i][3]);
+      acc[i][0] = __fmaf_rn(x.w, w3.x, acc[i][0]); acc[i][1] = __fmaf_rn(x.w, w3.y, acc[i][1]);
+      acc[i][2] = __fmaf_rn(x.w, w3.z, acc[i][2]); acc[i][3] = __fmaf_rn(x.w, w3.w, acc[i][3]);
+    }
+  }
+  for (; k < K; ++k) {
+    const float4 w0 = __ldg(w4 + (size_t)k * CG);
+#pragma unroll
+    for (int i = 0; i < TM; ++i) {
+      const float x = xr[i * ldx + k];
+      acc[i][0] = __fmaf_rn(x, w0.x, acc[i][0]); acc[i][1] = __fmaf_rn(x, w0.y, acc[i][1]);
+      acc[i][2] = __fmaf_rn(x, w0.z, acc[i][2]); acc[i][3] = __fmaf_rn(x, w0.w, acc[i][3]);
+    }
+  }
+#pragma unroll
+  for (int i = 0; i < TM; ++i) epi(rg * TM + i, cg * 4, acc[i]);
+}
+
+// K = 3 input layer (never a tensor layer): out[r][c] = relu(fmaf chain + b), converted for the next layer.
+template <int MODE, int R>
+__device__ __forceinline__ void input_layer3(const float* __restrict__ F /*[R][4] smem*/, const LayerP& L,
+                                             float inv_sx_next, float* __restrict__ Y, int ldy) {
+  const int N = L.N;
+  for (int idx = threadIdx.x; idx < R * N; idx += kMlpThreads) {
+    const int r = idx / N, c = idx % N;
+    float acc = 0.0f;
+    acc = __fmaf_rn(F[r * 4 + 0], __ldg(L.Wt + c), acc);
+    acc = __fmaf_rn(F[r * 4 + 1], __ldg(L.Wt + N + c), acc);
+    acc = __fmaf_rn(F[r * 4 + 2], __ldg(L.Wt + 2 * N + c), acc);
+    float y = __fadd_rn(acc, __ldg(L.bias + c));
+    y = y > 0.0f ? y : 0.0f;
+    Y[r * ldy + c] = to_operand<MODE>(y, inv_sx_next);
+  }
+}
+
+// ============================================================================================================
+// S1: hit-embedding MLP (sec. 5.1; R2, R3): 3 -> D -> ... -> D -> 4, ReLU on hidden layers only.
+template <int MODE, int D>
+__global__ void __launch_bounds__(kMlpThreads) embed_simt_kernel(EmbArgs a) {
+  constexpr int R = kTileRows, LD = D + 4;
+  extern __shared__ __align__(16) float smem[];
+  float* A = smem;                 // [R][LD]
+  float* B = smem + R * LD;        // [R][LD]
+  float* F = B + R * LD;           // [R][4]
+  const int H = a.n_layers - 1;
+  for (int tile = blockIdx.x; tile * R < a.n_rows; tile += gridDim.x) {
+    const int row0 = tile * R;
+    __syncthreads();
+    if (threadIdx.x < R) {
+      const int row = row0 + threadIdx.x;
+      float4 f = row < a.n_rows ? a.feat[row] : make_float4(0.f, 0.f, 0.f, 0.f);
+      *reinterpret_cast<float4*>(F + threadIdx.x * 4) = f;
+    }
+    __syncthreads();
+    input_layer3<MODE, R>(F, a.layers[0], a.layers[1].inv_sx, A, LD);
+    __syncthreads();
+    float* cur = A; float* nxt = B;
+    for (int l = 1; l < H; ++l) {
+      const LayerP L = a.layers[l];
+      const float inv_next = a.layers[l + 1].inv_sx;
+      int32_t* tap = (a.tap && a.tap_layer == L.index) ? a.tap : nullptr;
+      dense_tile<D, R>(cur, LD, L.K, L.Wt, [&](int r, int c, const float* acc) {
+        float4 sc = __ldg(reinterpret_cast<const float4*>(L.scale + c)), bi = __ldg(reinterpret_cast<const float4*>(L.bias + c));
+        float y[4] = {__fmaf_rn(acc[0], sc.x, bi.x), __fmaf_rn(acc[1], sc.y, bi.y), __fmaf_rn(acc[2], sc.z, bi.z), __fmaf_rn(acc[3], sc.w, bi.w)};
+#pragma unroll
+        for (int j = 0; j < 4; ++j) { y[j] = y[j] > 0.0f ? y[j] : 0.0f; y[j] = to_operand<MODE>(y[j], inv_next); }
+        *reinterpret_cast<float4*>(nxt + r * LD + c) = make_float4(y[0], y[1], y[2], y[3]);
+        if (tap && row0 + r < a.n_rows)
+          for (int j = 0; j < 4; ++j) tap[(size_t)(row0 + r) * D + c + j] = (int32_t)acc[j];
+      });
+      __syncthreads();
+      float* t = cur; cur = nxt; nxt = t;
+    }
+    // output layer D -> 4, linear, fp32 result (R20: the embedding output is not rounded)
+    {
+      const LayerP L = a.layers[H];
+      const int r = threadIdx.x / 4, c = threadIdx.x % 4;       // R * 4 == 256 threads
+      float acc = 0.0f;
+      const float* x = cur + r * LD;
+      for (int j = 0; j < L.K; ++j) acc = __fmaf_rn(x[j], __ldg(L.Wt + j * 4 + c), acc);
+      const float y = __fmaf_rn(acc, __ldg(L.scale + c), __ldg(L.bias + c));
+      if (row0 + r < a.n_rows) {
+        reinterpret_cast<float*>(a.emb)[(size_t)(row0 + r) * 4 + c] = y;
+        if (a.tap && a.tap_layer == L.index) a.tap[(size_t)(row0 + r) * 4 + c] = (int32_t)acc;
+      }
+    }
+  }
+}
+
+// ============================================================================================================
+// S4a/b/d/e (+ S4f): the four two-layer MLPs of the interaction network (sec. 5.2).
+//   node encoder  h0 = MLP(f)                                   (L133)
+//   edge encoder  e0 = MLP(|f_dst - f_src|)  or MLP([h0_s,h0_d]) (R10, R11)
+//   node network  h <- h + MLP([h, m_out, m_in])                (L140, R12, R14)
+//   edge network  e <- e + MLP([h_src, h_dst, e]), updated h    (L140, R13); optional head z = w.e + b (R16)
+template <int KIND, int MODE, typename ST, int D>
+__global__ void __launch_bounds__(kMlpThreads) gnn_mlp_simt_kernel(GnnArgs a) {
+  constexpr int R = kTileRows;
+  constexpr int K0MAX = 3 * D, LDX = K0MAX + 4, LDY = D + 4;
+  extern __shared__ __align__(16) float smem[];
+  float* X = smem;                       // [R][LDX]
+  float* Y = X + R * LDX;                // [R][LDY]
+  int* IDX = reinterpret_cast<int*>(Y + R * LDY);   // [2][R] src, dst
+  const int n_rows = a.n_rows_ptr ? *a.n_rows_ptr : a.n_rows;
+  const bool is_edge = (KIND == kEdgeEnc || KIND == kEdgeNet);
+  const LayerP L0 = a.l0, L1 = a.l1;
+  const bool quant_in = (MODE == kModeInt8) && L0.tensor;
+
+  for (int tile = blockIdx.x; (size_t)tile * R < (size_t)n_rows; tile += gridDim.x) {
+    const int row0 = tile * R;
+    __syncthreads();
+    if (is_edge && threadIdx.x < 2 * R) {
+      const int r = threadIdx.x % R, which = threadIdx.x / R;
+      const int row = row0 + r;
+      IDX[which * R + r] = row < n_rows ? (which ? a.dst[row] : a.src[row]) : 0;
+    }
+    __syncthreads();
+    // ---- assemble the layer-0 input ------------------------------------------------------------------------
+    if (KIND == kNodeEnc || (KIND == kEdgeEnc && a.edge_enc_input == 0)) {
+      if (threadIdx.x < R) {
+        const int r = threadIdx.x, row = row0 + r;
+        float4 f = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (row < n_rows) {
+          if (KIND == kNodeEnc) f = a.feat[row];
+          else {
+            const float4 fs = a.feat[IDX[r]], fd = a.feat[IDX[R + r]];
+            f = make_float4(fabsf(__fsub_rn(fd.x, fs.x)), fabsf(__fsub_rn(fd.y, fs.y)), fabsf(__fsub_rn(fd.z, fs.z)), 0.f);
+          }
+        }
+        *reinterpret_cast<float4*>(Y + r * 4) = f;       // Y doubles as the [R][4] feature buffer
+      }
+      __syncthreads();
+      // layer 0 (K = 3) writes its output (the layer-1 operand) into X, then Y is free again
+      input_layer3<MODE, R>(Y, L0, L1.inv_sx, X, LDX);
+      __syncthreads();
+    } else {
+      const int K0 = L0.K;                               // 2D (paper's edge encoder) or 3D
+      const int c4n = K0 / 4, seg4 = D / 4;
+      for (int idx = threadIdx.x; idx < R * c4n; idx += kMlpThreads) {
+        const int r = idx / c4n, c4 = idx % c4n, seg = c4 / seg4, within = (c4 % seg4) * 4;
+        const int row = row0 + r;
+        float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (row < n_rows) {
+          if (KIND == kNodeNet) {
+            v = seg == 0 ? State<ST>::ld4(a.h, (size_t)row * D + within)
+                         : State<ST>::ld4(a.m, (size_t)row * 2 * D + (size_t)(seg - 1) * D + within);
+          } else {
+            if (seg == 0) v = State<ST>::ld4(a.h, (size_t)IDX[r] * D + within);
+            else if (seg == 1) v = State<ST>::ld4(a.h, (size_t)IDX[R + r] * D + within);
+            else v = State<ST>::ld4(a.e, (size_t)row * D + within);
+          }
+        }
+        if (quant_in) { v.x = quant_i8(v.x, L0.inv_sx); v.y = quant_i8(v.y, L0.inv_sx); v.z = quant_i8(v.z, L0.inv_sx); v.w = quant_i8(v.w, L0.inv_sx); }
+        *reinterpret_cast<float4*>(X + r * LDX + c4 * 4) = v;
+      }
+      __syncthreads();
+      // layer 0: K0 -> D, ReLU, operand conversion for layer 1
+      int32_t* tap0 = (a.tap && a.tap_layer == L0.index) ? a.tap : nullptr;
+      dense_tile<D, R>(X, LDX, K0, L0.Wt, [&](int r, int c, const float* acc) {
+        float4 sc = __ldg(reinterpret_cast<const float4*>(L0.scale + c)), bi = __ldg(reinterpret_cast<const float4*>(L0.bias + c));
+        float y[4] = {__fmaf_rn(acc[0], sc.x, bi.x), __fmaf_rn(acc[1], sc.y, bi.y), __fmaf_rn(acc[2], sc.z, bi.z), __fmaf_rn(acc[3], sc.w, bi.w)};
+#pragma unroll
+        for (int j = 0; j < 4; ++j) { y[j] = y[j] > 0.0f ? y[j] : 0.0f; y[j] = to_operand<MODE>(y[j], L1.inv_sx); }
+        *reinterpret_cast<float4*>(Y + r * LDY + c) = make_float4(y[0], y[1], y[2], y[3]);
+        if (tap0 && row0 + r < n_rows)
+          for (int j = 0; j < 4; ++j) tap0[(size_t)(row0 + r) * D + c + j] = (int32_t)acc[j];
+      });
+      __syncthreads();
+    }
+    const bool hidden_in_x = (KIND == kNodeEnc || (KIND == kEdgeEnc && a.edge_enc_input == 0));
+    const float* HID = hidden_in_x ? X : Y;
+    const int ldh = hidden_in_x ? LDX : LDY;
+    float* OUT = hidden_in_x ? Y : X;           // staging of the new state rows for the fused head
+    const int ldo = hidden_in_x ? LDY : LDX;
+    // ---- layer 1: D -> D, linear; residual for the networks; store the state --------------------------------
+    int32_t* tap1 = (a.tap && a.tap_layer == L1.index) ? a.tap : nullptr;
+    void* state = is_edge ? a.e : a.h;
+    dense_tile<D, R>(HID, ldh, D, L1.Wt, [&](int r, int c, const float* acc) {
+      const int row = row0 + r;
+      float4 sc = __ldg(reinterpret_cast<const float4*>(L1.scale + c)), bi = __ldg(reinterpret_cast<const float4*>(L1.bias + c));
+      float4 y = make_float4(__fmaf_rn(acc[0], sc.x, bi.x), __fmaf_rn(acc[1], sc.y, bi.y), __fmaf_rn(acc[2], sc.z, bi.z), __fmaf_rn(acc[3], sc.w, bi.w));
+      if (row < n_rows) {
+        if (KIND == kNodeNet || KIND == kEdgeNet) {
+          const float4 old = State<ST>::ld4(state, (size_t)row * D + c);
+          y = make_float4(__fadd_rn(old.x, y.x), __fadd_rn(old.y, y.y), __fadd_rn(old.z, y.z), __fadd_rn(old.w, y.w));
+        }
+        y = make_float4(State<ST>::round(y.x), State<ST>::round(y.y), State<ST>::round(y.z), State<ST>::round(y.w));
+        State<ST>::st4(state, (size_t)row * D + c, y);
+        if (tap1) for (int j = 0; j < 4; ++j) tap1[(size_t)row * D + c + j] = (int32_t)acc[j];
+      }
+      if (is_edge && a.do_head) *reinterpret_cast<float4*>(OUT + r * ldo + c) = y;
+    });
+    // ---- S4f: edge classifier on the final edge state (L80, L142; R16): z = w.e + b, score = sigmoid(z) -----
+    if (is_edge && a.do_head) {
+      __syncthreads();
+      if (threadIdx.x < R && row0 + threadIdx.x < n_rows) {
+        const float* x = OUT + threadIdx.x * ldo;
+        float acc = 0.0f;
+        for (int j = 0; j < D; ++j) acc = __fmaf_rn(x[j], __ldg(a.head.Wt + j), acc);
+        const float z = __fadd_rn(acc, __ldg(a.head.bias));
+        a.logit[row0 + threadIdx.x] = z;
+        a.score[row0 + threadIdx.x] = 1.0f / (1.0f + expf(-z));
+      }
+    }
+  }
+}
+
+// ============================================================================================================
+// S4c: message building, Eq.(4): m_l = [ sum_{l->j} e_lj , sum_{i->l} e_il ].
+// The paper needed a scatter_add TensorRT plugin (global atomics, L253).  Here nothing is scattered: the
+// out-edges of a node are a contiguous run of e (edges are src-sorted) and its in-edges are listed by the
+// CSC, so each node's sums are sequential fp32 adds in ascending edge id (R22) -- deterministic, no atomics.
+// One group of D/4 lanes per node, 4 columns per lane.
+template <typename ST, int D>
+__global__ void __launch_bounds__(256) scatter_kernel(const void* __restrict__ e, const int32_t* __restrict__ row_ptr,
+                                                      const int32_t* __restrict__ col_ptr, const int32_t* __restrict__ in_edge,
+                                                      void* __restrict__ m, int n_hits) {
+  constexpr int LPN = D / 4;                              // lanes per node
+  const int gid = blockIdx.x * (256 / LPN) + threadIdx.x / LPN;
+  const int c = (threadIdx.x % LPN) * 4;
+  if (gid >= n_hits) return;
+  float4 so = make_float4(0.f, 0.f, 0.f, 0.f), si = so;
+  const int a0 = row_ptr[gid], a1 = row_ptr[gid + 1];
+  for (int i = a0; i < a1; ++i) {
+    const float4 v = State<ST>::ld4(e, (size_t)i * D + c);
+    so.x = __fadd_rn(so.x, v.x); so.y = __fadd_rn(so.y, v.y); so.z = __fadd_rn(so.z, v.z); so.w = __fadd_rn(so.w, v.w);
+  }
+  const int b0 = col_ptr[gid], b1 = col_ptr[gid + 1];
+  for (int i = b0; i < b1; ++i) {
+    const float4 v = State<ST>::ld4(e, (size_t)in_edge[i] * D + c);
+    si.x = __fadd_rn(si.x, v.x); si.y = __fadd_rn(si.y, v.y); si.z = __fadd_rn(si.z, v.z); si.w = __fadd_rn(si.w, v.w);
+  }
+  so = make_float4(State<ST>::round(so.x), State<ST>::round(so.y), State<ST>::round(so.z), State<ST>::round(so.w));
+  si = make_float4(State<ST>::round(si.x), State<ST>::round(si.y), State<ST>::round(si.z), State<ST>::round(si.w));
+  State<ST>::st4(m, (size_t)gid * 2 * D + c, so);
+  State<ST>::st4(m, (size_t)gid * 2 * D + D + c, si);
+}
+
+// ------------------------------------------------------------------------------------------------------------
+template <int D> static size_t gnn_smem() { return sizeof(float) * kTileRows * ((3 * D + 4) + (D + 4)) + sizeof(int) * 2 * kTileRows; }
+template <int D> static size_t emb_smem() { return sizeof(float) * kTileRows * (2 * (D + 4) + 4); }
+
+template <int KIND, int MODE, typename ST, int D>
+static void gnn_launch_one(etx_ctx* c, const GnnArgs& a, int max_rows, cudaStream_t s) {
+  auto kern = gnn_mlp_simt_kernel<KIND, MODE, ST, D>;
+  static bool configured = false;
+  if (!configured) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gnn_smem<D>()); configured = true; }
+  const int tiles = (max_rows + kTileRows - 1) / kTileRows;
+  const int grid = tiles < c->sm_count * 3 ? tiles : c->sm_count * 3;
+  if (grid <= 0) return;
+  kern<<<grid, kMlpThreads, gnn_smem<D>(), s>>>(a);
+  c->launches++;
+}
+
+template <int MODE, typename ST, int D>
+static void gnn_launch_kind(etx_ctx* c, int kind, const GnnArgs& a, int max_rows, cudaStream_t s) {
+  switch (kind) {
+    case kNodeEnc: gnn_launch_one<kNodeEnc, MODE, ST, D>(c, a, max_rows, s); break;
+    case kEdgeEnc: gnn_launch_one<kEdgeEnc, MODE, ST, D>(c, a, max_rows, s); break;
+    case kNodeNet: gnn_launch_one<kNodeNet, MODE, ST, D>(c, a, max_rows, s); break;
+    default:       gnn_launch_one<kEdgeNet, MODE, ST, D>(c, a, max_rows, s); break;
+  }
+}
+
+template <int D>
+static void gnn_launch_d(etx_ctx* c, int kind, const GnnArgs& a, int max_rows, cudaStream_t s) {
+  if (c->precision == ETX_FP32) gnn_launch_kind<kModeF32, float, D>(c, kind, a, max_rows, s);
+  else if (c->precision == ETX_BF16) gnn_launch_kind<kModeBf16, __nv_bfloat16, D>(c, kind, a, max_rows, s);
+  else gnn_launch_kind<kModeInt8, float, D>(c, kind, a, max_rows, s);
+}
+
+void fill_gnn_args(etx_ctx* c, int kind, int iter, int n_hits, bool do_head, GnnArgs& a) {
+  const bool is_edge = (kind == kEdgeEnc || kind == kEdgeNet);
+  int i0;
+  if (kind == kNodeEnc) i0 = c->i_nenc;
+  else if (kind == kEdgeEnc) i0 = c->i_eenc;
+  else if (kind == kNodeNet) i0 = c->i_iter0 + 4 * iter;
+  else i0 = c->i_iter0 + 4 * iter + 2;
+  a.l0 = c->layers[i0].dev; a.l1 = c->layers[i0 + 1].dev; a.head = c->layers[c->i_head].dev;
+  a.feat = c->feat; a.src = c->src; a.dst = c->dst;
+  a.n_rows_ptr = is_edge ? c->n_edges : nullptr;
+  a.n_rows = n_hits;
+  a.h = c->h; a.e = c->e; a.m = c->m; a.logit = c->logit; a.score = c->score;
+  a.do_head = do_head ? 1 : 0;
+  a.edge_enc_input = c->hp.edge_enc_input;
+  a.tap = c->tap_layer >= 0 ? c->tap : nullptr;
+  a.tap_layer = c->tap_layer;
+}
+
+void launch_gnn_mlp_simt(etx_ctx* c, int kind, int iter, int n_hits, bool do_head, cudaStream_t s) {
+  GnnArgs a;
+  fill_gnn_args(c, kind, iter, n_hits, do_head, a);
+  const bool is_edge = (kind == kEdgeEnc || kind == kEdgeNet);
+  // edge kernels: E is only known on the device; size the grid for the capacity k * n_hits
+  const long long max_rows_ll = is_edge ? (long long)n_hits * c->hp.k : n_hits;
+  const int max_rows = (int)(max_rows_ll > 0x7fffffff ? 0x7fffffff : max_rows_ll);
+  if (c->hp.gnn_latent == 32) gnn_launch_d<32>(c, kind, a, max_rows, s);
+  else gnn_launch_d<64>(c, kind, a, max_rows, s);
+}
+
+template <int MODE, int D>
+static void emb_launch(etx_ctx* c, const EmbArgs& a, cudaStream_t s) {
+  auto kern = embed_simt_kernel<MODE, D>;
+  static bool configured = false;
+  if (!configured) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)emb_smem<D>()); configured = true; }
+  const int tiles = (a.n_rows + kTileRows - 1) / kTileRows;
+  const int grid = tiles < c->sm_count * 3 ? tiles : c->sm_count * 3;
+  if (grid <= 0) return;
+  kern<<<grid, kMlpThreads, emb_smem<D>(), s>>>(a);
+  c->launches++;
+}
+
+void launch_embed_simt(etx_ctx* c, int n_hits, cudaStream_t s) {
+  EmbArgs a;
+  a.n_layers = c->hp.emb_n_hidden_layers + 1;
+  for (int l = 0; l < a.n_layers; ++l) a.layers[l] = c->layers[c->i_emb0 + l].dev;
+  a.feat = c->feat; a.emb = c->emb; a.n_rows = n_hits;
+  a.tap = c->tap_layer >= 0 ? c->tap : nullptr; a.tap_layer = c->tap_layer;
+  const int D = c->hp.emb_hidden;
+#define ETX_EMB(MODE)                                   \
+  if (D == 64) emb_launch<MODE, 64>(c, a, s);           \
+  else emb_launch<MODE, 128>(c, a, s);
+  if (c->precision == ETX_FP32) { ETX_EMB(kModeF32) }
+  else if (c->precision == ETX_BF16) { ETX_EMB(kModeBf16) }
+  else { ETX_EMB(kModeInt8) }
+#undef ETX_EMB
+}
+
+void launch_scatter(etx_ctx* c, int n_hits, cudaStream_t s) {
+  if (n_hits == 0) return;
+  const int d = c->hp.gnn_latent;
+  const int npb = 256 / (d / 4);
+  const int grid = (n_hits + npb - 1) / npb;
+  if (c->state_bf16) {
+    if (d == 32) scatter_kernel<__nv_bfloat16, 32><<<grid, 256, 0, s>>>(c->e, c->row_ptr, c->col_ptr, c->in_edge, c->m, n_hits);
+    else scatter_kernel<__nv_bfloat16, 64><<<grid, 256, 0, s>>>(c->e, c->row_ptr, c->col_ptr, c->in_edge, c->m, n_hits);
+  } else {
+    if (d == 32) scatter_kernel<float, 32><<<grid, 256, 0, s>>>(c->e, c->row_ptr, c->col_ptr, c->in_edge, c->m, n_hits);
+    else scatter_kernel<float, 64><<<grid, 256, 0, s>>>(c->e, c->row_ptr, c->col_ptr, c->in_edge, c->m, n_hits);
+  }
+  c->launches++;
+}
+
+void simt_configure(etx_ctx*) {}
+
+}  // namespace etx

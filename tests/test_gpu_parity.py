@@ -1,0 +1,282 @@
+"""GPU parity: the CUDA path (through the C-ABI, via the ctypes binding) against the CPU oracle on identical
+seeded inputs.  Protocol: DESIGN.md sec. 6 (stage-isolated, chained, end-to-end).  Bars (BASELINE.json
+north_star): k-NN edge list and track ids bit-exact; scores within 1e-4 (fp32) / 2e-2 (bf16) absolute;
+int32 accumulators of the INT8 path bit-exact."""
+import numpy as np
+import pytest
+import torch
+
+import datagen
+import oracle
+from gpu_utils import dev, make_ctx, run_gpu, state
+from helpers import centred_parity_weights, check_edge_invariants, check_track_invariants
+
+pytestmark = pytest.mark.gpu
+F = np.float32
+
+
+def _setup(name, n_events=None, preset="parity", precision=None, seed=None):
+    cfg = datagen.get_config(name)
+    if precision:
+        cfg = cfg.replace(precision=precision)
+    b = datagen.generate_batch(cfg, n_events=n_events, seed=seed)
+    W = centred_parity_weights(cfg, b) if preset == "parity" else datagen.make_weights(cfg, preset)
+    return cfg, b, W
+
+
+def _oracle_all(cfg, b, blob, precision):
+    o = oracle.Oracle(blob, precision)
+    r = o.run(b.xyz, b.plane, b.event_offsets, cfg.k, cfg.window, cfg.d2_max, cfg.threshold)
+    r["col_ptr"], r["in_edge"] = oracle.csc(r["dst"], b.n_hits)
+    return o, r
+
+
+# ---------------------------------------------------------------------------------- S0 + S2 + S3
+@pytest.mark.parametrize("name,n_events", [("cfg0", 1), ("cfg1", 5), ("cfg4", 2)])
+def test_knn_and_edge_list_bit_exact_on_oracle_embedding(name, n_events):
+    cfg, b, W = _setup(name, n_events, precision="fp32")
+    blob = datagen.pack_blob(cfg, W)
+    o, r = _oracle_all(cfg, b, blob, "fp32")
+    ctx = make_ctx(cfg, blob, b, precision="fp32")
+    g = run_gpu(ctx, b, emb=r["emb"], last_stage=3)
+    assert g["n_edges"] == r["src"].size
+    assert np.array_equal(g["src"], r["src"]) and np.array_equal(g["dst"], r["dst"])
+    assert np.array_equal(g["row_ptr"], r["row_ptr"])
+    assert np.array_equal(g["col_ptr"], r["col_ptr"]) and np.array_equal(g["in_edge"], r["in_edge"])
+    check_edge_invariants(g["src"], g["dst"], g["row_ptr"], b.plane, b.event_offsets, cfg.k, cfg.window)
+
+
+@pytest.mark.parametrize("k,w,d2max", [(4, 1, np.inf), (10, 2, np.inf), (16, 3, 2.0), (3, 25, np.inf), (33, 2, np.inf)])
+def test_knn_ties_duplicates_radius_and_ragged_events(k, w, d2max):
+    # integer-valued embeddings: many exact ties and duplicated points; events of ragged sizes incl. empty
+    rng = np.random.default_rng(100 + k)
+    sizes = [0, 37, 1, 0, 900, 130, 0]
+    planes, off = [], [0]
+    for n in sizes:
+        planes.append(np.sort(rng.integers(0, 26, n)).astype(np.int32)); off.append(off[-1] + n)
+    plane = np.concatenate(planes); off = np.asarray(off, np.int32)
+    emb = np.round(rng.normal(0, 1.5, (plane.size, 4))).astype(F)
+    cfg = datagen.get_config("cfg1").replace(k=k, window=w, d2_max=float(d2max), precision="fp32", gnn_iters=1)
+    blob = datagen.pack_blob(cfg, datagen.make_weights(cfg, "parity"))
+    b = datagen.EventBatch(np.zeros((plane.size, 3), F), plane, off, np.zeros(plane.size, np.int64))
+    nbr, deg = oracle.knn(emb, plane, off, k, w, d2max)
+    src, dst, row_ptr = oracle.build_edges(nbr, deg)
+    col_ptr, in_edge = oracle.csc(dst, plane.size)
+    ctx = make_ctx(cfg, blob, b)
+    g = run_gpu(ctx, b, emb=emb, last_stage=3)
+    assert np.array_equal(g["src"], src) and np.array_equal(g["dst"], dst)
+    assert np.array_equal(g["row_ptr"], row_ptr) and np.array_equal(g["col_ptr"], col_ptr)
+    assert np.array_equal(g["in_edge"], in_edge)
+
+
+def test_knn_candidate_window_larger_than_the_shared_memory_tile():
+    # one event, two planes, 3000 candidates per query: spans several 1024-candidate tiles + a ragged tail
+    rng = np.random.default_rng(7)
+    n0, n1 = 150, 3000
+    plane = np.concatenate([np.full(n0, 10), np.full(n1, 11)]).astype(np.int32)
+    off = np.array([0, n0 + n1], np.int32)
+    emb = rng.normal(0, 1, (n0 + n1, 4)).astype(F)
+    cfg = datagen.get_config("cfg4").replace(precision="fp32", gnn_iters=1)
+    blob = datagen.pack_blob(cfg, datagen.make_weights(cfg, "parity"))
+    b = datagen.EventBatch(np.zeros((plane.size, 3), F), plane, off, np.zeros(plane.size, np.int64))
+    nbr, deg = oracle.knn(emb, plane, off, cfg.k, cfg.window)
+    src, dst, _ = oracle.build_edges(nbr, deg)
+    g = run_gpu(make_ctx(cfg, blob, b), b, emb=emb, last_stage=3)
+    assert np.array_equal(g["src"], src) and np.array_equal(g["dst"], dst)
+
+
+# ---------------------------------------------------------------------------------- S1
+@pytest.mark.parametrize("name,precision", [("cfg0", "fp32"), ("cfg1", "fp32"), ("cfg1", "bf16"), ("cfg1", "int8")])
+def test_embedding_simt_engine_bit_exact(name, precision):
+    cfg, b, W = _setup(name, 3 if name != "cfg0" else 1, precision=precision)
+    scales = None
+    if precision == "int8":
+        scales = oracle.calibrate_int8(datagen.pack_blob(cfg, W), b.xyz, b.plane, b.event_offsets, cfg.k, cfg.window)
+    blob = datagen.pack_blob(cfg, W, scales)
+    want = oracle.Oracle(blob, precision).embed(b.xyz)
+    ctx = make_ctx(cfg, blob, b, engine="simt")
+    g = run_gpu(ctx, b, last_stage=1)
+    assert np.array_equal(g["emb"], want)
+
+
+# ---------------------------------------------------------------------------------- S4
+@pytest.mark.parametrize("name,n_events,eei", [("cfg0", 1, 0), ("cfg1", 3, 0), ("cfg0", 1, 1)])
+def test_gnn_fp32_on_oracle_edges(name, n_events, eei):
+    cfg, b, W = _setup(name, n_events, precision="fp32")
+    if eei:
+        cfg = cfg.replace(edge_enc_input=1)
+        W = datagen.make_weights(cfg, "parity")
+    blob = datagen.pack_blob(cfg, W)
+    o, r = _oracle_all(cfg, b, blob, "fp32")
+    og = o.gnn(b.xyz, r["src"], r["dst"], want_states=True, m_iter=cfg.gnn_iters - 1)
+    ctx = make_ctx(cfg, blob, b)
+    g = run_gpu(ctx, b, emb=r["emb"], src=r["src"], dst=r["dst"], last_stage=5)
+    d = cfg.gnn_latent
+    assert np.array_equal(state(ctx, "m", b.n_hits, 2 * d), og["m"])          # ascending-edge-id sums (R22)
+    assert np.array_equal(state(ctx, "h", b.n_hits, d), og["h"])
+    assert np.array_equal(state(ctx, "e", r["src"].size, d), og["e"])
+    assert np.array_equal(g["logit"], og["logit"])                            # pinned order => bit-exact
+    assert np.abs(g["score"] - og["score"]).max() <= 1e-4                     # north_star fp32 bar
+    assert np.array_equal(g["track_id"], r["track_id"])
+    mid = np.mean((og["score"] > 0.01) & (og["score"] < 0.99))
+    assert mid > 0.5, "scores must be informative for this comparison to mean anything"
+
+
+@pytest.mark.parametrize("precision", ["bf16", "int8"])
+def test_gnn_simt_engine_reproduces_the_oracles_rounding_points(precision):
+    cfg, b, W = _setup("cfg1", 2, precision=precision)
+    scales = None
+    if precision == "int8":
+        scales = oracle.calibrate_int8(datagen.pack_blob(cfg, W), b.xyz, b.plane, b.event_offsets, cfg.k, cfg.window)
+    blob = datagen.pack_blob(cfg, W, scales)
+    o, r = _oracle_all(cfg, b, blob, precision)
+    og = o.gnn(b.xyz, r["src"], r["dst"], want_states=True)
+    ctx = make_ctx(cfg, blob, b, engine="simt")
+    g = run_gpu(ctx, b, emb=r["emb"], src=r["src"], dst=r["dst"])
+    assert np.array_equal(state(ctx, "e", r["src"].size, cfg.gnn_latent), og["e"])
+    assert np.array_equal(g["logit"], og["logit"])
+    assert np.abs(g["score"] - og["score"]).max() <= (2e-2 if precision == "bf16" else 1e-4)
+
+
+def test_int8_accumulators_bit_exact_simt_engine():
+    cfg, b, W = _setup("cfg1", 2, precision="int8")
+    scales = oracle.calibrate_int8(datagen.pack_blob(cfg, W), b.xyz, b.plane, b.event_offsets, cfg.k, cfg.window)
+    blob = datagen.pack_blob(cfg, W, scales)
+    o, r = _oracle_all(cfg, b, blob, "int8")
+    names = [n for n, _, _ in datagen.layer_shapes(cfg)]
+    ctx = make_ctx(cfg, blob, b, engine="simt")
+    for lname, rows in (("emb2", b.n_hits), ("node3_0", b.n_hits), ("edge5_0", r["src"].size), ("edge0_1", r["src"].size)):
+        li = names.index(lname)
+        width = datagen.layer_shapes(cfg)[li][1]
+        tap = np.zeros((rows, width), np.int32)
+        o.set_tap(li, tap)
+        o.embed(b.xyz); o.gnn(b.xyz, r["src"], r["dst"])
+        o.set_tap(-1, None)
+        ctx.tap_layer(li)
+        run_gpu(ctx, b, emb=r["emb"] if not lname.startswith("emb") else None, src=r["src"], dst=r["dst"])
+        got = ctx.buffer("tap", torch.int32).cpu().numpy()[: rows * width].reshape(rows, width)
+        ctx.tap_layer(-1)
+        assert np.array_equal(got, tap), lname
+        assert np.abs(tap).max() > 100
+
+
+# ---------------------------------------------------------------------------------- S5
+def test_components_bit_exact_on_oracle_logits():
+    cfg, b, W = _setup("cfg1", 6, precision="fp32")
+    blob = datagen.pack_blob(cfg, W)
+    o, r = _oracle_all(cfg, b, blob, "fp32")
+    ctx = make_ctx(cfg, blob, b)
+    rng = np.random.default_rng(3)
+    for trial, logit in enumerate([r["logit"], rng.normal(0, 1, r["src"].size).astype(F),
+                                   rng.normal(2.5, 1, r["src"].size).astype(F), np.full(r["src"].size, -1, F),
+                                   np.zeros(r["src"].size, F)]):
+        want = oracle.components(r["src"], r["dst"], logit, oracle.logit_threshold(cfg.threshold), b.n_hits)
+        g = run_gpu(ctx, b, emb=r["emb"], src=r["src"], dst=r["dst"], logit=logit)
+        assert np.array_equal(g["track_id"], want), trial
+        check_track_invariants(g["track_id"], r["src"], r["dst"], logit >= 0, b.event_offsets)
+
+
+# ---------------------------------------------------------------------------------- end to end
+@pytest.mark.parametrize("name,n_events,preset", [("cfg0", 1, "parity"), ("cfg0", 1, "he"), ("cfg1", 6, "parity"),
+                                                   ("cfg1", 3, "he")])
+def test_end_to_end_fp32_bit_exact_edges_and_track_ids(name, n_events, preset):
+    cfg, b, W = _setup(name, n_events, preset=preset, precision="fp32")
+    blob = datagen.pack_blob(cfg, W)
+    o, r = _oracle_all(cfg, b, blob, "fp32")
+    ctx = make_ctx(cfg, blob, b)
+    g = run_gpu(ctx, b, debug=False)                     # the plain etx_run call
+    assert np.array_equal(g["emb"], r["emb"])
+    assert np.array_equal(g["src"], r["src"]) and np.array_equal(g["dst"], r["dst"])
+    assert np.abs(g["score"] - r["score"]).max() <= 1e-4
+    assert np.array_equal(g["track_id"], r["track_id"])
+    assert np.unique(g["track_id"]).size == np.unique(r["track_id"]).size
+
+
+def test_repeated_runs_on_one_handle_are_identical_and_smaller_batches_work():
+    cfg, b, W = _setup("cfg1", 4, precision="fp32")
+    blob = datagen.pack_blob(cfg, W)
+    ctx = make_ctx(cfg, blob, b)
+    g1 = run_gpu(ctx, b, debug=False)
+    b2 = b.slice_events(1, 3)
+    g2 = run_gpu(ctx, b2, debug=False)
+    r2 = oracle.Oracle(blob, "fp32").run(b2.xyz, b2.plane, b2.event_offsets, cfg.k, cfg.window)
+    assert np.array_equal(g2["src"], r2["src"]) and np.array_equal(g2["track_id"], r2["track_id"])
+    g3 = run_gpu(ctx, b, debug=False)
+    for key in ("src", "dst", "logit", "track_id"):
+        assert np.array_equal(g1[key], g3[key])
+
+
+# ---------------------------------------------------------------------------------- edge cases + errors
+def test_empty_batches_and_empty_events():
+    cfg = datagen.get_config("cfg0")
+    W = datagen.make_weights(cfg, "parity")
+    blob = datagen.pack_blob(cfg, W)
+    empty = datagen.EventBatch(np.zeros((0, 3), F), np.zeros(0, np.int32), np.zeros(1, np.int32), np.zeros(0, np.int64))
+    ctx = make_ctx(cfg, blob, empty, max_events=8, max_hits=4096)
+    g = run_gpu(ctx, empty, debug=False)                                   # n_events = 0
+    assert g["n_edges"] == 0 and g["track_id"].size == 0
+    empty3 = datagen.EventBatch(np.zeros((0, 3), F), np.zeros(0, np.int32), np.zeros(4, np.int32), np.zeros(0, np.int64))
+    g = run_gpu(ctx, empty3, debug=False)                                  # three empty events
+    assert g["n_edges"] == 0
+    b = datagen.generate_batch(cfg, n_events=2)
+    o = b.event_offsets
+    off = np.array([0, 0, o[1], o[1], o[1], o[2], o[2]], np.int32)         # empty first / middle / last events
+    bb = datagen.EventBatch(b.xyz, b.plane, off, b.particle)
+    r = oracle.Oracle(blob, "fp32").run(bb.xyz, bb.plane, bb.event_offsets, cfg.k, cfg.window)
+    g = run_gpu(ctx, bb, debug=False)
+    assert np.array_equal(g["src"], r["src"]) and np.array_equal(g["track_id"], r["track_id"])
+    # a hit on plane 25 only, and a single-hit event
+    hb = datagen.hand_batch([[(10.0, 0.0, 25)], [(7.0, 7.0, 3)], [(10.0, 1.0, 3), (10.1, 1.0, 4), (10.2, 1.1, 5)]])
+    r = oracle.Oracle(blob, "fp32").run(hb.xyz, hb.plane, hb.event_offsets, cfg.k, cfg.window)
+    g = run_gpu(ctx, hb, debug=False)
+    assert np.array_equal(g["src"], r["src"]) and np.array_equal(g["dst"], r["dst"])
+    assert np.array_equal(g["track_id"], r["track_id"]) and g["n_edges"] == 2
+
+
+def test_error_codes_capacity_blob_order_unsupported():
+    import paper_2407_12119_b200 as etx
+    cfg = datagen.get_config("cfg0")
+    W = datagen.make_weights(cfg, "parity")
+    blob = datagen.pack_blob(cfg, W)
+    b = datagen.generate_batch(cfg, n_events=2)
+    with pytest.raises(etx.EtxError) as ei:
+        make_ctx(cfg, blob[:-4], b)
+    assert ei.value.status == -2
+    with pytest.raises(etx.EtxError) as ei:
+        make_ctx(cfg, b"\0" * len(blob), b)
+    assert ei.value.status == -2
+    with pytest.raises(etx.EtxError) as ei:
+        make_ctx(cfg.replace(gnn_latent=48), datagen.pack_blob(cfg.replace(gnn_latent=48), datagen.make_weights(cfg.replace(gnn_latent=48))), b)
+    assert ei.value.status == -6
+    ctx = make_ctx(cfg, blob, b, max_events=1, max_hits=b.n_hits, validate=True)
+    with pytest.raises(etx.EtxError) as ei:
+        run_gpu(ctx, b, debug=False)
+    assert ei.value.status == -3
+    ctx = make_ctx(cfg, blob, b, max_events=4, max_hits=10)
+    with pytest.raises(etx.EtxError) as ei:
+        run_gpu(ctx, b, debug=False)
+    assert ei.value.status == -3
+    # unsorted planes are detected on the device and reported by the next call
+    ctx = make_ctx(cfg, blob, b, validate=True)
+    bad = datagen.EventBatch(b.xyz, b.plane[::-1].copy(), b.event_offsets, b.particle)
+    run_gpu(ctx, bad, debug=False, ) if False else ctx.results(ctx.run(dev(bad.xyz), dev(bad.plane), bad.event_offsets))
+    with pytest.raises(etx.EtxError) as ei:
+        ctx.run(dev(b.xyz), dev(b.plane), b.event_offsets)
+    assert ei.value.status == -4
+    g = run_gpu(ctx, b, debug=False)                                       # the handle stays usable
+    assert g["n_edges"] > 0
+
+
+def test_run_host_matches_device_run():
+    cfg, b, W = _setup("cfg1", 3, precision="fp32")
+    blob = datagen.pack_blob(cfg, W)
+    ctx = make_ctx(cfg, blob, b)
+    g = run_gpu(ctx, b, debug=False)
+    cap = cfg.k * b.n_hits
+    h_xyz = torch.from_numpy(b.xyz).pin_memory(); h_plane = torch.from_numpy(b.plane).pin_memory()
+    sc = torch.empty(cap, dtype=torch.float32).pin_memory(); s_ = torch.empty(cap, dtype=torch.int32).pin_memory()
+    d_ = torch.empty(cap, dtype=torch.int32).pin_memory(); tid = torch.empty(b.n_hits, dtype=torch.int32).pin_memory()
+    E = ctx.run_host(h_xyz, h_plane, b.event_offsets, sc, s_, d_, tid)
+    assert E == g["n_edges"]
+    assert np.array_equal(s_.numpy()[:E], g["src"]) and np.array_equal(d_.numpy()[:E], g["dst"])
+    assert np.array_equal(sc.numpy()[:E], g["score"]) and np.array_equal(tid.numpy(), g["track_id"])
