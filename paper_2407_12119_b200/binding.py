@@ -231,14 +231,14 @@ class Etx:
 
     @staticmethod
     def _copy_out(ptr, nbytes: int, dtype, shape=None):
+        """Clone `nbytes` of library-owned device memory into a fresh torch tensor of `dtype`."""
         import torch
-        esz = torch.empty(0, dtype=dtype).element_size()
-        out = torch.empty(nbytes // esz, dtype=dtype, device="cuda")
-        if nbytes:
-            err = torch.cuda.cudart().cudaMemcpy(out.data_ptr(), int(ptr), nbytes, 3)   # device -> device
-            code = err[0] if isinstance(err, tuple) else err
-            if int(code) != 0:
-                raise RuntimeError(f"cudaMemcpy failed: {err}")
+        if not nbytes:
+            out = torch.empty(0, dtype=dtype, device="cuda")
+        else:
+            class _Raw:     # zero-copy view of the raw pointer through the CUDA array interface
+                __cuda_array_interface__ = {"shape": (int(nbytes),), "typestr": "|u1", "data": (int(ptr), False), "version": 2}
+            out = torch.as_tensor(_Raw(), device="cuda").clone().view(dtype)
         return out.view(shape) if shape is not None else out
 
     def results(self, out: EtxOutput) -> dict:
