@@ -128,7 +128,7 @@ def main():
     ap.add_argument("--impl", default="etx", choices=["etx", "reference"])
     ap.add_argument("--config", default="cfg2")
     ap.add_argument("--events", type=int, default=None, help="override the batch size (debugging only)")
-    ap.add_argument("--engine", default="auto", choices=["auto", "simt"])
+    ap.add_argument("--engine", default="auto", choices=["auto", "simt", "tc_serial"])
     ap.add_argument("--cpu-events", type=int, default=32, help="oracle sample size for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

@@ -48,8 +48,10 @@ typedef enum { ETX_FP32 = 0, ETX_BF16 = 1, ETX_INT8 = 2 } etx_precision;
  * always fp32 FFMA in a pinned order, R4/R20/R21). */
 typedef enum {
   ETX_ENGINE_AUTO = 0,       /* fp32: FFMA kernels; bf16 / int8: tcgen05 tensor-core kernels  */
-  ETX_ENGINE_SIMT = 1        /* FFMA kernels in every precision (bf16 / int8 rounding points
+  ETX_ENGINE_SIMT = 1,       /* FFMA kernels in every precision (bf16 / int8 rounding points
                                 reproduced exactly; the deterministic debugging path)         */
+  ETX_ENGINE_TC_SERIAL = 2   /* tensor-core kernels without warp specialisation (one tile at a
+                                time per CTA); same arithmetic as AUTO, kept as a cross-check */
 } etx_engine;
 
 typedef struct {

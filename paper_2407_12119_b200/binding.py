@@ -11,7 +11,7 @@ _LIB_PATH = os.path.join(HERE, "libetx.so")
 _HEADER = os.path.join(HERE, "..", "include", "etx.h")
 
 PRECISION = {"fp32": 0, "bf16": 1, "int8": 2}
-ENGINE = {"auto": 0, "simt": 1}
+ENGINE = {"auto": 0, "simt": 1, "tc_serial": 2}
 STAGE_NAMES = ["S0_plane_offsets", "S1_embedding", "S2_knn", "S3_compaction_csc", "S4_encoders",
                "S4c_scatter", "S4d_node_net", "S4e_edge_net_head", "S5_components"]
 STATUS = {0: "ETX_OK", -1: "ETX_ERR_ARG", -2: "ETX_ERR_BLOB", -3: "ETX_ERR_CAPACITY", -4: "ETX_ERR_INPUT_ORDER",

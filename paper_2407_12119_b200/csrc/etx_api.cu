@@ -175,7 +175,7 @@ etx_status run_impl(etx_ctx* c, const float* d_xyz, const int32_t* d_plane, cons
     c->n_ev = 0; c->spans.clear();
     c->last_n_hits = n_hits;
     StageTimer tm{c, s};
-    const bool tensor_engine = (c->precision != ETX_FP32) && c->engine == ETX_ENGINE_AUTO;
+    const bool tensor_engine = (c->precision != ETX_FP32) && c->engine != ETX_ENGINE_SIMT;
     if (n_hits > 0) {
       // ---- S0
       tm.begin(0);
@@ -219,7 +219,8 @@ etx_status run_impl(etx_ctx* c, const float* d_xyz, const int32_t* d_plane, cons
         } else {
           const int L = c->hp.gnn_iters;
           auto mlp = [&](int kind, int it, bool head) {
-            if (tensor_engine) launch_gnn_mlp_umma(c, kind, it, n_hits, head, s);
+            if (tensor_engine && c->precision == ETX_BF16 && c->engine != ETX_ENGINE_TC_SERIAL) launch_gnn_mlp_ws(c, kind, it, n_hits, head, s);
+            else if (tensor_engine) launch_gnn_mlp_umma(c, kind, it, n_hits, head, s);
             else launch_gnn_mlp_simt(c, kind, it, n_hits, head, s);
           };
           tm.begin(4);
@@ -265,7 +266,7 @@ etx_status etx_create(const void* blob, size_t blob_bytes, const etx_hyperparams
   c->hp = *hp;
   c->precision = hp->precision; c->engine = hp->engine;
   auto bail = [&](etx_status st) { etx_destroy(c); return st; };
-  if (hp->precision < 0 || hp->precision > 2 || hp->engine < 0 || hp->engine > 1) return bail(ETX_ERR_ARG);
+  if (hp->precision < 0 || hp->precision > 2 || hp->engine < 0 || hp->engine > 2) return bail(ETX_ERR_ARG);
   if (hp->n_planes < 1 || hp->n_planes > 1024 || hp->k < 1 || hp->window < 1 || hp->max_events < 0 || hp->max_hits < 0 ||
       hp->gnn_iters < 0 || hp->gnn_iters > 64 || hp->emb_n_hidden_layers < 1 || hp->emb_n_hidden_layers > 8 ||
       !(hp->threshold >= 0.0f && hp->threshold <= 1.0f) || isnan(hp->d2_max))
@@ -322,7 +323,7 @@ etx_status etx_create(const void* blob, size_t blob_bytes, const etx_hyperparams
     ETX_CUDA(cudaEventCreateWithFlags(&c->staging_free, cudaEventDisableTiming));
     for (int i = 0; i < 256; ++i) ETX_CUDA(cudaEventCreate(&c->ev[i]));
     simt_configure(c);
-    if (c->precision != ETX_FP32 && c->engine == ETX_ENGINE_AUTO) {
+    if (c->precision != ETX_FP32 && c->engine != ETX_ENGINE_SIMT) {
       if (!umma_supported(c)) { c->error = "tensor-core engine not available for these shapes"; return bail(ETX_ERR_UNSUPPORTED); }
       umma_configure(c);
     }

@@ -139,5 +139,7 @@ bool umma_supported(const etx_ctx* c);
 void umma_configure(etx_ctx* c);
 void launch_embed_umma(etx_ctx* c, int n_hits, cudaStream_t s);
 void launch_gnn_mlp_umma(etx_ctx* c, int kind, int iter, int n_hits, bool do_head, cudaStream_t s);
+// k_mlp_ws.cu (bf16: warp-specialised, pipelined)
+void launch_gnn_mlp_ws(etx_ctx* c, int kind, int iter, int n_hits, bool do_head, cudaStream_t s);
 
 }  // namespace etx
