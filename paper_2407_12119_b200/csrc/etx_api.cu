@@ -236,7 +236,7 @@ etx_status run_impl(etx_ctx* c, const float* d_xyz, const int32_t* d_plane, cons
       }
       if (last >= 5) {
         tm.begin(8);
-        launch_components(c, c->logit, n_hits, s);
+        launch_components(c, c->logit, n_events, n_hits, s);
         tm.end();
       }
     }

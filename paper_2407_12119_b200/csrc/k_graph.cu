@@ -75,37 +75,56 @@ void launch_validate(etx_ctx* c, const int32_t* plane, int n_events, int n_hits,
 // event on planes p+1 .. min(p+w, P-1): one contiguous index range given by the plane offsets.  The result
 // is the first min(k, #kept) candidates in ascending (d2, index) order, d2 < d2_max strict.
 //
-// The paper's kernel is one thread per query with a sequential scan ("lacks parallelisation over the
-// neighbours", L286).  Here a CTA owns one (event, plane) bucket: the candidate range is staged through
-// shared memory in tiles (so capacity never depends on the window size), and every query is scanned by
-// LANES cooperating lanes (lane j takes candidates j, j+LANES, ...), each keeping a sorted top-k of 64-bit
-// keys (d2 bits << 32 | index) in registers; the LANES partial lists are merged with warp shuffles.
-// Keys are unique, so the merged list does not depend on how candidates were split.
+// The paper's kernel is one thread per query scanning global memory.  Here a CTA owns one (event, plane)
+// bucket and stages the candidate range through shared memory in tiles (so capacity never depends on the
+// window size); one thread per query walks the tile in ascending candidate index, all lanes of a warp reading
+// the same candidate (a shared-memory broadcast).  Each thread keeps its k best (d2, index) pairs sorted in
+// registers.  Because the walk is in ascending index and the insertion is stable (a candidate goes behind
+// every stored entry with d2 <= its own), the list is ordered by (d2, index) without ever comparing indices,
+// and `d2 < worst` (strict) rejects exactly the candidates that lose under that order (R5).  The empty slots
+// hold d2_max, so the radius cut `d2 < d2_max` (R6) is the same comparison.
 template <int KCAP>
 struct TopK {
-  unsigned long long key[KCAP];
-  __device__ __forceinline__ void init() {
+  float key[KCAP];
+  int idx[KCAP];
+  __device__ __forceinline__ void init(float d2_max) {
 #pragma unroll
-    for (int s = 0; s < KCAP; ++s) key[s] = ~0ull;
+    for (int s = 0; s < KCAP; ++s) { key[s] = d2_max; idx[s] = -1; }
   }
-  // insert into the ascending list of the first k slots
-  __device__ __forceinline__ void insert(unsigned long long cur, int k) {
+  // stable insertion into the ascending list of all KCAP slots; the entry pushed out of the last slot is dropped.
+  // The first k entries of a top-KCAP list are the top-k list, so k < KCAP needs no special case (and no
+  // run-time slot index, which would push the arrays into local memory).
+  __device__ __forceinline__ void insert(float d2, int id) {
+    // the list is ascending, so lt[s] = (d2 < key[s]) is monotone in s: slot s takes the new entry if it is the
+    // first slot with lt, the old slot s-1 if lt[s-1] already held, and keeps its own otherwise.  Entries equal
+    // to d2 stay in front of it (stable).  Walking down keeps key[s-1] / idx[s-1] old when slot s is written.
 #pragma unroll
-    for (int s = 0; s < KCAP; ++s) {
-      if (s < k) {
-        unsigned long long old = key[s];
-        bool lt = cur < old;
-        key[s] = lt ? cur : old;
-        cur = lt ? old : cur;
-      }
+    for (int s = KCAP - 1; s > 0; --s) {
+      const bool lt = d2 < key[s], ltp = d2 < key[s - 1];
+      key[s] = lt ? (ltp ? key[s - 1] : d2) : key[s];
+      idx[s] = lt ? (ltp ? idx[s - 1] : id) : idx[s];
     }
+    const bool lt0 = d2 < key[0];
+    key[0] = lt0 ? d2 : key[0];
+    idx[0] = lt0 ? id : idx[0];
   }
+  __device__ __forceinline__ float worst() const { return key[KCAP - 1]; }
 };
 
 constexpr int kKnnThreads = 128;
 constexpr int kKnnTile = 1024;       // candidates per shared-memory tile (16 KB)
 
-template <int KCAP, int LANES>
+// Eq.(1) in the pinned order: t0*t0, then fma(t_i, t_i, d2)   (R4)
+__device__ __forceinline__ float knn_d2(const float4 a, const float4 b) {
+  float t = __fsub_rn(a.x, b.x);
+  float d2 = __fmul_rn(t, t);
+  t = __fsub_rn(a.y, b.y); d2 = __fmaf_rn(t, t, d2);
+  t = __fsub_rn(a.z, b.z); d2 = __fmaf_rn(t, t, d2);
+  t = __fsub_rn(a.w, b.w); d2 = __fmaf_rn(t, t, d2);
+  return d2;
+}
+
+template <int KCAP>
 __global__ void __launch_bounds__(kKnnThreads)
 knn_kernel(const float4* __restrict__ emb, const int32_t* __restrict__ plane_off, int P, int k, int w,
            float d2_max, int32_t* __restrict__ nbr, int32_t* __restrict__ deg) {
@@ -117,60 +136,48 @@ knn_kernel(const float4* __restrict__ emb, const int32_t* __restrict__ plane_off
   if (q_lo == q_hi) return;
   const int p_hi = min(p + w, P - 1);
   const int c_lo = po[p + 1], c_hi = (p + 1 <= p_hi) ? po[p_hi + 1] : po[p + 1];
-  constexpr int QPB = kKnnThreads / LANES;       // queries per pass
-  const int sub = threadIdx.x % LANES, qslot = threadIdx.x / LANES;
-
-  for (int q0 = q_lo; q0 < q_hi; q0 += QPB) {
-    const int q = q0 + qslot;
+  const bool single = (c_hi - c_lo) <= kKnnTile;   // the usual case: stage the window once for every pass
+  if (single) {
+    for (int i = threadIdx.x; i < c_hi - c_lo; i += kKnnThreads) cand[i] = emb[c_lo + i];
+    __syncthreads();
+  }
+  for (int q0 = q_lo; q0 < q_hi; q0 += kKnnThreads) {
+    const int q = q0 + threadIdx.x;
     const bool active = q < q_hi;
-    float4 a = active ? emb[q] : make_float4(0.f, 0.f, 0.f, 0.f);
+    const float4 a = active ? emb[q] : make_float4(0.f, 0.f, 0.f, 0.f);
     TopK<KCAP> top;
-    top.init();
-    unsigned long long worst = ~0ull;
+    top.init(d2_max);
+    float worst = d2_max;
     for (int t0 = c_lo; t0 < c_hi; t0 += kKnnTile) {
       const int nt = min(kKnnTile, c_hi - t0);
-      __syncthreads();
-      for (int i = threadIdx.x; i < nt; i += kKnnThreads) cand[i] = emb[t0 + i];
-      __syncthreads();
+      if (!single) {
+        __syncthreads();
+        for (int i = threadIdx.x; i < nt; i += kKnnThreads) cand[i] = emb[t0 + i];
+        __syncthreads();
+      }
       if (active) {
-        for (int i = sub; i < nt; i += LANES) {
-          const float4 b = cand[i];
-          // Eq.(1) in the pinned order: t0*t0, then fma(t_i, t_i, d2)   (R4)
-          float t = __fsub_rn(a.x, b.x);
-          float d2 = __fmul_rn(t, t);
-          t = __fsub_rn(a.y, b.y); d2 = __fmaf_rn(t, t, d2);
-          t = __fsub_rn(a.z, b.z); d2 = __fmaf_rn(t, t, d2);
-          t = __fsub_rn(a.w, b.w); d2 = __fmaf_rn(t, t, d2);
-          if (d2 < d2_max) {
-            unsigned long long key = ((unsigned long long)__float_as_uint(d2) << 32) | (unsigned)(t0 + i);
-            if (key < worst) {
-              top.insert(key, k);
-#pragma unroll
-              for (int s = 0; s < KCAP; ++s) if (s == k - 1) worst = top.key[s];
-            }
-          }
+        int i = 0;
+        for (; i + 4 <= nt; i += 4) {
+          const float d0 = knn_d2(a, cand[i]), d1 = knn_d2(a, cand[i + 1]);
+          const float d2 = knn_d2(a, cand[i + 2]), d3 = knn_d2(a, cand[i + 3]);
+          if (d0 < worst) { top.insert(d0, t0 + i); worst = top.worst(); }
+          if (d1 < worst) { top.insert(d1, t0 + i + 1); worst = top.worst(); }
+          if (d2 < worst) { top.insert(d2, t0 + i + 2); worst = top.worst(); }
+          if (d3 < worst) { top.insert(d3, t0 + i + 3); worst = top.worst(); }
+        }
+        for (; i < nt; ++i) {
+          const float d0 = knn_d2(a, cand[i]);
+          if (d0 < worst) { top.insert(d0, t0 + i); worst = top.worst(); }
         }
       }
     }
-    // merge the LANES partial lists: round r folds lane (sub ^ r)'s list into ours
-    if (LANES > 1) {
-#pragma unroll
-      for (int r = 1; r < LANES; r <<= 1) {
-        unsigned long long other[KCAP];
-#pragma unroll
-        for (int s = 0; s < KCAP; ++s) other[s] = __shfl_xor_sync(0xffffffffu, top.key[s], r);
-#pragma unroll
-        for (int s = 0; s < KCAP; ++s) if (s < k && other[s] != ~0ull) top.insert(other[s], k);
-      }
-    }
-    if (active && sub == 0) {
+    if (active) {
       int cnt = 0;
 #pragma unroll
       for (int s = 0; s < KCAP; ++s) {
         if (s < k) {
-          const bool valid = top.key[s] != ~0ull;
-          nbr[(size_t)q * k + s] = valid ? (int32_t)(unsigned)(top.key[s] & 0xffffffffull) : -1;
-          cnt += valid;
+          nbr[(size_t)q * k + s] = top.idx[s];
+          cnt += top.idx[s] >= 0;
         }
       }
       deg[q] = cnt;
@@ -181,8 +188,8 @@ knn_kernel(const float4* __restrict__ emb, const int32_t* __restrict__ plane_off
 template <int KCAP>
 static void knn_dispatch(etx_ctx* c, int n_buckets, cudaStream_t s) {
   const etx_hyperparams& hp = c->hp;
-  knn_kernel<KCAP, 4><<<n_buckets, kKnnThreads, 0, s>>>(c->emb, c->plane_off, hp.n_planes, hp.k, hp.window,
-                                                       hp.d2_max, c->nbr, c->deg);
+  knn_kernel<KCAP><<<n_buckets, kKnnThreads, 0, s>>>(c->emb, c->plane_off, hp.n_planes, hp.k, hp.window,
+                                                    hp.d2_max, c->nbr, c->deg);
 }
 
 void launch_knn(etx_ctx* c, const int32_t* plane, int n_events, int n_hits, cudaStream_t s) {
@@ -369,43 +376,74 @@ __device__ __forceinline__ int uf_find(int32_t* parent_, int x) {
   return x;
 }
 
-__global__ void uf_init_kernel(int32_t* __restrict__ parent, int n) {
-  int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < n) parent[i] = i;
-}
-
-__global__ void uf_union_kernel(const int32_t* __restrict__ src, const int32_t* __restrict__ dst,
-                                const float* __restrict__ logit, const int32_t* __restrict__ n_edges, float tau,
-                                int32_t* parent) {
-  const int E = *n_edges;
-  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < E; i += gridDim.x * blockDim.x) {
-    if (!(logit[i] >= tau)) continue;
-    int a = uf_find(parent, src[i]), b = uf_find(parent, dst[i]);
-    while (a != b) {
-      if (a > b) { int t = a; a = b; b = t; }       // a < b : hang root b under a
-      int old = atomicCAS(&parent[b], b, a);
-      if (old == b) break;
-      b = uf_find(parent, old);                     // b was no longer a root: retry from its new root
-      a = uf_find(parent, a);
-    }
+// hang the root of one endpoint's set under the root of the other; `par` may be shared or global memory
+__device__ __forceinline__ void uf_union(int32_t* par, int a, int b) {
+  a = uf_find(par, a); b = uf_find(par, b);
+  while (a != b) {
+    if (a > b) { int t = a; a = b; b = t; }         // a < b : hang root b under a
+    int old = atomicCAS(&par[b], b, a);
+    if (old == b) break;
+    b = uf_find(par, old);                          // b was no longer a root: retry from its new root
+    a = uf_find(par, a);
   }
 }
 
-__global__ void uf_flatten_kernel(int32_t* parent, int n) {
-  int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
-  volatile int32_t* vp = parent;
-  int r = i;
-  while (true) { int p = vp[r]; if (p == r) break; r = p; }
-  vp[i] = r;     // racing readers still see an ancestor of i
+// Components never cross an event (R8), so one CTA labels one event with its parent array in shared memory
+// (local hit indices; the paper's per-event smem labelling, L261, made exact).  The event's edges are the
+// contiguous range row_ptr[first hit] .. row_ptr[end hit) because edges are sorted by src (R9); src, dst and
+// logit are read once, coalesced.  Events with more hits than the shared array use their slice of the global
+// output as the parent array, with the same code.
+constexpr int kUfThreads = 512;
+constexpr int kUfSmemHits = 16384;                  // 64 KB
+
+__global__ void __launch_bounds__(kUfThreads)
+uf_event_kernel(const int32_t* __restrict__ src, const int32_t* __restrict__ dst, const float* __restrict__ logit,
+                const int32_t* __restrict__ row_ptr, const int32_t* __restrict__ event_off, int n_events, float tau,
+                int32_t* track_id) {
+  extern __shared__ int32_t uf_smem[];
+  for (int e = blockIdx.x; e < n_events; e += gridDim.x) {
+    const int h0 = event_off[e], n = event_off[e + 1] - h0;
+    if (n <= 0) continue;
+    const int e0 = row_ptr[h0], e1 = row_ptr[h0 + n];
+    const bool in_smem = n <= kUfSmemHits;
+    int32_t* par = in_smem ? uf_smem : track_id + h0;
+    for (int i = threadIdx.x; i < n; i += kUfThreads) par[i] = i;
+    __syncthreads();
+    for (int i = e0 + threadIdx.x; i < e1; i += kUfThreads) {
+      if (!(logit[i] >= tau)) continue;             // R17: kept iff z >= tau
+      const unsigned a = (unsigned)(src[i] - h0), b = (unsigned)(dst[i] - h0);
+      if (a >= (unsigned)n || b >= (unsigned)n) continue;   // cannot happen for edges built by S2 (R8)
+      uf_union(par, (int)a, (int)b);
+    }
+    __syncthreads();
+    if (in_smem) {
+      for (int i = threadIdx.x; i < n; i += kUfThreads) {
+        int r = i;
+        while (true) { const int p = par[r]; if (p == r) break; r = p; }
+        track_id[h0 + i] = h0 + r;
+      }
+    } else {
+      volatile int32_t* vp = par;
+      for (int i = threadIdx.x; i < n; i += kUfThreads) {
+        int r = i;
+        while (true) { const int p = vp[r]; if (p == r) break; r = p; }
+        vp[i] = r;                                  // racing readers still see an ancestor of i
+      }
+      __syncthreads();
+      for (int i = threadIdx.x; i < n; i += kUfThreads) par[i] += h0;
+    }
+    __syncthreads();
+  }
 }
 
-void launch_components(etx_ctx* c, const float* logit, int n_hits, cudaStream_t s) {
-  if (n_hits == 0) return;
-  uf_init_kernel<<<(n_hits + 255) / 256, 256, 0, s>>>(c->track_id, n_hits);
-  uf_union_kernel<<<c->sm_count * 8, 256, 0, s>>>(c->src, c->dst, logit, c->n_edges, c->tau, c->track_id);
-  uf_flatten_kernel<<<(n_hits + 255) / 256, 256, 0, s>>>(c->track_id, n_hits);
-  c->launches += 3;
+void launch_components(etx_ctx* c, const float* logit, int n_events, int n_hits, cudaStream_t s) {
+  if (n_hits == 0 || n_events == 0) return;
+  static bool configured = false;
+  constexpr int smem = kUfSmemHits * (int)sizeof(int32_t);
+  if (!configured) { cudaFuncSetAttribute(uf_event_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); configured = true; }
+  const int grid = n_events < c->sm_count * 3 ? n_events : c->sm_count * 3;
+  uf_event_kernel<<<grid, kUfThreads, smem, s>>>(c->src, c->dst, logit, c->row_ptr, c->event_off, n_events, c->tau, c->track_id);
+  c->launches += 1;
 }
 
 }  // namespace etx

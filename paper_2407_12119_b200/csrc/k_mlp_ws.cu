@@ -30,6 +30,9 @@ constexpr int kFeatStages = 8;              // ring of 2 KB feature tiles when l
 constexpr int kEpiWarps = 8, kProdWarps = 4;
 constexpr int kMmaWarp = kEpiWarps + kProdWarps;
 constexpr int kWsThreads = (kMmaWarp + 1) * 32;   // 416
+// ptxas budgets 65536 / 512 = 128 registers per thread for a 416-thread CTA; the producer warpgroup gives 64 of
+// them back (setmaxnreg) and the two epilogue warpgroups take 32 each: 256 * 160 + 128 * 64 + 32 * 128 = 53248.
+constexpr int kProdRegs = 64, kEpiRegs = 160;
 
 __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
@@ -101,6 +104,7 @@ __global__ void __launch_bounds__(kWsThreads, 1) gnn_mlp_ws_kernel(GnnArgs a) {
 
   if (warp >= kEpiWarps && warp < kMmaWarp) {
     // ================================================================================================ producers
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kProdRegs));
     const int pw = warp - kEpiWarps;
     if (L0T) {
       constexpr int LAG = kStages - 1;
@@ -205,6 +209,7 @@ __global__ void __launch_bounds__(kWsThreads, 1) gnn_mlp_ws_kernel(GnnArgs a) {
     }
   } else {
     // ================================================================================================ epilogue
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kEpiRegs));
     const int g = warp >> 2, q = warp & 3;                    // warpgroup, TMEM lane quarter
     const int r = q * 32 + lane;                              // row of the tile owned by this thread
     const uint32_t lane_base = (uint32_t)(q * 32) << 16;
