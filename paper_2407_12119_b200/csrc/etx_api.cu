@@ -219,7 +219,8 @@ etx_status run_impl(etx_ctx* c, const float* d_xyz, const int32_t* d_plane, cons
         } else {
           const int L = c->hp.gnn_iters;
           auto mlp = [&](int kind, int it, bool head) {
-            if (tensor_engine && c->precision == ETX_BF16 && c->engine != ETX_ENGINE_TC_SERIAL) launch_gnn_mlp_ws(c, kind, it, n_hits, head, s);
+            if (kind == kEdgeNet && c->edge_tma) launch_edge_net_tma(c, it, n_hits, head, s);
+            else if (tensor_engine && c->precision == ETX_BF16 && c->engine != ETX_ENGINE_TC_SERIAL) launch_gnn_mlp_ws(c, kind, it, n_hits, head, s);
             else if (tensor_engine) launch_gnn_mlp_umma(c, kind, it, n_hits, head, s);
             else launch_gnn_mlp_simt(c, kind, it, n_hits, head, s);
           };
@@ -326,6 +327,10 @@ etx_status etx_create(const void* blob, size_t blob_bytes, const etx_hyperparams
     if (c->precision != ETX_FP32 && c->engine != ETX_ENGINE_SIMT) {
       if (!umma_supported(c)) { c->error = "tensor-core engine not available for these shapes"; return bail(ETX_ERR_UNSUPPORTED); }
       umma_configure(c);
+      if (c->precision == ETX_BF16 && c->engine == ETX_ENGINE_AUTO) {
+        if (!edge_tma_configure(c)) { c->error = "edge-network TMA setup failed"; return bail(ETX_ERR_CUDA); }
+        c->edge_tma = true;
+      }
     }
     ETX_CUDA(cudaDeviceSynchronize());
   } catch (const CudaFail& f) {

@@ -1,0 +1,465 @@
+// S4e, bf16 mode: the interaction network's edge update  e <- e + MLP_k([h_src, h_dst, e])  (PAPER.md L140,
+// L148) and, on the last step, the d -> 1 edge classifier (L80, L142), as one persistent tcgen05 kernel whose
+// edge-state traffic is moved entirely by TMA.
+//
+// This is the kernel that decides the step time: per launch it must read and write the whole edge state
+// (2 * E * d * 2 bytes, 2.5 GB at cfg 2), so everything is arranged to keep HBM requests in flight and the
+// per-tile epilogue short:
+//
+//   * the tile of `e` being updated (128 consecutive rows = one contiguous 16 KB block) is loaded by one TMA
+//     instruction into a 128B-swizzled slot of a 5-deep ring, updated IN PLACE in shared memory by the epilogue,
+//     and written back by one TMA store from the same slot;
+//   * h[src] and h[dst] (L2-resident: edges are sorted by src and dst lies in the same event) are gathered with
+//     16-byte cp.async into a separate 3-deep ring, so the depth of the HBM ring does not pay for them;
+//   * bias and residual are folded into the MMAs: acc0 = 1 * b0' + [h_src | h_dst | e] * W0^T and
+//     acc1 = 1 * b1' + hidden * W1^T + e * I, where b' is the fp32 bias split exactly into three bf16 terms and I
+//     is the identity (a bf16 value times 1.0 is exact in the fp32 accumulator).  The epilogues are then
+//     TMEM -> cvt(.relu).bf16x2 -> 16-byte shared-memory stores and nothing else;
+//   * the hidden activations overwrite the h_src segment of their gather slot (dead once layer 0 has finished),
+//     so no separate operand / staging buffers are needed.
+//
+// Rounding points are those of DESIGN.md R20 (operands and stored state bf16 RNE, accumulation fp32); the order of
+// the fp32 additions inside the tensor core is not specified, which the bf16 tolerance covers.
+//
+// Warp roles (15 warps, one CTA per SM):
+//   0-7   epilogue, two warpgroups; warpgroup g owns the CTA's tiles it = g (mod 2)
+//   8-11  gather producers (cp.async)
+//   12    MMA issuer (one thread)
+//   13    TMA loader (one thread)       14    TMA storer (one thread)
+#include <cuda.h>
+#include <string.h>
+
+#include "umma_common.cuh"
+
+namespace etx {
+
+namespace {
+
+using namespace umma;
+
+constexpr int kNE = 5;                      // ring of edge-state tiles (HBM latency)
+constexpr int kNH = 3;                      // ring of gathered [h_src | h_dst] tile pairs (L2 latency)
+constexpr int kEpiWarps = 8, kGatherWarps = 4;
+constexpr int kMmaWarp = kEpiWarps + kGatherWarps, kLoadWarp = kMmaWarp + 1, kStoreWarp = kMmaWarp + 2;
+constexpr int kThreads = (kStoreWarp + 1) * 32;   // 480
+// ptxas budgets 65536 / 512 = 128 registers per thread; the gather warpgroup hands 64 of them back and the two
+// epilogue warpgroups take 32 each: 256 * 160 + 128 * 64 + 96 * 128 = 61440 = 480 * 128.
+constexpr int kGatherRegs = 64, kEpiRegs = 160;
+
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+// TMA: one box of a 2-D tensor (inner coordinate x, row y) global -> shared, completing on an mbarrier
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, int x, int y, uint64_t* bar) {
+  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+               ::"r"(dst), "l"(reinterpret_cast<uint64_t>(map)), "r"(smem_u32(bar)), "r"(x), "r"(y) : "memory");
+}
+// TMA: shared -> global, tracked by the issuing thread's bulk async-group
+__device__ __forceinline__ void tma_store_2d(const CUtensorMap* map, uint32_t src, int x, int y) {
+  asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%2, %3}], [%1];"
+               ::"l"(reinterpret_cast<uint64_t>(map)), "r"(src), "r"(x), "r"(y) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+
+// two fp32 -> bf16x2 (RNE), lo in the low half; the .relu form clamps negative inputs to +0 first, which for a
+// monotone rounding is the same as rounding relu(x) (R3, R20)
+__device__ __forceinline__ uint32_t pack_bf16x2_relu(float lo, float hi) {
+  uint32_t r;
+  asm("cvt.rn.relu.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
+  return r;
+}
+
+// 32 lanes x 32 columns without the wait (so that two loads can be in flight)
+__device__ __forceinline__ void tmem_ld32_nowait(uint32_t taddr, uint32_t (&v)[32]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+      "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+      : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+        "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]),
+        "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]),
+        "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+      : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+
+struct EtSmem { int self, aux, w0, w1, ident, ones, b0, b1, headw, bar, total; };
+template <int D>
+__host__ __device__ constexpr EtSmem et_layout() {
+  constexpr int KB = D * 2, BLK = kRows * KB;
+  EtSmem s{};
+  s.self = 0;                          // kNE x [128][KB]             edge-state tiles (TMA in, in-place update, TMA out)
+  s.aux = s.self + kNE * BLK;          // kNH x 2 x [128][KB]         h_src | h_dst; hidden overwrites h_src
+  s.w0 = s.aux + kNH * 2 * BLK;        // W0 image: 3 K-blocks [D][KB]
+  s.w1 = s.w0 + 3 * D * KB;            // W1 image
+  s.ident = s.w1 + D * KB;             // identity [D][KB]
+  s.ones = s.ident + D * KB;           // [128][32 B]: columns 0..2 = 1.0 (32B swizzle)
+  s.b0 = s.ones + kRows * 32;          // [D][32 B]: row n = (hi, mid, lo) of b0[n]
+  s.b1 = s.b0 + D * 32;
+  s.headw = s.b1 + D * 32;             // fp32 [D]
+  s.bar = s.headw + D * 4;
+  s.total = s.bar + 256;
+  return s;
+}
+
+struct EdgeTmaArgs {
+  const void* w0_img; const void* w1_img; const void* ident_img; const void* b0_img; const void* b1_img;
+  const float* head_w; const float* head_b;
+  const __nv_bfloat16* h;
+  const int32_t* src; const int32_t* dst;
+  const int32_t* n_rows_ptr;
+  float* logit; float* score;
+  int do_head;
+};
+
+// all MMAs of one K-block: kbytes of K, 32 bytes (16 bf16) per instruction
+template <int KB>
+__device__ __forceinline__ void issue_block(uint32_t a_blk, uint32_t b_blk, uint32_t tmem_d, uint32_t idesc) {
+#pragma unroll
+  for (int s = 0; s < KB / 32; ++s)
+    umma::umma<kBf16>(tmem_d, make_desc<KB>(a_blk + s * 32), make_desc<KB>(b_blk + s * 32), idesc, 1u);
+}
+
+template <int D>
+__global__ void __launch_bounds__(kThreads, 1)
+edge_net_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeTmaArgs a) {
+  constexpr int KB = D * 2;                                  // bytes per state row = swizzle width
+  constexpr int CPR = KB / 16;                               // 16-byte chunks per row
+  constexpr int BLK = kRows * KB;
+  constexpr EtSmem L = et_layout<D>();
+  constexpr uint32_t TMEM_COLS = 4 * D;                      // acc0[2] | acc1[2]
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+  float* headw = reinterpret_cast<float*>(smem + L.headw);
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + L.bar);
+  uint64_t *self_full = bars, *self_empty = bars + kNE, *out_ready = bars + 2 * kNE;
+  uint64_t *aux_full = bars + 3 * kNE, *aux_empty = aux_full + kNH;
+  uint64_t *acc0_full = aux_empty + kNH, *hid_full = acc0_full + 2, *acc1_full = acc0_full + 4, *bar_w = acc0_full + 6;
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc0_full + 7);
+
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int n_rows = *a.n_rows_ptr;
+  const int n_tiles = (n_rows + kRows - 1) / kRows;
+
+  if (tid == 0) {
+    for (int s = 0; s < kNE; ++s) { mbar_init(&self_full[s], 1); mbar_init(&self_empty[s], 1); mbar_init(&out_ready[s], 128); }
+    for (int s = 0; s < kNH; ++s) { mbar_init(&aux_full[s], kGatherWarps * 32); mbar_init(&aux_empty[s], 1); }
+    for (int g = 0; g < 2; ++g) { mbar_init(&acc0_full[g], 1); mbar_init(&hid_full[g], 128); mbar_init(&acc1_full[g], 1); }
+    mbar_init(bar_w, 1);
+    fence_barrier_init();
+  }
+  if (warp == kMmaWarp) tmem_alloc(tmem_slot, TMEM_COLS);
+  for (int i = tid; i < D; i += kThreads) headw[i] = a.head_w[i];
+  // the ones tile: row r holds 1.0 in its first three bf16 columns (the three terms of the split bias)
+  for (int r = tid; r < kRows; r += kThreads) {
+    uint4* row = reinterpret_cast<uint4*>(smem + L.ones + r * 32);
+    row[0] = make_uint4(0u, 0u, 0u, 0u); row[1] = make_uint4(0u, 0u, 0u, 0u);
+    *reinterpret_cast<uint4*>(smem + L.ones + swz<32>(r, 0)) = make_uint4(0x3f803f80u, 0x00003f80u, 0u, 0u);
+  }
+  fence_proxy_async();
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = *tmem_slot;
+  const uint32_t self_addr = smem_u32(smem + L.self), aux_addr = smem_u32(smem + L.aux);
+
+  if (warp >= kEpiWarps && warp < kMmaWarp) {
+    // ================================================================================================ gather
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kGatherRegs));
+    const int pw = warp - kEpiWarps;
+    constexpr int LAG = kNH - 1;
+    int it = 0;
+    for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
+      const int s = it % kNH;
+      int row = tile * kRows + pw * 32 + lane;
+      if (row >= n_rows) row = n_rows - 1;                    // dead rows of the last tile: any valid row
+      const int is = __ldg(a.src + row), id = __ldg(a.dst + row);
+      // Publish the tile issued LAG iterations ago BEFORE waiting for a free slot: the slot of tile it-kNH is
+      // released by layer 1 of that tile, which the MMA thread issues only after layer 0 of tile it-kNH+1, i.e.
+      // after that tile has been published -- publishing after the wait would deadlock.
+      if (it >= LAG) {
+        cp_async_wait<LAG - 1>();
+        fence_proxy_async();                                  // generic-proxy writes -> visible to the tensor core
+        mbar_arrive(&aux_full[(it - LAG) % kNH]);
+      }
+      mbar_wait(&aux_empty[s], ((it / kNH) & 1) ^ 1);
+      const uint32_t st = aux_addr + s * 2 * BLK;
+#pragma unroll
+      for (int i = 0; i < CPR; ++i) {
+        const int c = i * 32 + lane, rl = c / CPR, piece = c % CPR;
+        const int r = pw * 32 + rl;
+        const int js = __shfl_sync(0xffffffffu, is, rl), jd = __shfl_sync(0xffffffffu, id, rl);
+        const uint32_t off = swz<KB>(r, piece);
+        cp_async16(st + off, a.h + (size_t)js * D + piece * 8);
+        cp_async16(st + BLK + off, a.h + (size_t)jd * D + piece * 8);
+      }
+      cp_async_commit();
+    }
+    cp_async_wait<0>();
+    fence_proxy_async();
+    for (int j = it - (it < LAG ? it : LAG); j < it; ++j) mbar_arrive(&aux_full[j % kNH]);
+  } else if (warp == kLoadWarp) {
+    // ================================================================================================ TMA loads
+    if (lane == 0) {
+      int it = 0;
+      for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
+        const int s = it % kNE;
+        mbar_wait(&self_empty[s], ((it / kNE) & 1) ^ 1);
+        mbar_expect_tx(&self_full[s], BLK);
+        tma_load_2d(self_addr + s * BLK, &e_map, 0, tile * kRows, &self_full[s]);
+      }
+    }
+  } else if (warp == kStoreWarp) {
+    // ================================================================================================ TMA stores
+    if (lane == 0) {
+      int it = 0;
+      for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
+        const int s = it % kNE;
+        mbar_wait(&out_ready[s], (it / kNE) & 1);
+        tma_store_2d(&e_map, self_addr + s * BLK, 0, tile * kRows);
+        bulk_commit();
+        bulk_wait_read0();                                    // the slot has been read: hand it back to the loader
+        mbar_arrive(&self_empty[s]);
+      }
+      bulk_wait0();
+    }
+  } else if (warp == kMmaWarp) {
+    // ================================================================================================ MMA issuer
+    if (lane == 0) {
+      const uint32_t wb0 = 3 * D * KB, wb1 = D * KB, bb = D * 32;
+      mbar_expect_tx(bar_w, wb0 + 2 * wb1 + 2 * bb);
+      bulk_g2s(smem + L.w0, a.w0_img, wb0, bar_w);
+      bulk_g2s(smem + L.w1, a.w1_img, wb1, bar_w);
+      bulk_g2s(smem + L.ident, a.ident_img, wb1, bar_w);
+      bulk_g2s(smem + L.b0, a.b0_img, bb, bar_w);
+      bulk_g2s(smem + L.b1, a.b1_img, bb, bar_w);
+      mbar_wait(bar_w, 0);
+      const uint32_t idesc = make_idesc<kBf16>(D);
+      const uint32_t w0_addr = smem_u32(smem + L.w0), w1_addr = smem_u32(smem + L.w1), id_addr = smem_u32(smem + L.ident);
+      const uint64_t ones_desc = make_desc<32>(smem_u32(smem + L.ones));
+      const uint64_t b0_desc = make_desc<32>(smem_u32(smem + L.b0)), b1_desc = make_desc<32>(smem_u32(smem + L.b1));
+      auto layer1 = [&](int j) {                              // acc1 = 1*b1' + hidden*W1^T + e*I   (tile j of this CTA)
+        const int g = j & 1, se = j % kNE, sh = j % kNH;
+        mbar_wait(&hid_full[g], (j >> 1) & 1);
+        tc_fence_after();
+        const uint32_t d1 = tmem + 2 * D + g * D;
+        umma::umma<kBf16>(d1, ones_desc, b1_desc, idesc, 0u);
+        issue_block<KB>(aux_addr + sh * 2 * BLK, w1_addr, d1, idesc);
+        issue_block<KB>(self_addr + se * BLK, id_addr, d1, idesc);
+        umma_commit(&acc1_full[g]);
+        umma_commit(&aux_empty[sh]);                          // the gather slot (hidden included) is free again
+      };
+      int it = 0;
+      for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
+        const int g = it & 1, se = it % kNE, sh = it % kNH;
+        mbar_wait(&aux_full[sh], (it / kNH) & 1);
+        mbar_wait(&self_full[se], (it / kNE) & 1);
+        tc_fence_after();
+        // acc0[g] was drained by epilogue 0 of tile it-2: hid_full, waited on for layer 1 of it-2, covers it
+        const uint32_t d0 = tmem + g * D;
+        umma::umma<kBf16>(d0, ones_desc, b0_desc, idesc, 0u);
+        issue_block<KB>(aux_addr + sh * 2 * BLK, w0_addr, d0, idesc);                      // h_src
+        issue_block<KB>(aux_addr + sh * 2 * BLK + BLK, w0_addr + D * KB, d0, idesc);       // h_dst
+        issue_block<KB>(self_addr + se * BLK, w0_addr + 2 * D * KB, d0, idesc);            // e
+        umma_commit(&acc0_full[g]);
+        if (it > 0) layer1(it - 1);
+      }
+      if (it > 0) layer1(it - 1);
+    }
+  } else {
+    // ================================================================================================ epilogue
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kEpiRegs));
+    const int g = warp >> 2, q = warp & 3;                    // warpgroup, TMEM lane quarter
+    const int r = q * 32 + lane;                              // row of the tile owned by this thread
+    const uint32_t lane_base = (uint32_t)(q * 32) << 16;
+    const float head_b = a.head_b[0];
+    int j = 0;
+    for (int it = g; blockIdx.x + (long long)it * gridDim.x < n_tiles; it += 2, ++j) {
+      const int tile = blockIdx.x + it * gridDim.x;
+      const int row = tile * kRows + r;
+      uint8_t* hid = smem + L.aux + (it % kNH) * 2 * BLK;     // h_src segment of the gather slot
+      uint8_t* out = smem + L.self + (it % kNE) * BLK;        // the e tile, updated in place
+      // ---- epilogue 0: relu(acc0) -> bf16 -> layer-1 operand (R3, R20); the bias is already in acc0
+      mbar_wait(&acc0_full[g], j & 1);
+      tc_fence_after();
+#pragma unroll
+      for (int c0 = 0; c0 < D; c0 += 32) {
+        uint32_t v[32];
+        tmem_ld32_nowait(tmem + lane_base + g * D + c0, v);
+        tmem_ld_wait();
+#pragma unroll
+        for (int ch = 0; ch < 4; ++ch) {
+          uint4 qv;
+          qv.x = pack_bf16x2_relu(__uint_as_float(v[ch * 8 + 0]), __uint_as_float(v[ch * 8 + 1]));
+          qv.y = pack_bf16x2_relu(__uint_as_float(v[ch * 8 + 2]), __uint_as_float(v[ch * 8 + 3]));
+          qv.z = pack_bf16x2_relu(__uint_as_float(v[ch * 8 + 4]), __uint_as_float(v[ch * 8 + 5]));
+          qv.w = pack_bf16x2_relu(__uint_as_float(v[ch * 8 + 6]), __uint_as_float(v[ch * 8 + 7]));
+          *reinterpret_cast<uint4*>(hid + swz<KB>(r, c0 / 8 + ch)) = qv;
+        }
+      }
+      tc_fence_before();
+      fence_proxy_async();
+      mbar_arrive(&hid_full[g]);
+      // ---- epilogue 1: acc1 (= b1 + W1 hidden + old e) -> bf16 -> the slot, optional classifier (R14, R16, R20)
+      mbar_wait(&acc1_full[g], j & 1);
+      tc_fence_after();
+      float hacc = 0.0f;
+#pragma unroll
+      for (int c0 = 0; c0 < D; c0 += 32) {
+        uint32_t v[32];
+        tmem_ld32_nowait(tmem + lane_base + 2 * D + g * D + c0, v);
+        tmem_ld_wait();
+#pragma unroll
+        for (int ch = 0; ch < 4; ++ch) {
+          uint4 qv;
+          qv.x = pack_bf16x2(__uint_as_float(v[ch * 8 + 0]), __uint_as_float(v[ch * 8 + 1]));
+          qv.y = pack_bf16x2(__uint_as_float(v[ch * 8 + 2]), __uint_as_float(v[ch * 8 + 3]));
+          qv.z = pack_bf16x2(__uint_as_float(v[ch * 8 + 4]), __uint_as_float(v[ch * 8 + 5]));
+          qv.w = pack_bf16x2(__uint_as_float(v[ch * 8 + 6]), __uint_as_float(v[ch * 8 + 7]));
+          *reinterpret_cast<uint4*>(out + swz<KB>(r, c0 / 8 + ch)) = qv;
+          if (a.do_head) {                                    // the classifier sees the stored bf16 state, ascending j
+            const float* hw = headw + c0 + ch * 8;
+            hacc = __fmaf_rn(bf16_lo(qv.x), hw[0], hacc); hacc = __fmaf_rn(bf16_hi(qv.x), hw[1], hacc);
+            hacc = __fmaf_rn(bf16_lo(qv.y), hw[2], hacc); hacc = __fmaf_rn(bf16_hi(qv.y), hw[3], hacc);
+            hacc = __fmaf_rn(bf16_lo(qv.z), hw[4], hacc); hacc = __fmaf_rn(bf16_hi(qv.z), hw[5], hacc);
+            hacc = __fmaf_rn(bf16_lo(qv.w), hw[6], hacc); hacc = __fmaf_rn(bf16_hi(qv.w), hw[7], hacc);
+          }
+        }
+      }
+      tc_fence_before();                                      // acc1[g] may be overwritten after our next hid_full arrive
+      fence_proxy_async();                                    // generic-proxy writes -> visible to the TMA store
+      mbar_arrive(&out_ready[it % kNE]);
+      if (a.do_head && row < n_rows) {
+        const float z = __fadd_rn(hacc, head_b);
+        a.logit[row] = z;
+        a.score[row] = 1.0f / (1.0f + expf(-z));
+      }
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == kMmaWarp) tmem_dealloc(tmem, TMEM_COLS);
+}
+
+// ---------------------------------------------------------------------------------------------- host side
+uint16_t bf16_bits_rne(float x) {
+  const __nv_bfloat16 b = __float2bfloat16_rn(x);
+  uint16_t u; memcpy(&u, &b, 2);
+  return u;
+}
+float bf16_value(uint16_t u) { uint32_t w = (uint32_t)u << 16; float f; memcpy(&f, &w, 4); return f; }
+
+// [n][32 B] image (32B swizzle) whose row n holds, in its first three bf16 columns, an exact split of v[n]:
+// hi = rn(v), mid = rn(v - hi), lo = v - hi - mid (at most 8 significant bits are left, so lo is exact)
+std::vector<uint8_t> pack_split_rows(const std::vector<float>& v) {
+  const int n = (int)v.size();
+  std::vector<uint8_t> img((size_t)n * 32, 0);
+  for (int r = 0; r < n; ++r) {
+    float rest = v[r];
+    uint16_t t[3];
+    for (int i = 0; i < 3; ++i) { t[i] = bf16_bits_rne(rest); rest -= bf16_value(t[i]); }
+    const uint32_t lin = (uint32_t)r * 32;
+    const size_t off = lin + ((((lin >> 7)) & 1u) << 4);      // chunk 0 of the row under the 32B swizzle
+    memcpy(&img[off], t, 6);
+  }
+  return img;
+}
+
+// identity [D][KB] in the K-major swizzled operand layout (row n has 1.0 at column n)
+std::vector<uint8_t> pack_identity(int D) {
+  const int KB = D * 2;
+  std::vector<uint8_t> img((size_t)D * KB, 0);
+  for (int n = 0; n < D; ++n) {
+    const int b = n * 2, chunk = b / 16;
+    const uint32_t lin = (uint32_t)n * KB;
+    const size_t off = lin + (((chunk ^ (lin >> 7)) & (KB / 16 - 1)) << 4) + (b & 15);
+    img[off] = 0x80; img[off + 1] = 0x3f;
+  }
+  return img;
+}
+
+void* upload_bytes(etx_ctx* c, const std::vector<uint8_t>& v) {
+  void* p = nullptr;
+  if (cudaMalloc(&p, v.size()) != cudaSuccess) return nullptr;
+  c->allocs.push_back(p);
+  cudaMemcpy(p, v.data(), v.size(), cudaMemcpyHostToDevice);
+  return p;
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+template <int D>
+void edge_tma_launch(etx_ctx* c, const EdgeTmaArgs& a, int max_rows, cudaStream_t s) {
+  auto kern = edge_net_tma_kernel<D>;
+  constexpr int smem = et_layout<D>().total + 1024;
+  static bool configured = false;
+  if (!configured) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); configured = true; }
+  const int tiles = (max_rows + kRows - 1) / kRows;
+  const int grid = tiles < c->sm_count ? tiles : c->sm_count;     // one persistent CTA per SM
+  if (grid <= 0) return;
+  CUtensorMap map;
+  memcpy(&map, c->e_map, sizeof(map));
+  kern<<<grid, kThreads, smem, s>>>(map, a);
+  c->launches++;
+}
+
+}  // namespace
+
+// bf16 mode, tensor engine: per-step bias / identity images and the tensor map of the edge state
+bool edge_tma_configure(etx_ctx* c) {
+  const int D = c->hp.gnn_latent, L = c->hp.gnn_iters;
+  static_assert(sizeof(CUtensorMap) == sizeof(c->e_map), "etx_ctx::e_map must hold a CUtensorMap");
+  c->ident_img = upload_bytes(c, pack_identity(D));
+  if (!c->ident_img) return false;
+  c->edge_bias_img.assign(2 * (size_t)L, nullptr);
+  for (int it = 0; it < L; ++it)
+    for (int l = 0; l < 2; ++l) {
+      void* p = upload_bytes(c, pack_split_rows(c->layers[c->i_iter0 + 4 * it + 2 + l].b));
+      if (!p) return false;
+      c->edge_bias_img[2 * it + l] = p;
+    }
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn) return false;
+  const cuuint64_t rows = c->max_edges > 0 ? (cuuint64_t)c->max_edges : 1;
+  const cuuint64_t gdim[2] = {(cuuint64_t)D, rows};
+  const cuuint64_t gstride[1] = {(cuuint64_t)D * 2};
+  const cuuint32_t box[2] = {(cuuint32_t)D, (cuuint32_t)kRows};
+  const cuuint32_t estr[2] = {1, 1};
+  CUtensorMap map;
+  const CUresult r = reinterpret_cast<EncodeTiledFn>(fn)(
+      &map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, c->e, gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+      D == 64 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return false;
+  memcpy(c->e_map, &map, sizeof(map));
+  return true;
+}
+
+void launch_edge_net_tma(etx_ctx* c, int iter, int n_hits, bool do_head, cudaStream_t s) {
+  const int i0 = c->i_iter0 + 4 * iter + 2;
+  EdgeTmaArgs a;
+  a.w0_img = c->layers[i0].dev.Wtc; a.w1_img = c->layers[i0 + 1].dev.Wtc; a.ident_img = c->ident_img;
+  a.b0_img = c->edge_bias_img[2 * iter]; a.b1_img = c->edge_bias_img[2 * iter + 1];
+  a.head_w = c->layers[c->i_head].dev.Wt; a.head_b = c->layers[c->i_head].dev.bias;
+  a.h = static_cast<const __nv_bfloat16*>(c->h);
+  a.src = c->src; a.dst = c->dst; a.n_rows_ptr = c->n_edges;
+  a.logit = c->logit; a.score = c->score; a.do_head = do_head ? 1 : 0;
+  const long long max_rows_ll = (long long)n_hits * c->hp.k;
+  const int max_rows = (int)(max_rows_ll > 0x7fffffff ? 0x7fffffff : max_rows_ll);
+  if (c->hp.gnn_latent == 32) edge_tma_launch<32>(c, a, max_rows, s);
+  else edge_tma_launch<64>(c, a, max_rows, s);
+}
+
+}  // namespace etx
