@@ -92,6 +92,32 @@ __device__ __forceinline__ void tmem_ld32_nowait(uint32_t taddr, uint32_t (&v)[3
 }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
+__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&v)[32]) {
+  asm volatile(
+      "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
+      "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, "
+      "%17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31, %32};"
+      :: "r"(taddr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]),
+         "r"(v[8]), "r"(v[9]), "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]),
+         "r"(v[16]), "r"(v[17]), "r"(v[18]), "r"(v[19]), "r"(v[20]), "r"(v[21]), "r"(v[22]), "r"(v[23]),
+         "r"(v[24]), "r"(v[25]), "r"(v[26]), "r"(v[27]), "r"(v[28]), "r"(v[29]), "r"(v[30]), "r"(v[31]) : "memory");
+}
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&v)[32]) {
+  asm volatile(
+      "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], "
+      "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};"
+      :: "r"(taddr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]),
+         "r"(v[8]), "r"(v[9]), "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]) : "memory");
+}
+__device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+
+// D[tmem] (+)= A[tmem] * B[smem]^T: A is a 128-lane x K block of tensor memory, two bf16 per 32-bit column
+__device__ __forceinline__ void umma_ts(uint32_t tmem_d, uint32_t tmem_a, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+  asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+               "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
+               ::"r"(tmem_d), "r"(tmem_a), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
+}
+
 struct EtSmem { int self, aux, w0, w1, ident, ones, b0, b1, headw, bar, total; };
 template <int D>
 __host__ __device__ constexpr EtSmem et_layout() {
@@ -136,7 +162,7 @@ edge_net_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeTmaArgs
   constexpr int CPR = KB / 16;                               // 16-byte chunks per row
   constexpr int BLK = kRows * KB;
   constexpr EtSmem L = et_layout<D>();
-  constexpr uint32_t TMEM_COLS = 4 * D;                      // acc0[2] | acc1[2]
+  constexpr uint32_t TMEM_COLS = 8 * D;                      // acc0[2] | acc1[2] | hidden[2] (D/2 packed columns each), pow2
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
   float* headw = reinterpret_cast<float*>(smem + L.headw);
@@ -152,7 +178,7 @@ edge_net_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeTmaArgs
 
   if (tid == 0) {
     for (int s = 0; s < kNE; ++s) { mbar_init(&self_full[s], 1); mbar_init(&self_empty[s], 1); mbar_init(&out_ready[s], 128); }
-    for (int s = 0; s < kNH; ++s) { mbar_init(&aux_full[s], kGatherWarps * 32); mbar_init(&aux_empty[s], 1); }
+    for (int s = 0; s < kNH; ++s) { mbar_init(&aux_full[s], 32); mbar_init(&aux_empty[s], 1); }
     for (int g = 0; g < 2; ++g) { mbar_init(&acc0_full[g], 1); mbar_init(&hid_full[g], 128); mbar_init(&acc1_full[g], 1); }
     mbar_init(bar_w, 1);
     fence_barrier_init();
@@ -175,38 +201,41 @@ edge_net_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeTmaArgs
   if (warp >= kEpiWarps && warp < kMmaWarp) {
     // ================================================================================================ gather
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kGatherRegs));
+    // Warp pw < kNH owns slot pw of the gather ring and gathers whole tiles it = pw (mod kNH): wait for the slot,
+    // issue the tile's 2 x 128 rows as 16-byte cp.async (64 per lane), wait for them, publish.  Up to kNH tiles are
+    // in flight per SM and a tile is published the moment it has landed.  (One warp per slot keeps every waiter at
+    // most one mbarrier phase ahead, which the parity wait requires; the warpgroup's fourth warp only donates its
+    // registers.)
     const int pw = warp - kEpiWarps;
-    constexpr int LAG = kNH - 1;
-    int it = 0;
-    for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
+    for (int it = pw; pw < kNH && blockIdx.x + (long long)it * gridDim.x < n_tiles; it += kNH) {
+      const int tile = blockIdx.x + it * gridDim.x;
       const int s = it % kNH;
-      int row = tile * kRows + pw * 32 + lane;
-      if (row >= n_rows) row = n_rows - 1;                    // dead rows of the last tile: any valid row
-      const int is = __ldg(a.src + row), id = __ldg(a.dst + row);
-      // Publish the tile issued LAG iterations ago BEFORE waiting for a free slot: the slot of tile it-kNH is
-      // released by layer 1 of that tile, which the MMA thread issues only after layer 0 of tile it-kNH+1, i.e.
-      // after that tile has been published -- publishing after the wait would deadlock.
-      if (it >= LAG) {
-        cp_async_wait<LAG - 1>();
-        fence_proxy_async();                                  // generic-proxy writes -> visible to the tensor core
-        mbar_arrive(&aux_full[(it - LAG) % kNH]);
+      int isv[4], idv[4];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        int row = tile * kRows + j * 32 + lane;
+        if (row >= n_rows) row = n_rows - 1;                  // dead rows of the last tile: any valid row
+        isv[j] = __ldg(a.src + row); idv[j] = __ldg(a.dst + row);
       }
       mbar_wait(&aux_empty[s], ((it / kNH) & 1) ^ 1);
       const uint32_t st = aux_addr + s * 2 * BLK;
 #pragma unroll
-      for (int i = 0; i < CPR; ++i) {
-        const int c = i * 32 + lane, rl = c / CPR, piece = c % CPR;
-        const int r = pw * 32 + rl;
-        const int js = __shfl_sync(0xffffffffu, is, rl), jd = __shfl_sync(0xffffffffu, id, rl);
-        const uint32_t off = swz<KB>(r, piece);
-        cp_async16(st + off, a.h + (size_t)js * D + piece * 8);
-        cp_async16(st + BLK + off, a.h + (size_t)jd * D + piece * 8);
+      for (int j = 0; j < 4; ++j) {
+#pragma unroll
+        for (int i = 0; i < CPR; ++i) {
+          const int c = i * 32 + lane, rl = c / CPR, piece = c % CPR;
+          const int r = j * 32 + rl;
+          const int js = __shfl_sync(0xffffffffu, isv[j], rl), jd = __shfl_sync(0xffffffffu, idv[j], rl);
+          const uint32_t off = swz<KB>(r, piece);
+          cp_async16(st + off, a.h + (size_t)js * D + piece * 8);
+          cp_async16(st + BLK + off, a.h + (size_t)jd * D + piece * 8);
+        }
       }
       cp_async_commit();
+      cp_async_wait<0>();
+      fence_proxy_async();                                    // generic-proxy writes -> visible to the tensor core
+      mbar_arrive(&aux_full[s]);
     }
-    cp_async_wait<0>();
-    fence_proxy_async();
-    for (int j = it - (it < LAG ? it : LAG); j < it; ++j) mbar_arrive(&aux_full[j % kNH]);
   } else if (warp == kLoadWarp) {
     // ================================================================================================ TMA loads
     if (lane == 0) {
@@ -248,15 +277,16 @@ edge_net_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeTmaArgs
       const uint64_t ones_desc = make_desc<32>(smem_u32(smem + L.ones));
       const uint64_t b0_desc = make_desc<32>(smem_u32(smem + L.b0)), b1_desc = make_desc<32>(smem_u32(smem + L.b1));
       auto layer1 = [&](int j) {                              // acc1 = 1*b1' + hidden*W1^T + e*I   (tile j of this CTA)
-        const int g = j & 1, se = j % kNE, sh = j % kNH;
+        const int g = j & 1, se = j % kNE;
         mbar_wait(&hid_full[g], (j >> 1) & 1);
         tc_fence_after();
-        const uint32_t d1 = tmem + 2 * D + g * D;
+        const uint32_t d1 = tmem + 2 * D + g * D, hid = tmem + 4 * D + g * (D / 2);
         umma::umma<kBf16>(d1, ones_desc, b1_desc, idesc, 0u);
-        issue_block<KB>(aux_addr + sh * 2 * BLK, w1_addr, d1, idesc);
+#pragma unroll
+        for (int k = 0; k < D / 16; ++k)                      // A = hidden in tensor memory, 8 packed columns per K = 16
+          umma_ts(d1, hid + 8 * k, make_desc<KB>(w1_addr + k * 32), idesc, 1u);
         issue_block<KB>(self_addr + se * BLK, id_addr, d1, idesc);
         umma_commit(&acc1_full[g]);
-        umma_commit(&aux_empty[sh]);                          // the gather slot (hidden included) is free again
       };
       int it = 0;
       for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
@@ -271,6 +301,7 @@ edge_net_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeTmaArgs
         issue_block<KB>(aux_addr + sh * 2 * BLK + BLK, w0_addr + D * KB, d0, idesc);       // h_dst
         issue_block<KB>(self_addr + se * BLK, w0_addr + 2 * D * KB, d0, idesc);            // e
         umma_commit(&acc0_full[g]);
+        umma_commit(&aux_empty[sh]);                          // layer 0 was the gather slot's only reader
         if (it > 0) layer1(it - 1);
       }
       if (it > 0) layer1(it - 1);
@@ -286,28 +317,29 @@ edge_net_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeTmaArgs
     for (int it = g; blockIdx.x + (long long)it * gridDim.x < n_tiles; it += 2, ++j) {
       const int tile = blockIdx.x + it * gridDim.x;
       const int row = tile * kRows + r;
-      uint8_t* hid = smem + L.aux + (it % kNH) * 2 * BLK;     // h_src segment of the gather slot
       uint8_t* out = smem + L.self + (it % kNE) * BLK;        // the e tile, updated in place
-      // ---- epilogue 0: relu(acc0) -> bf16 -> layer-1 operand (R3, R20); the bias is already in acc0
+      // ---- epilogue 0: relu(acc0) -> bf16, packed two per column -> tensor memory, the A operand of layer 1 (R3, R20);
+      //      the bias is already in acc0
       mbar_wait(&acc0_full[g], j & 1);
       tc_fence_after();
 #pragma unroll
-      for (int c0 = 0; c0 < D; c0 += 32) {
-        uint32_t v[32];
+      for (int c0 = 0; c0 < D; c0 += 64) {
+        uint32_t v[32], w[32], pk[32];
         tmem_ld32_nowait(tmem + lane_base + g * D + c0, v);
+        if (D > 32) tmem_ld32_nowait(tmem + lane_base + g * D + c0 + 32, w);
         tmem_ld_wait();
 #pragma unroll
-        for (int ch = 0; ch < 4; ++ch) {
-          uint4 qv;
-          qv.x = pack_bf16x2_relu(__uint_as_float(v[ch * 8 + 0]), __uint_as_float(v[ch * 8 + 1]));
-          qv.y = pack_bf16x2_relu(__uint_as_float(v[ch * 8 + 2]), __uint_as_float(v[ch * 8 + 3]));
-          qv.z = pack_bf16x2_relu(__uint_as_float(v[ch * 8 + 4]), __uint_as_float(v[ch * 8 + 5]));
-          qv.w = pack_bf16x2_relu(__uint_as_float(v[ch * 8 + 6]), __uint_as_float(v[ch * 8 + 7]));
-          *reinterpret_cast<uint4*>(hid + swz<KB>(r, c0 / 8 + ch)) = qv;
+        for (int i = 0; i < 16; ++i) pk[i] = pack_bf16x2_relu(__uint_as_float(v[2 * i]), __uint_as_float(v[2 * i + 1]));
+        if (D > 32) {
+#pragma unroll
+          for (int i = 0; i < 16; ++i) pk[16 + i] = pack_bf16x2_relu(__uint_as_float(w[2 * i]), __uint_as_float(w[2 * i + 1]));
+          tmem_st32(tmem + lane_base + 4 * D + g * (D / 2) + c0 / 2, pk);
+        } else {
+          tmem_st16(tmem + lane_base + 4 * D + g * (D / 2), pk);
         }
       }
+      tmem_st_wait();
       tc_fence_before();
-      fence_proxy_async();
       mbar_arrive(&hid_full[g]);
       // ---- epilogue 1: acc1 (= b1 + W1 hidden + old e) -> bf16 -> the slot, optional classifier (R14, R16, R20)
       mbar_wait(&acc1_full[g], j & 1);
