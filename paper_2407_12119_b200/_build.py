@@ -44,7 +44,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
     def compile_one(so):
         s, o = so
-        cmd = [_nvcc(), *NVCC_FLAGS, "-c", s, "-o", o] + (["-Xptxas", "-v"] if verbose else [])
+        cmd = [_nvcc(), *NVCC_FLAGS, *os.environ.get("ETX_NVCC_EXTRA", "").split(), "-c", s, "-o", o] + (["-Xptxas", "-v"] if verbose else [])
         r = subprocess.run(cmd, capture_output=True, text=True)
         if r.returncode != 0:
             raise RuntimeError("nvcc failed:\n" + " ".join(cmd) + "\n" + r.stdout + r.stderr)
