@@ -49,13 +49,6 @@ constexpr int kGatherRegs = 64, kEpiRegs = 160;
 __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
-// one lane of the (converged) warp; ptxas knows the guarded region runs single-threaded, so operands of the
-// tcgen05 instructions move to uniform registers without a per-instruction broadcast loop
-__device__ __forceinline__ bool elect_one() {
-  uint32_t p;
-  asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(p));
-  return p != 0;
-}
 __device__ __forceinline__ bool mbar_test(uint64_t* bar, uint32_t parity) {      // non-blocking
   uint32_t done;
   asm volatile(

@@ -155,7 +155,7 @@ __global__ void __launch_bounds__(kUmmaThreads) gnn_mlp_umma_kernel(GnnArgs a) {
       tc_fence_before();
       __syncthreads();
       // ---- layer 0 on the tensor cores: acc0 = A * W0^T ---------------------------------------------------------------
-      if (tid == 0) {
+      if (warp == 0 && elect_one()) {
         tc_fence_after();
         issue_layer<PREC, KB>(a_addr, w0_addr, nseg * KB, D, tmem, idesc);
         umma_commit(bar_mma);
@@ -198,7 +198,7 @@ __global__ void __launch_bounds__(kUmmaThreads) gnn_mlp_umma_kernel(GnnArgs a) {
     tc_fence_before();
     __syncthreads();
     // ---- layer 1: acc1 = H * W1^T ---------------------------------------------------------------------------------------
-    if (tid == 0) {
+    if (warp == 0 && elect_one()) {
       tc_fence_after();
       issue_layer<PREC, KB>(h_addr, w1_addr, KB, D, tmem + D, idesc);
       umma_commit(bar_mma);
@@ -368,7 +368,7 @@ __global__ void __launch_bounds__(kUmmaThreads) embed_umma_kernel(EmbArgs a) {
       fence_proxy_async();
       tc_fence_before();
       __syncthreads();
-      if (tid == 0) {
+      if (warp == 0 && elect_one()) {
         tc_fence_after();
         issue_layer<PREC, KB>(a_addr, w_addr + l * (D * ROWB), ROWB, D, tmem, idesc_mid);
         umma_commit(bar_mma);
@@ -389,7 +389,7 @@ __global__ void __launch_bounds__(kUmmaThreads) embed_umma_kernel(EmbArgs a) {
     fence_proxy_async();
     tc_fence_before();
     __syncthreads();
-    if (tid == 0) {
+    if (warp == 0 && elect_one()) {
       tc_fence_after();
       issue_layer<PREC, KB>(a_addr, w_addr + n_mid * (D * ROWB), ROWB, 16, tmem + 128, idesc_out);
       umma_commit(bar_mma);

@@ -175,7 +175,7 @@ __global__ void __launch_bounds__(kWsThreads, 1) gnn_mlp_ws_kernel(GnnArgs a) {
     }
   } else if (warp == kMmaWarp) {
     // ================================================================================================ MMA issuer
-    if (lane == 0) {
+    if (elect_one()) {
       const uint32_t b0 = L0T ? (uint32_t)(nseg * D * KB) : 0u, b1 = (uint32_t)(D * KB);
       mbar_expect_tx(bar_w, b0 + b1);
       if (L0T) bulk_g2s(smem + L.w0, a.l0.Wtc, b0, bar_w);

@@ -32,6 +32,14 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
     if (!done && spins > (1u << 24)) __trap();       // never hang the GPU: a lost arrival becomes an error
   }
 }
+// one lane of the (converged) warp.  ptxas knows a region guarded by elect.sync runs single-threaded, so the
+// operands of the tcgen05 instructions inside it move to uniform registers without a per-instruction
+// ELECT / R2UR.BROADCAST loop (which `lane == 0` costs: ~75 cycles per MMA instead of a few)
+__device__ __forceinline__ bool elect_one() {
+  uint32_t p;
+  asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(p));
+  return p != 0;
+}
 __device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
