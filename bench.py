@@ -28,6 +28,9 @@ sys.path.insert(0, ROOT)
 
 import datagen  # noqa: E402
 
+# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel (S4e edge network) from the
+# `ncu --set full` capture summarised in profiles/r1e_edge_net_full.md, per workload; bench.py cannot run ncu itself.
+NCU_TRAFFIC_BYTES = {("cfg2", 500): 2.7036e9}
 METRIC = "events_per_s"
 UNIT = "events/s"
 DTYPE = {"fp32": "f32", "bf16": "bf16", "int8": "int8"}
@@ -271,7 +274,8 @@ def main():
     dom_bytes = model[dom][1] / L
     roofline = {"kernel": "edge network MLP (S4e), one launch per message-passing step", "bound": "hbm",
                 "achieved": dom_bytes / (dom_ms * 1e-3) / 1e9 if dom_ms > 0 else None, "peak": peaks["hbm"], "unit": "GB/s",
-                "frac": (dom_bytes / (dom_ms * 1e-3) / 1e9 / peaks["hbm"]) if dom_ms > 0 else None, "traffic": None,
+                "frac": (dom_bytes / (dom_ms * 1e-3) / 1e9 / peaks["hbm"]) if dom_ms > 0 else None,
+                "traffic": NCU_TRAFFIC_BYTES.get((cfg.name, cfg.n_events)),
                 "peak_source": peaks["source"], "avg_launch_ms": dom_ms, "algorithmic_bytes_per_launch": dom_bytes,
                 "share_of_step": stage_ms[dom] / (ms / args.steps) if ms > 0 else None}
     cpu_baseline = None

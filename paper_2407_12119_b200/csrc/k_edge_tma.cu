@@ -14,18 +14,25 @@
 //   * bias and residual are folded into the MMAs: acc0 = 1 * b0' + [h_src | h_dst | e] * W0^T and
 //     acc1 = 1 * b1' + hidden * W1^T + e * I, where b' is the fp32 bias split exactly into three bf16 terms and I
 //     is the identity (a bf16 value times 1.0 is exact in the fp32 accumulator).  The epilogues are then
-//     TMEM -> cvt(.relu).bf16x2 -> 16-byte shared-memory stores and nothing else;
-//   * the hidden activations overwrite the h_src segment of their gather slot (dead once layer 0 has finished),
-//     so no separate operand / staging buffers are needed.
+//     TMEM -> cvt(.relu).bf16x2 -> store and nothing else;
+//   * the hidden activations never touch shared memory: epilogue 0 writes them back to tensor memory (two bf16
+//     per 32-bit column, tcgen05.st) and layer 1 takes its A operand from there, so the gather slot is released
+//     as soon as layer 0 has finished;
+//   * every tcgen05.mma / commit is issued under elect.sync, which lets ptxas keep descriptors and tensor-memory
+//     addresses in uniform registers (with `lane == 0` each MMA cost an ELECT / R2UR.BROADCAST loop, ~75 cycles,
+//     and the issuing thread was the bottleneck: 22 MMAs per tile).
 //
 // Rounding points are those of DESIGN.md R20 (operands and stored state bf16 RNE, accumulation fp32); the order of
 // the fp32 additions inside the tensor core is not specified, which the bf16 tolerance covers.
 //
 // Warp roles (15 warps, one CTA per SM):
 //   0-7   epilogue, two warpgroups; warpgroup g owns the CTA's tiles it = g (mod 2)
-//   8-11  gather producers (cp.async)
-//   12    MMA issuer (one thread)
+//   8-10  gather producers (cp.async), one per slot of the gather ring; warp 11 only donates registers
+//   12    MMA issuer (one elected thread)
 //   13    TMA loader (one thread)       14    TMA storer (one thread)
+// mbarriers: self_full / self_empty / out_ready [kNE] (TMA load -> MMA, TMA store read -> loader, epilogue 1 ->
+// storer), aux_full / aux_empty [kNH] (gather -> MMA, tcgen05.commit after layer 0 -> gather), acc0_full /
+// hid_full / acc1_full [2] (commit -> epilogue 0, epilogue 0 -> MMA, commit -> epilogue 1).
 #include <cuda.h>
 #include <string.h>
 

@@ -299,7 +299,10 @@ __global__ void __launch_bounds__(256) scatter_kernel(const void* __restrict__ e
                                                       const int32_t* __restrict__ col_ptr, const int32_t* __restrict__ in_edge,
                                                       void* __restrict__ m, int n_hits) {
   constexpr int LPN = D / 4;                              // lanes per node
-  const int gid = blockIdx.x * (256 / LPN) + threadIdx.x / LPN;
+  // Nodes are walked from the last to the first: the edge network that ran just before wrote e in ascending
+  // order, so the tail of e is what the L2 still holds, and the next edge network starts at the head, which this
+  // pass reads last.
+  const int gid = (gridDim.x - 1 - blockIdx.x) * (256 / LPN) + threadIdx.x / LPN;
   const int c = (threadIdx.x % LPN) * 4;
   if (gid >= n_hits) return;
   float4 so = make_float4(0.f, 0.f, 0.f, 0.f), si = so;
