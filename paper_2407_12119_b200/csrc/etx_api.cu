@@ -220,6 +220,7 @@ etx_status run_impl(etx_ctx* c, const float* d_xyz, const int32_t* d_plane, cons
           const int L = c->hp.gnn_iters;
           auto mlp = [&](int kind, int it, bool head) {
             if (kind == kEdgeNet && c->edge_tma) launch_edge_net_tma(c, it, n_hits, head, s);
+            else if (kind == kEdgeEnc && c->edge_tma && c->hp.edge_enc_input == 0 && !head) launch_edge_enc_tma(c, n_hits, s);
             else if (tensor_engine && c->precision == ETX_BF16 && c->engine != ETX_ENGINE_TC_SERIAL) launch_gnn_mlp_ws(c, kind, it, n_hits, head, s);
             else if (tensor_engine) launch_gnn_mlp_umma(c, kind, it, n_hits, head, s);
             else launch_gnn_mlp_simt(c, kind, it, n_hits, head, s);

@@ -97,6 +97,7 @@ struct etx_ctx {
   // k_edge_tma.cu: identity operand image, split-bias images [2 * iter + layer], CUtensorMap of `e` (opaque here)
   bool edge_tma = false;
   void* ident_img = nullptr;
+  void* eenc_b1_img = nullptr;
   std::vector<void*> edge_bias_img;
   alignas(64) unsigned char e_map[128] = {};
   int32_t* tap = nullptr;
@@ -150,5 +151,6 @@ void launch_gnn_mlp_ws(etx_ctx* c, int kind, int iter, int n_hits, bool do_head,
 // k_edge_tma.cu (bf16: the edge network with TMA-moved edge state, bias and residual inside the MMAs)
 bool edge_tma_configure(etx_ctx* c);
 void launch_edge_net_tma(etx_ctx* c, int iter, int n_hits, bool do_head, cudaStream_t s);
+void launch_edge_enc_tma(etx_ctx* c, int n_hits, cudaStream_t s);
 
 }  // namespace etx

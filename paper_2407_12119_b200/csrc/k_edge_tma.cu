@@ -446,6 +446,202 @@ edge_net_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeTmaArgs
   if (warp == kMmaWarp) tmem_dealloc(tmem, TMEM_COLS);
 }
 
+// ---------------------------------------------------------------------------------------------- S4b edge encoder
+// e0 = W1 relu(W0 |f_dst - f_src| + b0) + b1  (PAPER.md L133 with the configs' K = 3 input, R10 / R11).
+// The stage only WRITES the edge state (E * d * 2 bytes), so it is bound by that write plus the FFMA work of the
+// K = 3 layer, which stays on the fp32 pipe in the pinned order (R3, R20).  Four warpgroups each own the CTA's
+// tiles it = w (mod 4) from front to back: gather the two feature rows (prefetched one tile ahead, their indices
+// two tiles ahead), layer 0 on the FFMA pipe, relu -> bf16 -> tensor memory (the A operand of layer 1), wait for
+// the MMA, TMEM -> bf16 -> the warpgroup's swizzled shared-memory slot, and one TMA store per tile.
+constexpr int kEncGroups = 4;
+constexpr int kEncMmaWarp = kEncGroups * 4, kEncStoreWarp = kEncMmaWarp + 1;
+constexpr int kEncThreads = (kEncStoreWarp + 1) * 32;      // 576
+
+struct EncSmem { int out, w1, ones, b1, w3, bar, total; };
+template <int D>
+__host__ __device__ constexpr EncSmem enc_layout() {
+  constexpr int KB = D * 2, BLK = kRows * KB;
+  EncSmem s{};
+  s.out = 0;                           // kEncGroups x [128][KB] output staging
+  s.w1 = s.out + kEncGroups * BLK;     // W1 image [D][KB]
+  s.ones = s.w1 + D * KB;              // [128][32 B]
+  s.b1 = s.ones + kRows * 32;          // [D][32 B] split bias of layer 1
+  s.w3 = s.b1 + D * 32;                // fp32: W0^T [3][D], b0 [D]
+  s.bar = s.w3 + 4 * D * 4;
+  s.total = s.bar + 256;
+  return s;
+}
+
+struct EdgeEncArgs {
+  const void* w1_img; const void* b1_img;
+  const float* w0t;          // [3][D] fp32 (W0 transposed)
+  const float* b0;           // [D]
+  const float4* feat;
+  const int32_t* src; const int32_t* dst;
+  const int32_t* n_rows_ptr;
+};
+
+template <int D>
+__global__ void __launch_bounds__(kEncThreads, 1)
+edge_enc_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeEncArgs a) {
+  constexpr int KB = D * 2, BLK = kRows * KB;
+  constexpr EncSmem L = enc_layout<D>();
+  constexpr uint32_t TMEM_COLS = 8 * D;                      // acc[4] (D each) | hidden[4] (D/2 each), pow2
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+  float* w3 = reinterpret_cast<float*>(smem + L.w3);         // [0..3D) W0^T, [3D..4D) b0
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + L.bar);
+  uint64_t *hid_full = bars, *acc_full = bars + kEncGroups, *out_ready = bars + 2 * kEncGroups,
+           *slot_free = bars + 3 * kEncGroups, *bar_w = bars + 4 * kEncGroups;
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bar_w + 1);
+
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int n_rows = *a.n_rows_ptr;
+  const int n_tiles = (n_rows + kRows - 1) / kRows;
+
+  if (tid == 0) {
+    for (int g = 0; g < kEncGroups; ++g) {
+      mbar_init(&hid_full[g], 128); mbar_init(&acc_full[g], 1); mbar_init(&out_ready[g], 128); mbar_init(&slot_free[g], 1);
+    }
+    mbar_init(bar_w, 1);
+    fence_barrier_init();
+  }
+  if (warp == kEncMmaWarp) tmem_alloc(tmem_slot, TMEM_COLS);
+  for (int i = tid; i < 3 * D; i += kEncThreads) w3[i] = a.w0t[i];
+  for (int i = tid; i < D; i += kEncThreads) w3[3 * D + i] = a.b0[i];
+  for (int r = tid; r < kRows; r += kEncThreads) {
+    uint4* row = reinterpret_cast<uint4*>(smem + L.ones + r * 32);
+    row[0] = make_uint4(0u, 0u, 0u, 0u); row[1] = make_uint4(0u, 0u, 0u, 0u);
+    *reinterpret_cast<uint4*>(smem + L.ones + swz<32>(r, 0)) = make_uint4(0x3f803f80u, 0x00003f80u, 0u, 0u);
+  }
+  fence_proxy_async();
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = *tmem_slot;
+  const uint32_t out_addr = smem_u32(smem + L.out);
+
+  if (warp == kEncStoreWarp) {
+    // ================================================================================================ TMA stores
+    if (lane == 0) {
+      int it = 0;
+      for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
+        const int g = it % kEncGroups;
+        mbar_wait(&out_ready[g], (it / kEncGroups) & 1);
+        tma_store_2d(&e_map, out_addr + g * BLK, 0, tile * kRows);
+        bulk_commit();
+        bulk_wait_read0();
+        mbar_arrive(&slot_free[g]);
+      }
+      bulk_wait0();
+    }
+  } else if (warp == kEncMmaWarp) {
+    // ================================================================================================ MMA issuer
+    if (elect_one()) {
+      const uint32_t wb1 = D * KB, bb = D * 32;
+      mbar_expect_tx(bar_w, wb1 + bb);
+      bulk_g2s(smem + L.w1, a.w1_img, wb1, bar_w);
+      bulk_g2s(smem + L.b1, a.b1_img, bb, bar_w);
+      mbar_wait(bar_w, 0);
+      const uint32_t idesc = make_idesc<kBf16>(D);
+      const uint32_t w1_addr = smem_u32(smem + L.w1);
+      const uint64_t ones_desc = make_desc<32>(smem_u32(smem + L.ones)), b1_desc = make_desc<32>(smem_u32(smem + L.b1));
+      int it = 0;
+      for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
+        const int g = it % kEncGroups;
+        mbar_wait(&hid_full[g], (it / kEncGroups) & 1);       // also: the group has drained acc[g] of its last tile
+        tc_fence_after();
+        const uint32_t d1 = tmem + g * D, hid = tmem + kEncGroups * D + g * (D / 2);
+        umma::umma<kBf16>(d1, ones_desc, b1_desc, idesc, 0u);
+#pragma unroll
+        for (int k = 0; k < D / 16; ++k) umma_ts(d1, hid + 8 * k, make_desc<KB>(w1_addr + k * 32), idesc, 1u);
+        umma_commit(&acc_full[g]);
+      }
+    }
+  } else {
+    // ================================================================================================ compute groups
+    const int g = warp >> 2, q = warp & 3;
+    const int r = q * 32 + lane;                              // row of the tile owned by this thread
+    const uint32_t lane_base = (uint32_t)(q * 32) << 16;
+    uint8_t* out = smem + L.out + g * BLK;
+    auto tile_of = [&](int j) { return blockIdx.x + (long long)(g + j * kEncGroups) * gridDim.x; };
+    auto load_idx = [&](int j, int& is, int& id) {
+      const long long t = tile_of(j);
+      is = 0; id = 0;
+      if (t < n_tiles) {
+        long long row = t * kRows + r;
+        if (row >= n_rows) row = n_rows - 1;
+        is = __ldg(a.src + row); id = __ldg(a.dst + row);
+      }
+    };
+    int is_n, id_n;                                           // indices of tile j + 1
+    float4 fs, fd;                                            // features of tile j
+    {
+      int is0, id0;
+      load_idx(0, is0, id0);
+      load_idx(1, is_n, id_n);
+      fs = __ldg(a.feat + is0); fd = __ldg(a.feat + id0);
+    }
+    for (int j = 0; tile_of(j) < n_tiles; ++j) {
+      const long long tile = tile_of(j);
+      // R11: component-wise |f_dst - f_src| of the normalised features
+      const float fx = fabsf(__fsub_rn(fd.x, fs.x)), fy = fabsf(__fsub_rn(fd.y, fs.y)), fz = fabsf(__fsub_rn(fd.z, fs.z));
+      // prefetch: features of tile j + 1 (their indices are here), indices of tile j + 2
+      fs = __ldg(a.feat + is_n); fd = __ldg(a.feat + id_n);
+      load_idx(j + 2, is_n, id_n);
+      // ---- layer 0 on the FFMA pipe, pinned order (R3); relu -> bf16 -> tensor memory
+#pragma unroll
+      for (int c0 = 0; c0 < D; c0 += 64) {
+        uint32_t pk[32];
+#pragma unroll
+        for (int i = 0; i < (D > 32 ? 32 : 16); ++i) {
+          float y[2];
+#pragma unroll
+          for (int h = 0; h < 2; ++h) {
+            const int c = c0 + 2 * i + h;
+            float acc = __fmaf_rn(fx, w3[c], 0.0f);
+            acc = __fmaf_rn(fy, w3[D + c], acc);
+            acc = __fmaf_rn(fz, w3[2 * D + c], acc);
+            y[h] = __fadd_rn(acc, w3[3 * D + c]);
+          }
+          pk[i] = pack_bf16x2_relu(y[0], y[1]);
+        }
+        if (D > 32) tmem_st32(tmem + lane_base + kEncGroups * D + g * (D / 2) + c0 / 2, pk);
+        else tmem_st16(tmem + lane_base + kEncGroups * D + g * (D / 2), pk);
+      }
+      tmem_st_wait();
+      tc_fence_before();
+      mbar_arrive(&hid_full[g]);
+      // ---- layer 1 result (bias already inside): TMEM -> bf16 -> the group's slot -> TMA store (R20)
+      mbar_wait(&slot_free[g], (j & 1) ^ 1);                  // the store of tile j - 1 has read the slot
+      mbar_wait(&acc_full[g], j & 1);
+      tc_fence_after();
+#pragma unroll
+      for (int c0 = 0; c0 < D; c0 += 32) {
+        uint32_t v[32];
+        tmem_ld32_nowait(tmem + lane_base + g * D + c0, v);
+        tmem_ld_wait();
+#pragma unroll
+        for (int ch = 0; ch < 4; ++ch) {
+          uint4 qv;
+          qv.x = pack_bf16x2(__uint_as_float(v[ch * 8 + 0]), __uint_as_float(v[ch * 8 + 1]));
+          qv.y = pack_bf16x2(__uint_as_float(v[ch * 8 + 2]), __uint_as_float(v[ch * 8 + 3]));
+          qv.z = pack_bf16x2(__uint_as_float(v[ch * 8 + 4]), __uint_as_float(v[ch * 8 + 5]));
+          qv.w = pack_bf16x2(__uint_as_float(v[ch * 8 + 6]), __uint_as_float(v[ch * 8 + 7]));
+          *reinterpret_cast<uint4*>(out + swz<KB>(r, c0 / 8 + ch)) = qv;
+        }
+      }
+      tc_fence_before();
+      fence_proxy_async();
+      mbar_arrive(&out_ready[g]);
+      (void)tile;
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == kEncMmaWarp) tmem_dealloc(tmem, TMEM_COLS);
+}
+
 // ---------------------------------------------------------------------------------------------- host side
 uint16_t bf16_bits_rne(float x) {
   const __nv_bfloat16 b = __float2bfloat16_rn(x);
@@ -510,6 +706,21 @@ void edge_tma_launch(etx_ctx* c, const EdgeTmaArgs& a, int max_rows, cudaStream_
   c->launches++;
 }
 
+template <int D>
+void edge_enc_launch(etx_ctx* c, const EdgeEncArgs& a, int max_rows, cudaStream_t s) {
+  auto kern = edge_enc_tma_kernel<D>;
+  constexpr int smem = enc_layout<D>().total + 1024;
+  static bool configured = false;
+  if (!configured) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); configured = true; }
+  const int tiles = (max_rows + kRows - 1) / kRows;
+  const int grid = tiles < c->sm_count ? tiles : c->sm_count;     // one persistent CTA per SM (512 TMEM columns)
+  if (grid <= 0) return;
+  CUtensorMap map;
+  memcpy(&map, c->e_map, sizeof(map));
+  kern<<<grid, kEncThreads, smem, s>>>(map, a);
+  c->launches++;
+}
+
 }  // namespace
 
 // bf16 mode, tensor engine: per-step bias / identity images and the tensor map of the edge state
@@ -525,6 +736,8 @@ bool edge_tma_configure(etx_ctx* c) {
       if (!p) return false;
       c->edge_bias_img[2 * it + l] = p;
     }
+  c->eenc_b1_img = upload_bytes(c, pack_split_rows(c->layers[c->i_eenc + 1].b));
+  if (!c->eenc_b1_img) return false;
   void* fn = nullptr;
   cudaDriverEntryPointQueryResult qres;
   if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn) return false;
@@ -556,6 +769,19 @@ void launch_edge_net_tma(etx_ctx* c, int iter, int n_hits, bool do_head, cudaStr
   const int max_rows = (int)(max_rows_ll > 0x7fffffff ? 0x7fffffff : max_rows_ll);
   if (c->hp.gnn_latent == 32) edge_tma_launch<32>(c, a, max_rows, s);
   else edge_tma_launch<64>(c, a, max_rows, s);
+}
+
+// S4b with the configs' K = 3 edge-encoder input (edge_enc_input == 0)
+void launch_edge_enc_tma(etx_ctx* c, int n_hits, cudaStream_t s) {
+  const int i0 = c->i_eenc;
+  EdgeEncArgs a;
+  a.w1_img = c->layers[i0 + 1].dev.Wtc; a.b1_img = c->eenc_b1_img;
+  a.w0t = c->layers[i0].dev.Wt; a.b0 = c->layers[i0].dev.bias;
+  a.feat = c->feat; a.src = c->src; a.dst = c->dst; a.n_rows_ptr = c->n_edges;
+  const long long max_rows_ll = (long long)n_hits * c->hp.k;
+  const int max_rows = (int)(max_rows_ll > 0x7fffffff ? 0x7fffffff : max_rows_ll);
+  if (c->hp.gnn_latent == 32) edge_enc_launch<32>(c, a, max_rows, s);
+  else edge_enc_launch<64>(c, a, max_rows, s);
 }
 
 }  // namespace etx
