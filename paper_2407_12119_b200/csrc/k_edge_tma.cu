@@ -474,8 +474,8 @@ __host__ __device__ constexpr EncSmem enc_layout() {
 
 struct EdgeEncArgs {
   const void* w1_img; const void* b1_img;
-  const float* w0t;          // [3][D] fp32 (W0 transposed)
-  const float* b0;           // [D]
+  float w0t[3 * 64];         // [3][D] fp32 (W0 transposed) and b0[D], passed BY VALUE: kernel parameters live in the
+  float b0[64];              // constant bank, so the FFMAs of layer 0 take them as operands without any load
   const float4* feat;
   const int32_t* src; const int32_t* dst;
   const int32_t* n_rows_ptr;
@@ -489,7 +489,6 @@ edge_enc_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeEncArgs
   constexpr uint32_t TMEM_COLS = 8 * D;                      // acc[4] (D each) | hidden[4] (D/2 each), pow2
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
-  float* w3 = reinterpret_cast<float*>(smem + L.w3);         // [0..3D) W0^T, [3D..4D) b0
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + L.bar);
   uint64_t *hid_full = bars, *acc_full = bars + kEncGroups, *out_ready = bars + 2 * kEncGroups,
            *slot_free = bars + 3 * kEncGroups, *bar_w = bars + 4 * kEncGroups;
@@ -507,8 +506,6 @@ edge_enc_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeEncArgs
     fence_barrier_init();
   }
   if (warp == kEncMmaWarp) tmem_alloc(tmem_slot, TMEM_COLS);
-  for (int i = tid; i < 3 * D; i += kEncThreads) w3[i] = a.w0t[i];
-  for (int i = tid; i < D; i += kEncThreads) w3[3 * D + i] = a.b0[i];
   for (int r = tid; r < kRows; r += kEncThreads) {
     uint4* row = reinterpret_cast<uint4*>(smem + L.ones + r * 32);
     row[0] = make_uint4(0u, 0u, 0u, 0u); row[1] = make_uint4(0u, 0u, 0u, 0u);
@@ -582,13 +579,16 @@ edge_enc_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeEncArgs
       load_idx(1, is_n, id_n);
       fs = __ldg(a.feat + is0); fd = __ldg(a.feat + id0);
     }
+    PROF_DECL
     for (int j = 0; tile_of(j) < n_tiles; ++j) {
       const long long tile = tile_of(j);
+      PROF(0)
       // R11: component-wise |f_dst - f_src| of the normalised features
       const float fx = fabsf(__fsub_rn(fd.x, fs.x)), fy = fabsf(__fsub_rn(fd.y, fs.y)), fz = fabsf(__fsub_rn(fd.z, fs.z));
       // prefetch: features of tile j + 1 (their indices are here), indices of tile j + 2
       fs = __ldg(a.feat + is_n); fd = __ldg(a.feat + id_n);
       load_idx(j + 2, is_n, id_n);
+      PROF(1)
       // ---- layer 0 on the FFMA pipe, pinned order (R3); relu -> bf16 -> tensor memory
 #pragma unroll
       for (int c0 = 0; c0 < D; c0 += 64) {
@@ -599,10 +599,10 @@ edge_enc_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeEncArgs
 #pragma unroll
           for (int h = 0; h < 2; ++h) {
             const int c = c0 + 2 * i + h;
-            float acc = __fmaf_rn(fx, w3[c], 0.0f);
-            acc = __fmaf_rn(fy, w3[D + c], acc);
-            acc = __fmaf_rn(fz, w3[2 * D + c], acc);
-            y[h] = __fadd_rn(acc, w3[3 * D + c]);
+            float acc = __fmaf_rn(fx, a.w0t[c], 0.0f);
+            acc = __fmaf_rn(fy, a.w0t[D + c], acc);
+            acc = __fmaf_rn(fz, a.w0t[2 * D + c], acc);
+            y[h] = __fadd_rn(acc, a.b0[c]);
           }
           pk[i] = pack_bf16x2_relu(y[0], y[1]);
         }
@@ -612,9 +612,11 @@ edge_enc_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeEncArgs
       tmem_st_wait();
       tc_fence_before();
       mbar_arrive(&hid_full[g]);
+      PROF(2)
       // ---- layer 1 result (bias already inside): TMEM -> bf16 -> the group's slot -> TMA store (R20)
       mbar_wait(&slot_free[g], (j & 1) ^ 1);                  // the store of tile j - 1 has read the slot
       mbar_wait(&acc_full[g], j & 1);
+      PROF(3)
       tc_fence_after();
 #pragma unroll
       for (int c0 = 0; c0 < D; c0 += 32) {
@@ -635,7 +637,9 @@ edge_enc_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeEncArgs
       fence_proxy_async();
       mbar_arrive(&out_ready[g]);
       (void)tile;
+      PROF(4)
     }
+    PROF_OUT("enc[tail,feat,ffma,wait_acc,epi]")
   }
   tc_fence_before();
   __syncthreads();
@@ -776,7 +780,11 @@ void launch_edge_enc_tma(etx_ctx* c, int n_hits, cudaStream_t s) {
   const int i0 = c->i_eenc;
   EdgeEncArgs a;
   a.w1_img = c->layers[i0 + 1].dev.Wtc; a.b1_img = c->eenc_b1_img;
-  a.w0t = c->layers[i0].dev.Wt; a.b0 = c->layers[i0].dev.bias;
+  const int D = c->hp.gnn_latent;                            // 32 or 64 (umma_supported)
+  for (int n = 0; n < D; ++n) {
+    for (int k = 0; k < 3; ++k) a.w0t[k * D + n] = c->layers[i0].W[(size_t)n * 3 + k];
+    a.b0[n] = c->layers[i0].b[n];
+  }
   a.feat = c->feat; a.src = c->src; a.dst = c->dst; a.n_rows_ptr = c->n_edges;
   const long long max_rows_ll = (long long)n_hits * c->hp.k;
   const int max_rows = (int)(max_rows_ll > 0x7fffffff ? 0x7fffffff : max_rows_ll);
