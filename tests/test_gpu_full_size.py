@@ -1,0 +1,138 @@
+"""GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times (engine auto, the
+whole batch in one etx_run).  The oracle cannot recompute a 500-event batch in seconds, so (DESIGN.md sec. 6,
+"Full size"): properties that hold at any size are checked on the whole output, and a sample of events --
+first, last, largest, smallest non-empty, a few seeded random ones -- is recomputed by the oracle one by one.
+Events are independent in every stage, so an event cut out of the batch is a valid oracle
+input on its own; edges and track ids are compared after rebasing hit indices."""
+import numpy as np
+import pytest
+import torch
+
+import datagen
+import oracle
+from gpu_utils import make_ctx, run_gpu
+from helpers import centred_parity_weights, check_edge_invariants, check_track_invariants
+
+pytestmark = pytest.mark.gpu
+
+
+def _sample_events(b, n_random=3, seed=5):
+    sizes = np.diff(b.event_offsets)
+    nz = np.flatnonzero(sizes > 0)
+    pick = {0, b.n_events - 1, int(np.argmax(sizes)), int(nz[np.argmin(sizes[nz])])}
+    rng = np.random.default_rng(seed)
+    pick.update(int(x) for x in rng.integers(0, b.n_events, n_random))
+    return sorted(pick)
+
+
+def _check_sampled_events(cfg, b, g, blob, precision, events, score_tol=None, logit_rel=None):
+    o = oracle.Oracle(blob, precision)
+    tau = oracle.logit_threshold(cfg.threshold)
+    eo, rp = b.event_offsets, g["row_ptr"]
+    worst = 0.0
+    for ev in events:
+        h0, h1 = int(eo[ev]), int(eo[ev + 1])
+        e0, e1 = int(rp[h0]), int(rp[h1])
+        sub = b.slice_events(ev, ev + 1)
+        # chained: oracle S2 + S3 on the GPU's own embedding of this event == the GPU's edges (bit-exact)
+        nbr, deg = oracle.knn(g["emb"][h0:h1], sub.plane, sub.event_offsets, cfg.k, cfg.window, cfg.d2_max)
+        src, dst, _ = oracle.build_edges(nbr, deg)
+        assert src.size == e1 - e0, (ev, src.size, e1 - e0)
+        assert np.array_equal(g["src"][e0:e1] - h0, src) and np.array_equal(g["dst"][e0:e1] - h0, dst), ev
+        # S4 on those edges: scores / logits within the bar
+        og = o.gnn(sub.xyz, src, dst)
+        if score_tol is not None and src.size:
+            err = float(np.abs(g["score"][e0:e1] - og["score"]).max())
+            worst = max(worst, err)
+            assert err <= score_tol, (ev, err)
+        if logit_rel is not None and src.size:
+            scale = float(np.abs(og["logit"]).max())
+            assert np.isfinite(g["logit"][e0:e1]).all()
+            assert np.abs(g["logit"][e0:e1] - og["logit"]).max() <= logit_rel * max(scale, 1.0), ev
+        # chained: oracle S5 on the GPU's own logits == the GPU's track ids (bit-exact)
+        tid = oracle.components(src, dst, g["logit"][e0:e1], tau, h1 - h0)
+        assert np.array_equal(g["track_id"][h0:h1] - h0, tid), ev
+    return worst
+
+
+def _whole_batch_invariants(cfg, b, g):
+    assert g["n_edges"] == g["src"].size == g["row_ptr"][-1]
+    check_edge_invariants(g["src"], g["dst"], g["row_ptr"], b.plane, b.event_offsets, cfg.k, cfg.window)
+    keep = g["logit"] >= oracle.logit_threshold(cfg.threshold)
+    check_track_invariants(g["track_id"], g["src"], g["dst"], keep, b.event_offsets)
+    assert np.isfinite(g["score"]).all() and (g["score"] >= 0).all() and (g["score"] <= 1).all()
+    # CSC: a permutation of the edge ids, grouped by dst, ascending inside every group (R9, R22)
+    ie, cp = g["in_edge"], g["col_ptr"]
+    assert np.array_equal(np.sort(ie), np.arange(ie.size, dtype=ie.dtype))
+    assert np.array_equal(np.repeat(np.arange(b.n_hits), np.diff(cp)), g["dst"][ie])
+    inner = np.ones(ie.size, bool); inner[cp[:-1][np.diff(cp) > 0]] = False
+    assert (np.diff(ie)[inner[1:]] > 0).all()
+
+
+@pytest.mark.parametrize("name,preset", [("cfg2", "he"), ("cfg2", "parity"), ("cfg4", "parity")])
+def test_full_size_bf16_invariants_and_sampled_events(name, preset):
+    cfg = datagen.get_config(name)                              # bf16, 500 / 200 events: the bench configuration
+    b = datagen.generate_batch(cfg)
+    if preset == "he":
+        W = datagen.make_weights(cfg, "he")                     # BASELINE.json: what bench.py times
+    else:
+        W = centred_parity_weights(cfg, b.slice_events(0, 2))   # logits O(1): score parity is informative
+    blob = datagen.pack_blob(cfg, W)
+    ctx = make_ctx(cfg, blob, b)
+    g = run_gpu(ctx, b, debug=False)
+    torch.cuda.synchronize()
+    _whole_batch_invariants(cfg, b, g)
+    events = _sample_events(b, n_random=3 if name == "cfg2" else 1)
+    if name == "cfg4":
+        events = events[:3]                                     # ~9,000-hit events: the oracle takes seconds each
+    if preset == "he":
+        worst = _check_sampled_events(cfg, b, g, blob, "bf16", events, logit_rel=0.05)
+    else:
+        worst = _check_sampled_events(cfg, b, g, blob, "bf16", events, score_tol=2e-2)
+        mid = np.mean((g["score"] > 0.01) & (g["score"] < 0.99))
+        assert mid > 0.3, mid
+    print(f"{name}/{preset}: N={b.n_hits} E={g['n_edges']} sampled events {events} max|score err|={worst:.2e}")
+    ctx.destroy()
+
+
+def test_full_size_fp32_cfg1_end_to_end_sampled_events():
+    cfg = datagen.get_config("cfg1")                            # 64 events, fp32 throughout
+    b = datagen.generate_batch(cfg)
+    W = centred_parity_weights(cfg, b.slice_events(0, 2))
+    blob = datagen.pack_blob(cfg, W)
+    ctx = make_ctx(cfg, blob, b)
+    g = run_gpu(ctx, b, debug=False)
+    _whole_batch_invariants(cfg, b, g)
+    worst = _check_sampled_events(cfg, b, g, blob, "fp32", _sample_events(b, 2), score_tol=1e-4)
+    print(f"cfg1/fp32: N={b.n_hits} E={g['n_edges']} max|score err|={worst:.2e}")
+    ctx.destroy()
+
+
+def test_full_size_int8_cfg3_bit_exact_on_sampled_events():
+    # 1000 events, INT8 MLPs (R21): integer accumulation is order-free and every other op is a single pinned fp32
+    # op, so on sampled events the embedding, the edges, the logits and the track ids must equal the oracle's bits
+    cfg = datagen.get_config("cfg3")
+    b = datagen.generate_batch(cfg)
+    W = centred_parity_weights(cfg.replace(precision="fp32"), b.slice_events(0, 2))
+    cal = datagen.generate_batch(datagen.get_config("cfg1"), n_events=datagen.configs.CALIBRATION_EVENTS,
+                                 seed=datagen.configs.CALIBRATION_SEED)
+    scales = oracle.calibrate_int8(datagen.pack_blob(cfg, W), cal.xyz, cal.plane, cal.event_offsets, cfg.k, cfg.window)
+    blob = datagen.pack_blob(cfg, W, scales)
+    ctx = make_ctx(cfg, blob, b)
+    g = run_gpu(ctx, b, debug=False)
+    _whole_batch_invariants(cfg, b, g)
+    o = oracle.Oracle(blob, "int8")
+    eo, rp = b.event_offsets, g["row_ptr"]
+    events = _sample_events(b, n_random=2)
+    for ev in events:
+        h0, h1 = int(eo[ev]), int(eo[ev + 1])
+        e0, e1 = int(rp[h0]), int(rp[h1])
+        sub = b.slice_events(ev, ev + 1)
+        r = o.run(sub.xyz, sub.plane, sub.event_offsets, cfg.k, cfg.window, cfg.d2_max, cfg.threshold)
+        assert np.array_equal(g["emb"][h0:h1], r["emb"]), ev
+        assert np.array_equal(g["src"][e0:e1] - h0, r["src"]) and np.array_equal(g["dst"][e0:e1] - h0, r["dst"]), ev
+        assert np.array_equal(g["logit"][e0:e1], r["logit"]), ev
+        assert np.abs(g["score"][e0:e1] - r["score"]).max(initial=0.0) <= 1e-4
+        assert np.array_equal(g["track_id"][h0:h1] - h0, r["track_id"]), ev
+    print(f"cfg3/int8: N={b.n_hits} E={g['n_edges']} sampled events {events} bit-exact")
+    ctx.destroy()
