@@ -175,6 +175,7 @@ etx_status run_impl(etx_ctx* c, const float* d_xyz, const int32_t* d_plane, cons
     c->n_ev = 0; c->spans.clear();
     c->last_n_hits = n_hits;
     StageTimer tm{c, s};
+    bool edges_marked = false;
     const bool tensor_engine = (c->precision != ETX_FP32) && c->engine != ETX_ENGINE_SIMT;
     if (n_hits > 0) {
       // ---- S0
@@ -206,6 +207,11 @@ etx_status run_impl(etx_ctx* c, const float* d_xyz, const int32_t* d_plane, cons
           tm.begin(3);
           launch_pack_edges(c, n_hits, s);
         }
+        // E and the edge list are final here: mirror E to the host and mark the point (etx_run_host starts the
+        // D2H copy of src / dst on its copy stream from this event, under the GNN)
+        ETX_CUDA(cudaMemcpyAsync(c->h_n_edges, c->n_edges, sizeof(int32_t), cudaMemcpyDeviceToHost, s));
+        ETX_CUDA(cudaEventRecord(c->edges_ready, s));
+        edges_marked = true;
         if (last >= 3) launch_csc(c, n_hits, s);
         tm.end();
       }
@@ -242,7 +248,10 @@ etx_status run_impl(etx_ctx* c, const float* d_xyz, const int32_t* d_plane, cons
         tm.end();
       }
     }
-    ETX_CUDA(cudaMemcpyAsync(c->h_n_edges, c->n_edges, sizeof(int32_t), cudaMemcpyDeviceToHost, s));
+    if (!edges_marked) {
+      ETX_CUDA(cudaMemcpyAsync(c->h_n_edges, c->n_edges, sizeof(int32_t), cudaMemcpyDeviceToHost, s));
+      ETX_CUDA(cudaEventRecord(c->edges_ready, s));
+    }
     if (c->hp.validate_input) {
       ETX_CUDA(cudaMemcpyAsync(c->h_flags, c->flags, sizeof(int32_t), cudaMemcpyDeviceToHost, s));
       ETX_CUDA(cudaMemsetAsync(c->flags, 0, sizeof(int32_t), s));
@@ -323,6 +332,9 @@ etx_status etx_create(const void* blob, size_t blob_bytes, const etx_hyperparams
     ETX_CUDA(cudaMallocHost(&c->h_flags, sizeof(int32_t)));
     c->h_n_edges[0] = 0; c->h_flags[0] = 0;
     ETX_CUDA(cudaEventCreateWithFlags(&c->staging_free, cudaEventDisableTiming));
+    ETX_CUDA(cudaEventCreateWithFlags(&c->edges_ready, cudaEventDisableTiming));
+    ETX_CUDA(cudaEventCreateWithFlags(&c->copies_done, cudaEventDisableTiming));
+    ETX_CUDA(cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
     for (int i = 0; i < 256; ++i) ETX_CUDA(cudaEventCreate(&c->ev[i]));
     simt_configure(c);
     if (c->precision != ETX_FP32 && c->engine != ETX_ENGINE_SIMT) {
@@ -351,6 +363,9 @@ etx_status etx_destroy(etx_handle c) {
   if (c->h_n_edges) cudaFreeHost(c->h_n_edges);
   if (c->h_flags) cudaFreeHost(c->h_flags);
   if (c->staging_free) cudaEventDestroy(c->staging_free);
+  if (c->edges_ready) cudaEventDestroy(c->edges_ready);
+  if (c->copies_done) cudaEventDestroy(c->copies_done);
+  if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
   for (int i = 0; i < 256; ++i) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
   delete c;
   return ETX_OK;
@@ -384,17 +399,21 @@ etx_status etx_run_host(etx_handle c, const float* h_xyz, const int32_t* h_plane
     etx_output o;
     etx_status st = run_impl(c, c->d_xyz_in, c->d_plane_in, h_event_offsets, n_events, s, nullptr, &o);
     if (st != ETX_OK) return st;
-    if (h_track_id && n_hits > 0)
-      ETX_CUDA(cudaMemcpyAsync(h_track_id, c->track_id, sizeof(int32_t) * (size_t)n_hits, cudaMemcpyDeviceToHost, s));
-    ETX_CUDA(cudaStreamSynchronize(s));            // E is needed on the host to size the edge copies
+    // src / dst are final after S3: their D2H copy runs on the copy stream while the GNN is still computing
+    ETX_CUDA(cudaEventSynchronize(c->edges_ready));
     const int E = c->h_n_edges[0];
     *n_edges_out = E;
-    if (E > 0) {
-      if (h_edge_score) ETX_CUDA(cudaMemcpyAsync(h_edge_score, c->score, sizeof(float) * (size_t)E, cudaMemcpyDeviceToHost, s));
-      if (h_edge_src) ETX_CUDA(cudaMemcpyAsync(h_edge_src, c->src, sizeof(int32_t) * (size_t)E, cudaMemcpyDeviceToHost, s));
-      if (h_edge_dst) ETX_CUDA(cudaMemcpyAsync(h_edge_dst, c->dst, sizeof(int32_t) * (size_t)E, cudaMemcpyDeviceToHost, s));
-      ETX_CUDA(cudaStreamSynchronize(s));
+    if (E > 0 && (h_edge_src || h_edge_dst)) {
+      ETX_CUDA(cudaStreamWaitEvent(c->copy_stream, c->edges_ready, 0));
+      if (h_edge_src) ETX_CUDA(cudaMemcpyAsync(h_edge_src, c->src, sizeof(int32_t) * (size_t)E, cudaMemcpyDeviceToHost, c->copy_stream));
+      if (h_edge_dst) ETX_CUDA(cudaMemcpyAsync(h_edge_dst, c->dst, sizeof(int32_t) * (size_t)E, cudaMemcpyDeviceToHost, c->copy_stream));
+      ETX_CUDA(cudaEventRecord(c->copies_done, c->copy_stream));
+      ETX_CUDA(cudaStreamWaitEvent(s, c->copies_done, 0));      // the caller's stream stays the single point to wait on
     }
+    if (h_track_id && n_hits > 0)
+      ETX_CUDA(cudaMemcpyAsync(h_track_id, c->track_id, sizeof(int32_t) * (size_t)n_hits, cudaMemcpyDeviceToHost, s));
+    if (E > 0 && h_edge_score) ETX_CUDA(cudaMemcpyAsync(h_edge_score, c->score, sizeof(float) * (size_t)E, cudaMemcpyDeviceToHost, s));
+    ETX_CUDA(cudaStreamSynchronize(s));
   } catch (const CudaFail& f) {
     return fail(c, ETX_ERR_CUDA, std::string(f.what) + ": " + cudaGetErrorString(f.err));
   }

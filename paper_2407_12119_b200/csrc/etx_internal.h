@@ -108,6 +108,8 @@ struct etx_ctx {
   int32_t* h_n_edges = nullptr;           // pinned mirror
   int32_t* h_flags = nullptr;             // pinned mirror
   cudaEvent_t staging_free = nullptr;
+  cudaEvent_t edges_ready = nullptr, copies_done = nullptr;   // etx_run_host: src / dst D2H under the GNN
+  cudaStream_t copy_stream = nullptr;
   // staging for etx_run_host
   float* d_xyz_in = nullptr;
   int32_t* d_plane_in = nullptr;
