@@ -212,7 +212,7 @@ etx_status run_impl(etx_ctx* c, const float* d_xyz, const int32_t* d_plane, cons
         ETX_CUDA(cudaMemcpyAsync(c->h_n_edges, c->n_edges, sizeof(int32_t), cudaMemcpyDeviceToHost, s));
         ETX_CUDA(cudaEventRecord(c->edges_ready, s));
         edges_marked = true;
-        if (last >= 3) launch_csc(c, n_hits, s);
+        if (last >= 3) launch_csc(c, n_events, n_hits, !(inj && inj->d_src), s);
         tm.end();
       }
       if (last >= 4) {

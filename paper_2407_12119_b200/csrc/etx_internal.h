@@ -134,7 +134,7 @@ void launch_validate(etx_ctx* c, const int32_t* plane, int n_events, int n_hits,
 void launch_knn(etx_ctx* c, const int32_t* plane, int n_events, int n_hits, cudaStream_t s);
 void launch_pack_edges(etx_ctx* c, int n_hits, cudaStream_t s);                 // deg, nbr -> row_ptr, src, dst, n_edges
 void launch_rows_from_src(etx_ctx* c, int n_hits, int n_edges, cudaStream_t s); // injected edge list -> row_ptr
-void launch_csc(etx_ctx* c, int n_hits, cudaStream_t s);                        // dst -> col_ptr, in_edge
+void launch_csc(etx_ctx* c, int n_events, int n_hits, bool windowed, cudaStream_t s);                        // dst -> col_ptr, in_edge
 void launch_components(etx_ctx* c, const float* logit, int n_events, int n_hits, cudaStream_t s);
 // k_mlp_simt.cu
 void launch_embed_simt(etx_ctx* c, int n_hits, cudaStream_t s);
