@@ -347,51 +347,48 @@ __global__ void csc_sort_kernel(const int32_t* __restrict__ col_ptr, int n_hits,
   }
 }
 
-// Fill + sort of one (event, plane) bucket of dst hits per CTA, in shared memory.  Edges are sorted by src and a
-// k-NN edge goes from plane q to a plane in q+1 .. q+w (R7, R25), so every in-edge of a hit on plane p lies in the
-// contiguous edge range of the src planes p-w .. p-1 of the same event.  The CTA scans that range once (coalesced
-// dst reads), drops each edge whose dst is in its bucket into the dst's group with a shared-memory cursor, sorts
-// every group (ascending edge id, R9 / R22; groups are short) and writes its slice of in_edge once, coalesced.
-// Needs col_ptr (the scan of the in-degrees).  Buckets that do not fit fall back to global cursors + in-place sort.
-constexpr int kCscThreads = 256;
-constexpr int kCscHits = 2048;                       // hits per bucket held in shared memory (8 KB)
-constexpr int kCscEdges = 10240;                     // in-edges per bucket held in shared memory (40 KB)
+// Stable fill of one (event, plane) bucket of dst hits per WARP -- no sort.  Edges are sorted by src and a k-NN edge
+// goes from plane q to a plane in q+1 .. q+w (R7, R25), so every in-edge of a hit on plane p lies in the contiguous
+// edge range of the src planes p-w .. p-1 of the same event.  The warp walks that range in ascending edge id, 32
+// edges per step (coalesced dst reads); inside a step the lanes with the same dst are ranked with match.any, the
+// lowest of them advances the dst's cursor by the group size, and each lane writes its edge id at cursor + rank.
+// Steps are sequential and ranks follow the lane order, so every dst group comes out in ascending edge id
+// (R9 / R22) by construction.  The cursors of a bucket are touched by this warp only (plain loads / stores, in
+// shared memory, or in the global scratch `cursor` for a bucket of more than kCscHits hits; initialised from
+// col_ptr), so there is no capacity limit and no atomic.
+constexpr int kCscWarps = 8;
+constexpr int kCscHits = 1024;                       // cursors per warp in shared memory (4 KB)
 
-__global__ void __launch_bounds__(kCscThreads)
+__global__ void __launch_bounds__(kCscWarps * 32)
 csc_bucket_kernel(const int32_t* __restrict__ dst, const int32_t* __restrict__ row_ptr, const int32_t* __restrict__ col_ptr,
-                  const int32_t* __restrict__ plane_off, int P, int w, int32_t* __restrict__ g_cursor, int32_t* __restrict__ in_edge) {
-  __shared__ int32_t cur_s[kCscHits];
-  __shared__ int32_t list_s[kCscEdges];
-  const int e = blockIdx.x / P, p = blockIdx.x % P;
+                  const int32_t* __restrict__ plane_off, int n_buckets, int P, int w, int32_t* cursor, int32_t* __restrict__ in_edge) {
+  const int bucket = blockIdx.x * kCscWarps + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+  if (bucket >= n_buckets) return;
+  const int e = bucket / P, p = bucket % P;
   const int32_t* po = plane_off + (size_t)e * (P + 1);
   const int h0 = po[p], n = po[p + 1] - h0;
   if (n == 0) return;
-  const int base = col_ptr[h0], m = col_ptr[h0 + n] - base;         // this bucket's slice of in_edge
-  if (m == 0) return;
+  if (col_ptr[h0 + n] == col_ptr[h0]) return;                       // no in-edges at all
   const int q_lo = p - w > 0 ? p - w : 0;
   const int e0 = row_ptr[po[q_lo]], e1 = row_ptr[h0];               // out-edges of the src planes p-w .. p-1
-  const bool fits = n <= kCscHits && m <= kCscEdges;
-  int32_t* cur = fits ? cur_s : g_cursor + h0;                      // running fill position, relative to base
-  int32_t* list = fits ? list_s : in_edge + base;
-  for (int i = threadIdx.x; i < n; i += kCscThreads) cur[i] = col_ptr[h0 + i] - base;
-  __syncthreads();
-  for (int i = e0 + threadIdx.x; i < e1; i += kCscThreads) {
-    const unsigned d = (unsigned)(dst[i] - h0);
-    if (d < (unsigned)n) list[atomicAdd(&cur[d], 1)] = i;
-  }
-  __syncthreads();
-  for (int l = threadIdx.x; l < n; l += kCscThreads) {
-    const int a = col_ptr[h0 + l] - base, b = col_ptr[h0 + l + 1] - base;
-    for (int i = a + 1; i < b; ++i) {
-      const int v = list[i];
-      int j = i - 1;
-      while (j >= a && list[j] > v) { list[j + 1] = list[j]; --j; }
-      list[j + 1] = v;
+  __shared__ int32_t cur_s[kCscWarps][kCscHits];
+  volatile int32_t* cur = n <= kCscHits ? cur_s[threadIdx.x >> 5] : cursor + h0;   // shared unless the bucket is huge
+  for (int i = lane; i < n; i += 32) cur[i] = col_ptr[h0 + i];
+  __syncwarp();
+  for (int i0 = e0; i0 < e1; i0 += 32) {
+    const int i = i0 + lane;
+    const unsigned d = i < e1 ? (unsigned)(dst[i] - h0) : 0xffffffffu;
+    const bool mine = d < (unsigned)n;
+    const unsigned active = __ballot_sync(0xffffffffu, mine);
+    if (mine) {
+      const unsigned peers = __match_any_sync(active, d);
+      const int leader = __ffs(peers) - 1, rank = __popc(peers & ((1u << lane) - 1u));
+      int pos = 0;
+      if (lane == leader) { pos = cur[d]; cur[d] = pos + __popc(peers); }
+      pos = __shfl_sync(peers, pos, leader);
+      in_edge[pos + rank] = i;
     }
-  }
-  if (fits) {
-    __syncthreads();
-    for (int i = threadIdx.x; i < m; i += kCscThreads) in_edge[base + i] = list_s[i];
+    __syncwarp();
   }
 }
 
@@ -403,8 +400,9 @@ void launch_csc(etx_ctx* c, int n_events, int n_hits, bool windowed, cudaStream_
   indegree_kernel<<<grid, 256, 0, s>>>(c->dst, c->n_edges, c->cursor);
   exclusive_scan(c, c->cursor, n_hits, c->col_ptr, nullptr, s);
   if (windowed && n_events > 0) {
-    csc_bucket_kernel<<<n_events * c->hp.n_planes, kCscThreads, 0, s>>>(c->dst, c->row_ptr, c->col_ptr, c->plane_off, c->hp.n_planes,
-                                                                     c->hp.window, c->cursor, c->in_edge);
+    const int nb = n_events * c->hp.n_planes;
+    csc_bucket_kernel<<<(nb + kCscWarps - 1) / kCscWarps, kCscWarps * 32, 0, s>>>(c->dst, c->row_ptr, c->col_ptr, c->plane_off, nb,
+                                                                                c->hp.n_planes, c->hp.window, c->cursor, c->in_edge);
     c->launches += 2;
     return;
   }
