@@ -293,33 +293,59 @@ __global__ void __launch_bounds__(kMlpThreads) gnn_mlp_simt_kernel(GnnArgs a) {
 // The paper needed a scatter_add TensorRT plugin (global atomics, L253).  Here nothing is scattered: the
 // out-edges of a node are a contiguous run of e (edges are src-sorted) and its in-edges are listed by the
 // CSC, so each node's sums are sequential fp32 adds in ascending edge id (R22) -- deterministic, no atomics.
-// One group of D/4 lanes per node, 4 columns per lane.
+// One group of lanes per node, 16 bytes of the row per lane (8 bf16 or 4 fp32 columns).  The pass is bound by
+// instruction issue as much as by bytes (ncu: 61 % of the issue slots at 69 % of the HBM peak with 8-byte loads), so
+// the widest load is what counts.
+template <typename ST> struct Vec16;
+template <> struct Vec16<float> {
+  static constexpr int V = 4;
+  static __device__ __forceinline__ void add(const void* base, size_t elem, float (&s)[4]) {
+    const float4 v = *reinterpret_cast<const float4*>(static_cast<const float*>(base) + elem);
+    s[0] = __fadd_rn(s[0], v.x); s[1] = __fadd_rn(s[1], v.y); s[2] = __fadd_rn(s[2], v.z); s[3] = __fadd_rn(s[3], v.w);
+  }
+  static __device__ __forceinline__ void st(void* base, size_t elem, const float (&x)[4]) {
+    *reinterpret_cast<float4*>(static_cast<float*>(base) + elem) = make_float4(x[0], x[1], x[2], x[3]);
+  }
+};
+template <> struct Vec16<__nv_bfloat16> {
+  static constexpr int V = 8;
+  static __device__ __forceinline__ void add(const void* base, size_t elem, float (&s)[8]) {
+    const uint4 u = *reinterpret_cast<const uint4*>(static_cast<const __nv_bfloat16*>(base) + elem);
+    s[0] = __fadd_rn(s[0], __uint_as_float(u.x << 16)); s[1] = __fadd_rn(s[1], __uint_as_float(u.x & 0xffff0000u));
+    s[2] = __fadd_rn(s[2], __uint_as_float(u.y << 16)); s[3] = __fadd_rn(s[3], __uint_as_float(u.y & 0xffff0000u));
+    s[4] = __fadd_rn(s[4], __uint_as_float(u.z << 16)); s[5] = __fadd_rn(s[5], __uint_as_float(u.z & 0xffff0000u));
+    s[6] = __fadd_rn(s[6], __uint_as_float(u.w << 16)); s[7] = __fadd_rn(s[7], __uint_as_float(u.w & 0xffff0000u));
+  }
+  static __device__ __forceinline__ void st(void* base, size_t elem, const float (&x)[8]) {   // RNE to bf16 (R20)
+    uint4 u;
+    u.x = (__float_as_uint(bf16r(x[0])) >> 16) | (__float_as_uint(bf16r(x[1])) & 0xffff0000u);
+    u.y = (__float_as_uint(bf16r(x[2])) >> 16) | (__float_as_uint(bf16r(x[3])) & 0xffff0000u);
+    u.z = (__float_as_uint(bf16r(x[4])) >> 16) | (__float_as_uint(bf16r(x[5])) & 0xffff0000u);
+    u.w = (__float_as_uint(bf16r(x[6])) >> 16) | (__float_as_uint(bf16r(x[7])) & 0xffff0000u);
+    *reinterpret_cast<uint4*>(static_cast<__nv_bfloat16*>(base) + elem) = u;
+  }
+};
+
 template <typename ST, int D>
 __global__ void __launch_bounds__(256) scatter_kernel(const void* __restrict__ e, const int32_t* __restrict__ row_ptr,
                                                       const int32_t* __restrict__ col_ptr, const int32_t* __restrict__ in_edge,
                                                       void* __restrict__ m, int n_hits) {
-  constexpr int LPN = D / 4;                              // lanes per node
+  constexpr int V = Vec16<ST>::V, LPN = D / V;            // lanes per node
   // Nodes are walked from the last to the first: the edge network that ran just before wrote e in ascending
   // order, so the tail of e is what the L2 still holds, and the next edge network starts at the head, which this
   // pass reads last.
   const int gid = (gridDim.x - 1 - blockIdx.x) * (256 / LPN) + threadIdx.x / LPN;
-  const int c = (threadIdx.x % LPN) * 4;
+  const int c = (threadIdx.x % LPN) * V;
   if (gid >= n_hits) return;
-  float4 so = make_float4(0.f, 0.f, 0.f, 0.f), si = so;
+  float so[V], si[V];
+#pragma unroll
+  for (int j = 0; j < V; ++j) { so[j] = 0.0f; si[j] = 0.0f; }
   const int a0 = row_ptr[gid], a1 = row_ptr[gid + 1];
-  for (int i = a0; i < a1; ++i) {
-    const float4 v = State<ST>::ld4(e, (size_t)i * D + c);
-    so.x = __fadd_rn(so.x, v.x); so.y = __fadd_rn(so.y, v.y); so.z = __fadd_rn(so.z, v.z); so.w = __fadd_rn(so.w, v.w);
-  }
+  for (int i = a0; i < a1; ++i) Vec16<ST>::add(e, (size_t)i * D + c, so);
   const int b0 = col_ptr[gid], b1 = col_ptr[gid + 1];
-  for (int i = b0; i < b1; ++i) {
-    const float4 v = State<ST>::ld4(e, (size_t)in_edge[i] * D + c);
-    si.x = __fadd_rn(si.x, v.x); si.y = __fadd_rn(si.y, v.y); si.z = __fadd_rn(si.z, v.z); si.w = __fadd_rn(si.w, v.w);
-  }
-  so = make_float4(State<ST>::round(so.x), State<ST>::round(so.y), State<ST>::round(so.z), State<ST>::round(so.w));
-  si = make_float4(State<ST>::round(si.x), State<ST>::round(si.y), State<ST>::round(si.z), State<ST>::round(si.w));
-  State<ST>::st4(m, (size_t)gid * 2 * D + c, so);
-  State<ST>::st4(m, (size_t)gid * 2 * D + D + c, si);
+  for (int i = b0; i < b1; ++i) Vec16<ST>::add(e, (size_t)in_edge[i] * D + c, si);
+  Vec16<ST>::st(m, (size_t)gid * 2 * D + c, so);
+  Vec16<ST>::st(m, (size_t)gid * 2 * D + D + c, si);
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -415,7 +441,7 @@ void launch_embed_simt(etx_ctx* c, int n_hits, cudaStream_t s) {
 void launch_scatter(etx_ctx* c, int n_hits, cudaStream_t s) {
   if (n_hits == 0) return;
   const int d = c->hp.gnn_latent;
-  const int npb = 256 / (d / 4);
+  const int npb = 256 / (d / (c->state_bf16 ? 8 : 4));
   const int grid = (n_hits + npb - 1) / npb;
   if (c->state_bf16) {
     if (d == 32) scatter_kernel<__nv_bfloat16, 32><<<grid, 256, 0, s>>>(c->e, c->row_ptr, c->col_ptr, c->in_edge, c->m, n_hits);
