@@ -462,9 +462,17 @@ uf_event_kernel(const int32_t* __restrict__ src, const int32_t* __restrict__ dst
     int32_t* par = in_smem ? uf_smem : track_id + h0;
     for (int i = threadIdx.x; i < n; i += kUfThreads) par[i] = i;
     __syncthreads();
-    for (int i = e0 + threadIdx.x; i < e1; i += kUfThreads) {
-      if (!(logit[i] >= tau)) continue;             // R17: kept iff z >= tau
-      const unsigned a = (unsigned)(src[i] - h0), b = (unsigned)(dst[i] - h0);
+    // the three streams are read one iteration ahead: the loop body (finds, CAS) depends on them, and an edge per
+    // ~1 us of load latency per thread is what this kernel would otherwise run at
+    int i = e0 + threadIdx.x;
+    float z = 0.0f; int s_ = 0, d_ = 0;
+    if (i < e1) { z = logit[i]; s_ = src[i]; d_ = dst[i]; }
+    while (i < e1) {
+      const float zc = z; const int sc = s_, dc = d_;
+      i += kUfThreads;
+      if (i < e1) { z = logit[i]; s_ = src[i]; d_ = dst[i]; }
+      if (!(zc >= tau)) continue;                   // R17: kept iff z >= tau
+      const unsigned a = (unsigned)(sc - h0), b = (unsigned)(dc - h0);
       if (a >= (unsigned)n || b >= (unsigned)n) continue;   // cannot happen for edges built by S2 (R8)
       uf_union(par, (int)a, (int)b);
     }
@@ -494,7 +502,7 @@ void launch_components(etx_ctx* c, const float* logit, int n_events, int n_hits,
   static bool configured = false;
   constexpr int smem = kUfSmemHits * (int)sizeof(int32_t);
   if (!configured) { cudaFuncSetAttribute(uf_event_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); configured = true; }
-  const int grid = n_events < c->sm_count * 3 ? n_events : c->sm_count * 3;
+  const int grid = n_events;                          // one CTA per event; the hardware balances them
   uf_event_kernel<<<grid, kUfThreads, smem, s>>>(c->src, c->dst, logit, c->row_ptr, c->event_off, n_events, c->tau, c->track_id);
   c->launches += 1;
 }
