@@ -375,9 +375,11 @@ csc_bucket_kernel(const int32_t* __restrict__ dst, const int32_t* __restrict__ r
   volatile int32_t* cur = n <= kCscHits ? cur_s[threadIdx.x >> 5] : cursor + h0;   // shared unless the bucket is huge
   for (int i = lane; i < n; i += 32) cur[i] = col_ptr[h0 + i];
   __syncwarp();
+  int d_next = e0 + lane < e1 ? dst[e0 + lane] : -1;                 // dst is read one step ahead of its use
   for (int i0 = e0; i0 < e1; i0 += 32) {
     const int i = i0 + lane;
-    const unsigned d = i < e1 ? (unsigned)(dst[i] - h0) : 0xffffffffu;
+    const unsigned d = i < e1 ? (unsigned)(d_next - h0) : 0xffffffffu;
+    d_next = i + 32 < e1 ? dst[i + 32] : -1;
     const bool mine = d < (unsigned)n;
     const unsigned active = __ballot_sync(0xffffffffu, mine);
     if (mine) {
@@ -446,7 +448,7 @@ __device__ __forceinline__ void uf_union(int32_t* par, int a, int b) {
 // contiguous range row_ptr[first hit] .. row_ptr[end hit) because edges are sorted by src (R9); src, dst and
 // logit are read once, coalesced.  Events with more hits than the shared array use their slice of the global
 // output as the parent array, with the same code.
-constexpr int kUfThreads = 512;
+constexpr int kUfThreads = 1024;
 constexpr int kUfSmemHits = 16384;                  // 64 KB
 
 __global__ void __launch_bounds__(kUfThreads)
