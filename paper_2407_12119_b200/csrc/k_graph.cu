@@ -357,6 +357,7 @@ __global__ void csc_sort_kernel(const int32_t* __restrict__ col_ptr, int n_hits,
 // shared memory, or in the global scratch `cursor` for a bucket of more than kCscHits hits; initialised from
 // col_ptr), so there is no capacity limit and no atomic.
 constexpr int kCscWarps = 8;
+constexpr int kCscAhead = 8;                         // steps of 32 edges whose dst values are loaded together
 constexpr int kCscHits = 1024;                       // cursors per warp in shared memory (4 KB)
 
 __global__ void __launch_bounds__(kCscWarps * 32)
@@ -375,22 +376,29 @@ csc_bucket_kernel(const int32_t* __restrict__ dst, const int32_t* __restrict__ r
   volatile int32_t* cur = n <= kCscHits ? cur_s[threadIdx.x >> 5] : cursor + h0;   // shared unless the bucket is huge
   for (int i = lane; i < n; i += 32) cur[i] = col_ptr[h0 + i];
   __syncwarp();
-  int d_next = e0 + lane < e1 ? dst[e0 + lane] : -1;                 // dst is read one step ahead of its use
-  for (int i0 = e0; i0 < e1; i0 += 32) {
-    const int i = i0 + lane;
-    const unsigned d = i < e1 ? (unsigned)(d_next - h0) : 0xffffffffu;
-    d_next = i + 32 < e1 ? dst[i + 32] : -1;
-    const bool mine = d < (unsigned)n;
-    const unsigned active = __ballot_sync(0xffffffffu, mine);
-    if (mine) {
-      const unsigned peers = __match_any_sync(active, d);
-      const int leader = __ffs(peers) - 1, rank = __popc(peers & ((1u << lane) - 1u));
-      int pos = 0;
-      if (lane == leader) { pos = cur[d]; cur[d] = pos + __popc(peers); }
-      pos = __shfl_sync(peers, pos, leader);
-      in_edge[pos + rank] = i;
+  // The walk is sequential, so its speed is one global-load latency per batch of dst values: kCscAhead steps
+  // (32 edges each) are loaded at once, then ranked and placed one after the other.
+  for (int i0 = e0; i0 < e1; i0 += 32 * kCscAhead) {
+    int dq[kCscAhead];
+#pragma unroll
+    for (int u = 0; u < kCscAhead; ++u) { const int i = i0 + 32 * u + lane; dq[u] = i < e1 ? dst[i] : -1; }
+#pragma unroll
+    for (int u = 0; u < kCscAhead; ++u) {
+      const int i = i0 + 32 * u + lane;
+      if (i0 + 32 * u >= e1) break;                                  // warp-uniform
+      const unsigned d = (unsigned)(dq[u] - h0);                     // -1 - h0 wraps above n
+      const bool mine = dq[u] >= 0 && d < (unsigned)n;
+      const unsigned active = __ballot_sync(0xffffffffu, mine);
+      if (mine) {
+        const unsigned peers = __match_any_sync(active, d);
+        const int leader = __ffs(peers) - 1, rank = __popc(peers & ((1u << lane) - 1u));
+        int pos = 0;
+        if (lane == leader) { pos = cur[d]; cur[d] = pos + __popc(peers); }
+        pos = __shfl_sync(peers, pos, leader);
+        in_edge[pos + rank] = i;
+      }
+      __syncwarp();
     }
-    __syncwarp();
   }
 }
 
