@@ -376,3 +376,35 @@ def test_bf16_tensor_core_paper_edge_encoder_and_literal_he_weights():
     g = run_gpu(make_ctx(cfg, blob, b), b, emb=r["emb"], src=r["src"], dst=r["dst"])
     scale = np.abs(r["logit"]).max()
     assert np.isfinite(g["logit"]).all() and np.abs(g["logit"] - r["logit"]).max() <= 0.05 * scale
+
+
+@pytest.mark.parametrize("d", [32, 64])
+def test_bf16_tma_kernels_edge_cases_no_edges_tile_boundaries_and_handle_reuse(d):
+    # the TMA-fed bf16 kernels (edge encoder, edge network): zero edges, one edge, edge counts on both sides of a
+    # multiple of the 128-row tile, and one handle reused for a smaller batch after a larger one (stale rows behind
+    # n_edges in the workspace must never leak into live rows).  Scores against the oracle on the oracle's edges.
+    cfg = datagen.get_config("cfg1").replace(precision="bf16", gnn_latent=d, gnn_iters=2)
+    big = datagen.generate_batch(cfg, n_events=2)
+    W = centred_parity_weights(cfg, big)
+    blob = datagen.pack_blob(cfg, W)
+    o = oracle.Oracle(blob, "bf16")
+    ctx = make_ctx(cfg, blob, big)
+    r = o.run(big.xyz, big.plane, big.event_offsets, cfg.k, cfg.window, cfg.d2_max, cfg.threshold)
+    E = r["src"].size
+    assert E > 1000
+    for n_e in (E, 1, 127, 128, 129, 5 * 128, 5 * 128 + 1, E):       # (no edge at all: below, through S2)
+        # a prefix of the oracle's (src-sorted) edge list is itself a valid src-sorted edge list
+        src, dst = r["src"][:n_e], r["dst"][:n_e]
+        og = o.gnn(big.xyz, src, dst)
+        g = run_gpu(ctx, big, emb=r["emb"], src=src, dst=dst)
+        assert g["n_edges"] == n_e
+        if n_e:
+            assert np.isfinite(g["score"]).all()
+            assert np.abs(g["score"] - og["score"]).max() <= 2e-2, n_e
+        tid = oracle.components(src, dst, g["logit"], oracle.logit_threshold(cfg.threshold), big.n_hits)
+        assert np.array_equal(g["track_id"], tid), n_e
+    # no candidate passes the radius cut: S2 yields no edge at all, every hit is its own track
+    cfg0 = cfg.replace(d2_max=1e-30)
+    ctx0 = make_ctx(cfg0, blob, big)
+    g = run_gpu(ctx0, big, debug=False)
+    assert g["n_edges"] == 0 and np.array_equal(g["track_id"], np.arange(big.n_hits, dtype=np.int32))
