@@ -187,7 +187,9 @@ etx_status run_impl(etx_ctx* c, const float* d_xyz, const int32_t* d_plane, cons
       // ---- S1
       tm.begin(1);
       if (inj && inj->d_emb) ETX_CUDA(cudaMemcpyAsync(c->emb, inj->d_emb, sizeof(float4) * (size_t)n_hits, cudaMemcpyDeviceToDevice, s));
-      else if (tensor_engine) launch_embed_umma(c, n_hits, s);
+      else if (tensor_engine) {
+        if (!(c->engine == ETX_ENGINE_AUTO && launch_embed_ws(c, n_hits, s))) launch_embed_umma(c, n_hits, s);
+      }
       else launch_embed_simt(c, n_hits, s);
       tm.end();
       if (last >= 2) {

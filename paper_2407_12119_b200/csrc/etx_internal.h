@@ -150,6 +150,8 @@ void launch_gnn_mlp_umma(etx_ctx* c, int kind, int iter, int n_hits, bool do_hea
 // k_mlp_ws.cu (bf16: warp-specialised, pipelined)
 void launch_gnn_mlp_ws(etx_ctx* c, int kind, int iter, int n_hits, bool do_head, cudaStream_t s);
 
+// k_embed_ws.cu (bf16: four tiles in flight per SM; false = shape not covered, nothing launched)
+bool launch_embed_ws(etx_ctx* c, int n_hits, cudaStream_t s);
 // k_edge_tma.cu (bf16: the edge network with TMA-moved edge state, bias and residual inside the MMAs)
 bool edge_tma_configure(etx_ctx* c);
 void launch_edge_net_tma(etx_ctx* c, int iter, int n_hits, bool do_head, cudaStream_t s);

@@ -34,9 +34,6 @@ constexpr int kWsThreads = (kMmaWarp + 1) * 32;   // 416
 // them back (setmaxnreg) and the two epilogue warpgroups take 32 each: 256 * 160 + 128 * 64 + 32 * 128 = 53248.
 constexpr int kProdRegs = 64, kEpiRegs = 160;
 
-__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
 __device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
 }
