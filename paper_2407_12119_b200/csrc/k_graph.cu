@@ -350,19 +350,21 @@ __global__ void csc_sort_kernel(const int32_t* __restrict__ col_ptr, int n_hits,
 // Stable fill of one (event, plane) bucket of dst hits per WARP -- no sort.  Edges are sorted by src and a k-NN edge
 // goes from plane q to a plane in q+1 .. q+w (R7, R25), so every in-edge of a hit on plane p lies in the contiguous
 // edge range of the src planes p-w .. p-1 of the same event.  The warp walks that range in ascending edge id, 32
-// edges per step (coalesced dst reads); inside a step the lanes with the same dst are ranked with match.any, the
-// lowest of them advances the dst's cursor by the group size, and each lane writes its edge id at cursor + rank.
-// Steps are sequential and ranks follow the lane order, so every dst group comes out in ascending edge id
-// (R9 / R22) by construction.  The cursors of a bucket are touched by this warp only (plain loads / stores, in
-// shared memory, or in the global scratch `cursor` for a bucket of more than kCscHits hits; initialised from
-// col_ptr), so there is no capacity limit and no atomic.
+// edges per step (coalesced src / dst reads, eight steps loaded at once).  The neighbours of one src are distinct,
+// so two lanes of a step can only meet on a dst if they belong to different src hits: the step is split into
+// phases, one per src it spans (at most a handful), and in a phase every lane of that src advances its dst's
+// cursor with a plain read-modify-write.  Phases and steps are sequential, so every dst group comes out in
+// ascending edge id (R9 / R22) by construction.  (match.any would rank the lanes of a step in one go, but costs
+// ~1,400 cycles a step on this part.)  The cursors of a bucket are touched by this warp only (in shared memory, or
+// in the global scratch `cursor` for a bucket of more than kCscHits hits; initialised from col_ptr), so there is no
+// capacity limit and no atomic.
 constexpr int kCscWarps = 8;
 constexpr int kCscAhead = 8;                         // steps of 32 edges whose dst values are loaded together
 constexpr int kCscHits = 1024;                       // cursors per warp in shared memory (4 KB)
 
 __global__ void __launch_bounds__(kCscWarps * 32)
-csc_bucket_kernel(const int32_t* __restrict__ dst, const int32_t* __restrict__ row_ptr, const int32_t* __restrict__ col_ptr,
-                  const int32_t* __restrict__ plane_off, int n_buckets, int P, int w, int32_t* cursor, int32_t* __restrict__ in_edge) {
+csc_bucket_kernel(const int32_t* __restrict__ src, const int32_t* __restrict__ dst, const int32_t* __restrict__ row_ptr,
+                  const int32_t* __restrict__ col_ptr, const int32_t* __restrict__ plane_off, int n_buckets, int P, int w, int32_t* cursor, int32_t* __restrict__ in_edge) {
   const int bucket = blockIdx.x * kCscWarps + (threadIdx.x >> 5), lane = threadIdx.x & 31;
   if (bucket >= n_buckets) return;
   const int e = bucket / P, p = bucket % P;
@@ -379,25 +381,24 @@ csc_bucket_kernel(const int32_t* __restrict__ dst, const int32_t* __restrict__ r
   // The walk is sequential, so its speed is one global-load latency per batch of dst values: kCscAhead steps
   // (32 edges each) are loaded at once, then ranked and placed one after the other.
   for (int i0 = e0; i0 < e1; i0 += 32 * kCscAhead) {
-    int dq[kCscAhead];
+    int dq[kCscAhead], sq[kCscAhead];
 #pragma unroll
-    for (int u = 0; u < kCscAhead; ++u) { const int i = i0 + 32 * u + lane; dq[u] = i < e1 ? dst[i] : -1; }
+    for (int u = 0; u < kCscAhead; ++u) {
+      const int i = i0 + 32 * u + lane;
+      dq[u] = i < e1 ? dst[i] : -1;
+      sq[u] = i < e1 ? src[i] : 0x7fffffff;
+    }
 #pragma unroll
     for (int u = 0; u < kCscAhead; ++u) {
       const int i = i0 + 32 * u + lane;
       if (i0 + 32 * u >= e1) break;                                  // warp-uniform
       const unsigned d = (unsigned)(dq[u] - h0);                     // -1 - h0 wraps above n
       const bool mine = dq[u] >= 0 && d < (unsigned)n;
-      const unsigned active = __ballot_sync(0xffffffffu, mine);
-      if (mine) {
-        const unsigned peers = __match_any_sync(active, d);
-        const int leader = __ffs(peers) - 1, rank = __popc(peers & ((1u << lane) - 1u));
-        int pos = 0;
-        if (lane == leader) { pos = cur[d]; cur[d] = pos + __popc(peers); }
-        pos = __shfl_sync(peers, pos, leader);
-        in_edge[pos + rank] = i;
+      unsigned s_now = (unsigned)__shfl_sync(0xffffffffu, sq[u], 0);
+      while (s_now < 0x7fffffffu) {                                  // one phase per src hit the step spans
+        if (mine && (unsigned)sq[u] == s_now) { const int pos = cur[d]; cur[d] = pos + 1; in_edge[pos] = i; }
+        s_now = __reduce_min_sync(0xffffffffu, (unsigned)sq[u] > s_now ? (unsigned)sq[u] : 0x7fffffffu);   // also orders the phases
       }
-      __syncwarp();
     }
   }
 }
@@ -411,7 +412,7 @@ void launch_csc(etx_ctx* c, int n_events, int n_hits, bool windowed, cudaStream_
   exclusive_scan(c, c->cursor, n_hits, c->col_ptr, nullptr, s);
   if (windowed && n_events > 0) {
     const int nb = n_events * c->hp.n_planes;
-    csc_bucket_kernel<<<(nb + kCscWarps - 1) / kCscWarps, kCscWarps * 32, 0, s>>>(c->dst, c->row_ptr, c->col_ptr, c->plane_off, nb,
+    csc_bucket_kernel<<<(nb + kCscWarps - 1) / kCscWarps, kCscWarps * 32, 0, s>>>(c->src, c->dst, c->row_ptr, c->col_ptr, c->plane_off, nb,
                                                                                 c->hp.n_planes, c->hp.window, c->cursor, c->in_edge);
     c->launches += 2;
     return;
