@@ -79,8 +79,10 @@ class ClockSampler(threading.Thread):
                 "reasons": sorted(reasons), "samples": len(self.samples)}
 
 
-def workload(cfg, rank: int):
-    batch = datagen.generate_batch(cfg, first_event=rank * cfg.n_events)
+def workload(cfg, rank: int, world: int = 1):
+    from paper_2407_12119_b200.sharding import rank_events
+    first, n = rank_events(rank, world, cfg.n_events)
+    batch = datagen.generate_batch(cfg, n_events=n, first_event=first)
     layers = datagen.make_weights(cfg, "he")                      # BASELINE.json: He-uniform, zero bias
     return batch, layers
 
@@ -183,7 +185,7 @@ def main():
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
-    batch, layers = workload(cfg, rank)
+    batch, layers = workload(cfg, rank, world)
     scales = int8_scales(cfg, layers) if cfg.precision == "int8" else None
     blob = datagen.pack_blob(cfg, layers, scales)
     hp = etx.hyperparams_from_config(cfg, batch.n_events, batch.n_hits, engine=args.engine)
@@ -217,15 +219,8 @@ def main():
     launches = ctx.launch_count() - launches0
     stage_ms = ctx.stage_times()                      # CUDA events of the last timed step, on the launching stream
     ctx.enable_timing(False)
-    if dist is not None:
-        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-        cnt = torch.tensor([batch.n_events, N, E], device="cuda", dtype=torch.float64)
-        dist.all_reduce(cnt)
-        tot_events, tot_hits, _ = [float(x) for x in cnt.tolist()]
-    else:
-        tot_events, tot_hits = float(batch.n_events), float(N)
+    from paper_2407_12119_b200.sharding import whole_job
+    ms, (tot_events, tot_hits, _) = whole_job(ms, [batch.n_events, N, E], dist, "cuda")
     value = tot_events * args.steps / (ms * 1e-3)
 
     # ---- end to end through etx_run_host: pinned host buffers, H2D + D2H inside the timed region
@@ -241,10 +236,7 @@ def main():
         E2 = ctx.run_host(h_xyz, h_plane, batch.event_offsets, h_score, h_src, h_dst, h_tid)
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
-    if dist is not None:
-        t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s, _ = whole_job(e2e_s, [], dist, "cuda")
     e2e = {"value": tot_events * args.steps / e2e_s, "unit": UNIT,
            "h2d_bytes_per_step": int(16 * N + 4 * (batch.n_events + 1)), "d2h_bytes_per_step": int(12 * E2 + 4 * N + 4)}
 
