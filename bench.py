@@ -128,13 +128,13 @@ def run_oracle_sample(cfg, batch, layers, n_events, scales=None):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="etx", choices=["etx", "reference"])
     ap.add_argument("--config", default="cfg2")
     ap.add_argument("--events", type=int, default=None, help="override the batch size (debugging only)")
     ap.add_argument("--engine", default="auto", choices=["auto", "simt", "tc_serial"])
-    ap.add_argument("--cpu-events", type=int, default=32, help="oracle sample size for cpu_baseline")
+    ap.add_argument("--cpu-events", type=int, default=500, help="oracle sample size for cpu_baseline (about 10 s of CPU work at cfg2)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
 
