@@ -128,7 +128,7 @@ def run_oracle_sample(cfg, batch, layers, n_events, scales=None):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--steps", type=int, default=30)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="etx", choices=["etx", "reference"])
     ap.add_argument("--config", default="cfg2")

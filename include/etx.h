@@ -108,7 +108,9 @@ etx_status etx_run(etx_handle h, const float* d_xyz, const int32_t* d_plane,
 /* The same call with HOST buffers (the end-to-end measurement of bench.py): copies xyz / plane to the
  * device, runs S0..S5, copies edge_score [n_edges], edge_src/dst (if non-NULL) and track_id [n_hits]
  * back, and synchronises `stream`.  h_* output buffers must hold k*n_hits (edges) / n_hits entries.
- * Pinned host memory makes the copies asynchronous; pageable memory works too.  *n_edges_out = E. */
+ * Pinned host memory makes the copies asynchronous (src / dst are copied under the GNN, and the scores
+ * are written by the classifier straight into a pinned h_edge_score, which is device-addressable);
+ * pageable memory works too.  *n_edges_out = E. */
 etx_status etx_run_host(etx_handle h, const float* h_xyz, const int32_t* h_plane,
                         const int32_t* h_event_offsets, int32_t n_events, etx_stream stream,
                         float* h_edge_score, int32_t* h_edge_src, int32_t* h_edge_dst,

@@ -222,7 +222,7 @@ etx_status run_impl(etx_ctx* c, const float* d_xyz, const int32_t* d_plane, cons
         if (inj && inj->d_logit) {
           tm.begin(7);
           if (inj->n_edges > 0) ETX_CUDA(cudaMemcpyAsync(c->logit, inj->d_logit, sizeof(float) * (size_t)inj->n_edges, cudaMemcpyDeviceToDevice, s));
-          sigmoid_kernel<<<c->sm_count * 4, 256, 0, s>>>(c->logit, c->n_edges, c->score); c->launches++;
+          sigmoid_kernel<<<c->sm_count * 4, 256, 0, s>>>(c->logit, c->n_edges, c->score_out); c->launches++;
           tm.end();
         } else {
           const int L = c->hp.gnn_iters;
@@ -324,6 +324,7 @@ etx_status etx_create(const void* blob, size_t blob_bytes, const etx_hyperparams
     c->e = dev_alloc<uint8_t>(c, E * d * sb + 256);
     c->logit = dev_alloc<float>(c, E);
     c->score = dev_alloc<float>(c, E);
+    c->score_out = c->score;
     c->track_id = dev_alloc<int32_t>(c, N);
     c->d_xyz_in = dev_alloc<float>(c, N * 3);
     c->d_plane_in = dev_alloc<int32_t>(c, N);
@@ -398,8 +399,21 @@ etx_status etx_run_host(etx_handle c, const float* h_xyz, const int32_t* h_plane
       ETX_CUDA(cudaMemcpyAsync(c->d_xyz_in, h_xyz, sizeof(float) * 3 * (size_t)n_hits, cudaMemcpyHostToDevice, s));
       ETX_CUDA(cudaMemcpyAsync(c->d_plane_in, h_plane, sizeof(int32_t) * (size_t)n_hits, cudaMemcpyHostToDevice, s));
     }
+    // Pinned (page-locked) host memory is addressable from the device: the classifier then writes the scores
+    // straight into the caller's buffer while it computes, and the 4 E byte copy after the run disappears.
+    bool score_direct = false;
+    if (h_edge_score) {
+      cudaPointerAttributes attr;
+      if (cudaPointerGetAttributes(&attr, h_edge_score) == cudaSuccess && attr.type == cudaMemoryTypeHost && attr.devicePointer) {
+        c->score_out = static_cast<float*>(attr.devicePointer);
+        score_direct = true;
+      } else {
+        (void)cudaGetLastError();                              // pageable memory: not an error, take the copy path
+      }
+    }
     etx_output o;
     etx_status st = run_impl(c, c->d_xyz_in, c->d_plane_in, h_event_offsets, n_events, s, nullptr, &o);
+    c->score_out = c->score;
     if (st != ETX_OK) return st;
     // src / dst are final after S3: their D2H copy runs on the copy stream while the GNN is still computing
     ETX_CUDA(cudaEventSynchronize(c->edges_ready));
@@ -414,7 +428,7 @@ etx_status etx_run_host(etx_handle c, const float* h_xyz, const int32_t* h_plane
     }
     if (h_track_id && n_hits > 0)
       ETX_CUDA(cudaMemcpyAsync(h_track_id, c->track_id, sizeof(int32_t) * (size_t)n_hits, cudaMemcpyDeviceToHost, s));
-    if (E > 0 && h_edge_score) ETX_CUDA(cudaMemcpyAsync(h_edge_score, c->score, sizeof(float) * (size_t)E, cudaMemcpyDeviceToHost, s));
+    if (E > 0 && h_edge_score && !score_direct) ETX_CUDA(cudaMemcpyAsync(h_edge_score, c->score, sizeof(float) * (size_t)E, cudaMemcpyDeviceToHost, s));
     ETX_CUDA(cudaStreamSynchronize(s));
   } catch (const CudaFail& f) {
     return fail(c, ETX_ERR_CUDA, std::string(f.what) + ": " + cudaGetErrorString(f.err));

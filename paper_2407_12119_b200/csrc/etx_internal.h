@@ -93,6 +93,7 @@ struct etx_ctx {
   int32_t* flags = nullptr;               // device: [0] input-order violation
   void *h = nullptr, *e = nullptr, *m = nullptr;
   float *logit = nullptr, *score = nullptr;
+  float* score_out = nullptr;             // where the classifier writes scores: `score`, or the caller's mapped host buffer (etx_run_host)
   int32_t *track_id = nullptr;
   // k_edge_tma.cu: identity operand image, split-bias images [2 * iter + layer], CUtensorMap of `e` (opaque here)
   bool edge_tma = false;

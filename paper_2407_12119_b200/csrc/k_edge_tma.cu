@@ -734,7 +734,7 @@ void launch_edge_net_tma(etx_ctx* c, int iter, int n_hits, bool do_head, cudaStr
   a.head_w = c->layers[c->i_head].dev.Wt; a.head_b = c->layers[c->i_head].dev.bias;
   a.h = static_cast<const __nv_bfloat16*>(c->h);
   a.src = c->src; a.dst = c->dst; a.n_rows_ptr = c->n_edges;
-  a.logit = c->logit; a.score = c->score; a.do_head = do_head ? 1 : 0;
+  a.logit = c->logit; a.score = c->score_out; a.do_head = do_head ? 1 : 0;
   const long long max_rows_ll = (long long)n_hits * c->hp.k;
   const int max_rows = (int)(max_rows_ll > 0x7fffffff ? 0x7fffffff : max_rows_ll);
   if (c->hp.gnn_latent == 32) edge_tma_launch<32>(c, a, max_rows, s);

@@ -392,7 +392,7 @@ void fill_gnn_args(etx_ctx* c, int kind, int iter, int n_hits, bool do_head, Gnn
   a.feat = c->feat; a.src = c->src; a.dst = c->dst;
   a.n_rows_ptr = is_edge ? c->n_edges : nullptr;
   a.n_rows = n_hits;
-  a.h = c->h; a.e = c->e; a.m = c->m; a.logit = c->logit; a.score = c->score;
+  a.h = c->h; a.e = c->e; a.m = c->m; a.logit = c->logit; a.score = c->score_out;
   a.do_head = do_head ? 1 : 0;
   a.edge_enc_input = c->hp.edge_enc_input;
   a.tap = c->tap_layer >= 0 ? c->tap : nullptr;

@@ -267,19 +267,27 @@ def test_error_codes_capacity_blob_order_unsupported():
     assert g["n_edges"] > 0
 
 
-def test_run_host_matches_device_run():
-    cfg, b, W = _setup("cfg1", 3, precision="fp32")
+@pytest.mark.parametrize("precision,pinned", [("fp32", True), ("fp32", False), ("bf16", True), ("bf16", False)])
+def test_run_host_matches_device_run(precision, pinned):
+    # pinned buffers: src / dst are copied under the GNN and the scores are written by the classifier straight into
+    # the (device-addressable) host buffer; pageable buffers: plain copies after the run.  Same bits either way.
+    cfg, b, W = _setup("cfg1", 3, precision=precision)
     blob = datagen.pack_blob(cfg, W)
     ctx = make_ctx(cfg, blob, b)
     g = run_gpu(ctx, b, debug=False)
     cap = cfg.k * b.n_hits
-    h_xyz = torch.from_numpy(b.xyz).pin_memory(); h_plane = torch.from_numpy(b.plane).pin_memory()
-    sc = torch.empty(cap, dtype=torch.float32).pin_memory(); s_ = torch.empty(cap, dtype=torch.int32).pin_memory()
-    d_ = torch.empty(cap, dtype=torch.int32).pin_memory(); tid = torch.empty(b.n_hits, dtype=torch.int32).pin_memory()
-    E = ctx.run_host(h_xyz, h_plane, b.event_offsets, sc, s_, d_, tid)
-    assert E == g["n_edges"]
-    assert np.array_equal(s_.numpy()[:E], g["src"]) and np.array_equal(d_.numpy()[:E], g["dst"])
-    assert np.array_equal(sc.numpy()[:E], g["score"]) and np.array_equal(tid.numpy(), g["track_id"])
+    mk = (lambda t: t.pin_memory()) if pinned else (lambda t: t)
+    h_xyz = mk(torch.from_numpy(b.xyz)); h_plane = mk(torch.from_numpy(b.plane))
+    sc = mk(torch.full((cap,), -1.0, dtype=torch.float32)); s_ = mk(torch.empty(cap, dtype=torch.int32))
+    d_ = mk(torch.empty(cap, dtype=torch.int32)); tid = mk(torch.empty(b.n_hits, dtype=torch.int32))
+    for _ in range(2):                                       # twice: the direct-write redirection must not stick
+        E = ctx.run_host(h_xyz, h_plane, b.event_offsets, sc, s_, d_, tid)
+        assert E == g["n_edges"]
+        assert np.array_equal(s_.numpy()[:E], g["src"]) and np.array_equal(d_.numpy()[:E], g["dst"])
+        assert np.array_equal(sc.numpy()[:E], g["score"]) and np.array_equal(tid.numpy(), g["track_id"])
+        assert (sc.numpy()[E:] == -1.0).all()                # nothing is written behind the E scores
+    g2 = run_gpu(ctx, b, debug=False)                        # and a device run afterwards still fills its own buffer
+    assert np.array_equal(g2["score"], g["score"])
 
 
 # ================================================================================== tcgen05 engine (bf16 / int8)
