@@ -428,8 +428,8 @@ template <int D>
 __host__ __device__ constexpr EncSmem enc_layout() {
   constexpr int KB = D * 2, BLK = kRows * KB;
   EncSmem s{};
-  s.out = 0;                           // kEncGroups x [128][KB] output staging
-  s.w1 = s.out + kEncGroups * BLK;     // W1 image [D][KB]
+  s.out = 0;                           // 2 x kEncGroups x [128][KB] output staging (two slots per warpgroup)
+  s.w1 = s.out + 2 * kEncGroups * BLK; // W1 image [D][KB]
   s.ones = s.w1 + D * KB;              // [128][32 B]
   s.b1 = s.ones + kRows * 32;          // [D][32 B] split bias of layer 1
   s.w3 = s.b1 + D * 32;                // fp32: W0^T [3][D], b0 [D]
@@ -457,7 +457,7 @@ edge_enc_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeEncArgs
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + L.bar);
   uint64_t *hid_full = bars, *acc_full = bars + kEncGroups, *out_ready = bars + 2 * kEncGroups,
-           *slot_free = bars + 3 * kEncGroups, *bar_w = bars + 4 * kEncGroups;
+           *slot_free = bars + 4 * kEncGroups, *bar_w = bars + 6 * kEncGroups;
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bar_w + 1);
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -466,7 +466,8 @@ edge_enc_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeEncArgs
 
   if (tid == 0) {
     for (int g = 0; g < kEncGroups; ++g) {
-      mbar_init(&hid_full[g], 128); mbar_init(&acc_full[g], 1); mbar_init(&out_ready[g], 128); mbar_init(&slot_free[g], 1);
+      mbar_init(&hid_full[g], 128); mbar_init(&acc_full[g], 1);
+      for (int b = 0; b < 2; ++b) { mbar_init(&out_ready[2 * g + b], 128); mbar_init(&slot_free[2 * g + b], 1); }
     }
     mbar_init(bar_w, 1);
     fence_barrier_init();
@@ -490,11 +491,12 @@ edge_enc_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeEncArgs
       int it = 0;
       for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
         const int g = it % kEncGroups;
-        mbar_wait(&out_ready[g], (it / kEncGroups) & 1);
-        tma_store_2d(&e_map, out_addr + g * BLK, 0, tile * kRows);
+        const int jj = it / kEncGroups, sl = 2 * g + (jj & 1);  // the group's tiles alternate between its two slots
+        mbar_wait(&out_ready[sl], (jj >> 1) & 1);
+        tma_store_2d(&e_map, out_addr + sl * BLK, 0, tile * kRows);
         bulk_commit();
         bulk_wait_read0();
-        mbar_arrive(&slot_free[g]);
+        mbar_arrive(&slot_free[sl]);
       }
       bulk_wait0();
     }
@@ -526,7 +528,6 @@ edge_enc_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeEncArgs
     const int g = warp >> 2, q = warp & 3;
     const int r = q * 32 + lane;                              // row of the tile owned by this thread
     const uint32_t lane_base = (uint32_t)(q * 32) << 16;
-    uint8_t* out = smem + L.out + g * BLK;
     auto tile_of = [&](int j) { return blockIdx.x + (long long)(g + j * kEncGroups) * gridDim.x; };
     auto load_idx = [&](int j, int& is, int& id) {
       const long long t = tile_of(j);
@@ -580,7 +581,9 @@ edge_enc_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeEncArgs
       mbar_arrive(&hid_full[g]);
       PROF(2)
       // ---- layer 1 result (bias already inside): TMEM -> bf16 -> the group's slot -> TMA store (R20)
-      mbar_wait(&slot_free[g], (j & 1) ^ 1);                  // the store of tile j - 1 has read the slot
+      const int sl = 2 * g + (j & 1);
+      uint8_t* out = smem + L.out + sl * BLK;
+      mbar_wait(&slot_free[sl], ((j >> 1) & 1) ^ 1);          // the store of tile j - 2 has read the slot
       mbar_wait(&acc_full[g], j & 1);
       PROF(3)
       tc_fence_after();
@@ -601,7 +604,7 @@ edge_enc_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeEncArgs
       }
       tc_fence_before();
       fence_proxy_async();
-      mbar_arrive(&out_ready[g]);
+      mbar_arrive(&out_ready[sl]);
       (void)tile;
       PROF(4)
     }
