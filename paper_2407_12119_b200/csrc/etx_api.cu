@@ -228,7 +228,8 @@ etx_status run_impl(etx_ctx* c, const float* d_xyz, const int32_t* d_plane, cons
           const int L = c->hp.gnn_iters;
           auto mlp = [&](int kind, int it, bool head) {
             if (kind == kEdgeNet && c->edge_tma) launch_edge_net_tma(c, it, n_hits, head, s);
-            else if (kind == kEdgeEnc && c->edge_tma && c->hp.edge_enc_input == 0 && !head) launch_edge_enc_tma(c, n_hits, s);
+            else if (kind == kEdgeEnc && c->edge_tma && c->hp.edge_enc_input == 0 && !head) launch_edge_enc_tma(c, n_hits, false, s);
+            else if (kind == kNodeEnc && c->edge_tma) launch_edge_enc_tma(c, n_hits, true, s);
             else if (tensor_engine && c->precision == ETX_BF16 && c->engine != ETX_ENGINE_TC_SERIAL) launch_gnn_mlp_ws(c, kind, it, n_hits, head, s);
             else if (tensor_engine && kind == kEdgeNet && c->precision == ETX_INT8 && c->engine == ETX_ENGINE_AUTO && c->tap_layer < 0)
               launch_edge_net_i8(c, it, n_hits, head, s);

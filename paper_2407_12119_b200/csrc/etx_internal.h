@@ -99,8 +99,10 @@ struct etx_ctx {
   bool edge_tma = false;
   void* ident_img = nullptr;
   void* eenc_b1_img = nullptr;
+  void* nenc_b1_img = nullptr;
   std::vector<void*> edge_bias_img;
   alignas(64) unsigned char e_map[128] = {};
+  alignas(64) unsigned char h_map[128] = {};   // CUtensorMap of `h` (node encoder output)
   int32_t* tap = nullptr;
   size_t tap_bytes = 0;
   int tap_layer = -1;
@@ -158,6 +160,6 @@ bool launch_embed_ws(etx_ctx* c, int n_hits, cudaStream_t s);
 // k_edge_tma.cu (bf16: the edge network with TMA-moved edge state, bias and residual inside the MMAs)
 bool edge_tma_configure(etx_ctx* c);
 void launch_edge_net_tma(etx_ctx* c, int iter, int n_hits, bool do_head, cudaStream_t s);
-void launch_edge_enc_tma(etx_ctx* c, int n_hits, cudaStream_t s);
+void launch_edge_enc_tma(etx_ctx* c, int n_hits, bool node, cudaStream_t s);
 
 }  // namespace etx

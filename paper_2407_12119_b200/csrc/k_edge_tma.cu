@@ -444,7 +444,9 @@ struct EdgeEncArgs {
   float b0[64];              // constant bank, so the FFMAs of layer 0 take them as operands without any load
   const float4* feat;
   const int32_t* src; const int32_t* dst;
-  const int32_t* n_rows_ptr;
+  const int32_t* n_rows_ptr; // edge encoder: E on the device
+  int n_rows;                // node encoder (S4a): number of hits
+  int node;                  // 1: h0 = MLP(f) over hits, rows are the hits themselves; 0: e0 = MLP(|f_dst - f_src|) over edges
 };
 
 template <int D>
@@ -461,7 +463,7 @@ edge_enc_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeEncArgs
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bar_w + 1);
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int n_rows = *a.n_rows_ptr;
+  const int n_rows = a.node ? a.n_rows : *a.n_rows_ptr;
   const int n_tiles = (n_rows + kRows - 1) / kRows;
 
   if (tid == 0) {
@@ -535,7 +537,8 @@ edge_enc_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeEncArgs
       if (t < n_tiles) {
         long long row = t * kRows + r;
         if (row >= n_rows) row = n_rows - 1;
-        is = __ldg(a.src + row); id = __ldg(a.dst + row);
+        if (a.node) { is = (int)row; id = (int)row; }
+        else { is = __ldg(a.src + row); id = __ldg(a.dst + row); }
       }
     };
     int is_n, id_n;                                           // indices of tile j + 1
@@ -551,7 +554,8 @@ edge_enc_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeEncArgs
       const long long tile = tile_of(j);
       PROF(0)
       // R11: component-wise |f_dst - f_src| of the normalised features
-      const float fx = fabsf(__fsub_rn(fd.x, fs.x)), fy = fabsf(__fsub_rn(fd.y, fs.y)), fz = fabsf(__fsub_rn(fd.z, fs.z));
+      float fx = fabsf(__fsub_rn(fd.x, fs.x)), fy = fabsf(__fsub_rn(fd.y, fs.y)), fz = fabsf(__fsub_rn(fd.z, fs.z));
+      if (a.node) { fx = fs.x; fy = fs.y; fz = fs.z; }        // S4a: the hit's own normalised features
       // prefetch: features of tile j + 1 (their indices are here), indices of tile j + 2
       fs = __ldg(a.feat + is_n); fd = __ldg(a.feat + id_n);
       load_idx(j + 2, is_n, id_n);
@@ -680,7 +684,7 @@ void edge_tma_launch(etx_ctx* c, const EdgeTmaArgs& a, int max_rows, cudaStream_
 }
 
 template <int D>
-void edge_enc_launch(etx_ctx* c, const EdgeEncArgs& a, int max_rows, cudaStream_t s) {
+void edge_enc_launch(etx_ctx* c, const EdgeEncArgs& a, const unsigned char* out_map, int max_rows, cudaStream_t s) {
   auto kern = edge_enc_tma_kernel<D>;
   constexpr int smem = enc_layout<D>().total + 1024;
   static bool configured = false;
@@ -689,7 +693,7 @@ void edge_enc_launch(etx_ctx* c, const EdgeEncArgs& a, int max_rows, cudaStream_
   const int grid = tiles < c->sm_count ? tiles : c->sm_count;     // one persistent CTA per SM (512 TMEM columns)
   if (grid <= 0) return;
   CUtensorMap map;
-  memcpy(&map, c->e_map, sizeof(map));
+  memcpy(&map, out_map, sizeof(map));
   kern<<<grid, kEncThreads, smem, s>>>(map, a);
   c->launches++;
 }
@@ -710,7 +714,8 @@ bool edge_tma_configure(etx_ctx* c) {
       c->edge_bias_img[2 * it + l] = p;
     }
   c->eenc_b1_img = upload_bytes(c, pack_split_rows(c->layers[c->i_eenc + 1].b));
-  if (!c->eenc_b1_img) return false;
+  c->nenc_b1_img = upload_bytes(c, pack_split_rows(c->layers[c->i_nenc + 1].b));
+  if (!c->eenc_b1_img || !c->nenc_b1_img) return false;
   void* fn = nullptr;
   cudaDriverEntryPointQueryResult qres;
   if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn) return false;
@@ -726,6 +731,13 @@ bool edge_tma_configure(etx_ctx* c) {
       CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) return false;
   memcpy(c->e_map, &map, sizeof(map));
+  const cuuint64_t hdim[2] = {(cuuint64_t)D, c->hp.max_hits > 0 ? (cuuint64_t)c->hp.max_hits : 1};
+  const CUresult r2 = reinterpret_cast<EncodeTiledFn>(fn)(
+      &map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, c->h, hdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+      D == 64 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r2 != CUDA_SUCCESS) return false;
+  memcpy(c->h_map, &map, sizeof(map));
   return true;
 }
 
@@ -744,21 +756,23 @@ void launch_edge_net_tma(etx_ctx* c, int iter, int n_hits, bool do_head, cudaStr
   else edge_tma_launch<64>(c, a, max_rows, s);
 }
 
-// S4b with the configs' K = 3 edge-encoder input (edge_enc_input == 0)
-void launch_edge_enc_tma(etx_ctx* c, int n_hits, cudaStream_t s) {
-  const int i0 = c->i_eenc;
+// S4b with the configs' K = 3 edge-encoder input (edge_enc_input == 0), or S4a (node = true): the same kernel over hits
+void launch_edge_enc_tma(etx_ctx* c, int n_hits, bool node, cudaStream_t s) {
+  const int i0 = node ? c->i_nenc : c->i_eenc;
   EdgeEncArgs a;
-  a.w1_img = c->layers[i0 + 1].dev.Wtc; a.b1_img = c->eenc_b1_img;
+  a.w1_img = c->layers[i0 + 1].dev.Wtc; a.b1_img = node ? c->nenc_b1_img : c->eenc_b1_img;
   const int D = c->hp.gnn_latent;                            // 32 or 64 (umma_supported)
   for (int n = 0; n < D; ++n) {
     for (int k = 0; k < 3; ++k) a.w0t[k * D + n] = c->layers[i0].W[(size_t)n * 3 + k];
     a.b0[n] = c->layers[i0].b[n];
   }
   a.feat = c->feat; a.src = c->src; a.dst = c->dst; a.n_rows_ptr = c->n_edges;
-  const long long max_rows_ll = (long long)n_hits * c->hp.k;
+  a.n_rows = n_hits; a.node = node ? 1 : 0;
+  const long long max_rows_ll = node ? (long long)n_hits : (long long)n_hits * c->hp.k;
   const int max_rows = (int)(max_rows_ll > 0x7fffffff ? 0x7fffffff : max_rows_ll);
-  if (c->hp.gnn_latent == 32) edge_enc_launch<32>(c, a, max_rows, s);
-  else edge_enc_launch<64>(c, a, max_rows, s);
+  const unsigned char* map = node ? c->h_map : c->e_map;
+  if (c->hp.gnn_latent == 32) edge_enc_launch<32>(c, a, map, max_rows, s);
+  else edge_enc_launch<64>(c, a, map, max_rows, s);
 }
 
 }  // namespace etx
