@@ -416,3 +416,28 @@ def test_bf16_tma_kernels_edge_cases_no_edges_tile_boundaries_and_handle_reuse(d
     ctx0 = make_ctx(cfg0, blob, big)
     g = run_gpu(ctx0, big, debug=False)
     assert g["n_edges"] == 0 and np.array_equal(g["track_id"], np.arange(big.n_hits, dtype=np.int32))
+
+
+def test_two_handles_on_two_streams_run_concurrently_and_agree_with_sequential_runs():
+    # One handle serves one stream at a time, several handles may run at once (include/etx.h): two bf16 handles,
+    # each enqueuing several batches on its own stream without any synchronisation in between, must give the bits
+    # of a sequential run (persistent one-CTA-per-SM kernels of the two streams interleave on the device).
+    cfg, b, W = _setup("cfg1", 4, precision="bf16")
+    blob = datagen.pack_blob(cfg, W)
+    b2 = b.slice_events(1, 4)
+    ref = [run_gpu(make_ctx(cfg, blob, x), x, debug=False) for x in (b, b2)]
+    ctxs = [make_ctx(cfg, blob, b), make_ctx(cfg, blob, b)]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    ins = [(dev(x.xyz), dev(x.plane), x.event_offsets) for x in (b, b2)]
+    torch.cuda.synchronize()
+    outs = [None, None]
+    for rep in range(3):
+        for k in (0, 1):
+            with torch.cuda.stream(streams[k]):
+                outs[k] = ctxs[k].run(*ins[k])
+    for k in (0, 1):
+        with torch.cuda.stream(streams[k]):
+            r = ctxs[k].results(outs[k])
+        assert r["n_edges"] == ref[k]["n_edges"]
+        for name in ("src", "dst", "score", "logit", "track_id"):
+            assert np.array_equal(r[name].cpu().numpy(), ref[k][name]), (k, name)
