@@ -231,7 +231,7 @@ etx_status run_impl(etx_ctx* c, const float* d_xyz, const int32_t* d_plane, cons
             else if (kind == kEdgeEnc && c->edge_tma && c->hp.edge_enc_input == 0 && !head) launch_edge_enc_tma(c, n_hits, false, s);
             else if (kind == kNodeEnc && c->edge_tma) launch_edge_enc_tma(c, n_hits, true, s);
             else if (tensor_engine && c->precision == ETX_BF16 && c->engine != ETX_ENGINE_TC_SERIAL) launch_gnn_mlp_ws(c, kind, it, n_hits, head, s);
-            else if (tensor_engine && kind == kEdgeNet && c->precision == ETX_INT8 && c->engine == ETX_ENGINE_AUTO && c->tap_layer < 0)
+            else if (kind == kEdgeNet && c->edge_i8 && c->tap_layer < 0)
               launch_edge_net_i8(c, it, n_hits, head, s);
             else if (tensor_engine) launch_gnn_mlp_umma(c, kind, it, n_hits, head, s);
             else launch_gnn_mlp_simt(c, kind, it, n_hits, head, s);
@@ -346,6 +346,10 @@ etx_status etx_create(const void* blob, size_t blob_bytes, const etx_hyperparams
     if (c->precision != ETX_FP32 && c->engine != ETX_ENGINE_SIMT) {
       if (!umma_supported(c)) { c->error = "tensor-core engine not available for these shapes"; return bail(ETX_ERR_UNSUPPORTED); }
       umma_configure(c);
+      if (c->precision == ETX_INT8 && c->engine == ETX_ENGINE_AUTO) {
+        if (!edge_i8_configure(c)) { c->error = "INT8 edge-network TMA setup failed"; return bail(ETX_ERR_CUDA); }
+        c->edge_i8 = true;
+      }
       if (c->precision == ETX_BF16 && c->engine == ETX_ENGINE_AUTO) {
         if (!edge_tma_configure(c)) { c->error = "edge-network TMA setup failed"; return bail(ETX_ERR_CUDA); }
         c->edge_tma = true;

@@ -97,6 +97,7 @@ struct etx_ctx {
   int32_t *track_id = nullptr;
   // k_edge_tma.cu: identity operand image, split-bias images [2 * iter + layer], CUtensorMap of `e` (opaque here)
   bool edge_tma = false;
+  bool edge_i8 = false;                   // k_edge_i8.cu usable (INT8, auto engine, tensor map of fp32 `e` encoded)
   void* ident_img = nullptr;
   void* eenc_b1_img = nullptr;
   void* nenc_b1_img = nullptr;
@@ -154,6 +155,7 @@ void launch_gnn_mlp_umma(etx_ctx* c, int kind, int iter, int n_hits, bool do_hea
 void launch_gnn_mlp_ws(etx_ctx* c, int kind, int iter, int n_hits, bool do_head, cudaStream_t s);
 
 // k_edge_i8.cu (int8: warp-specialised edge network with quantising producers)
+bool edge_i8_configure(etx_ctx* c);
 void launch_edge_net_i8(etx_ctx* c, int iter, int n_hits, bool do_head, cudaStream_t s);
 // k_embed_ws.cu (bf16: four tiles in flight per SM; false = shape not covered, nothing launched)
 bool launch_embed_ws(etx_ctx* c, int n_hits, cudaStream_t s);

@@ -3,16 +3,20 @@
 // its embedding (L265-269) and names the GNN as the step where INT8 would pay most (L271).
 //
 // Same arithmetic, operation for operation, as gnn_mlp_umma_kernel<kEdgeNet, kInt8, D> (every int32 accumulator is
-// reproduced bit for bit, and every other op is a single pinned fp32 op), but warp-specialised and pipelined:
+// reproduced bit for bit, and every other op is a single pinned fp32 op), but warp-specialised and pipelined, with
+// the fp32 edge state moved by TMA as in the bf16 kernel (k_edge_tma.cu):
 //
-//   producers  (8 warps)  read the fp32 rows h[src] | h[dst] | e of the next tiles, quantise them
-//                         (q = clamp(rne(x * (1 / s_x)), +-127)) and write the int8 A tile in the swizzled UMMA
-//                         layout, kI8Stages tiles ahead -- the quantisation is ~1,000 ALU instructions per row and
-//                         is what the serial kernel could not hide;
+//   TMA loader (1 thread) the 128-row fp32 tile of e (contiguous) -> a 128B-swizzled slot of a kI8E-deep ring;
+//   producers  (8 warps)  gather the fp32 rows h[src] | h[dst] from global memory (L2 hits), take e from the slot,
+//                         quantise all three (q = clamp(rne(x * (1 / s_x)), +-127)) into the int8 A tile;
 //   MMA issuer (1 thread) layer 0 of tile i+1 is issued before layer 1 of tile i; accumulators double-buffered in TMEM;
 //   epilogue   (2 x 4 warps) warpgroup g owns tiles i = g (mod 2): acc0 -> fmaf(acc, s_x s_w, b) -> relu -> int8 ->
-//                         layer-1 operand; acc1 -> fmaf -> + old e (fp32, re-read: an L2 hit) -> e, and the
-//                         classifier dot product on the last step.
+//                         layer-1 operand; acc1 -> fmaf -> + old e, IN PLACE in the slot, and the classifier dot
+//                         product on the last step;
+//   TMA storer (1 thread) the slot -> e, then hands the slot back to the loader.
+#include <cuda.h>
+#include <string.h>
+
 #include "umma_common.cuh"
 
 namespace etx {
@@ -21,36 +25,53 @@ namespace {
 
 using namespace umma;
 
-constexpr int kI8Stages = 4;
+constexpr int kI8E = 4;                                    // ring of fp32 edge-state tiles
+constexpr int kI8A = 2;                                    // ring of int8 operand tiles
 constexpr int kI8EpiWarps = 8, kI8ProdWarps = 8;
-constexpr int kI8MmaWarp = kI8EpiWarps + kI8ProdWarps;
-constexpr int kI8Threads = (kI8MmaWarp + 1) * 32;          // 544
+constexpr int kI8MmaWarp = kI8EpiWarps + kI8ProdWarps, kI8LoadWarp = kI8MmaWarp + 1, kI8StoreWarp = kI8MmaWarp + 2;
+constexpr int kI8Threads = (kI8StoreWarp + 1) * 32;        // 608
 constexpr int kI8ProdThreads = kI8ProdWarps * 32;
-// ptxas compiles the 544-thread CTA with 96 registers per thread; the two producer warpgroups hand 16 each to the
-// two epilogue warpgroups: 256 * 80 + 256 * 112 + 32 * 96 = 52224 = 544 * 96.
+// ptxas compiles the 608-thread CTA with 96 registers per thread; the two producer warpgroups hand 16 each to the
+// two epilogue warpgroups: 256 * 80 + 256 * 112 + 96 * 96 = 58368 = 608 * 96.
 constexpr int kI8ProdRegs = 80, kI8EpiRegs = 112;
+constexpr int kI8Sub = kRows * 128;                        // one TMA box of the fp32 tile: [128 rows][32 floats]
 
-struct I8Smem { int a, h, stg, w0, w1, par, bar, total; };
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, int x, int y, uint64_t* bar) {
+  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+               ::"r"(dst), "l"(reinterpret_cast<uint64_t>(map)), "r"(smem_u32(bar)), "r"(x), "r"(y) : "memory");
+}
+__device__ __forceinline__ void tma_store_2d(const CUtensorMap* map, uint32_t src, int x, int y) {
+  asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%2, %3}], [%1];"
+               ::"l"(reinterpret_cast<uint64_t>(map)), "r"(src), "r"(x), "r"(y) : "memory");
+}
+
+// byte offset of floats [4 c4, 4 c4 + 4) of row r inside an fp32 tile slot (boxes of 32 floats, 128B swizzle)
+__device__ __forceinline__ uint32_t e_off(uint32_t r, uint32_t c4) {
+  return (c4 >> 3) * kI8Sub + r * 128 + (((c4 & 7) ^ (r & 7)) << 4);
+}
+
+struct I8Smem { int e, a, h, w0, w1, par, bar, total; };
 template <int D>
 __host__ __device__ constexpr I8Smem i8_layout() {
   I8Smem s{};
-  s.a = 0;                                   // kI8Stages x 3 K-blocks [128][D] int8
-  s.h = s.a + kI8Stages * 3 * kRows * D;     // 2 x [128][D]: layer-1 operand per epilogue warpgroup
-  s.stg = s.h + 2 * kRows * D;               // 2 x [128][D] fp32: output staging per epilogue warpgroup (chunk-swizzled)
-  s.w0 = s.stg + 2 * kRows * D * 4;          // W0 image: 3 K-blocks [D][D]
+  s.e = 0;                                   // kI8E x [128][D] fp32, as D/32 boxes [128][128 B]
+  s.a = s.e + kI8E * kRows * D * 4;          // kI8A x 3 K-blocks [128][D] int8
+  s.h = s.a + kI8A * 3 * kRows * D;          // 2 x [128][D]: layer-1 operand per epilogue warpgroup
+  s.w0 = s.h + 2 * kRows * D;                // W0 image: 3 K-blocks [D][D]
   s.w1 = s.w0 + 3 * D * D;                   // W1 image
   s.par = s.w1 + D * D;                      // fp32: scale0, bias0, scale1, bias1, head w
   s.bar = s.par + 5 * D * 4;
-  s.total = s.bar + 128;
+  s.total = s.bar + 256;
   return s;
 }
 
 template <int D>
-__global__ void __launch_bounds__(kI8Threads, 1) edge_net_i8_kernel(GnnArgs a) {
+__global__ void __launch_bounds__(kI8Threads, 1) edge_net_i8_kernel(const __grid_constant__ CUtensorMap e_map, GnnArgs a) {
   constexpr int KB = D;                                      // bytes per int8 segment row = swizzle width (32 / 64)
   constexpr int CPR = KB / 16;                               // 16-byte chunks per segment row
   constexpr int BLK = kRows * KB;
   constexpr int STAGE = 3 * BLK;
+  constexpr int ETILE = kRows * D * 4;
   constexpr I8Smem L = i8_layout<D>();
   constexpr uint32_t TMEM_COLS = 4 * D;                      // acc0[2] | acc1[2]
   extern __shared__ uint8_t smem_raw[];
@@ -58,8 +79,9 @@ __global__ void __launch_bounds__(kI8Threads, 1) edge_net_i8_kernel(GnnArgs a) {
   float* par = reinterpret_cast<float*>(smem + L.par);
   float *scale0 = par, *bias0 = par + D, *scale1 = par + 2 * D, *bias1 = par + 3 * D, *headw = par + 4 * D;
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + L.bar);
-  uint64_t *full = bars, *empty = bars + kI8Stages, *acc0_full = bars + 2 * kI8Stages, *hid_full = acc0_full + 2,
-           *acc1_full = acc0_full + 4, *bar_w = acc0_full + 6;
+  uint64_t *e_full = bars, *e_free = bars + kI8E, *out_ready = bars + 2 * kI8E, *a_full = bars + 3 * kI8E,
+           *a_empty = a_full + kI8A, *acc0_full = a_empty + kI8A, *hid_full = acc0_full + 2, *acc1_full = acc0_full + 4,
+           *bar_w = acc0_full + 6;
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc0_full + 7);
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -67,7 +89,8 @@ __global__ void __launch_bounds__(kI8Threads, 1) edge_net_i8_kernel(GnnArgs a) {
   const int n_tiles = (n_rows + kRows - 1) / kRows;
 
   if (tid == 0) {
-    for (int s = 0; s < kI8Stages; ++s) { mbar_init(&full[s], kI8ProdThreads); mbar_init(&empty[s], 1); }
+    for (int s = 0; s < kI8E; ++s) { mbar_init(&e_full[s], 1); mbar_init(&e_free[s], 1); mbar_init(&out_ready[s], 128); }
+    for (int s = 0; s < kI8A; ++s) { mbar_init(&a_full[s], kI8ProdThreads); mbar_init(&a_empty[s], 1); }
     for (int g = 0; g < 2; ++g) { mbar_init(&acc0_full[g], 1); mbar_init(&hid_full[g], 128); mbar_init(&acc1_full[g], 1); }
     mbar_init(bar_w, 1);
     fence_barrier_init();
@@ -81,6 +104,7 @@ __global__ void __launch_bounds__(kI8Threads, 1) edge_net_i8_kernel(GnnArgs a) {
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = *tmem_slot;
+  const uint32_t e_addr = smem_u32(smem + L.e);
 
   if (warp >= kI8EpiWarps && warp < kI8MmaWarp) {
     // ================================================================================================ producers
@@ -88,36 +112,77 @@ __global__ void __launch_bounds__(kI8Threads, 1) edge_net_i8_kernel(GnnArgs a) {
     const int pt = tid - kI8EpiWarps * 32;                   // 0 .. 255
     const float inv_sx0 = a.l0.inv_sx;
     const float* hbase = static_cast<const float*>(a.h);
-    const float* ebase = static_cast<const float*>(a.e);
+    auto quant16 = [&](const float4& f0, const float4& f1, const float4& f2, const float4& f3) {
+      uint4 q;
+      q.x = pack_i8x4(quant_i8(f0.x, inv_sx0), quant_i8(f0.y, inv_sx0), quant_i8(f0.z, inv_sx0), quant_i8(f0.w, inv_sx0));
+      q.y = pack_i8x4(quant_i8(f1.x, inv_sx0), quant_i8(f1.y, inv_sx0), quant_i8(f1.z, inv_sx0), quant_i8(f1.w, inv_sx0));
+      q.z = pack_i8x4(quant_i8(f2.x, inv_sx0), quant_i8(f2.y, inv_sx0), quant_i8(f2.z, inv_sx0), quant_i8(f2.w, inv_sx0));
+      q.w = pack_i8x4(quant_i8(f3.x, inv_sx0), quant_i8(f3.y, inv_sx0), quant_i8(f3.z, inv_sx0), quant_i8(f3.w, inv_sx0));
+      return q;
+    };
     int it = 0;
     for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
-      const int s = it % kI8Stages;
-      mbar_wait(&empty[s], ((it / kI8Stages) & 1) ^ 1);
-      uint8_t* st = smem + L.a + s * STAGE;
-      // item c = (row r, 16-byte chunk `piece` of the int8 row) = 16 consecutive fp32 of the source row; CPR
-      // consecutive threads share a row, so a warp reads 32 / CPR whole rows (coalesced for the contiguous e tile)
+      const int sa = it % kI8A, se = it % kI8E;
+      uint8_t* st = smem + L.a + sa * STAGE;
+      const uint8_t* es = smem + L.e + se * ETILE;
+      bool first = true;
+      // item c = (row r, 16-byte chunk `piece` of the int8 row) = 16 consecutive fp32 of the source row
 #pragma unroll
-      for (int i = 0; i < (kRows * CPR) / kI8ProdThreads; ++i) {
-        const int c = i * kI8ProdThreads + pt, r = c / CPR, piece = c % CPR;
-        int grow = tile * kRows + r;
-        if (grow >= n_rows) grow = n_rows - 1;                // dead rows of the last tile: any valid row (never stored)
-        const int js = __ldg(a.src + grow), jd = __ldg(a.dst + grow);
-        const float* p[3] = {hbase + (size_t)js * D + piece * 16, hbase + (size_t)jd * D + piece * 16,
-                             ebase + (size_t)grow * D + piece * 16};
-#pragma unroll
-        for (int sg = 0; sg < 3; ++sg) {
-          const float4* q4 = reinterpret_cast<const float4*>(p[sg]);
-          const float4 f0 = __ldg(q4), f1 = __ldg(q4 + 1), f2 = __ldg(q4 + 2), f3 = __ldg(q4 + 3);
-          uint4 q;
-          q.x = pack_i8x4(quant_i8(f0.x, inv_sx0), quant_i8(f0.y, inv_sx0), quant_i8(f0.z, inv_sx0), quant_i8(f0.w, inv_sx0));
-          q.y = pack_i8x4(quant_i8(f1.x, inv_sx0), quant_i8(f1.y, inv_sx0), quant_i8(f1.z, inv_sx0), quant_i8(f1.w, inv_sx0));
-          q.z = pack_i8x4(quant_i8(f2.x, inv_sx0), quant_i8(f2.y, inv_sx0), quant_i8(f2.z, inv_sx0), quant_i8(f2.w, inv_sx0));
-          q.w = pack_i8x4(quant_i8(f3.x, inv_sx0), quant_i8(f3.y, inv_sx0), quant_i8(f3.z, inv_sx0), quant_i8(f3.w, inv_sx0));
-          *reinterpret_cast<uint4*>(st + sg * BLK + swz<KB>(r, piece)) = q;
+      for (int i = 0; i < (kRows * CPR + kI8ProdThreads - 1) / kI8ProdThreads; ++i) {
+        const int c = i * kI8ProdThreads + pt;
+        if (c < kRows * CPR) {
+          const int r = c / CPR, piece = c % CPR;
+          int grow = tile * kRows + r;
+          if (grow >= n_rows) grow = n_rows - 1;              // dead rows of the last tile: any valid row (never stored)
+          const int js = __ldg(a.src + grow), jd = __ldg(a.dst + grow);
+          const float4* ps = reinterpret_cast<const float4*>(hbase + (size_t)js * D + piece * 16);
+          const float4* pd = reinterpret_cast<const float4*>(hbase + (size_t)jd * D + piece * 16);
+          const float4 s0 = __ldg(ps), s1 = __ldg(ps + 1), s2 = __ldg(ps + 2), s3 = __ldg(ps + 3);
+          const float4 d0 = __ldg(pd), d1 = __ldg(pd + 1), d2 = __ldg(pd + 2), d3 = __ldg(pd + 3);
+          if (first) {                                        // the gathers are in flight while we wait for the slots
+            mbar_wait(&a_empty[sa], ((it / kI8A) & 1) ^ 1);
+            mbar_wait(&e_full[se], (it / kI8E) & 1);
+            first = false;
+          }
+          const float4 e0 = *reinterpret_cast<const float4*>(es + e_off(r, piece * 4 + 0));
+          const float4 e1 = *reinterpret_cast<const float4*>(es + e_off(r, piece * 4 + 1));
+          const float4 e2 = *reinterpret_cast<const float4*>(es + e_off(r, piece * 4 + 2));
+          const float4 e3 = *reinterpret_cast<const float4*>(es + e_off(r, piece * 4 + 3));
+          *reinterpret_cast<uint4*>(st + 2 * BLK + swz<KB>(r, piece)) = quant16(e0, e1, e2, e3);
+          *reinterpret_cast<uint4*>(st + swz<KB>(r, piece)) = quant16(s0, s1, s2, s3);
+          *reinterpret_cast<uint4*>(st + BLK + swz<KB>(r, piece)) = quant16(d0, d1, d2, d3);
         }
       }
+      if (first) { mbar_wait(&a_empty[sa], ((it / kI8A) & 1) ^ 1); mbar_wait(&e_full[se], (it / kI8E) & 1); }
       fence_proxy_async();                                    // generic-proxy writes -> visible to the tensor core
-      mbar_arrive(&full[s]);
+      mbar_arrive(&a_full[sa]);
+    }
+  } else if (warp == kI8LoadWarp) {
+    // ================================================================================================ TMA loads
+    if (lane == 0) {
+      int it = 0;
+      for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
+        const int s = it % kI8E;
+        mbar_wait(&e_free[s], ((it / kI8E) & 1) ^ 1);
+        mbar_expect_tx(&e_full[s], ETILE);
+#pragma unroll
+        for (int b = 0; b < D / 32; ++b) tma_load_2d(e_addr + s * ETILE + b * kI8Sub, &e_map, 32 * b, tile * kRows, &e_full[s]);
+      }
+    }
+  } else if (warp == kI8StoreWarp) {
+    // ================================================================================================ TMA stores
+    if (lane == 0) {
+      int it = 0;
+      for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
+        const int s = it % kI8E;
+        mbar_wait(&out_ready[s], (it / kI8E) & 1);
+#pragma unroll
+        for (int b = 0; b < D / 32; ++b) tma_store_2d(&e_map, e_addr + s * ETILE + b * kI8Sub, 32 * b, tile * kRows);
+        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+        mbar_arrive(&e_free[s]);
+      }
+      asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
     }
   } else if (warp == kI8MmaWarp) {
     // ================================================================================================ MMA issuer
@@ -139,13 +204,13 @@ __global__ void __launch_bounds__(kI8Threads, 1) edge_net_i8_kernel(GnnArgs a) {
       };
       int it = 0;
       for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
-        const int s = it % kI8Stages, g = it & 1;
-        mbar_wait(&full[s], (it / kI8Stages) & 1);
+        const int s = it % kI8A, g = it & 1;
+        mbar_wait(&a_full[s], (it / kI8A) & 1);
         tc_fence_after();
         // acc0[g] was drained by epilogue 0 of tile it-2, which hid_full (waited on for layer 1 of it-2) covers
         issue_layer<kInt8, KB>(a_addr + s * STAGE, w0_addr, 3 * KB, D, tmem + g * D, idesc);
         umma_commit(&acc0_full[g]);
-        umma_commit(&empty[s]);                               // layer 0 is the stage's only reader
+        umma_commit(&a_empty[s]);                             // layer 0 is the operand tile's only reader
         if (it > 0) layer1(it - 1);
       }
       if (it > 0) layer1(it - 1);
@@ -157,16 +222,14 @@ __global__ void __launch_bounds__(kI8Threads, 1) edge_net_i8_kernel(GnnArgs a) {
     const int r = q * 32 + lane;                              // row of the tile owned by this thread
     const uint32_t lane_base = (uint32_t)(q * 32) << 16;
     uint8_t* Hg = smem + L.h + g * BLK;
-    uint8_t* Sg = smem + L.stg + g * (kRows * D * 4);         // fp32 staging tile of this warpgroup
-    auto stg_off = [](int row_, int chunk) { return row_ * (D * 4) + ((chunk ^ (row_ & (D / 4 - 1))) << 4); };
     const float head_b = a.head.bias[0];
     const float inv_sx1 = a.l1.inv_sx;
-    float* state = static_cast<float*>(a.e);
     int j = 0;                                                // this warpgroup's tile counter
     for (int it = g; blockIdx.x + (long long)it * gridDim.x < n_tiles; it += 2, ++j) {
       const long long tile = blockIdx.x + (long long)it * gridDim.x;
       const long long row = tile * kRows + r;
       const bool live = row < n_rows;
+      uint8_t* es = smem + L.e + (it % kI8E) * ETILE;         // this tile's fp32 edge state, updated in place
       // ---- epilogue 0: relu(fmaf(acc0, s_x s_w, b0)) -> int8 codes -> layer-1 operand (R21)
       mbar_wait(&acc0_full[g], j & 1);
       tc_fence_after();
@@ -179,67 +242,49 @@ __global__ void __launch_bounds__(kI8Threads, 1) edge_net_i8_kernel(GnnArgs a) {
       tc_fence_before();
       fence_proxy_async();
       mbar_arrive(&hid_full[g]);
-      // ---- epilogue 1: fmaf(acc1, s_x s_w, b1) + old e -> e (fp32), optional classifier (R14, R16, R21).
-      //      The thread that owns a row dequantises it into a shared staging tile; the residual add and the store
-      //      then run over the tile in global-memory order (16 bytes per thread, whole rows per group of threads):
-      //      a row-per-thread read-modify-write of e cost a third of the kernel.
+      // ---- epilogue 1: fmaf(acc1, s_x s_w, b1) + old e -> e (fp32, in the slot), optional classifier (R14, R16, R21)
       mbar_wait(&acc1_full[g], j & 1);
       tc_fence_after();
+      float hacc = 0.0f;
 #pragma unroll
       for (int c0 = 0; c0 < D; c0 += 32) {
         uint32_t v[32];
         tmem_ld32(tmem + lane_base + 2 * D + g * D + c0, v);
 #pragma unroll
         for (int ch = 0; ch < 8; ++ch) {
-          float4 y;
           const int c = c0 + ch * 4;
-          y.x = __fmaf_rn((float)(int)v[ch * 4 + 0], scale1[c + 0], bias1[c + 0]);
-          y.y = __fmaf_rn((float)(int)v[ch * 4 + 1], scale1[c + 1], bias1[c + 1]);
-          y.z = __fmaf_rn((float)(int)v[ch * 4 + 2], scale1[c + 2], bias1[c + 2]);
-          y.w = __fmaf_rn((float)(int)v[ch * 4 + 3], scale1[c + 3], bias1[c + 3]);
-          *reinterpret_cast<float4*>(Sg + stg_off(r, c / 4)) = y;
+          float4* p = reinterpret_cast<float4*>(es + e_off(r, c / 4));
+          const float4 o = *p;
+          float4 y;
+          y.x = __fadd_rn(o.x, __fmaf_rn((float)(int)v[ch * 4 + 0], scale1[c + 0], bias1[c + 0]));
+          y.y = __fadd_rn(o.y, __fmaf_rn((float)(int)v[ch * 4 + 1], scale1[c + 1], bias1[c + 1]));
+          y.z = __fadd_rn(o.z, __fmaf_rn((float)(int)v[ch * 4 + 2], scale1[c + 2], bias1[c + 2]));
+          y.w = __fadd_rn(o.w, __fmaf_rn((float)(int)v[ch * 4 + 3], scale1[c + 3], bias1[c + 3]));
+          *p = y;
+          if (a.do_head) {                                    // ascending j (R16)
+            hacc = __fmaf_rn(y.x, headw[c + 0], hacc); hacc = __fmaf_rn(y.y, headw[c + 1], hacc);
+            hacc = __fmaf_rn(y.z, headw[c + 2], hacc); hacc = __fmaf_rn(y.w, headw[c + 3], hacc);
+          }
         }
       }
       tc_fence_before();                                      // acc1[g] may be overwritten after our next hid_full arrive
-      asm volatile("bar.sync %0, 128;" ::"r"(1 + g) : "memory");
-      {
-        constexpr int CH = D / 4;                             // 16-byte chunks per row = threads per row
-        const int t = (warp & 3) * 32 + lane, cc = t % CH;
-#pragma unroll 4
-        for (int rr = t / CH; rr < kRows; rr += 128 / CH) {
-          const long long grow = tile * kRows + rr;
-          if (grow < n_rows) {
-            float* gp = state + (size_t)grow * D + cc * 4;
-            const float4 o = *reinterpret_cast<const float4*>(gp);
-            float4 y = *reinterpret_cast<const float4*>(Sg + stg_off(rr, cc));
-            y.x = __fadd_rn(o.x, y.x); y.y = __fadd_rn(o.y, y.y); y.z = __fadd_rn(o.z, y.z); y.w = __fadd_rn(o.w, y.w);
-            *reinterpret_cast<float4*>(gp) = y;
-            if (a.do_head) *reinterpret_cast<float4*>(Sg + stg_off(rr, cc)) = y;
-          }
-        }
+      fence_proxy_async();                                    // generic-proxy writes -> visible to the TMA store
+      mbar_arrive(&out_ready[it % kI8E]);
+      if (a.do_head && live) {
+        const float z = __fadd_rn(hacc, head_b);
+        a.logit[row] = z;
+        a.score[row] = 1.0f / (1.0f + expf(-z));
       }
-      if (a.do_head) {                                        // the classifier: ascending j over the row's new state (R16)
-        asm volatile("bar.sync %0, 128;" ::"r"(1 + g) : "memory");
-        if (live) {
-          float hacc = 0.0f;
-#pragma unroll
-          for (int c4 = 0; c4 < D / 4; ++c4) {
-            const float4 y = *reinterpret_cast<const float4*>(Sg + stg_off(r, c4));
-            hacc = __fmaf_rn(y.x, headw[c4 * 4 + 0], hacc); hacc = __fmaf_rn(y.y, headw[c4 * 4 + 1], hacc);
-            hacc = __fmaf_rn(y.z, headw[c4 * 4 + 2], hacc); hacc = __fmaf_rn(y.w, headw[c4 * 4 + 3], hacc);
-          }
-          const float z = __fadd_rn(hacc, head_b);
-          a.logit[row] = z;
-          a.score[row] = 1.0f / (1.0f + expf(-z));
-        }
-      }
-      asm volatile("bar.sync %0, 128;" ::"r"(1 + g) : "memory");   // the staging tile is free for the next tile
     }
   }
   tc_fence_before();
   __syncthreads();
   if (warp == kI8MmaWarp) tmem_dealloc(tmem, TMEM_COLS);
 }
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
 template <int D>
 void edge_i8_launch(etx_ctx* c, const GnnArgs& a, int max_rows, cudaStream_t s) {
@@ -250,11 +295,33 @@ void edge_i8_launch(etx_ctx* c, const GnnArgs& a, int max_rows, cudaStream_t s) 
   const int tiles = (max_rows + kRows - 1) / kRows;
   const int grid = tiles < c->sm_count ? tiles : c->sm_count;     // one persistent CTA per SM
   if (grid <= 0) return;
-  kern<<<grid, kI8Threads, smem, s>>>(a);
+  CUtensorMap map;
+  memcpy(&map, c->e_map, sizeof(map));
+  kern<<<grid, kI8Threads, smem, s>>>(map, a);
   c->launches++;
 }
 
 }  // namespace
+
+// INT8 mode: tensor map of the fp32 edge state (boxes of 128 rows x 32 floats, 128B swizzle)
+bool edge_i8_configure(etx_ctx* c) {
+  static_assert(sizeof(CUtensorMap) == sizeof(c->e_map), "etx_ctx::e_map must hold a CUtensorMap");
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn) return false;
+  const int D = c->hp.gnn_latent;
+  const cuuint64_t gdim[2] = {(cuuint64_t)D, c->max_edges > 0 ? (cuuint64_t)c->max_edges : 1};
+  const cuuint64_t gstride[1] = {(cuuint64_t)D * 4};
+  const cuuint32_t box[2] = {32, (cuuint32_t)kRows};
+  const cuuint32_t estr[2] = {1, 1};
+  CUtensorMap map;
+  const CUresult r = reinterpret_cast<EncodeTiledFn>(fn)(
+      &map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, c->e, gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+      CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return false;
+  memcpy(c->e_map, &map, sizeof(map));
+  return true;
+}
 
 // INT8 mode, fp32 state, no accumulator tap requested (the tap stays with gnn_mlp_umma_kernel)
 void launch_edge_net_i8(etx_ctx* c, int iter, int n_hits, bool do_head, cudaStream_t s) {
