@@ -233,6 +233,8 @@ etx_status run_impl(etx_ctx* c, const float* d_xyz, const int32_t* d_plane, cons
             else if (tensor_engine && c->precision == ETX_BF16 && c->engine != ETX_ENGINE_TC_SERIAL) launch_gnn_mlp_ws(c, kind, it, n_hits, head, s);
             else if (kind == kEdgeNet && c->edge_i8 && c->tap_layer < 0)
               launch_edge_net_i8(c, it, n_hits, head, s);
+            else if (kind == kNodeNet && c->edge_i8 && c->tap_layer < 0)
+              launch_node_net_i8(c, it, n_hits, s);
             else if (tensor_engine) launch_gnn_mlp_umma(c, kind, it, n_hits, head, s);
             else launch_gnn_mlp_simt(c, kind, it, n_hits, head, s);
           };

@@ -157,6 +157,7 @@ void launch_gnn_mlp_ws(etx_ctx* c, int kind, int iter, int n_hits, bool do_head,
 // k_edge_i8.cu (int8: warp-specialised edge network with quantising producers)
 bool edge_i8_configure(etx_ctx* c);
 void launch_edge_net_i8(etx_ctx* c, int iter, int n_hits, bool do_head, cudaStream_t s);
+void launch_node_net_i8(etx_ctx* c, int iter, int n_hits, cudaStream_t s);
 // k_embed_ws.cu (bf16: four tiles in flight per SM; false = shape not covered, nothing launched)
 bool launch_embed_ws(etx_ctx* c, int n_hits, cudaStream_t s);
 // k_edge_tma.cu (bf16: the edge network with TMA-moved edge state, bias and residual inside the MMAs)

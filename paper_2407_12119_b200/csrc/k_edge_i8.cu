@@ -65,7 +65,9 @@ __host__ __device__ constexpr I8Smem i8_layout() {
   return s;
 }
 
-template <int D>
+// NODE = false: S4e over edges (self state e, K-block 2; gathered h[src], h[dst]);  NODE = true: S4d over hits
+// (self state h, K-block 0; m_out, m_in of the same row).
+template <int D, bool NODE>
 __global__ void __launch_bounds__(kI8Threads, 1) edge_net_i8_kernel(const __grid_constant__ CUtensorMap e_map, GnnArgs a) {
   constexpr int KB = D;                                      // bytes per int8 segment row = swizzle width (32 / 64)
   constexpr int CPR = KB / 16;                               // 16-byte chunks per segment row
@@ -85,8 +87,9 @@ __global__ void __launch_bounds__(kI8Threads, 1) edge_net_i8_kernel(const __grid
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc0_full + 7);
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int n_rows = *a.n_rows_ptr;
+  const int n_rows = NODE ? a.n_rows : *a.n_rows_ptr;
   const int n_tiles = (n_rows + kRows - 1) / kRows;
+  constexpr int SELF = NODE ? 0 : 2, AUX0 = NODE ? 1 : 0, AUX1 = NODE ? 2 : 1;   // K-blocks of the A tile
 
   if (tid == 0) {
     for (int s = 0; s < kI8E; ++s) { mbar_init(&e_full[s], 1); mbar_init(&e_free[s], 1); mbar_init(&out_ready[s], 128); }
@@ -134,9 +137,15 @@ __global__ void __launch_bounds__(kI8Threads, 1) edge_net_i8_kernel(const __grid
           const int r = c / CPR, piece = c % CPR;
           int grow = tile * kRows + r;
           if (grow >= n_rows) grow = n_rows - 1;              // dead rows of the last tile: any valid row (never stored)
-          const int js = __ldg(a.src + grow), jd = __ldg(a.dst + grow);
-          const float4* ps = reinterpret_cast<const float4*>(hbase + (size_t)js * D + piece * 16);
-          const float4* pd = reinterpret_cast<const float4*>(hbase + (size_t)jd * D + piece * 16);
+          const float4 *ps, *pd;
+          if (NODE) {
+            ps = reinterpret_cast<const float4*>(static_cast<const float*>(a.m) + (size_t)grow * 2 * D + piece * 16);
+            pd = ps + D / 4;
+          } else {
+            const int js = __ldg(a.src + grow), jd = __ldg(a.dst + grow);
+            ps = reinterpret_cast<const float4*>(hbase + (size_t)js * D + piece * 16);
+            pd = reinterpret_cast<const float4*>(hbase + (size_t)jd * D + piece * 16);
+          }
           const float4 s0 = __ldg(ps), s1 = __ldg(ps + 1), s2 = __ldg(ps + 2), s3 = __ldg(ps + 3);
           const float4 d0 = __ldg(pd), d1 = __ldg(pd + 1), d2 = __ldg(pd + 2), d3 = __ldg(pd + 3);
           if (first) {                                        // the gathers are in flight while we wait for the slots
@@ -148,9 +157,9 @@ __global__ void __launch_bounds__(kI8Threads, 1) edge_net_i8_kernel(const __grid
           const float4 e1 = *reinterpret_cast<const float4*>(es + e_off(r, piece * 4 + 1));
           const float4 e2 = *reinterpret_cast<const float4*>(es + e_off(r, piece * 4 + 2));
           const float4 e3 = *reinterpret_cast<const float4*>(es + e_off(r, piece * 4 + 3));
-          *reinterpret_cast<uint4*>(st + 2 * BLK + swz<KB>(r, piece)) = quant16(e0, e1, e2, e3);
-          *reinterpret_cast<uint4*>(st + swz<KB>(r, piece)) = quant16(s0, s1, s2, s3);
-          *reinterpret_cast<uint4*>(st + BLK + swz<KB>(r, piece)) = quant16(d0, d1, d2, d3);
+          *reinterpret_cast<uint4*>(st + SELF * BLK + swz<KB>(r, piece)) = quant16(e0, e1, e2, e3);
+          *reinterpret_cast<uint4*>(st + AUX0 * BLK + swz<KB>(r, piece)) = quant16(s0, s1, s2, s3);
+          *reinterpret_cast<uint4*>(st + AUX1 * BLK + swz<KB>(r, piece)) = quant16(d0, d1, d2, d3);
         }
       }
       if (first) { mbar_wait(&a_empty[sa], ((it / kI8A) & 1) ^ 1); mbar_wait(&e_full[se], (it / kI8E) & 1); }
@@ -261,7 +270,7 @@ __global__ void __launch_bounds__(kI8Threads, 1) edge_net_i8_kernel(const __grid
           y.z = __fadd_rn(o.z, __fmaf_rn((float)(int)v[ch * 4 + 2], scale1[c + 2], bias1[c + 2]));
           y.w = __fadd_rn(o.w, __fmaf_rn((float)(int)v[ch * 4 + 3], scale1[c + 3], bias1[c + 3]));
           *p = y;
-          if (a.do_head) {                                    // ascending j (R16)
+          if (!NODE && a.do_head) {                           // ascending j (R16)
             hacc = __fmaf_rn(y.x, headw[c + 0], hacc); hacc = __fmaf_rn(y.y, headw[c + 1], hacc);
             hacc = __fmaf_rn(y.z, headw[c + 2], hacc); hacc = __fmaf_rn(y.w, headw[c + 3], hacc);
           }
@@ -270,7 +279,7 @@ __global__ void __launch_bounds__(kI8Threads, 1) edge_net_i8_kernel(const __grid
       tc_fence_before();                                      // acc1[g] may be overwritten after our next hid_full arrive
       fence_proxy_async();                                    // generic-proxy writes -> visible to the TMA store
       mbar_arrive(&out_ready[it % kI8E]);
-      if (a.do_head && live) {
+      if (!NODE && a.do_head && live) {
         const float z = __fadd_rn(hacc, head_b);
         a.logit[row] = z;
         a.score[row] = 1.0f / (1.0f + expf(-z));
@@ -286,9 +295,9 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
-template <int D>
+template <int D, bool NODE>
 void edge_i8_launch(etx_ctx* c, const GnnArgs& a, int max_rows, cudaStream_t s) {
-  auto kern = edge_net_i8_kernel<D>;
+  auto kern = edge_net_i8_kernel<D, NODE>;
   constexpr int smem = i8_layout<D>().total + 1024;
   static bool configured = false;
   if (!configured) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); configured = true; }
@@ -296,7 +305,7 @@ void edge_i8_launch(etx_ctx* c, const GnnArgs& a, int max_rows, cudaStream_t s) 
   const int grid = tiles < c->sm_count ? tiles : c->sm_count;     // one persistent CTA per SM
   if (grid <= 0) return;
   CUtensorMap map;
-  memcpy(&map, c->e_map, sizeof(map));
+  memcpy(&map, NODE ? c->h_map : c->e_map, sizeof(map));
   kern<<<grid, kI8Threads, smem, s>>>(map, a);
   c->launches++;
 }
@@ -310,16 +319,19 @@ bool edge_i8_configure(etx_ctx* c) {
   cudaDriverEntryPointQueryResult qres;
   if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn) return false;
   const int D = c->hp.gnn_latent;
-  const cuuint64_t gdim[2] = {(cuuint64_t)D, c->max_edges > 0 ? (cuuint64_t)c->max_edges : 1};
   const cuuint64_t gstride[1] = {(cuuint64_t)D * 4};
   const cuuint32_t box[2] = {32, (cuuint32_t)kRows};
   const cuuint32_t estr[2] = {1, 1};
-  CUtensorMap map;
-  const CUresult r = reinterpret_cast<EncodeTiledFn>(fn)(
-      &map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, c->e, gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-      CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-  if (r != CUDA_SUCCESS) return false;
-  memcpy(c->e_map, &map, sizeof(map));
+  for (int node = 0; node < 2; ++node) {
+    const long long rows = node ? c->hp.max_hits : c->max_edges;
+    const cuuint64_t gdim[2] = {(cuuint64_t)D, rows > 0 ? (cuuint64_t)rows : 1};
+    CUtensorMap map;
+    const CUresult r = reinterpret_cast<EncodeTiledFn>(fn)(
+        &map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, node ? c->h : c->e, gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+        CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return false;
+    memcpy(node ? c->h_map : c->e_map, &map, sizeof(map));
+  }
   return true;
 }
 
@@ -329,8 +341,16 @@ void launch_edge_net_i8(etx_ctx* c, int iter, int n_hits, bool do_head, cudaStre
   fill_gnn_args(c, kEdgeNet, iter, n_hits, do_head, a);
   const long long max_rows_ll = (long long)n_hits * c->hp.k;
   const int max_rows = (int)(max_rows_ll > 0x7fffffff ? 0x7fffffff : max_rows_ll);
-  if (c->hp.gnn_latent == 32) edge_i8_launch<32>(c, a, max_rows, s);
-  else edge_i8_launch<64>(c, a, max_rows, s);
+  if (c->hp.gnn_latent == 32) edge_i8_launch<32, false>(c, a, max_rows, s);
+  else edge_i8_launch<64, false>(c, a, max_rows, s);
+}
+
+// S4d in INT8 mode: the same kernel over hits (self state h, second and third segment m_out, m_in)
+void launch_node_net_i8(etx_ctx* c, int iter, int n_hits, cudaStream_t s) {
+  GnnArgs a;
+  fill_gnn_args(c, kNodeNet, iter, n_hits, false, a);
+  if (c->hp.gnn_latent == 32) edge_i8_launch<32, true>(c, a, n_hits, s);
+  else edge_i8_launch<64, true>(c, a, n_hits, s);
 }
 
 }  // namespace etx
