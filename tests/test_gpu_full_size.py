@@ -69,9 +69,10 @@ def _whole_batch_invariants(cfg, b, g):
     assert (np.diff(ie)[inner[1:]] > 0).all()
 
 
-@pytest.mark.parametrize("name,preset", [("cfg2", "he"), ("cfg2", "parity"), ("cfg4", "parity")])
+@pytest.mark.parametrize("name,preset", [("cfg2", "he"), ("cfg2", "parity"), ("cfg4", "parity"), ("cfg5", "parity")])
 def test_full_size_bf16_invariants_and_sampled_events(name, preset):
     cfg = datagen.get_config(name)                              # bf16, 500 / 200 events: the bench configuration
+    # (cfg5: the paper's operating point -- k = 50 with a radius cut, latent 32, edge encoder on [h0_src, h0_dst])
     b = datagen.generate_batch(cfg)
     if preset == "he":
         W = datagen.make_weights(cfg, "he")                     # BASELINE.json: what bench.py times
