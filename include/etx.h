@@ -74,6 +74,12 @@ typedef struct {
   int32_t  max_events;               /* workspace capacity (L223: fixed memory per stream)              */
   int32_t  max_hits;                 /* max_edges = k * max_hits                                        */
   int32_t  validate_input;           /* 1: device-side check that hits are sorted by (event, plane)     */
+  /* Optional device-memory allocator (L223: Allen hands every algorithm memory from its own per-stream
+   * arena).  NULL alloc: cudaMalloc / cudaFree.  alloc must return device memory aligned to 256 bytes or
+   * NULL on failure; dealloc is called once per block from etx_destroy; alloc and dealloc go together.    */
+  void*  (*alloc)(size_t bytes, void* alloc_ctx);
+  void   (*dealloc)(void* ptr, void* alloc_ctx);
+  void*  alloc_ctx;
 } etx_hyperparams;
 
 typedef struct {                     /* device pointers into the handle's workspace (library-owned);   */
@@ -117,6 +123,9 @@ etx_status etx_run_host(etx_handle h, const float* h_xyz, const int32_t* h_plane
                         int32_t* h_track_id, int32_t* n_edges_out);
 
 etx_status etx_destroy(etx_handle h);
+
+/* Device bytes held by the handle (workspace + converted weights), as requested from the allocator. */
+size_t etx_workspace_bytes(etx_handle h);
 
 const char* etx_status_string(etx_status s);
 const char* etx_last_error(etx_handle h);         /* message of the last failing call on this handle */

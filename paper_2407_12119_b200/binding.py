@@ -24,13 +24,18 @@ class EtxError(RuntimeError):
         super().__init__(f"{STATUS.get(status, status)}: {msg}")
 
 
+ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)      # optional device allocator callbacks (include/etx.h)
+DEALLOC_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p)
+
+
 class Hyperparams(C.Structure):
     _fields_ = [("struct_size", C.c_uint32), ("n_planes", C.c_int32), ("norm_offset", C.c_float * 3),
                 ("norm_div", C.c_float * 3), ("emb_hidden", C.c_int32), ("emb_n_hidden_layers", C.c_int32),
                 ("emb_dim", C.c_int32), ("k", C.c_int32), ("window", C.c_int32), ("d2_max", C.c_float),
                 ("gnn_latent", C.c_int32), ("gnn_iters", C.c_int32), ("edge_enc_input", C.c_int32),
                 ("threshold", C.c_float), ("precision", C.c_int32), ("engine", C.c_int32),
-                ("max_events", C.c_int32), ("max_hits", C.c_int32), ("validate_input", C.c_int32)]
+                ("max_events", C.c_int32), ("max_hits", C.c_int32), ("validate_input", C.c_int32),
+                ("alloc", ALLOC_FN), ("dealloc", DEALLOC_FN), ("alloc_ctx", C.c_void_p)]
 
 
 class EtxOutput(C.Structure):
@@ -76,6 +81,8 @@ def load_library():
     L.etx_run_host.argtypes = [vp, vp, vp, i32p, C.c_int32, vp, vp, vp, vp, vp, i32p]
     L.etx_destroy.restype = C.c_int
     L.etx_destroy.argtypes = [vp]
+    L.etx_workspace_bytes.restype = C.c_size_t
+    L.etx_workspace_bytes.argtypes = [vp]
     L.etx_status_string.restype = C.c_char_p
     L.etx_status_string.argtypes = [C.c_int]
     L.etx_last_error.restype = C.c_char_p
@@ -217,6 +224,9 @@ class Etx:
         arr = (C.c_float * len(STAGE_NAMES))()
         self._check(self._L.etx_dbg_stage_times(self._h, arr), "etx_dbg_stage_times")
         return {n: float(v) for n, v in zip(STAGE_NAMES, arr)}
+
+    def workspace_bytes(self) -> int:
+        return int(self._L.etx_workspace_bytes(self._h))
 
     def launch_count(self) -> int:
         return int(self._L.etx_dbg_launch_count(self._h))

@@ -24,9 +24,8 @@ struct CudaFail { cudaError_t err; const char* what; };
 
 template <typename T>
 T* dev_alloc(etx_ctx* c, size_t n) {
-  void* p = nullptr;
-  ETX_CUDA(cudaMalloc(&p, (n ? n : 1) * sizeof(T)));
-  c->allocs.push_back(p);
+  void* p = etx::etx_device_alloc(c, (n ? n : 1) * sizeof(T));
+  if (!p) throw CudaFail{cudaErrorMemoryAllocation, "device allocation"};
   return static_cast<T*>(p);
 }
 
@@ -274,6 +273,27 @@ etx_status run_impl(etx_ctx* c, const float* d_xyz, const int32_t* d_plane, cons
 
 }  // namespace
 
+namespace etx {
+void* etx_device_alloc(etx_ctx* c, size_t bytes) {
+  void* p = nullptr;
+  if (c->hp.alloc) {
+    p = c->hp.alloc(bytes, c->hp.alloc_ctx);
+    if (p && (reinterpret_cast<uintptr_t>(p) & 255u)) {      // contract: 256-byte alignment (TMA, 16-byte vector access)
+      if (c->hp.dealloc) c->hp.dealloc(p, c->hp.alloc_ctx);
+      c->error = "alloc callback returned memory that is not aligned to 256 bytes";
+      return nullptr;
+    }
+  } else if (cudaMalloc(&p, bytes) != cudaSuccess) {
+    (void)cudaGetLastError();
+    p = nullptr;
+  }
+  if (!p) return nullptr;
+  c->allocs.push_back(p);
+  c->device_bytes += bytes;
+  return p;
+}
+}  // namespace etx
+
 extern "C" {
 
 etx_status etx_create(const void* blob, size_t blob_bytes, const etx_hyperparams* hp, etx_handle* out) {
@@ -285,6 +305,7 @@ etx_status etx_create(const void* blob, size_t blob_bytes, const etx_hyperparams
   c->precision = hp->precision; c->engine = hp->engine;
   auto bail = [&](etx_status st) { etx_destroy(c); return st; };
   if (hp->precision < 0 || hp->precision > 2 || hp->engine < 0 || hp->engine > 2) return bail(ETX_ERR_ARG);
+  if ((hp->alloc == nullptr) != (hp->dealloc == nullptr)) return bail(ETX_ERR_ARG);
   if (hp->n_planes < 1 || hp->n_planes > 1024 || hp->k < 1 || hp->window < 1 || hp->max_events < 0 || hp->max_hits < 0 ||
       hp->gnn_iters < 0 || hp->gnn_iters > 64 || hp->emb_n_hidden_layers < 1 || hp->emb_n_hidden_layers > 8 ||
       !(hp->threshold >= 0.0f && hp->threshold <= 1.0f) || isnan(hp->d2_max))
@@ -369,7 +390,7 @@ etx_status etx_create(const void* blob, size_t blob_bytes, const etx_hyperparams
 etx_status etx_destroy(etx_handle c) {
   if (!c) return ETX_OK;
   cudaDeviceSynchronize();
-  for (void* p : c->allocs) cudaFree(p);
+  for (void* p : c->allocs) { if (c->hp.alloc) { if (c->hp.dealloc) c->hp.dealloc(p, c->hp.alloc_ctx); } else cudaFree(p); }
   if (c->tap) cudaFree(c->tap);
   if (c->h_event_off) cudaFreeHost(c->h_event_off);
   if (c->h_n_edges) cudaFreeHost(c->h_n_edges);
@@ -459,6 +480,8 @@ const char* etx_status_string(etx_status s) {
 }
 
 const char* etx_last_error(etx_handle c) { return c ? c->error.c_str() : "null handle"; }
+
+size_t etx_workspace_bytes(etx_handle c) { return c ? c->device_bytes : 0; }
 
 etx_status etx_dbg_buffer(etx_handle c, const char* name, const void** d_ptr, size_t* bytes) {
   if (!c || !name || !d_ptr || !bytes) return ETX_ERR_ARG;

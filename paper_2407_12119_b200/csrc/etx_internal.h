@@ -79,7 +79,8 @@ struct etx_ctx {
   std::string error;
   std::vector<etx::HostLayer> layers;     // blob order
   int i_emb0 = 0, i_nenc = 0, i_eenc = 0, i_iter0 = 0, i_head = 0;
-  std::vector<void*> allocs;              // every cudaMalloc of this handle
+  std::vector<void*> allocs;              // every device block of this handle (etx_device_alloc)
+  size_t device_bytes = 0;
   // workspace
   int32_t* event_off = nullptr;           // [max_events + 1]
   int32_t* plane_off = nullptr;           // [max_events][P + 1]
@@ -131,6 +132,8 @@ struct etx_ctx {
 namespace etx {
 
 // ---- launchers (each file owns its kernels) -------------------------------------------------------------
+// etx_api.cu: device memory through the handle's allocator (hp.alloc or cudaMalloc); nullptr on failure
+void* etx_device_alloc(etx_ctx* c, size_t bytes);
 // k_graph.cu
 void launch_features(etx_ctx* c, const float* xyz, int n_hits, cudaStream_t s);
 void launch_plane_offsets(etx_ctx* c, const int32_t* plane, int n_events, cudaStream_t s);

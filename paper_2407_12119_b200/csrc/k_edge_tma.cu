@@ -657,9 +657,8 @@ std::vector<uint8_t> pack_identity(int D) {
 }
 
 void* upload_bytes(etx_ctx* c, const std::vector<uint8_t>& v) {
-  void* p = nullptr;
-  if (cudaMalloc(&p, v.size()) != cudaSuccess) return nullptr;
-  c->allocs.push_back(p);
+  void* p = etx_device_alloc(c, v.size());
+  if (!p) return nullptr;
   cudaMemcpy(p, v.data(), v.size(), cudaMemcpyHostToDevice);
   return p;
 }

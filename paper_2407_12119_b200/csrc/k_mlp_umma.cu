@@ -504,9 +504,8 @@ void umma_configure(etx_ctx* c) {
     int KB = seg * esz; if (KB > 128) KB = 128;
     const int n_pad = l.out < 16 ? 16 : l.out;
     std::vector<uint8_t> img = pack_weight_image(l.W, l.out, l.in, n_pad, esz, KB);
-    void* p = nullptr;
-    if (cudaMalloc(&p, img.size()) != cudaSuccess) { c->error = "cudaMalloc(weight image)"; return; }
-    c->allocs.push_back(p);
+    void* p = etx_device_alloc(c, img.size());
+    if (!p) { c->error = "device allocation (weight image)"; return; }
     cudaMemcpy(p, img.data(), img.size(), cudaMemcpyHostToDevice);
     l.dev.Wtc = p;
   }

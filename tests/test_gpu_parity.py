@@ -441,3 +441,45 @@ def test_two_handles_on_two_streams_run_concurrently_and_agree_with_sequential_r
         assert r["n_edges"] == ref[k]["n_edges"]
         for name in ("src", "dst", "score", "logit", "track_id"):
             assert np.array_equal(r[name].cpu().numpy(), ref[k][name]), (k, name)
+
+
+def test_custom_allocator_callbacks_serve_every_device_block():
+    # include/etx.h: hp.alloc / hp.dealloc (Allen-style arena).  Every device block of the handle must
+    # come from the callback (sum of requests == etx_workspace_bytes), results must equal the cudaMalloc handle's,
+    # every block must be handed back by etx_destroy, and a misaligned or half-specified allocator is refused.
+    import ctypes as C
+    import paper_2407_12119_b200 as etx
+    from paper_2407_12119_b200.binding import ALLOC_FN, DEALLOC_FN
+    cfg, b, W = _setup("cfg1", 2, precision="bf16")
+    blob = datagen.pack_blob(cfg, W)
+    ref = run_gpu(make_ctx(cfg, blob, b), b, debug=False)
+    live, total = {}, [0]
+
+    def alloc(nbytes, _ctx):
+        t = torch.empty(int(nbytes) + 256, dtype=torch.uint8, device="cuda")
+        p = (t.data_ptr() + 255) // 256 * 256
+        live[p] = t; total[0] += int(nbytes)
+        return p
+
+    def dealloc(p, _ctx):
+        if live.pop(p, None) is None:
+            del live[p - 16]                                 # the deliberately misaligned block of the last case
+
+    a_cb, d_cb = ALLOC_FN(alloc), DEALLOC_FN(dealloc)
+    hp = etx.hyperparams_from_config(cfg, b.n_events, b.n_hits)
+    hp.alloc, hp.dealloc = a_cb, d_cb
+    ctx = etx.Etx(blob, hp)
+    assert len(live) > 20 and ctx.workspace_bytes() == total[0]
+    g = run_gpu(ctx, b, debug=False)
+    for name in ("src", "dst", "score", "logit", "track_id"):
+        assert np.array_equal(g[name], ref[name]), name
+    ctx.destroy()
+    assert not live
+    hp2 = etx.hyperparams_from_config(cfg, b.n_events, b.n_hits)
+    hp2.alloc = a_cb                                         # alloc without dealloc
+    with pytest.raises(etx.EtxError):
+        etx.Etx(blob, hp2)
+    hp3 = etx.hyperparams_from_config(cfg, b.n_events, b.n_hits)
+    hp3.alloc, hp3.dealloc = ALLOC_FN(lambda n, c: alloc(n, c) + 16), d_cb      # misaligned blocks
+    with pytest.raises(etx.EtxError):
+        etx.Etx(blob, hp3)
