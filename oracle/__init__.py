@@ -89,6 +89,9 @@ def lib():
         L.etxo_logit_threshold.argtypes = [C.c_float]
         L.etxo_components.argtypes = [C.POINTER(C.c_int32), C.POINTER(C.c_int32), C.POINTER(C.c_float),
                                       C.c_int64, C.c_float, C.c_int64, C.POINTER(C.c_int32)]
+        L.etxo_tracks.restype = C.c_int64
+        L.etxo_tracks.argtypes = [C.POINTER(C.c_int32), C.c_int64, C.POINTER(C.c_int32), C.c_int64, C.c_int32,
+                                  C.POINTER(C.c_int32), C.POINTER(C.c_int32), C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
         _lib = L
     return _lib
 
@@ -166,6 +169,18 @@ def components(src, dst, logit, tau, n):
     lib().etxo_components(_p(src, C.c_int32), _p(dst, C.c_int32), _p(logit, C.c_float), src.size,
                           C.c_float(tau), n, _p(out, C.c_int32))
     return out
+
+
+def tracks(track_id, event_offsets, min_hits=3):
+    """Track containers from the per-hit component labels (etxo_tracks)."""
+    tid, eo = _i32(track_id), _i32(event_offsets)
+    n, B = tid.size, eo.size - 1
+    index = np.zeros(n, np.int32); offs = np.zeros(n + 1, np.int32); hits = np.zeros(max(n, 1), np.int32)
+    ev = np.zeros(B + 1, np.int32)
+    T = int(lib().etxo_tracks(_p(tid, C.c_int32), n, _p(eo, C.c_int32), B, int(min_hits), _p(index, C.c_int32),
+                              _p(offs, C.c_int32), _p(hits, C.c_int32), _p(ev, C.c_int32)))
+    return dict(n_tracks=T, track_index=index, track_offsets=offs[:T + 1].copy(), track_hits=hits[:offs[T]].copy(),
+                event_track_offsets=ev)
 
 
 class Oracle:

@@ -22,6 +22,7 @@
 //   scatter-sum  : dense 0/1 incidence-matrix product (Eq.(4))
 //   head         : sigmoid closed forms, threshold boundary (L80)
 //   components   : scipy.sparse.csgraph + BFS + the paper's plane sweeps iterated
+//   tracks       : dictionary-based regrouping in Python, partition / ordering invariants, truth particles
 //   The paper prints no worked numerical example, so no value
 //   here is pinned to a number printed by the paper.
 //
@@ -537,6 +538,45 @@ void etxo_components(const int32_t* src, const int32_t* dst, const float* logit,
     if (a < b) parent[b] = a; else parent[a] = b;
   }
   for (int64_t i = 0; i < n; ++i) track_id[i] = find((int32_t)i);
+}
+
+// ---------------------------------------------------------------------------
+// Track containers (a particle is reconstructible in the VELO with at
+// least three hits; L74, L82: the output of the pipeline is the set of tracks, each a list of hits).  A track is
+// a connected component with at least min_hits hits.  Tracks are numbered densely in ascending order of their
+// smallest hit index (= their track_id), so the tracks of one event are consecutive; hits inside a track are in
+// ascending hit index.  Outputs:
+//   track_index[n]        dense track number of the hit's track, or -1 (component too small)
+//   track_offsets[T + 1]  CSR offsets into track_hits            (capacity n + 1)
+//   track_hits[...]       hit indices, track after track          (capacity n)
+//   event_track_off[B+1]  first dense track number of every event
+// Returns T.  Plain loops: count, number, fill.
+int64_t etxo_tracks(const int32_t* track_id, int64_t n, const int32_t* event_off, int64_t n_events, int32_t min_hits,
+                    int32_t* track_index, int32_t* track_offsets, int32_t* track_hits, int32_t* event_track_off) {
+  std::vector<int32_t> size(n, 0), number(n, -1);
+  for (int64_t h = 0; h < n; ++h) size[track_id[h]] += 1;             // component size, stored at its root
+  int64_t T = 0;
+  track_offsets[0] = 0;
+  for (int64_t r = 0; r < n; ++r) {                                   // roots in ascending order
+    if (track_id[r] == r && size[r] >= min_hits) {
+      number[r] = (int32_t)T;
+      track_offsets[T + 1] = track_offsets[T] + size[r];
+      ++T;
+    }
+  }
+  std::vector<int32_t> cursor(track_offsets, track_offsets + T);
+  for (int64_t h = 0; h < n; ++h) {                                   // hits in ascending order -> ascending inside a track
+    const int32_t t = number[track_id[h]];
+    track_index[h] = t;
+    if (t >= 0) track_hits[cursor[t]++] = (int32_t)h;
+  }
+  for (int64_t e = 0; e <= n_events; ++e) {                           // tracks whose root lies before the event's first hit
+    int64_t cnt = 0;
+    const int64_t lim = e < n_events ? event_off[e] : n;
+    for (int64_t r = 0; r < lim; ++r) cnt += number[r] >= 0;
+    event_track_off[e] = (int32_t)cnt;
+  }
+  return T;
 }
 
 }  // extern "C"

@@ -515,3 +515,66 @@ def test_generator_shapes_follow_baseline_configs():
     assert 0.01 < np.mean(b1.particle < 0) < 0.035
     again = datagen.generate_batch(datagen.get_config("cfg1"), n_events=2, first_event=3)
     assert np.array_equal(again.xyz, b1.slice_events(3, 5).xyz)
+
+
+# ---------------------------------------------------------------------------------- track containers
+def _tracks_by_dict(track_id, event_offsets, min_hits):
+    """Independent regrouping with Python containers (no shared code with the oracle)."""
+    groups = {}
+    for h, t in enumerate(track_id.tolist()):
+        groups.setdefault(t, []).append(h)
+    kept = sorted(t for t, hs in groups.items() if len(hs) >= min_hits)
+    index = np.full(track_id.size, -1, np.int32)
+    hits, offs = [], [0]
+    for num, t in enumerate(kept):
+        index[groups[t]] = num
+        hits += sorted(groups[t]); offs.append(len(hits))
+    ev = [sum(1 for t in kept if t < lim) for lim in list(event_offsets[:-1]) + [track_id.size]]
+    return len(kept), index, np.asarray(offs, np.int32), np.asarray(hits, np.int32), np.asarray(ev, np.int32)
+
+
+@pytest.mark.parametrize("min_hits", [1, 3, 5])
+def test_tracks_equal_an_independent_regrouping_and_are_a_partition(min_hits):
+    rng = np.random.default_rng(11 + min_hits)
+    sizes = [0, 40, 3, 0, 120, 1]
+    off = np.concatenate([[0], np.cumsum(sizes)]).astype(np.int32)
+    n = int(off[-1])
+    tid = np.arange(n, dtype=np.int32)
+    for e in range(len(sizes)):                       # random components inside every event, label = smallest member
+        lo, hi = int(off[e]), int(off[e + 1])
+        lab = rng.integers(0, max(1, (hi - lo) // 4), hi - lo)
+        for v in np.unique(lab):
+            members = lo + np.flatnonzero(lab == v)
+            tid[members] = members.min()
+    r = oracle.tracks(tid, off, min_hits)
+    T, index, offs, hits, ev = _tracks_by_dict(tid, off, min_hits)
+    assert r["n_tracks"] == T
+    assert np.array_equal(r["track_index"], index) and np.array_equal(r["track_offsets"], offs)
+    assert np.array_equal(r["track_hits"], hits) and np.array_equal(r["event_track_offsets"], ev)
+    # invariants: kept hits are partitioned, every track has >= min_hits hits in ascending order, inside one event
+    assert np.array_equal(np.sort(r["track_hits"]), np.flatnonzero(r["track_index"] >= 0))
+    evt = np.repeat(np.arange(len(sizes)), sizes)
+    for t in range(T):
+        hs = r["track_hits"][r["track_offsets"][t]:r["track_offsets"][t + 1]]
+        assert hs.size >= min_hits and (np.diff(hs) > 0).all()
+        assert (r["track_index"][hs] == t).all() and np.unique(evt[hs]).size == 1 and tid[hs[0]] == hs[0]
+        assert r["event_track_offsets"][evt[hs[0]]] <= t < r["event_track_offsets"][evt[hs[0]] + 1]
+
+
+def test_tracks_on_a_noise_free_event_are_the_particles_with_three_hits():
+    # PAPER.md L42: reconstructible = at least three hits.  With the truth edge set every particle is one component,
+    # so the tracks at min_hits = 3 are exactly the generated particles that left >= 3 hits.
+    cfg = datagen.get_config("cfg0")
+    b = datagen.generate_batch(cfg, n_events=1, seed=5)
+    src, dst = [], []
+    for pid in np.unique(b.particle):
+        hs = np.flatnonzero(b.particle == pid)
+        src += hs[:-1].tolist(); dst += hs[1:].tolist()
+    src, dst = np.asarray(src, np.int32), np.asarray(dst, np.int32)
+    tid = oracle.components(src, dst, np.ones(src.size, np.float32), 0.0, b.n_hits)
+    r = oracle.tracks(tid, b.event_offsets, 3)
+    counts = np.bincount(b.particle.astype(np.int64))
+    assert r["n_tracks"] == int((counts >= 3).sum())
+    for t in range(r["n_tracks"]):
+        hs = r["track_hits"][r["track_offsets"][t]:r["track_offsets"][t + 1]]
+        assert np.unique(b.particle[hs]).size == 1 and hs.size == counts[b.particle[hs[0]]]
