@@ -122,6 +122,23 @@ etx_status etx_run_host(etx_handle h, const float* h_xyz, const int32_t* h_plane
                         float* h_edge_score, int32_t* h_edge_src, int32_t* h_edge_dst,
                         int32_t* h_track_id, int32_t* n_edges_out);
 
+/* Track containers (L42: a particle is reconstructible with at least three VELO hits; L74, L82: the product of
+ * the pipeline is the set of tracks, each a list of hits).  Enqueue on `stream`, after an etx_run on the same
+ * stream and handle, the regrouping of its track ids: a track is a component with at least min_hits hits; tracks
+ * are numbered densely in ascending order of their smallest hit index (so the tracks of an event are
+ * consecutive); the hits of a track are listed in ascending hit index.  Library-owned device pointers, valid
+ * until the next call on the handle; no synchronisation. */
+typedef struct {
+  const int32_t* d_track_index;          /* [n_hits]        dense track number of the hit, or -1            */
+  const int32_t* d_track_offsets;        /* [n_tracks + 1]  CSR offsets into d_track_hits                   */
+  const int32_t* d_track_hits;           /* [offsets[n_tracks]] hit indices, track after track              */
+  const int32_t* d_event_track_offsets;  /* [n_events + 1]  first track number of every event               */
+  const int32_t* d_n_tracks;             /* device scalar                                                   */
+  const int32_t* h_n_tracks;             /* pinned host mirror; valid once the stream has been synchronised */
+} etx_tracks_output;
+
+etx_status etx_tracks(etx_handle h, int32_t min_hits, etx_stream stream, etx_tracks_output* out);
+
 etx_status etx_destroy(etx_handle h);
 
 /* Device bytes held by the handle (workspace + converted weights), as requested from the allocator. */

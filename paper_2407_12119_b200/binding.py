@@ -44,6 +44,11 @@ class EtxOutput(C.Structure):
                 ("h_n_edges", C.POINTER(C.c_int32)), ("n_hits", C.c_int32)]
 
 
+class EtxTracks(C.Structure):
+    _fields_ = [("d_track_index", C.c_void_p), ("d_track_offsets", C.c_void_p), ("d_track_hits", C.c_void_p),
+                ("d_event_track_offsets", C.c_void_p), ("d_n_tracks", C.c_void_p), ("h_n_tracks", C.POINTER(C.c_int32))]
+
+
 class Inject(C.Structure):
     _fields_ = [("d_emb", C.c_void_p), ("d_src", C.c_void_p), ("d_dst", C.c_void_p), ("n_edges", C.c_int32),
                 ("d_logit", C.c_void_p), ("last_stage", C.c_int32)]
@@ -81,6 +86,8 @@ def load_library():
     L.etx_run_host.argtypes = [vp, vp, vp, i32p, C.c_int32, vp, vp, vp, vp, vp, i32p]
     L.etx_destroy.restype = C.c_int
     L.etx_destroy.argtypes = [vp]
+    L.etx_tracks.restype = C.c_int
+    L.etx_tracks.argtypes = [vp, C.c_int32, vp, C.POINTER(EtxTracks)]
     L.etx_workspace_bytes.restype = C.c_size_t
     L.etx_workspace_bytes.argtypes = [vp]
     L.etx_status_string.restype = C.c_char_p
@@ -224,6 +231,20 @@ class Etx:
         arr = (C.c_float * len(STAGE_NAMES))()
         self._check(self._L.etx_dbg_stage_times(self._h, arr), "etx_dbg_stage_times")
         return {n: float(v) for n, v in zip(STAGE_NAMES, arr)}
+
+    def tracks(self, n_hits: int, n_events: int, min_hits: int = 3) -> dict:
+        """etx_tracks on the current stream after a run over (n_events, n_hits); synchronises, returns torch tensors."""
+        import torch
+        out = EtxTracks()
+        self._check(self._L.etx_tracks(self._h, int(min_hits), self._stream(), C.byref(out)), "etx_tracks")
+        torch.cuda.current_stream().synchronize()
+        T = int(out.h_n_tracks[0])
+        offs = self._copy_out(out.d_track_offsets, 4 * (T + 1), torch.int32)
+        n_hits_kept = int(offs[-1].item()) if T else 0
+        return dict(n_tracks=T, track_offsets=offs,
+                    track_index=self._copy_out(out.d_track_index, 4 * n_hits, torch.int32),
+                    track_hits=self._copy_out(out.d_track_hits, 4 * n_hits_kept, torch.int32),
+                    event_track_offsets=self._copy_out(out.d_event_track_offsets, 4 * (n_events + 1), torch.int32))
 
     def workspace_bytes(self) -> int:
         return int(self._L.etx_workspace_bytes(self._h))

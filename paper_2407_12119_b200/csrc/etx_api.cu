@@ -172,7 +172,7 @@ etx_status run_impl(etx_ctx* c, const float* d_xyz, const int32_t* d_plane, cons
     ETX_CUDA(cudaEventRecord(c->staging_free, s));
     ETX_CUDA(cudaMemsetAsync(c->n_edges, 0, sizeof(int32_t), s));
     c->n_ev = 0; c->spans.clear();
-    c->last_n_hits = n_hits;
+    c->last_n_hits = n_hits; c->last_n_events = n_events;
     StageTimer tm{c, s};
     bool edges_marked = false;
     const bool tensor_engine = (c->precision != ETX_FP32) && c->engine != ETX_ENGINE_SIMT;
@@ -352,12 +352,19 @@ etx_status etx_create(const void* blob, size_t blob_bytes, const etx_hyperparams
     c->score = dev_alloc<float>(c, E);
     c->score_out = c->score;
     c->track_id = dev_alloc<int32_t>(c, N);
+    c->trk_size = dev_alloc<int32_t>(c, N); c->trk_keep = dev_alloc<int32_t>(c, N + 1);
+    c->trk_number = dev_alloc<int32_t>(c, N + 1); c->trk_ksize = dev_alloc<int32_t>(c, N + 1);
+    c->trk_index = dev_alloc<int32_t>(c, N); c->trk_offsets = dev_alloc<int32_t>(c, N + 1);
+    c->trk_hits = dev_alloc<int32_t>(c, N); c->trk_event_off = dev_alloc<int32_t>(c, B + 1);
+    c->n_tracks = dev_alloc<int32_t>(c, 1);
     c->d_xyz_in = dev_alloc<float>(c, N * 3);
     c->d_plane_in = dev_alloc<int32_t>(c, N);
     ETX_CUDA(cudaMemset(c->n_edges, 0, sizeof(int32_t)));
     ETX_CUDA(cudaMemset(c->flags, 0, sizeof(int32_t)));
     ETX_CUDA(cudaMallocHost(&c->h_event_off, sizeof(int32_t) * (B + 1)));
     ETX_CUDA(cudaMallocHost(&c->h_n_edges, sizeof(int32_t)));
+    ETX_CUDA(cudaMallocHost(&c->h_n_tracks, sizeof(int32_t)));
+    c->h_n_tracks[0] = 0;
     ETX_CUDA(cudaMallocHost(&c->h_flags, sizeof(int32_t)));
     c->h_n_edges[0] = 0; c->h_flags[0] = 0;
     ETX_CUDA(cudaEventCreateWithFlags(&c->staging_free, cudaEventDisableTiming));
@@ -394,6 +401,7 @@ etx_status etx_destroy(etx_handle c) {
   if (c->tap) cudaFree(c->tap);
   if (c->h_event_off) cudaFreeHost(c->h_event_off);
   if (c->h_n_edges) cudaFreeHost(c->h_n_edges);
+  if (c->h_n_tracks) cudaFreeHost(c->h_n_tracks);
   if (c->h_flags) cudaFreeHost(c->h_flags);
   if (c->staging_free) cudaEventDestroy(c->staging_free);
   if (c->edges_ready) cudaEventDestroy(c->edges_ready);
@@ -407,6 +415,19 @@ etx_status etx_destroy(etx_handle c) {
 etx_status etx_run(etx_handle c, const float* d_xyz, const int32_t* d_plane, const int32_t* h_event_offsets,
                    int32_t n_events, etx_stream stream, etx_output* out) {
   return run_impl(c, d_xyz, d_plane, h_event_offsets, n_events, static_cast<cudaStream_t>(stream), nullptr, out);
+}
+
+etx_status etx_tracks(etx_handle c, int32_t min_hits, etx_stream stream, etx_tracks_output* out) {
+  if (!c) return ETX_ERR_ARG;
+  if (!out || min_hits < 1) return fail(c, ETX_ERR_ARG, "etx_tracks: null output or min_hits < 1");
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  launch_tracks(c, c->last_n_events, c->last_n_hits, min_hits, s);
+  if (cudaMemcpyAsync(c->h_n_tracks, c->n_tracks, sizeof(int32_t), cudaMemcpyDeviceToHost, s) != cudaSuccess ||
+      cudaGetLastError() != cudaSuccess)
+    return fail(c, ETX_ERR_CUDA, "etx_tracks: launch failed");
+  out->d_track_index = c->trk_index; out->d_track_offsets = c->trk_offsets; out->d_track_hits = c->trk_hits;
+  out->d_event_track_offsets = c->trk_event_off; out->d_n_tracks = c->n_tracks; out->h_n_tracks = c->h_n_tracks;
+  return ETX_OK;
 }
 
 etx_status etx_dbg_run(etx_handle c, const float* d_xyz, const int32_t* d_plane, const int32_t* h_event_offsets,

@@ -96,6 +96,11 @@ struct etx_ctx {
   float *logit = nullptr, *score = nullptr;
   float* score_out = nullptr;             // where the classifier writes scores: `score`, or the caller's mapped host buffer (etx_run_host)
   int32_t *track_id = nullptr;
+  // track containers (etx_tracks): component sizes, keep flags / cursors, dense numbers, kept sizes, outputs
+  int32_t *trk_size = nullptr, *trk_keep = nullptr, *trk_number = nullptr, *trk_ksize = nullptr;
+  int32_t *trk_index = nullptr, *trk_offsets = nullptr, *trk_hits = nullptr, *trk_event_off = nullptr;
+  int32_t *n_tracks = nullptr, *h_n_tracks = nullptr;
+  int last_n_events = 0;
   // k_edge_tma.cu: identity operand image, split-bias images [2 * iter + layer], CUtensorMap of `e` (opaque here)
   bool edge_tma = false;
   bool edge_i8 = false;                   // k_edge_i8.cu usable (INT8, auto engine, tensor map of fp32 `e` encoded)
@@ -143,6 +148,7 @@ void launch_pack_edges(etx_ctx* c, int n_hits, cudaStream_t s);                 
 void launch_rows_from_src(etx_ctx* c, int n_hits, int n_edges, cudaStream_t s); // injected edge list -> row_ptr
 void launch_csc(etx_ctx* c, int n_events, int n_hits, bool windowed, cudaStream_t s);                        // dst -> col_ptr, in_edge
 void launch_components(etx_ctx* c, const float* logit, int n_events, int n_hits, cudaStream_t s);
+void launch_tracks(etx_ctx* c, int n_events, int n_hits, int min_hits, cudaStream_t s);
 // k_mlp_simt.cu
 void launch_embed_simt(etx_ctx* c, int n_hits, cudaStream_t s);
 void launch_gnn_mlp_simt(etx_ctx* c, int kind, int iter, int n_hits, bool do_head, cudaStream_t s);

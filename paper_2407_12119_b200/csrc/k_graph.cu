@@ -518,4 +518,86 @@ void launch_components(etx_ctx* c, const float* logit, int n_events, int n_hits,
   c->launches += 1;
 }
 
+// --------------------------------------------------------------------------------------------------------
+// Track containers (reconstructible = at least three hits; L74, L82: the pipeline's product is the
+// set of tracks, each a list of hits).  A track is a component with >= min_hits hits;
+// tracks are numbered densely in ascending order of their root (= smallest hit index = track_id), so the tracks
+// of an event are consecutive; hits inside a track ascend.
+__global__ void trk_size_kernel(const int32_t* __restrict__ track_id, int n, int32_t* __restrict__ size) {
+  const int h = blockIdx.x * blockDim.x + threadIdx.x;
+  if (h < n) atomicAdd(&size[track_id[h]], 1);
+}
+__global__ void trk_keep_kernel(const int32_t* __restrict__ track_id, const int32_t* __restrict__ size, int n, int min_hits,
+                                int32_t* __restrict__ keep) {
+  const int r = blockIdx.x * blockDim.x + threadIdx.x;
+  if (r < n) keep[r] = (track_id[r] == r && size[r] >= min_hits) ? 1 : 0;
+}
+// number[r] = exclusive scan of keep: dense number of root r.  Sizes of the kept tracks in dense order, and per hit
+// the dense number of its track (or -1).
+__global__ void trk_index_kernel(const int32_t* __restrict__ track_id, const int32_t* __restrict__ size,
+                                 const int32_t* __restrict__ number, int n, int min_hits,
+                                 int32_t* __restrict__ track_index, int32_t* __restrict__ ksize) {
+  const int h = blockIdx.x * blockDim.x + threadIdx.x;
+  if (h >= n) return;
+  const int r = track_id[h];
+  const bool kept = size[r] >= min_hits;
+  track_index[h] = kept ? number[r] : -1;
+  if (kept && r == h) ksize[number[r]] = size[r];
+}
+__global__ void trk_event_kernel(const int32_t* __restrict__ event_off, const int32_t* __restrict__ number, int n_events,
+                                 int32_t* __restrict__ event_track_off) {
+  const int e = blockIdx.x * blockDim.x + threadIdx.x;
+  if (e <= n_events) event_track_off[e] = number[event_off[e]];
+}
+// One warp per event walks the event's hits in ascending order, 32 per step; the lanes of a step that share a track
+// are ranked with match.any and the lowest advances the track's cursor, so every hit list ascends by construction.
+// The cursors of an event's tracks are touched by this warp only.
+__global__ void __launch_bounds__(256)
+trk_fill_kernel(const int32_t* __restrict__ track_index, const int32_t* __restrict__ track_offsets,
+                const int32_t* __restrict__ event_off, const int32_t* __restrict__ event_track_off, int n_events,
+                int32_t* cursor, int32_t* __restrict__ track_hits) {
+  const int e = blockIdx.x * 8 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+  if (e >= n_events) return;
+  const int h0 = event_off[e], h1 = event_off[e + 1];
+  const int t0 = event_track_off[e], t1 = event_track_off[e + 1];
+  volatile int32_t* cur = cursor;
+  for (int t = t0 + lane; t < t1; t += 32) cur[t] = track_offsets[t];
+  __syncwarp();
+  for (int i0 = h0; i0 < h1; i0 += 32) {
+    const int h = i0 + lane;
+    const int t = h < h1 ? track_index[h] : -1;
+    const unsigned active = __ballot_sync(0xffffffffu, t >= 0);
+    if (t >= 0) {
+      const unsigned peers = __match_any_sync(active, t);
+      const int leader = __ffs(peers) - 1, rank = __popc(peers & ((1u << lane) - 1u));
+      int pos = 0;
+      if (lane == leader) { pos = cur[t]; cur[t] = pos + __popc(peers); }
+      pos = __shfl_sync(peers, pos, leader);
+      track_hits[pos + rank] = h;
+    }
+    __syncwarp();
+  }
+}
+
+void launch_tracks(etx_ctx* c, int n_events, int n_hits, int min_hits, cudaStream_t s) {
+  cudaMemsetAsync(c->n_tracks, 0, sizeof(int32_t), s);
+  if (n_hits == 0 || n_events == 0) {
+    cudaMemsetAsync(c->trk_event_off, 0, sizeof(int32_t) * ((size_t)n_events + 1), s);
+    cudaMemsetAsync(c->trk_offsets, 0, sizeof(int32_t), s);
+    return;
+  }
+  const int g = (n_hits + 255) / 256;
+  cudaMemsetAsync(c->trk_size, 0, sizeof(int32_t) * (size_t)n_hits, s);
+  cudaMemsetAsync(c->trk_ksize, 0, sizeof(int32_t) * (size_t)n_hits, s);
+  trk_size_kernel<<<g, 256, 0, s>>>(c->track_id, n_hits, c->trk_size);
+  trk_keep_kernel<<<g, 256, 0, s>>>(c->track_id, c->trk_size, n_hits, min_hits, c->trk_keep);
+  exclusive_scan(c, c->trk_keep, n_hits, c->trk_number, c->n_tracks, s);
+  trk_index_kernel<<<g, 256, 0, s>>>(c->track_id, c->trk_size, c->trk_number, n_hits, min_hits, c->trk_index, c->trk_ksize);
+  exclusive_scan(c, c->trk_ksize, n_hits, c->trk_offsets, nullptr, s);       // entries >= n_tracks repeat the total
+  trk_event_kernel<<<(n_events + 256) / 256, 256, 0, s>>>(c->event_off, c->trk_number, n_events, c->trk_event_off);
+  trk_fill_kernel<<<(n_events + 7) / 8, 256, 0, s>>>(c->trk_index, c->trk_offsets, c->event_off, c->trk_event_off, n_events,
+                                                     c->trk_keep, c->trk_hits);      // trk_keep is free again: cursors
+  c->launches += 5;
+}
+
 }  // namespace etx

@@ -93,6 +93,15 @@ def test_full_size_bf16_invariants_and_sampled_events(name, preset):
         mid = np.mean((g["score"] > 0.01) & (g["score"] < 0.99))
         assert mid > 0.3, mid
     print(f"{name}/{preset}: N={b.n_hits} E={g['n_edges']} sampled events {events} max|score err|={worst:.2e}")
+    if name == "cfg2":
+        # track containers over the whole batch (integer work: every array equals the oracle's), and their cost
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record(); t = ctx.tracks(b.n_hits, b.n_events, 3); ev1.record(); torch.cuda.synchronize()
+        r = oracle.tracks(g["track_id"], b.event_offsets, 3)
+        assert t["n_tracks"] == r["n_tracks"]
+        for key in ("track_index", "track_offsets", "track_hits", "event_track_offsets"):
+            assert np.array_equal(t[key].cpu().numpy(), r[key]), key
+        print(f"{name}/{preset}: etx_tracks(min_hits=3): {r['n_tracks']} tracks, {ev0.elapsed_time(ev1):.2f} ms incl. the copies back")
     ctx.destroy()
 
 

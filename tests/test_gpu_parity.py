@@ -483,3 +483,28 @@ def test_custom_allocator_callbacks_serve_every_device_block():
     hp3.alloc, hp3.dealloc = ALLOC_FN(lambda n, c: alloc(n, c) + 16), d_cb      # misaligned blocks
     with pytest.raises(etx.EtxError):
         etx.Etx(blob, hp3)
+
+
+@pytest.mark.parametrize("name,n_events,precision,min_hits", [("cfg1", 5, "fp32", 3), ("cfg1", 5, "bf16", 1), ("cfg0", 1, "fp32", 3),
+                                                              ("cfg4", 1, "bf16", 4)])
+def test_track_containers_bit_exact_against_the_oracle(name, n_events, precision, min_hits):
+    # etx_tracks regroups the run's track ids: dense numbering by smallest hit, >= min_hits filter,
+    # ascending hit lists.  All integer work: every array must equal the oracle's on the GPU's own track ids.
+    cfg, b, W = _setup(name, n_events, precision=precision)
+    blob = datagen.pack_blob(cfg, W)
+    ctx = make_ctx(cfg, blob, b)
+    g = run_gpu(ctx, b, debug=False)
+    t = ctx.tracks(b.n_hits, b.n_events, min_hits)
+    r = oracle.tracks(g["track_id"], b.event_offsets, min_hits)
+    assert t["n_tracks"] == r["n_tracks"] and r["n_tracks"] > 0
+    for key in ("track_index", "track_offsets", "track_hits", "event_track_offsets"):
+        assert np.array_equal(t[key].cpu().numpy(), r[key]), key
+    # empty batch and a second call with another filter on the same handle
+    t2 = ctx.tracks(b.n_hits, b.n_events, min_hits + 2)
+    r2 = oracle.tracks(g["track_id"], b.event_offsets, min_hits + 2)
+    assert t2["n_tracks"] == r2["n_tracks"] and np.array_equal(t2["track_hits"].cpu().numpy(), r2["track_hits"])
+    ne = min(2, b.n_events)                                  # within the handle's max_events
+    empty = datagen.EventBatch(np.zeros((0, 3), F), np.zeros(0, np.int32), np.zeros(ne + 1, np.int32), np.zeros(0, np.int64))
+    run_gpu(ctx, empty, debug=False)
+    t3 = ctx.tracks(0, ne, 3)
+    assert t3["n_tracks"] == 0 and np.array_equal(t3["event_track_offsets"].cpu().numpy(), np.zeros(ne + 1, np.int32))
