@@ -128,8 +128,9 @@ def stage_model(cfg, N, E, pairs, peaks):
         "S2_knn": ("alu", pairs * 12.0, alu_lane, "lane-instr/s"),
         "S3_compaction_csc": ("hbm", 4.0 * k * N + 12.0 * E + 12.0 * E + 16.0 * N, peaks["hbm"], "GB/s"),
         "S4_encoders": (mlp_bound, 2.0 * (3 * d + d * d) * (N + E), mlp_peak, "TFLOP/s"),
-        "S4c_scatter": ("hbm", L * (2.0 * E * d * b + 2.0 * N * d * b + 4.0 * E + 8.0 * N), peaks["hbm"], "GB/s"),
-        "S4d_node_net": ("hbm", L * (5.0 * N * d * b), peaks["hbm"], "GB/s"),
+        # e is read from HBM once (the second direction finds its rows in L2: ncu, profiles/r1f_stage_rooflines.md)
+        "S4c_scatter": ("hbm", L * (1.0 * E * d * b + 2.0 * N * d * b + 4.0 * E + 8.0 * N), peaks["hbm"], "GB/s"),
+        "S4d_node_net": ("hbm", L * (4.0 * N * d * b), peaks["hbm"], "GB/s"),
         "S4e_edge_net_head": ("hbm", L * ((2.0 * d * b + 8.0) * E + N * d * b) + 8.0 * E, peaks["hbm"], "GB/s"),
         "S5_components": ("hbm", 12.0 * E + 8.0 * N, peaks["hbm"], "GB/s"),
     }
