@@ -16,6 +16,8 @@ N_PLANES = 26
 PLANE_Z0, PLANE_DZ = -300.0, 42.0  # BASELINE.json cfg 0: z_i = -300 + 42 i
 NORM_OFFSET = (0.0, 0.0, 300.0)    # features (x/40, y/40, (z+300)/1050)
 NORM_DIV = (40.0, 40.0, 1050.0)
+CYL_OFFSET = (-20.0, 0.0, 300.0)   # cylindrical embedding input ((r-20)/12, phi/pi, (z+300)/1050): DESIGN.md R27
+CYL_DIV = (12.0, 3.14159274, 1050.0)
 
 
 @dataclass(frozen=True)
@@ -41,6 +43,7 @@ class EtxConfig:
     threshold: float
     precision: str              # "fp32" | "bf16" | "int8"
     edge_enc_input: int = 0     # 0: |f_dst - f_src| (configs), 1: [h0_src, h0_dst]
+    emb_input: int = 0          # 0: the embedding reads the Cartesian features, 1: normalised (r, phi, z) (L96, R27)
     weights_seed: int = 7
 
     def replace(self, **kw) -> "EtxConfig":

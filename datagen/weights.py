@@ -9,7 +9,7 @@ Blob (little-endian):
     [0] magic 'ETXW' (0x57585445)  [1] version = 1
     [2] emb_hidden  [3] emb_n_hidden_layers  [4] emb_dim
     [5] gnn_latent  [6] gnn_iters            [7] edge_enc_input
-    [8] n_weight_floats  [9] n_act_scales    [10..15] zero
+    [8] n_weight_floats  [9] n_act_scales    [10] emb_input   [11..15] zero
   then fp32 tensors, each Linear as W[out][in] row-major followed by b[out], in
   this order: embedding layers 0..H; node encoder (2); edge encoder (2); for each
   iteration: node net (2), edge net (2); head (1).  Concatenated inputs are
@@ -104,7 +104,7 @@ def pack_blob(cfg: EtxConfig, layers, act_scales: np.ndarray | None = None) -> b
     n_floats = len(body) // 4
     sc = np.zeros(0, "<f4") if act_scales is None else np.ascontiguousarray(act_scales, dtype="<f4")
     hdr = [BLOB_MAGIC, BLOB_VERSION, cfg.emb_hidden, cfg.emb_n_hidden_layers, cfg.emb_dim,
-           cfg.gnn_latent, cfg.gnn_iters, cfg.edge_enc_input, n_floats, int(sc.size)] + [0] * 6
+           cfg.gnn_latent, cfg.gnn_iters, cfg.edge_enc_input, n_floats, int(sc.size), cfg.emb_input] + [0] * 5
     return struct.pack("<16I", *hdr) + body + sc.tobytes()
 
 

@@ -35,7 +35,7 @@ def build(force: bool = False) -> str:
 
 class _Params(C.Structure):
     _fields_ = [("n_planes", C.c_int32), ("norm_offset", C.c_float * 3), ("norm_div", C.c_float * 3),
-                ("precision", C.c_int32)]
+                ("precision", C.c_int32), ("cyl_offset", C.c_float * 3), ("cyl_div", C.c_float * 3)]
 
 
 _lib = None
@@ -73,6 +73,7 @@ def lib():
         L.etxo_plane_offsets.argtypes = [C.POINTER(C.c_int32), C.POINTER(C.c_int32), C.c_int, C.c_int,
                                          C.POINTER(C.c_int32)]
         L.etxo_features.argtypes = [C.c_void_p, C.POINTER(C.c_float), C.c_int64, C.POINTER(C.c_float)]
+        L.etxo_features_emb.argtypes = [C.c_void_p, C.POINTER(C.c_float), C.c_int64, C.POINTER(C.c_float)]
         L.etxo_embed.argtypes = [C.c_void_p, C.POINTER(C.c_float), C.c_int64, C.POINTER(C.c_float)]
         L.etxo_knn.argtypes = [C.POINTER(C.c_float), C.c_int64, C.c_int, C.POINTER(C.c_int32),
                                C.POINTER(C.c_int32), C.c_int, C.c_int, C.c_int, C.c_int, C.c_float,
@@ -187,9 +188,10 @@ class Oracle:
     """One model (weights blob + precision mode).  Methods mirror the stages of the hot path."""
 
     def __init__(self, blob: bytes, precision: str = "fp32", n_planes: int = 26,
-                 norm_offset=(0.0, 0.0, 300.0), norm_div=(40.0, 40.0, 1050.0)):
+                 norm_offset=(0.0, 0.0, 300.0), norm_div=(40.0, 40.0, 1050.0),
+                 cyl_offset=(-20.0, 0.0, 300.0), cyl_div=(12.0, 3.14159274, 1050.0)):
         prm = _Params(n_planes, (C.c_float * 3)(*norm_offset), (C.c_float * 3)(*norm_div),
-                      PRECISION[precision])
+                      PRECISION[precision], (C.c_float * 3)(*cyl_offset), (C.c_float * 3)(*cyl_div))
         self._blob = bytes(blob)
         self._h = lib().etxo_create(self._blob, len(self._blob), C.byref(prm))
         err = lib().etxo_error(self._h).decode()
@@ -202,6 +204,7 @@ class Oracle:
         import struct
         hdr = struct.unpack("<16I", self._blob[:64])
         self.emb_dim, self.latent = hdr[4], hdr[5]
+        self.emb_input = hdr[10]          # 0: Cartesian features, 1: cylindrical (R27)
 
     def __del__(self):
         if getattr(self, "_h", None):
@@ -212,6 +215,13 @@ class Oracle:
         xyz = _f32(xyz)
         out = np.zeros_like(xyz)
         lib().etxo_features(self._h, _p(xyz, C.c_float), xyz.shape[0], _p(out, C.c_float))
+        return out
+
+    def features_emb(self, xyz):
+        """Input of the embedding MLP (the Cartesian features, or normalised (r, phi, z) when the blob says so)."""
+        xyz = _f32(xyz)
+        out = np.zeros_like(xyz)
+        lib().etxo_features_emb(self._h, _p(xyz, C.c_float), xyz.shape[0], _p(out, C.c_float))
         return out
 
     def embed(self, xyz):

@@ -10,10 +10,11 @@
 // is never a fallback for it.
 //
 // Every function cites the passage it follows.  Where the paper is silent the
-// reading is the one listed in DESIGN.md section 4 ("Readings"), numbered R1..R26.
+// reading is the one listed in DESIGN.md section 4 ("Readings"), numbered R1..R27.
 //
 // Pins (tests/test_oracle_pins.py, run with -m "not gpu"):
-//   features/MLP : closed forms on hand-made weights, float64 matmul bound
+//   features/MLP : closed forms on hand-made weights, float64 matmul bound; cylindrical input (R27): float64
+//                  hypot / atan2 within 5e-7, quadrants, axes, signed zeros
 //   bf16 rounding: torch's CPU bfloat16 conversion on edge cases + random
 //   int8         : numpy int64 integer matmul, hand quantiser values
 //   distance     : Eq.(1) on integer embeddings
@@ -88,6 +89,8 @@ struct Linear {
 struct Model {
   int n_planes = 26;
   float norm_off[3] = {0, 0, 300}, norm_div[3] = {40, 40, 1050};
+  int emb_input = 0;                    // 0: the embedding reads the Cartesian features; 1: cylindrical (L96, R27)
+  float cyl_off[3] = {-20, 0, 300}, cyl_div[3] = {12, 3.14159274f, 1050};
   int emb_hidden = 0, emb_layers_hidden = 0, emb_dim = 4;
   int latent = 0, iters = 0, edge_enc_input = 0;
   int precision = P_FP32;
@@ -161,6 +164,38 @@ inline void features(const Model& M, const float* xyz, float* f) {
   for (int i = 0; i < 3; ++i) f[i] = (xyz[i] + M.norm_off[i]) / M.norm_div[i];
 }
 
+// Cylindrical embedding input (L96 "normalised cylindrical coordinates", R27).  r and phi in fp32, every step one
+// correctly rounded operation in this order so that the CUDA path can take the same steps:
+//   r   = sqrt(fma(y, y, x*x))
+//   phi = atan2(y, x) through an odd polynomial on [0, 1]:  a = min(|x|,|y|) / max(|x|,|y|)  (0 if both are 0),
+//         s = a*a,  q = Horner in s with fma over the nine coefficients below (degree 8, from c8 down to c0),
+//         p = a*q;  |y| > |x|: p = pi/2 - p;  x < 0 (sign bit clear test on the value, so x = -0 counts as +0):
+//         p = pi - p;  phi = copysign(p, y).
+// |phi - atan2(y,x)| <= 5e-7 (pinned against the float64 library atan2); phi(0,0) = 0.
+// The coefficients are a Chebyshev-node interpolant of atan(sqrt(s))/sqrt(s) on s in [0,1], rounded to fp32.
+constexpr float kAtanC[9] = {0x1.000000p+0f,  -0x1.55548ep-2f, 0x1.996efcp-3f,  -0x1.22c55ap-3f, 0x1.b2edb0p-4f,
+                             -0x1.316ecap-4f, 0x1.593100p-5f,  -0x1.01bda4p-6f, 0x1.6a9512p-9f};
+inline float atan2_poly(float y, float x) {
+  const float ax = std::fabs(x), ay = std::fabs(y);
+  const float mx = ax > ay ? ax : ay, mn = ax > ay ? ay : ax;
+  const float a = mx > 0.0f ? mn / mx : 0.0f;
+  const float s = a * a;
+  float q = kAtanC[8];
+  for (int i = 7; i >= 0; --i) q = std::fmaf(q, s, kAtanC[i]);
+  float p = a * q;
+  if (ay > ax) p = 1.57079637f - p;
+  if (x < 0.0f) p = 3.14159274f - p;
+  return std::copysign(p, y);
+}
+// Input of the embedding MLP: the Cartesian features (emb_input 0, BASELINE configs, R1) or
+// ((r, phi, z) + cyl_off) / cyl_div (emb_input 1, L96; same add-then-divide as R1).
+inline void features_emb(const Model& M, const float* xyz, float* f) {
+  if (!M.emb_input) { features(M, xyz, f); return; }
+  const float x = xyz[0], y = xyz[1];
+  const float c[3] = {std::sqrt(std::fmaf(y, y, x * x)), atan2_poly(y, x), xyz[2]};
+  for (int i = 0; i < 3; ++i) f[i] = (c[i] + M.cyl_off[i]) / M.cyl_div[i];
+}
+
 bool parse_blob(Model& M, const uint8_t* blob, size_t bytes) {
   if (bytes < 64) { M.error = "blob too small"; return false; }
   uint32_t h[16];
@@ -168,6 +203,8 @@ bool parse_blob(Model& M, const uint8_t* blob, size_t bytes) {
   if (h[0] != 0x57585445u || h[1] != 1u) { M.error = "bad magic/version"; return false; }
   M.emb_hidden = (int)h[2]; M.emb_layers_hidden = (int)h[3]; M.emb_dim = (int)h[4];
   M.latent = (int)h[5]; M.iters = (int)h[6]; M.edge_enc_input = (int)h[7];
+  M.emb_input = (int)h[10];
+  if (M.emb_input != 0 && M.emb_input != 1) { M.error = "bad emb_input"; return false; }
   const int D = M.emb_hidden, H = M.emb_layers_hidden, d = M.latent, L = M.iters;
   if (D < 1 || D > 256 || H < 1 || H > 8 || M.emb_dim < 1 || M.emb_dim > 16 || d < 1 || d > 85 ||
       L < 0 || L > 64) { M.error = "bad shapes"; return false; }
@@ -240,6 +277,8 @@ struct etxo_params {
   float norm_offset[3];
   float norm_div[3];
   int32_t precision;   // 0 fp32, 1 bf16-emulated, 2 int8
+  float cyl_offset[3]; // used when the blob says emb_input = 1 (R27)
+  float cyl_div[3];
 };
 
 void* etxo_create(const void* blob, uint64_t bytes, const etxo_params* prm) {
@@ -247,6 +286,7 @@ void* etxo_create(const void* blob, uint64_t bytes, const etxo_params* prm) {
   M->precision = prm->precision;
   M->n_planes = prm->n_planes;
   for (int i = 0; i < 3; ++i) { M->norm_off[i] = prm->norm_offset[i]; M->norm_div[i] = prm->norm_div[i]; }
+  for (int i = 0; i < 3; ++i) { M->cyl_off[i] = prm->cyl_offset[i]; M->cyl_div[i] = prm->cyl_div[i]; }
   if (!parse_blob(*M, static_cast<const uint8_t*>(blob), (size_t)bytes)) { /* keep M for the message */ }
   return M;
 }
@@ -325,6 +365,11 @@ void etxo_features(void* m, const float* xyz, int64_t n, float* f) {
   for (int64_t i = 0; i < n; ++i) features(M, xyz + 3 * i, f + 3 * i);
 }
 
+void etxo_features_emb(void* m, const float* xyz, int64_t n, float* f) {
+  const Model& M = *static_cast<Model*>(m);
+  for (int64_t i = 0; i < n; ++i) features_emb(M, xyz + 3 * i, f + 3 * i);
+}
+
 // ---------------------------------------------------------------------------
 // Step 1+2.  Hit embedding (section 5.1): e_h = MLP(normalised coords);
 // ReLU after hidden layers, linear output (R3).  bf16 mode rounds every hidden
@@ -335,7 +380,7 @@ void etxo_embed(void* m, const float* xyz, int64_t n, float* emb) {
 #pragma omp parallel for schedule(static)
   for (int64_t i = 0; i < n; ++i) {
     float a[256], t[256], f[3];
-    features(M, xyz + 3 * i, f);
+    features_emb(M, xyz + 3 * i, f);
     linear(M, M.emb[0], f, a, (size_t)i);
     relu(a, M.emb[0].out); state_round(M, a, M.emb[0].out);
     for (int l = 1; l < H; ++l) {

@@ -34,6 +34,61 @@ def test_features_closed_form_and_true_division():
     assert not np.array_equal(recip, want)
 
 
+def test_cylindrical_embedding_input_against_float64_and_special_cases():
+    # L96: the embedding reads normalised cylindrical coordinates.  R27 fixes r = sqrt(fma(y,y,x*x)) and a polynomial
+    # atan2; the pin is the float64 library hypot / atan2 (another routine entirely), quadrants, axes, zeros, and that
+    # the Cartesian features (what the GNN encoders read, L133) are unchanged by the switch.
+    cfg = toy_config().replace(emb_input=1)
+    o = oracle.Oracle(datagen.pack_blob(cfg, zero_layers(cfg)))
+    assert o.emb_input == 1
+    off, div = np.array(datagen.configs.CYL_OFFSET), np.array(datagen.configs.CYL_DIV)
+    rng = np.random.default_rng(3)
+    xyz = rng.uniform(-45, 45, (200000, 3)).astype(F)
+    xyz[:1000, 0] *= F(1e-4); xyz[1000:2000, 1] *= F(1e-4)          # near the axes, both ways round
+    xyz[2000:3000, 1] = xyz[2000:3000, 0] * rng.choice([-1, 1], 1000).astype(F)   # on the diagonals
+    xyz[:, 2] = rng.uniform(-300, 800, xyz.shape[0])
+    f = o.features_emb(xyz).astype(np.float64)
+    x, y, z = (xyz[:, i].astype(np.float64) for i in range(3))
+    r, phi = f[:, 0] * div[0] - off[0], f[:, 1] * div[1] - off[1]
+    assert np.abs(r - np.hypot(x, y)).max() <= 6e-6                   # 1 ulp at r ~ 64 plus the normalisation's roundings
+    assert np.abs(phi - np.arctan2(y, x)).max() <= 5e-7 + 4e-7       # R27's bound + the normalisation's roundings
+    assert np.array_equal(f[:, 2].astype(F), ((xyz[:, 2] + F(300)) / F(1050)))
+    assert np.abs(f[:, 1]).max() <= 1.0 + 1e-7                        # phi / pi stays in [-1, 1]
+    # special cases, exactly: axes, quadrant signs, zeros (x = -0 counts as +0, phi(0,0) = 0)
+    pts = np.array([[1, 0, 0], [0, 1, 0], [-1, 0, 0], [0, -1, 0], [0, 0, 0], [3, 4, 0], [-2, -2, 0], [-0.0, 0.0, 0]], F)
+    g = o.features_emb(pts)
+    pi, hpi = F(3.14159274), F(1.57079637)
+    want_phi = np.array([0, hpi, pi, -hpi, 0, np.nan, np.nan, 0], F)
+    want_r = np.array([1, 1, 1, 1, 0, 5, np.sqrt(F(8)), 0], F)
+    for i in range(len(pts)):
+        assert g[i, 0] == (want_r[i] + F(off[0])) / F(div[0]), i
+        if not np.isnan(want_phi[i]):
+            assert g[i, 1] == (want_phi[i] + F(off[1])) / F(div[1]), i
+    assert g[5, 1] > 0 and g[6, 1] < 0 and abs(float(g[6, 1]) * float(div[1]) + 3 * np.pi / 4) < 5e-7
+    # odd in y, and phi(y, -x) = pi - phi(y, x) in exact arithmetic (checked to the bound)
+    m = xyz.copy(); m[:, 1] = -m[:, 1]
+    assert np.array_equal(o.features_emb(m)[:, 1], -o.features_emb(xyz)[:, 1])
+    # the Cartesian features are what they were, and emb_input = 0 keeps the embedding on them
+    o0 = oracle.Oracle(datagen.pack_blob(toy_config(), zero_layers(toy_config())))
+    assert np.array_equal(o.features(xyz), o0.features(xyz)) and np.array_equal(o0.features_emb(xyz), o0.features(xyz))
+
+
+def test_cylindrical_input_reaches_the_embedding_mlp():
+    # the embedding MLP of an emb_input = 1 model applied to xyz == the same weights applied (as a Cartesian model with
+    # identity normalisation) to the cylindrical features: the switch changes the input and nothing else
+    cfg = toy_config(D=4, H=1).replace(emb_input=1)
+    L = zero_layers(cfg)
+    rng = np.random.default_rng(4)
+    for name, W, b in L:
+        if name.startswith("emb"):
+            W[...] = rng.uniform(-1, 1, W.shape); b[...] = rng.uniform(-1, 1, b.shape)
+    xyz = rng.uniform(-40, 40, (500, 3)).astype(F)
+    o1 = oracle.Oracle(datagen.pack_blob(cfg, L))
+    o0 = oracle.Oracle(datagen.pack_blob(cfg.replace(emb_input=0), L), norm_offset=(0, 0, 0), norm_div=(1, 1, 1))
+    assert np.array_equal(o1.embed(xyz), o0.embed(o1.features_emb(xyz)))
+    assert not np.array_equal(o1.embed(xyz), oracle.Oracle(datagen.pack_blob(cfg.replace(emb_input=0), L)).embed(xyz))
+
+
 # ------------------------------------------------------------------ MLP forward (L96; R3)
 def _emb_toy(D=4, H=2):
     cfg = toy_config(D=D, H=H)
