@@ -74,6 +74,14 @@ typedef struct {
   int32_t  max_events;               /* workspace capacity (L223: fixed memory per stream)              */
   int32_t  max_hits;                 /* max_edges = k * max_hits                                        */
   int32_t  validate_input;           /* 1: device-side check that hits are sorted by (event, plane)     */
+  int32_t  emb_input;                /* input of the embedding MLP.  0: the Cartesian features above (BASELINE
+                                        configs)  1: ((r, phi, z) + cyl_offset) / cyl_div, the paper's normalised
+                                        cylindrical coordinates (L96); r = sqrt(fma(y,y,x*x)), phi = the fp32
+                                        polynomial atan2 of DESIGN.md R27 (|error| <= 5e-7).  Must equal word 10
+                                        of the blob header.  The GNN encoders always read the Cartesian
+                                        features (L133).                                                   */
+  float    cyl_offset[3];
+  float    cyl_div[3];
   /* Optional device-memory allocator (L223: Allen hands every algorithm memory from its own per-stream
    * arena).  NULL alloc: cudaMalloc / cudaFree.  alloc must return device memory aligned to 256 bytes or
    * NULL on failure; dealloc is called once per block from etx_destroy; alloc and dealloc go together.    */

@@ -35,6 +35,7 @@ class Hyperparams(C.Structure):
                 ("gnn_latent", C.c_int32), ("gnn_iters", C.c_int32), ("edge_enc_input", C.c_int32),
                 ("threshold", C.c_float), ("precision", C.c_int32), ("engine", C.c_int32),
                 ("max_events", C.c_int32), ("max_hits", C.c_int32), ("validate_input", C.c_int32),
+                ("emb_input", C.c_int32), ("cyl_offset", C.c_float * 3), ("cyl_div", C.c_float * 3),
                 ("alloc", ALLOC_FN), ("dealloc", DEALLOC_FN), ("alloc_ctx", C.c_void_p)]
 
 
@@ -116,7 +117,8 @@ def lib():
 
 def hyperparams_from_config(cfg, max_events: int, max_hits: int, precision: str | None = None,
                             engine: str = "auto", validate_input: bool = False, n_planes: int = 26,
-                            norm_offset=(0.0, 0.0, 300.0), norm_div=(40.0, 40.0, 1050.0)) -> Hyperparams:
+                            norm_offset=(0.0, 0.0, 300.0), norm_div=(40.0, 40.0, 1050.0),
+                            cyl_offset=(-20.0, 0.0, 300.0), cyl_div=(12.0, 3.14159274, 1050.0)) -> Hyperparams:
     """etx_hyperparams from a datagen.EtxConfig-like object (attribute access only)."""
     hp = Hyperparams()
     hp.struct_size = C.sizeof(Hyperparams)
@@ -132,6 +134,9 @@ def hyperparams_from_config(cfg, max_events: int, max_hits: int, precision: str 
     hp.engine = ENGINE[engine]
     hp.max_events, hp.max_hits = max_events, max_hits
     hp.validate_input = int(validate_input)
+    hp.emb_input = getattr(cfg, "emb_input", 0)
+    hp.cyl_offset = (C.c_float * 3)(*cyl_offset)
+    hp.cyl_div = (C.c_float * 3)(*cyl_div)
     return hp
 
 

@@ -50,7 +50,7 @@ etx_status parse_blob(etx_ctx* c, const uint8_t* blob, size_t bytes) {
   memcpy(h, blob, 64);
   if (h[0] != kBlobMagic || h[1] != 1u) return fail(c, ETX_ERR_BLOB, "bad blob magic / version");
   if ((int)h[2] != hp.emb_hidden || (int)h[3] != hp.emb_n_hidden_layers || (int)h[4] != hp.emb_dim ||
-      (int)h[5] != hp.gnn_latent || (int)h[6] != hp.gnn_iters || (int)h[7] != hp.edge_enc_input)
+      (int)h[5] != hp.gnn_latent || (int)h[6] != hp.gnn_iters || (int)h[7] != hp.edge_enc_input || (int)h[10] != hp.emb_input)
     return fail(c, ETX_ERR_BLOB, "blob shapes differ from the hyper-parameters");
   const int D = hp.emb_hidden, H = hp.emb_n_hidden_layers, d = hp.gnn_latent, L = hp.gnn_iters;
   auto add = [&](int out, int in, bool head = false) {
@@ -310,10 +310,12 @@ etx_status etx_create(const void* blob, size_t blob_bytes, const etx_hyperparams
       hp->gnn_iters < 0 || hp->gnn_iters > 64 || hp->emb_n_hidden_layers < 1 || hp->emb_n_hidden_layers > 8 ||
       !(hp->threshold >= 0.0f && hp->threshold <= 1.0f) || isnan(hp->d2_max))
     return bail(ETX_ERR_ARG);
-  for (int i = 0; i < 3; ++i) if (!(hp->norm_div[i] != 0.0f)) return bail(ETX_ERR_ARG);
+  for (int i = 0; i < 3; ++i)
+    if (!(hp->norm_div[i] != 0.0f) || (hp->emb_input && !(hp->cyl_div[i] != 0.0f))) return bail(ETX_ERR_ARG);
   // shapes built into the kernels
   if (!(hp->emb_hidden == 64 || hp->emb_hidden == 128) || hp->emb_dim != 4 || !(hp->gnn_latent == 32 || hp->gnn_latent == 64) ||
-      hp->k > 64 || (hp->edge_enc_input != 0 && hp->edge_enc_input != 1))
+      hp->k > 64 || (hp->edge_enc_input != 0 && hp->edge_enc_input != 1) ||
+      (hp->emb_input != 0 && hp->emb_input != 1))
     return bail(ETX_ERR_UNSUPPORTED);
   if ((long long)hp->k * hp->max_hits > 0x7fffffffLL) return bail(ETX_ERR_CAPACITY);
   c->max_edges = hp->k * hp->max_hits;
@@ -333,6 +335,7 @@ etx_status etx_create(const void* blob, size_t blob_bytes, const etx_hyperparams
     c->event_off = dev_alloc<int32_t>(c, B + 1);
     c->plane_off = dev_alloc<int32_t>(c, B * (hp->n_planes + 1));
     c->feat = dev_alloc<float4>(c, N);
+    c->feat_emb = hp->emb_input ? dev_alloc<float4>(c, N) : c->feat;
     c->emb = dev_alloc<float4>(c, N);
     c->nbr = dev_alloc<int32_t>(c, N * hp->k);
     c->deg = dev_alloc<int32_t>(c, N);
@@ -511,6 +514,7 @@ etx_status etx_dbg_buffer(etx_handle c, const char* name, const void** d_ptr, si
   if (n == "plane_off") { *d_ptr = c->plane_off; *bytes = 0; return ETX_OK; }
   if (n == "emb") { *d_ptr = c->emb; *bytes = N * 16; return ETX_OK; }
   if (n == "feat") { *d_ptr = c->feat; *bytes = N * 16; return ETX_OK; }
+  if (n == "feat_emb") { *d_ptr = c->feat_emb; *bytes = N * 16; return ETX_OK; }
   if (n == "nbr") { *d_ptr = c->nbr; *bytes = N * c->hp.k * 4; return ETX_OK; }
   if (n == "deg") { *d_ptr = c->deg; *bytes = N * 4; return ETX_OK; }
   if (n == "row_ptr") { *d_ptr = c->row_ptr; *bytes = (N + 1) * 4; return ETX_OK; }

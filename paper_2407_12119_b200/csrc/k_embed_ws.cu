@@ -226,7 +226,7 @@ bool launch_embed_ws(etx_ctx* c, int n_hits, cudaStream_t s) {
   const HostLayer& lo = c->layers[c->i_emb0 + H];
   for (int n = 0; n < 4; ++n) a.bout[n] = lo.b[n];
   a.wout_img = lo.dev.Wtc;
-  a.feat = c->feat; a.emb = c->emb; a.n_rows = n_hits; a.n_mid = n_mid;
+  a.feat = c->feat_emb; a.emb = c->emb; a.n_rows = n_hits; a.n_mid = n_mid;
   return D == 64 ? emb_ws_launch<64>(c, a, s) : emb_ws_launch<128>(c, a, s);
 }
 

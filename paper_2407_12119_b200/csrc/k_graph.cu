@@ -8,21 +8,56 @@ namespace etx {
 // --------------------------------------------------------------------------------------------------------
 // C1 (PAPER.md L107 fn.5; R1): f = ((x,y,z) + offset) / div, one IEEE add and one correctly
 // rounded division.  Stored once as float4 so every later stage gathers 16 B per hit.
-__global__ void features_kernel(const float* __restrict__ xyz, float4* __restrict__ feat, int n,
-                                float ox, float oy, float oz, float dx, float dy, float dz) {
+struct FeatArgs { float o[3], d[3], co[3], cd[3]; };
+
+// phi = atan2(y, x) in fp32 as DESIGN.md R27 states it (every step one correctly rounded operation, in this order):
+// a = min(|x|,|y|) / max(|x|,|y|), an odd polynomial in a on [0,1] (Horner in a*a with fma, degree 8), then the
+// octant, half-plane and sign corrections.  |phi - atan2| <= 5e-7.
+__device__ __forceinline__ float atan2_r27(float y, float x) {
+  const float ax = fabsf(x), ay = fabsf(y);
+  const float mx = ax > ay ? ax : ay, mn = ax > ay ? ay : ax;
+  const float a = mx > 0.0f ? __fdiv_rn(mn, mx) : 0.0f;
+  const float s = __fmul_rn(a, a);
+  float q = 0x1.6a9512p-9f;
+  q = __fmaf_rn(q, s, -0x1.01bda4p-6f);
+  q = __fmaf_rn(q, s, 0x1.593100p-5f);
+  q = __fmaf_rn(q, s, -0x1.316ecap-4f);
+  q = __fmaf_rn(q, s, 0x1.b2edb0p-4f);
+  q = __fmaf_rn(q, s, -0x1.22c55ap-3f);
+  q = __fmaf_rn(q, s, 0x1.996efcp-3f);
+  q = __fmaf_rn(q, s, -0x1.55548ep-2f);
+  q = __fmaf_rn(q, s, 1.0f);
+  float p = __fmul_rn(a, q);
+  if (ay > ax) p = __fsub_rn(1.57079637f, p);
+  if (x < 0.0f) p = __fsub_rn(3.14159274f, p);
+  return copysignf(p, y);
+}
+
+template <bool CYL>
+__global__ void features_kernel(const float* __restrict__ xyz, float4* __restrict__ feat, float4* __restrict__ feat_emb,
+                                int n, FeatArgs a) {
   int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   float x = xyz[3 * (size_t)i], y = xyz[3 * (size_t)i + 1], z = xyz[3 * (size_t)i + 2];
-  feat[i] = make_float4(__fdiv_rn(__fadd_rn(x, ox), dx), __fdiv_rn(__fadd_rn(y, oy), dy),
-                        __fdiv_rn(__fadd_rn(z, oz), dz), 0.0f);
+  feat[i] = make_float4(__fdiv_rn(__fadd_rn(x, a.o[0]), a.d[0]), __fdiv_rn(__fadd_rn(y, a.o[1]), a.d[1]),
+                        __fdiv_rn(__fadd_rn(z, a.o[2]), a.d[2]), 0.0f);
+  if (CYL) {                                              // L96: the embedding reads normalised (r, phi, z)
+    const float r = __fsqrt_rn(__fmaf_rn(y, y, __fmul_rn(x, x)));
+    const float phi = atan2_r27(y, x);
+    feat_emb[i] = make_float4(__fdiv_rn(__fadd_rn(r, a.co[0]), a.cd[0]), __fdiv_rn(__fadd_rn(phi, a.co[1]), a.cd[1]),
+                              __fdiv_rn(__fadd_rn(z, a.co[2]), a.cd[2]), 0.0f);
+  }
 }
 
 void launch_features(etx_ctx* c, const float* xyz, int n_hits, cudaStream_t s) {
   if (n_hits == 0) return;
   const etx_hyperparams& hp = c->hp;
-  features_kernel<<<(n_hits + 255) / 256, 256, 0, s>>>(xyz, c->feat, n_hits, hp.norm_offset[0], hp.norm_offset[1],
-                                                       hp.norm_offset[2], hp.norm_div[0], hp.norm_div[1],
-                                                       hp.norm_div[2]);
+  FeatArgs a;
+  for (int i = 0; i < 3; ++i) {
+    a.o[i] = hp.norm_offset[i]; a.d[i] = hp.norm_div[i]; a.co[i] = hp.cyl_offset[i]; a.cd[i] = hp.cyl_div[i];
+  }
+  if (hp.emb_input) features_kernel<true><<<(n_hits + 255) / 256, 256, 0, s>>>(xyz, c->feat, c->feat_emb, n_hits, a);
+  else features_kernel<false><<<(n_hits + 255) / 256, 256, 0, s>>>(xyz, c->feat, c->feat_emb, n_hits, a);
   c->launches++;
 }
 

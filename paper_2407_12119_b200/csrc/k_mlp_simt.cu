@@ -426,7 +426,7 @@ void launch_embed_simt(etx_ctx* c, int n_hits, cudaStream_t s) {
   EmbArgs a;
   a.n_layers = c->hp.emb_n_hidden_layers + 1;
   for (int l = 0; l < a.n_layers; ++l) a.layers[l] = c->layers[c->i_emb0 + l].dev;
-  a.feat = c->feat; a.emb = c->emb; a.n_rows = n_hits;
+  a.feat = c->feat_emb; a.emb = c->emb; a.n_rows = n_hits;
   a.tap = c->tap_layer >= 0 ? c->tap : nullptr; a.tap_layer = c->tap_layer;
   const int D = c->hp.emb_hidden;
 #define ETX_EMB(MODE)                                   \
