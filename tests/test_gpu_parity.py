@@ -192,6 +192,46 @@ def test_end_to_end_fp32_bit_exact_edges_and_track_ids(name, n_events, preset):
     assert np.unique(g["track_id"]).size == np.unique(r["track_id"]).size
 
 
+@pytest.mark.parametrize("name,n_events,precision", [("cfg0", 1, "fp32"), ("cfg1", 4, "fp32"), ("cfg1", 4, "bf16"),
+                                                      ("cfg5", 3, "bf16")])
+def test_cylindrical_embedding_input(name, n_events, precision):
+    # L96 / R27: the embedding reads normalised (r, phi, z).  Every step of R27 is a single pinned fp32 operation, so
+    # the features equal the oracle's bits in every precision; fp32 then stays bit-exact end to end
+    cfg = datagen.get_config(name).replace(emb_input=1, precision=precision)
+    b = datagen.generate_batch(cfg, n_events=n_events)
+    xyz = b.xyz.copy()
+    xyz[0, :2] = (0.0, 0.0); xyz[1, :2] = (-7.0, 0.0); xyz[2, :2] = (0.0, -9.0); xyz[3, :2] = (-6.0, -6.0)   # axes, diagonal
+    xyz[4, :2] = (-0.0, 5.0); xyz[5, :2] = (-8.0, -0.0)
+    b = datagen.EventBatch(xyz, b.plane, b.event_offsets, b.particle)
+    W = centred_parity_weights(cfg, b)
+    blob = datagen.pack_blob(cfg, W)
+    o, r = _oracle_all(cfg, b, blob, precision)
+    ctx = make_ctx(cfg, blob, b)
+    g = run_gpu(ctx, b, debug=False)
+    fe = ctx.buffer("feat_emb", torch.float32).cpu().numpy().reshape(-1, 4)[:b.n_hits]
+    fc = ctx.buffer("feat", torch.float32).cpu().numpy().reshape(-1, 4)[:b.n_hits]
+    assert np.array_equal(fe[:, :3], o.features_emb(b.xyz)) and np.array_equal(fc[:, :3], o.features(b.xyz))
+    assert not np.array_equal(fe, fc)
+    if precision == "fp32":
+        assert np.array_equal(g["emb"], r["emb"])
+        assert np.array_equal(g["src"], r["src"]) and np.array_equal(g["dst"], r["dst"])
+        assert np.abs(g["score"] - r["score"]).max() <= 1e-4
+        assert np.array_equal(g["track_id"], r["track_id"])
+    else:
+        assert np.abs(g["emb"] - r["emb"]).max() <= 2e-2 * max(1.0, float(np.abs(r["emb"]).max()))
+        nbr, deg = oracle.knn(g["emb"], b.plane, b.event_offsets, cfg.k, cfg.window, cfg.d2_max)   # chained (sec. 6)
+        src, dst, _ = oracle.build_edges(nbr, deg)
+        assert np.array_equal(g["src"], src) and np.array_equal(g["dst"], dst)
+        og = o.gnn(b.xyz, src, dst)
+        assert np.abs(g["score"] - og["score"]).max(initial=0.0) <= 2e-2
+        tid = oracle.components(src, dst, g["logit"], oracle.logit_threshold(cfg.threshold), b.n_hits)
+        assert np.array_equal(g["track_id"], tid)
+    # a blob that says Cartesian is refused by a handle that says cylindrical
+    with pytest.raises(Exception):
+        make_ctx(cfg, datagen.pack_blob(cfg.replace(emb_input=0), W), b)
+    ctx.destroy()
+
+
 def test_repeated_runs_on_one_handle_are_identical_and_smaller_batches_work():
     cfg, b, W = _setup("cfg1", 4, precision="fp32")
     blob = datagen.pack_blob(cfg, W)
