@@ -131,7 +131,9 @@ def stage_model(cfg, N, E, pairs, peaks):
         # e is read from HBM once (the second direction finds its rows in L2: ncu, profiles/r1f_stage_rooflines.md)
         "S4c_scatter": ("hbm", L * (1.0 * E * d * b + 2.0 * N * d * b + 4.0 * E + 8.0 * N), peaks["hbm"], "GB/s"),
         "S4d_node_net": ("hbm", L * (4.0 * N * d * b), peaks["hbm"], "GB/s"),
-        "S4e_edge_net_head": ("hbm", L * ((2.0 * d * b + 8.0) * E + N * d * b) + 8.0 * E, peaks["hbm"], "GB/s"),
+        # e is read by every step and written by all but the last (e^L feeds only the classifier, which is fused)
+        "S4e_edge_net_head": ("hbm", L * ((2.0 * d * b + 8.0) * E + N * d * b) + 8.0 * E - (E * d * b if L else 0.0),
+                              peaks["hbm"], "GB/s"),
         "S5_components": ("hbm", 12.0 * E + 8.0 * N, peaks["hbm"], "GB/s"),
     }
 

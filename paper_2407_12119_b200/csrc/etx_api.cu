@@ -173,6 +173,7 @@ etx_status run_impl(etx_ctx* c, const float* d_xyz, const int32_t* d_plane, cons
     ETX_CUDA(cudaMemsetAsync(c->n_edges, 0, sizeof(int32_t), s));
     c->n_ev = 0; c->spans.clear();
     c->last_n_hits = n_hits; c->last_n_events = n_events;
+    c->keep_final_state = (inj != nullptr);   // e^L feeds only the classifier (L142); a plain run does not write it
     StageTimer tm{c, s};
     bool edges_marked = false;
     const bool tensor_engine = (c->precision != ETX_FP32) && c->engine != ETX_ENGINE_SIMT;

@@ -185,10 +185,12 @@ __global__ void __launch_bounds__(kI8Threads, 1) edge_net_i8_kernel(const __grid
       for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
         const int s = it % kI8E;
         mbar_wait(&out_ready[s], (it / kI8E) & 1);
+        if (a.do_head != 2) {                                 // 2: the new state is dead (last step of a plain etx_run)
 #pragma unroll
-        for (int b = 0; b < D / 32; ++b) tma_store_2d(&e_map, e_addr + s * ETILE + b * kI8Sub, 32 * b, tile * kRows);
-        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-        asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+          for (int b = 0; b < D / 32; ++b) tma_store_2d(&e_map, e_addr + s * ETILE + b * kI8Sub, 32 * b, tile * kRows);
+          asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+          asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+        }
         mbar_arrive(&e_free[s]);
       }
       asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
@@ -339,6 +341,7 @@ bool edge_i8_configure(etx_ctx* c) {
 void launch_edge_net_i8(etx_ctx* c, int iter, int n_hits, bool do_head, cudaStream_t s) {
   GnnArgs a;
   fill_gnn_args(c, kEdgeNet, iter, n_hits, do_head, a);
+  if (do_head && !c->keep_final_state) a.do_head = 2;        // e^L feeds only the classifier: do not write it back
   const long long max_rows_ll = (long long)n_hits * c->hp.k;
   const int max_rows = (int)(max_rows_ll > 0x7fffffff ? 0x7fffffff : max_rows_ll);
   if (c->hp.gnn_latent == 32) edge_i8_launch<32, false>(c, a, max_rows, s);

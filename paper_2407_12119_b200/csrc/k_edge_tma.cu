@@ -138,6 +138,7 @@ struct EdgeTmaArgs {
   const int32_t* n_rows_ptr;
   float* logit; float* score;
   int do_head;
+  int store_e;                 // 0: the new edge state is dead (last step of a plain etx_run: only the classifier reads it)
 };
 
 // all MMAs of one K-block: kbytes of K, 32 bytes (16 bf16) per instruction
@@ -260,9 +261,11 @@ edge_net_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeTmaArgs
         PROF(0)
         mbar_wait(&out_ready[s], (it / kNE) & 1);
         PROF(1)
-        tma_store_2d(&e_map, self_addr + s * BLK, 0, tile * kRows);
-        bulk_commit();
-        bulk_wait_read0();                                    // the slot has been read: hand it back to the loader
+        if (a.store_e) {
+          tma_store_2d(&e_map, self_addr + s * BLK, 0, tile * kRows);
+          bulk_commit();
+          bulk_wait_read0();                                  // the slot has been read: hand it back to the loader
+        }
         mbar_arrive(&self_empty[s]);
         PROF(2)
       }
@@ -385,7 +388,7 @@ edge_net_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeTmaArgs
           qv.y = pack_bf16x2(__uint_as_float(v[ch * 8 + 2]), __uint_as_float(v[ch * 8 + 3]));
           qv.z = pack_bf16x2(__uint_as_float(v[ch * 8 + 4]), __uint_as_float(v[ch * 8 + 5]));
           qv.w = pack_bf16x2(__uint_as_float(v[ch * 8 + 6]), __uint_as_float(v[ch * 8 + 7]));
-          *reinterpret_cast<uint4*>(out + swz<KB>(r, c0 / 8 + ch)) = qv;
+          if (a.store_e) *reinterpret_cast<uint4*>(out + swz<KB>(r, c0 / 8 + ch)) = qv;
           if (a.do_head) {                                    // the classifier sees the stored bf16 state, ascending j
             const float* hw = headw + c0 + ch * 8;
             hacc = __fmaf_rn(bf16_lo(qv.x), hw[0], hacc); hacc = __fmaf_rn(bf16_hi(qv.x), hw[1], hacc);
@@ -749,6 +752,7 @@ void launch_edge_net_tma(etx_ctx* c, int iter, int n_hits, bool do_head, cudaStr
   a.h = static_cast<const __nv_bfloat16*>(c->h);
   a.src = c->src; a.dst = c->dst; a.n_rows_ptr = c->n_edges;
   a.logit = c->logit; a.score = c->score_out; a.do_head = do_head ? 1 : 0;
+  a.store_e = (do_head && !c->keep_final_state) ? 0 : 1;
   const long long max_rows_ll = (long long)n_hits * c->hp.k;
   const int max_rows = (int)(max_rows_ll > 0x7fffffff ? 0x7fffffff : max_rows_ll);
   if (c->hp.gnn_latent == 32) edge_tma_launch<32>(c, a, max_rows, s);

@@ -232,6 +232,52 @@ def test_cylindrical_embedding_input(name, n_events, precision):
     ctx.destroy()
 
 
+def test_one_huge_event_takes_the_global_memory_paths():
+    # maximum sizes: twenty events merged into one of ~42,000 hits with ~1,600 hits per plane -- more than the 16,384
+    # hits the per-event union-find keeps in shared memory and more than the 1,024 cursors per bucket of the CSC walk, so
+    # both kernels run on their global-memory scratch; the k-NN walks several candidate tiles per bucket.  fp32: bit-exact
+    cfg = datagen.get_config("cfg1")
+    b20 = datagen.generate_batch(cfg, n_events=20)
+    order = np.argsort(b20.plane, kind="stable")
+    big = datagen.EventBatch(b20.xyz[order], b20.plane[order], np.array([0, b20.n_hits], np.int32), b20.particle[order])
+    small = datagen.generate_batch(cfg, n_events=2, seed=77)
+    b = datagen.EventBatch(np.concatenate([small.xyz, big.xyz]), np.concatenate([small.plane, big.plane]),
+                           np.concatenate([small.event_offsets, [small.n_hits + big.n_hits]]).astype(np.int32),
+                           np.concatenate([small.particle, big.particle]))
+    assert big.n_hits > 16384 and np.bincount(big.plane).max() > 1024
+    W = centred_parity_weights(cfg, small)
+    blob = datagen.pack_blob(cfg, W)
+    o, r = _oracle_all(cfg, b, blob, "fp32")
+    ctx = make_ctx(cfg, blob, b, validate=True)
+    g = run_gpu(ctx, b)
+    assert np.array_equal(g["src"], r["src"]) and np.array_equal(g["dst"], r["dst"])
+    assert np.array_equal(g["col_ptr"], r["col_ptr"]) and np.array_equal(g["in_edge"], r["in_edge"])
+    assert np.abs(g["score"] - r["score"]).max() <= 1e-4
+    assert np.array_equal(g["track_id"], r["track_id"])
+    t = ctx.tracks(b.n_hits, b.n_events, 3)
+    want = oracle.tracks(r["track_id"], b.event_offsets, 3)
+    for key in ("track_index", "track_offsets", "track_hits", "event_track_offsets"):
+        assert np.array_equal(t[key].cpu().numpy(), want[key]), key
+    ctx.destroy()
+
+
+@pytest.mark.parametrize("name,precision", [("cfg1", "bf16"), ("cfg5", "bf16"), ("cfg1", "int8")])
+def test_plain_run_skips_the_dead_final_edge_state_and_changes_nothing_else(name, precision):
+    # e^L feeds only the classifier (L142), which is fused into the last edge network: etx_run does not write it back,
+    # etx_dbg_run does.  Logits, scores and track ids must be the same bits either way
+    cfg, b, W = _setup(name, 3, precision=precision)
+    blob = _int8_blob(cfg, b, W) if precision == "int8" else datagen.pack_blob(cfg, W)
+    ctx = make_ctx(cfg, blob, b)
+    g1 = run_gpu(ctx, b, debug=False)
+    e1 = state(ctx, "e", g1["n_edges"], cfg.gnn_latent).copy()
+    g2 = run_gpu(ctx, b)
+    e2 = state(ctx, "e", g2["n_edges"], cfg.gnn_latent)
+    for key in ("src", "logit", "score", "track_id"):
+        assert np.array_equal(g1[key], g2[key]), key
+    assert not np.array_equal(e1, e2)                    # the plain run left e^(L-1) in place
+    ctx.destroy()
+
+
 def test_repeated_runs_on_one_handle_are_identical_and_smaller_batches_work():
     cfg, b, W = _setup("cfg1", 4, precision="fp32")
     blob = datagen.pack_blob(cfg, W)
@@ -349,10 +395,13 @@ def test_int8_tensor_core_path_is_bit_exact_end_to_end(name, n_events):
     assert np.array_equal(g["emb"], r["emb"])
     assert np.array_equal(g["src"], r["src"]) and np.array_equal(g["dst"], r["dst"])
     assert np.array_equal(state(ctx, "h", b.n_hits, cfg.gnn_latent), og["h"])
-    assert np.array_equal(state(ctx, "e", r["src"].size, cfg.gnn_latent), og["e"])
     assert np.array_equal(g["logit"], r["logit"])
     assert np.abs(g["score"] - r["score"]).max() <= 1e-4
     assert np.array_equal(g["track_id"], r["track_id"])
+    # a plain etx_run does not write e^L back (only the fused classifier reads it); etx_dbg_run does, with the same logits
+    g2 = run_gpu(ctx, b)
+    assert np.array_equal(state(ctx, "e", r["src"].size, cfg.gnn_latent), og["e"])
+    assert np.array_equal(g2["logit"], g["logit"]) and np.array_equal(g2["track_id"], g["track_id"])
 
 
 def test_int8_tensor_core_accumulators_bit_exact():
