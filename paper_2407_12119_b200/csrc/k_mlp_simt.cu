@@ -337,15 +337,17 @@ __global__ void __launch_bounds__(256) scatter_kernel(const void* __restrict__ e
   const int gid = (gridDim.x - 1 - blockIdx.x) * (256 / LPN) + threadIdx.x / LPN;
   const int c = (threadIdx.x % LPN) * V;
   if (gid >= n_hits) return;
-  float so[V], si[V];
+  float sum[V];
 #pragma unroll
-  for (int j = 0; j < V; ++j) { so[j] = 0.0f; si[j] = 0.0f; }
+  for (int j = 0; j < V; ++j) sum[j] = 0.0f;
   const int a0 = row_ptr[gid], a1 = row_ptr[gid + 1];
-  for (int i = a0; i < a1; ++i) Vec16<ST>::add(e, (size_t)i * D + c, so);
   const int b0 = col_ptr[gid], b1 = col_ptr[gid + 1];
-  for (int i = b0; i < b1; ++i) Vec16<ST>::add(e, (size_t)in_edge[i] * D + c, si);
-  Vec16<ST>::st(m, (size_t)gid * 2 * D + c, so);
-  Vec16<ST>::st(m, (size_t)gid * 2 * D + D + c, si);
+  for (int i = a0; i < a1; ++i) Vec16<ST>::add(e, (size_t)i * D + c, sum);
+  Vec16<ST>::st(m, (size_t)gid * 2 * D + c, sum);         // m_out is stored before m_in starts: one live accumulator set
+#pragma unroll
+  for (int j = 0; j < V; ++j) sum[j] = 0.0f;
+  for (int i = b0; i < b1; ++i) Vec16<ST>::add(e, (size_t)in_edge[i] * D + c, sum);
+  Vec16<ST>::st(m, (size_t)gid * 2 * D + D + c, sum);
 }
 
 // ------------------------------------------------------------------------------------------------------------
