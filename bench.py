@@ -28,9 +28,10 @@ sys.path.insert(0, ROOT)
 
 import datagen  # noqa: E402
 
-# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel (S4e edge network) from the
-# `ncu --set full` capture summarised in profiles/r1e_edge_net_full.md, per workload; bench.py cannot run ncu itself.
-NCU_TRAFFIC_BYTES = {("cfg2", 500): 2.7036e9}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel (S4e edge network): the mean over the
+# six launches of one pass (five write e back, the last does not) from the `ncu --set full` capture summarised in
+# profiles/r1h_launches_s4e_traffic.md, per workload; bench.py cannot run ncu itself.
+NCU_TRAFFIC_BYTES = {("cfg2", 500): 2.5150e9}
 METRIC = "events_per_s"
 UNIT = "events/s"
 DTYPE = {"fp32": "f32", "bf16": "bf16", "int8": "int8"}
