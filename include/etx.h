@@ -174,7 +174,8 @@ etx_status etx_dbg_run(etx_handle h, const float* d_xyz, const int32_t* d_plane,
                        const etx_inject* inj, etx_output* out);
 
 /* Device pointer + byte size of an internal buffer of the last run: "plane_off", "emb", "nbr", "deg",
- * "row_ptr", "col_ptr", "in_edge", "h", "e", "m", "logit", "tap", "feat", "feat_emb".  h / e / m are in the
+ * "row_ptr", "col_ptr", "in_edge", "h", "e", "m", "logit", "tap", "feat", "feat_emb".  "nbr" is [n_hits][k]; only the
+ * first deg[q] slots of a row are defined.  h / e / m are in the
  * state dtype (fp32 for ETX_FP32 and ETX_INT8, bf16 for ETX_BF16).  "e" holds the final edge state e^L only after
  * etx_dbg_run: in etx_run the last edge network feeds the fused classifier and does not write e^L back (the
  * tensor-core kernels; after etx_run "e" is then e^(L-1)). */

@@ -335,6 +335,7 @@ etx_status etx_create(const void* blob, size_t blob_bytes, const etx_hyperparams
     const size_t sb = c->state_bf16 ? 2 : 4;
     c->event_off = dev_alloc<int32_t>(c, B + 1);
     c->plane_off = dev_alloc<int32_t>(c, B * (hp->n_planes + 1));
+    c->knn_redo = dev_alloc<int32_t>(c, B * hp->n_planes + 1);
     c->feat = dev_alloc<float4>(c, N);
     c->feat_emb = hp->emb_input ? dev_alloc<float4>(c, N) : c->feat;
     c->emb = dev_alloc<float4>(c, N);

@@ -86,6 +86,7 @@ struct etx_ctx {
   int32_t* plane_off = nullptr;           // [max_events][P + 1]
   float4* feat = nullptr;                 // [max_hits]
   bool keep_final_state = false;          // etx_dbg_run: the last edge network still writes e^L (tests read it)
+  int32_t* knn_redo = nullptr;            // [max_events * n_planes] buckets knn_cut_kernel hands to knn_kernel
   float4* feat_emb = nullptr;             // [max_hits] input of the embedding MLP (= feat unless emb_input = 1)
   float4* emb = nullptr;                  // [max_hits]
   int32_t *nbr = nullptr, *deg = nullptr; // [max_hits][k], [max_hits]

@@ -162,9 +162,10 @@ __device__ __forceinline__ float knn_d2(const float4 a, const float4 b) {
 template <int KCAP>
 __global__ void __launch_bounds__(kKnnThreads)
 knn_kernel(const float4* __restrict__ emb, const int32_t* __restrict__ plane_off, int P, int k, int w,
-           float d2_max, int32_t* __restrict__ nbr, int32_t* __restrict__ deg) {
+           float d2_max, int32_t* __restrict__ nbr, int32_t* __restrict__ deg, const int32_t* __restrict__ only) {
   __shared__ float4 cand[kKnnTile];
   const int bucket = blockIdx.x;                 // e * P + p
+  if (only && !only[bucket]) return;             // second pass after knn_cut_kernel: flagged buckets only
   const int e = bucket / P, p = bucket % P;
   const int32_t* po = plane_off + (size_t)e * (P + 1);
   const int q_lo = po[p], q_hi = po[p + 1];
@@ -178,7 +179,7 @@ knn_kernel(const float4* __restrict__ emb, const int32_t* __restrict__ plane_off
   }
   for (int q0 = q_lo; q0 < q_hi; q0 += kKnnThreads) {
     const int q = q0 + threadIdx.x;
-    const bool active = q < q_hi;
+    const bool active = q < q_hi && (!only || deg[q] < 0);    // second pass: only the hits knn_cut_kernel gave up on
     const float4 a = active ? emb[q] : make_float4(0.f, 0.f, 0.f, 0.f);
     TopK<KCAP> top;
     top.init(d2_max);
@@ -211,8 +212,7 @@ knn_kernel(const float4* __restrict__ emb, const int32_t* __restrict__ plane_off
 #pragma unroll
       for (int s = 0; s < KCAP; ++s) {
         if (s < k) {
-          nbr[(size_t)q * k + s] = top.idx[s];
-          cnt += top.idx[s] >= 0;
+          if (top.idx[s] >= 0) { nbr[(size_t)q * k + s] = top.idx[s]; ++cnt; }   // slots past deg[q] are never read
         }
       }
       deg[q] = cnt;
@@ -220,24 +220,119 @@ knn_kernel(const float4* __restrict__ emb, const int32_t* __restrict__ plane_off
   }
 }
 
+// With a finite radius cut (the paper's regime, L101 / L257: ~14 of a hit's ~160 candidates lie inside d2_max and
+// "less than 0.1 % of hits have more than 50 neighbours") the sorted insertion is the wrong tool: almost every
+// candidate is rejected by the cut, yet the insertion code runs whenever any lane of the warp accepts one.  This
+// kernel only collects the candidates inside the cut, in scan order, in a per-thread shared-memory list of kKnnBuf
+// entries, then sorts that short list by d2 (stable, so equal distances stay in ascending index order: R5) and
+// writes its first k entries.  A hit with more than kKnnBuf candidates inside the cut gets deg = -1 and its bucket
+// a flag in `redo`; knn_kernel, which is exact for any count, then does those hits.
+constexpr int kKnnBuf = 64;            // >= the largest k
+constexpr int kKnnCutTile = 512;       // candidates per shared-memory tile (8 KB)
+constexpr int kKnnCutThreads = 96;     // a VELO bucket holds ~80 hits: three full warps; 56 KB per block, four blocks per SM
+
+__global__ void __launch_bounds__(kKnnCutThreads)
+knn_cut_kernel(const float4* __restrict__ emb, const int32_t* __restrict__ plane_off, int P, int k, int w,
+               float d2_max, int32_t* __restrict__ nbr, int32_t* __restrict__ deg, int32_t* __restrict__ redo) {
+  extern __shared__ float4 knn_smem[];
+  float4* cand = knn_smem;                                              // [kKnnCutTile]
+  float* bkey = reinterpret_cast<float*>(knn_smem + kKnnCutTile);       // [kKnnBuf][kKnnCutThreads]
+  int* bidx = reinterpret_cast<int*>(bkey + kKnnBuf * kKnnCutThreads);     // [kKnnBuf][kKnnCutThreads]
+  const int bucket = blockIdx.x, tid = threadIdx.x;
+  const int e = bucket / P, p = bucket % P;
+  const int32_t* po = plane_off + (size_t)e * (P + 1);
+  const int q_lo = po[p], q_hi = po[p + 1];
+  if (q_lo == q_hi) { if (tid == 0) redo[bucket] = 0; return; }
+  const int p_hi = min(p + w, P - 1);
+  const int c_lo = po[p + 1], c_hi = (p + 1 <= p_hi) ? po[p_hi + 1] : po[p + 1];
+  const bool single = (c_hi - c_lo) <= kKnnCutTile;
+  if (single) {
+    for (int i = tid; i < c_hi - c_lo; i += kKnnCutThreads) cand[i] = emb[c_lo + i];
+    __syncthreads();
+  }
+  int overflow = 0;
+  for (int q0 = q_lo; q0 < q_hi; q0 += kKnnCutThreads) {
+    const int q = q0 + tid;
+    const bool active = q < q_hi;
+    const float4 a = active ? emb[q] : make_float4(0.f, 0.f, 0.f, 0.f);
+    int cnt = 0;
+    for (int t0 = c_lo; t0 < c_hi; t0 += kKnnCutTile) {
+      const int nt = min(kKnnCutTile, c_hi - t0);
+      if (!single) {
+        __syncthreads();
+        for (int i = tid; i < nt; i += kKnnCutThreads) cand[i] = emb[t0 + i];
+        __syncthreads();
+      }
+      if (active) {
+#pragma unroll 4
+        for (int i = 0; i < nt; ++i) {
+          const float d = knn_d2(a, cand[i]);
+          if (d < d2_max) {                                             // R6: strict
+            if (cnt < kKnnBuf) { bkey[cnt * kKnnCutThreads + tid] = d; bidx[cnt * kKnnCutThreads + tid] = t0 + i; }
+            ++cnt;
+          }
+        }
+      }
+    }
+    // The lists of a warp's 32 hits are ordered one after the other by the whole warp: lane l ranks entries l and
+    // l + 32 of the list (rank = entries with a smaller d2, or an equal d2 met earlier in the scan: R5) and writes the
+    // entry to slot `rank` if that is one of the first k.  Ranking only reads the list, and the warp's cost is the sum
+    // of the list lengths, not 32 times the longest one.
+    const bool over = active && cnt > kKnnBuf;
+    if (over) { overflow = 1; deg[q] = -1; }                            // knn_kernel redoes this hit
+    const int my_n = (active && !over) ? cnt : 0;
+    if (active && !over) deg[q] = min(cnt, k);                          // slots past deg[q] are never read
+    __syncwarp();
+    const int lane = tid & 31, wbase = tid & ~31;
+    for (int l = 0; l < 32; ++l) {
+      const int n = __shfl_sync(0xffffffffu, my_n, l);
+      if (n == 0) continue;
+      const int col = wbase + l;
+      int32_t* out = nbr + (size_t)(q0 + col) * k;
+      for (int i = lane; i < n; i += 32) {
+        const float kd = bkey[i * kKnnCutThreads + col];
+        int rank = 0;
+        for (int j = 0; j < n; ++j) {
+          const float kj = bkey[j * kKnnCutThreads + col];
+          rank += (kj < kd) || (kj == kd && j < i);
+        }
+        if (rank < k) out[rank] = bidx[i * kKnnCutThreads + col];
+      }
+    }
+    __syncwarp();                                                       // the lists are rewritten by the next batch
+  }
+  overflow = __syncthreads_or(overflow);
+  if (tid == 0) redo[bucket] = overflow;
+}
+
 template <int KCAP>
-static void knn_dispatch(etx_ctx* c, int n_buckets, cudaStream_t s) {
+static void knn_dispatch(etx_ctx* c, int n_buckets, const int32_t* only, cudaStream_t s) {
   const etx_hyperparams& hp = c->hp;
   knn_kernel<KCAP><<<n_buckets, kKnnThreads, 0, s>>>(c->emb, c->plane_off, hp.n_planes, hp.k, hp.window,
-                                                    hp.d2_max, c->nbr, c->deg);
+                                                    hp.d2_max, c->nbr, c->deg, only);
+  c->launches++;
 }
 
 void launch_knn(etx_ctx* c, const int32_t* plane, int n_events, int n_hits, cudaStream_t s) {
   (void)plane;
   if (n_hits == 0 || n_events == 0) return;
-  const int nb = n_events * c->hp.n_planes;
-  const int k = c->hp.k;
-  if (k <= 4) knn_dispatch<4>(c, nb, s);
-  else if (k <= 10) knn_dispatch<10>(c, nb, s);
-  else if (k <= 16) knn_dispatch<16>(c, nb, s);
-  else if (k <= 32) knn_dispatch<32>(c, nb, s);
-  else knn_dispatch<64>(c, nb, s);
-  c->launches++;
+  const etx_hyperparams& hp = c->hp;
+  const int nb = n_events * hp.n_planes;
+  const int k = hp.k;
+  const int32_t* only = nullptr;
+  if (isfinite(hp.d2_max)) {
+    constexpr int smem = kKnnCutTile * (int)sizeof(float4) + kKnnBuf * kKnnCutThreads * 8;
+    static bool configured = false;
+    if (!configured) { cudaFuncSetAttribute(knn_cut_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); configured = true; }
+    knn_cut_kernel<<<nb, kKnnCutThreads, smem, s>>>(c->emb, c->plane_off, hp.n_planes, k, hp.window, hp.d2_max, c->nbr, c->deg, c->knn_redo);
+    c->launches++;
+    only = c->knn_redo;
+  }
+  if (k <= 4) knn_dispatch<4>(c, nb, only, s);
+  else if (k <= 10) knn_dispatch<10>(c, nb, only, s);
+  else if (k <= 16) knn_dispatch<16>(c, nb, only, s);
+  else if (k <= 32) knn_dispatch<32>(c, nb, only, s);
+  else knn_dispatch<64>(c, nb, only, s);
 }
 
 // --------------------------------------------------------------------------------------------------------

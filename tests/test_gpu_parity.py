@@ -46,7 +46,8 @@ def test_knn_and_edge_list_bit_exact_on_oracle_embedding(name, n_events):
     check_edge_invariants(g["src"], g["dst"], g["row_ptr"], b.plane, b.event_offsets, cfg.k, cfg.window)
 
 
-@pytest.mark.parametrize("k,w,d2max", [(4, 1, np.inf), (10, 2, np.inf), (16, 3, 2.0), (3, 25, np.inf), (33, 2, np.inf)])
+@pytest.mark.parametrize("k,w,d2max", [(4, 1, np.inf), (10, 2, np.inf), (16, 3, 2.0), (3, 25, np.inf), (33, 2, np.inf),
+                                       (50, 2, 1.0), (50, 2, 9.0), (64, 3, 1e30), (10, 2, 3.0), (7, 1, 1e-3)])
 def test_knn_ties_duplicates_radius_and_ragged_events(k, w, d2max):
     # integer-valued embeddings: many exact ties and duplicated points; events of ragged sizes incl. empty
     rng = np.random.default_rng(100 + k)
@@ -67,6 +68,34 @@ def test_knn_ties_duplicates_radius_and_ragged_events(k, w, d2max):
     assert np.array_equal(g["src"], src) and np.array_equal(g["dst"], dst)
     assert np.array_equal(g["row_ptr"], row_ptr) and np.array_equal(g["col_ptr"], col_ptr)
     assert np.array_equal(g["in_edge"], in_edge)
+
+
+@pytest.mark.parametrize("d2max", [0.05, 0.6, 50.0])
+def test_knn_radius_cut_kernel_short_lists_overflowing_lists_and_several_tiles(d2max):
+    # a finite cut takes the collect-then-sort kernel: 0.05 leaves a handful of candidates per hit (the paper's regime),
+    # 0.6 puts some hits above its 64-entry list and others below (flagged buckets are redone by the insertion kernel),
+    # 50.0 overflows every list; 1400 candidates per query span three of its 512-candidate tiles
+    rng = np.random.default_rng(11)
+    n0, n1, n2 = 300, 1400, 90
+    plane = np.concatenate([np.full(n0, 4), np.full(n1, 5), np.full(n2, 6)]).astype(np.int32)
+    off = np.array([0, plane.size], np.int32)
+    emb = rng.normal(0, 1, (plane.size, 4)).astype(F)
+    emb[:40] = np.round(emb[:40])                        # some exact ties
+    emb[n0:n0 + 200] = np.round(emb[n0:n0 + 200])
+    cfg = datagen.get_config("cfg5").replace(precision="fp32", gnn_iters=1, d2_max=d2max, window=1)
+    blob = datagen.pack_blob(cfg, datagen.make_weights(cfg, "parity"))
+    b = datagen.EventBatch(np.zeros((plane.size, 3), F), plane, off, np.zeros(plane.size, np.int64))
+    nbr, deg = oracle.knn(emb, plane, off, cfg.k, cfg.window, d2max)
+    inside = deg[:n0]
+    if d2max == 0.05:
+        assert inside.max() < 50
+    if d2max == 50.0:
+        assert inside.min() == 50
+    src, dst, _ = oracle.build_edges(nbr, deg)
+    ctx = make_ctx(cfg, blob, b)
+    g = run_gpu(ctx, b, emb=emb, last_stage=3)
+    assert np.array_equal(g["src"], src) and np.array_equal(g["dst"], dst)
+    ctx.destroy()
 
 
 def test_knn_candidate_window_larger_than_the_shared_memory_tile():
