@@ -98,6 +98,36 @@ def test_knn_radius_cut_kernel_short_lists_overflowing_lists_and_several_tiles(d
     ctx.destroy()
 
 
+@pytest.mark.parametrize("seed", range(10))
+def test_knn_seeded_random_shapes_cuts_and_k(seed):
+    # random k (1..64), window, cut (none / loose / tight), bucket sizes from empty to a few hundred hits, embeddings
+    # with a random share of exact duplicates: both k-NN kernels against the oracle, edge lists as arrays
+    rng = np.random.default_rng(4000 + seed)
+    k = int(rng.choice([1, 2, 4, 5, 10, 11, 16, 17, 32, 33, 50, 64]))
+    w = int(rng.integers(1, 5))
+    n_ev = int(rng.integers(1, 5))
+    planes, off = [], [0]
+    for _ in range(n_ev):
+        per_plane = rng.integers(0, int(rng.choice([3, 40, 300])), 26)
+        per_plane[rng.random(26) < 0.2] = 0
+        planes.append(np.repeat(np.arange(26), per_plane).astype(np.int32)); off.append(off[-1] + int(per_plane.sum()))
+    plane = np.concatenate(planes); off = np.asarray(off, np.int32)
+    emb = rng.normal(0, 1, (plane.size, 4)).astype(F)
+    dup = rng.random(plane.size) < rng.choice([0.0, 0.3, 0.9])
+    emb[dup] = np.round(emb[dup])
+    d2max = float(rng.choice([np.inf, 30.0, 1.5, 0.2, 1e-4]))
+    cfg = datagen.get_config("cfg1").replace(k=k, window=w, d2_max=d2max, precision="fp32", gnn_iters=1)
+    blob = datagen.pack_blob(cfg, datagen.make_weights(cfg, "parity"))
+    b = datagen.EventBatch(np.zeros((plane.size, 3), F), plane, off, np.zeros(plane.size, np.int64))
+    nbr, deg = oracle.knn(emb, plane, off, k, w, d2max)
+    src, dst, row_ptr = oracle.build_edges(nbr, deg)
+    ctx = make_ctx(cfg, blob, b)
+    g = run_gpu(ctx, b, emb=emb, last_stage=3)
+    assert np.array_equal(g["row_ptr"], row_ptr), (k, w, d2max)
+    assert np.array_equal(g["src"], src) and np.array_equal(g["dst"], dst), (k, w, d2max)
+    ctx.destroy()
+
+
 def test_knn_candidate_window_larger_than_the_shared_memory_tile():
     # one event, two planes, 3000 candidates per query: spans several 1024-candidate tiles + a ragged tail
     rng = np.random.default_rng(7)
