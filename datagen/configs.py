@@ -82,8 +82,9 @@ CONFIGS: dict[str, EtxConfig] = {
     # with a radius cut, w = 2, latent 32, n = 5 steps with distinct weights (L148), edge encoder on
     # [h0_src, h0_dst] (L133).  The paper's d2_max = 0.9 only means something for its trained embedding; with
     # seeded random weights the cut is set to the value that leaves ~14 edges per hit (L74: ~30,000 edges for
-    # ~2,200 hits), measured on six events of this generator with the oracle (0.06 % of the hits then fill all 50
-    # slots; the paper reports < 0.1 %, L257).  Embedding shape as cfg 2, input the paper's normalised cylindrical
+    # ~2,200 hits), measured on six events of this generator with the oracle.  On those six events 0.06 % of the
+    # hits fill all 50 slots (the paper reports < 0.1 %, L257); over the first 24 events it is 3 %, because the busiest
+    # events (> 4,500 hits) saturate 10-20 % of their hits -- a fixed cut on an untrained embedding tracks density.  Embedding shape as cfg 2, input the paper's normalised cylindrical
     # coordinates (L96, R27).
     "cfg5": EtxConfig(name="cfg5", n_events=500, fixed_pv=None, mu_pv=5.0, fixed_tracks=None,
                       mu_tracks=40.0, noise_frac=0.02, events_seed=1005,
