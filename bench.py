@@ -127,7 +127,7 @@ def stage_model(cfg, N, E, pairs, peaks):
         "S0_plane_offsets": ("hbm", 16.0 * N + 4.0 * N, peaks["hbm"], "GB/s"),
         "S1_embedding": (mlp_bound, N * 2.0 * (3 * D + (H - 1) * D * D + 4 * D), mlp_peak, "TFLOP/s"),
         "S2_knn": ("alu", pairs * 12.0, alu_lane, "lane-instr/s"),
-        "S3_compaction_csc": ("hbm", 4.0 * k * N + 12.0 * E + 12.0 * E + 16.0 * N, peaks["hbm"], "GB/s"),
+        "S3_compaction_csc": ("hbm", 4.0 * k * N + 12.0 * E + 8.0 * E + 16.0 * N, peaks["hbm"], "GB/s"),
         "S4_encoders": (mlp_bound, 2.0 * (3 * d + d * d) * (N + E), mlp_peak, "TFLOP/s"),
         # e is read from HBM once (the second direction finds its rows in L2: ncu, profiles/r1f_stage_rooflines.md)
         "S4c_scatter": ("hbm", L * (1.0 * E * d * b + 2.0 * N * d * b + 4.0 * E + 8.0 * N), peaks["hbm"], "GB/s"),
