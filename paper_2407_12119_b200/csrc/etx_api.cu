@@ -229,6 +229,7 @@ etx_status run_impl(etx_ctx* c, const float* d_xyz, const int32_t* d_plane, cons
           auto mlp = [&](int kind, int it, bool head) {
             if (kind == kEdgeNet && c->edge_tma) launch_edge_net_tma(c, it, n_hits, head, s);
             else if (kind == kEdgeEnc && c->edge_tma && c->hp.edge_enc_input == 0 && !head) launch_edge_enc_tma(c, n_hits, false, s);
+            else if (kind == kEdgeEnc && c->edge_tma && c->hp.edge_enc_input == 1) launch_edge_enc_h_tma(c, n_hits, head, s);
             else if (kind == kNodeEnc && c->edge_tma) launch_edge_enc_tma(c, n_hits, true, s);
             else if (tensor_engine && c->precision == ETX_BF16 && c->engine != ETX_ENGINE_TC_SERIAL) launch_gnn_mlp_ws(c, kind, it, n_hits, head, s);
             else if (kind == kEdgeNet && c->edge_i8 && c->tap_layer < 0)

@@ -108,6 +108,7 @@ struct etx_ctx {
   bool edge_tma = false;
   bool edge_i8 = false;                   // k_edge_i8.cu usable (INT8, auto engine, tensor map of fp32 `e` encoded)
   void* ident_img = nullptr;
+  void* eenc_b0_img = nullptr;
   void* eenc_b1_img = nullptr;
   void* nenc_b1_img = nullptr;
   std::vector<void*> edge_bias_img;
@@ -144,6 +145,7 @@ namespace etx {
 void* etx_device_alloc(etx_ctx* c, size_t bytes);
 // k_graph.cu
 void launch_features(etx_ctx* c, const float* xyz, int n_hits, cudaStream_t s);
+void launch_edge_enc_h_tma(etx_ctx* c, int n_hits, bool do_head, cudaStream_t s);
 void launch_plane_offsets(etx_ctx* c, const int32_t* plane, int n_events, cudaStream_t s);
 void launch_validate(etx_ctx* c, const int32_t* plane, int n_events, int n_hits, cudaStream_t s);
 void launch_knn(etx_ctx* c, const int32_t* plane, int n_events, int n_hits, cudaStream_t s);

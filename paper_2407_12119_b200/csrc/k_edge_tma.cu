@@ -139,6 +139,7 @@ struct EdgeTmaArgs {
   float* logit; float* score;
   int do_head;
   int store_e;                 // 0: the new edge state is dead (last step of a plain etx_run: only the classifier reads it)
+  int enc;                     // 1: S4b with the paper's input, e0 = MLP([h0_src, h0_dst]) (L133): no old state, K = 2d
 };
 
 // all MMAs of one K-block: kbytes of K, 32 bytes (16 bf16) per instruction
@@ -246,6 +247,7 @@ edge_net_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeTmaArgs
         PROF(0)
         mbar_wait(&self_empty[s], ((it / kNE) & 1) ^ 1);
         PROF(1)
+        if (a.enc) { mbar_arrive(&self_full[s]); continue; }  // no old state: the slot is only the output staging
         mbar_expect_tx(&self_full[s], BLK);
         tma_load_2d(self_addr + s * BLK, &e_map, 0, tile * kRows, &self_full[s]);
       }
@@ -275,7 +277,7 @@ edge_net_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeTmaArgs
   } else if (warp == kMmaWarp) {
     // ================================================================================================ MMA issuer
     if (elect_one()) {
-      const uint32_t wb0 = 3 * D * KB, wb1 = D * KB, bb = D * 32;
+      const uint32_t wb0 = (a.enc ? 2 : 3) * D * KB, wb1 = D * KB, bb = D * 32;
       mbar_expect_tx(bar_w, wb0 + 2 * wb1 + 2 * bb);
       bulk_g2s(smem + L.w0, a.w0_img, wb0, bar_w);
       bulk_g2s(smem + L.w1, a.w1_img, wb1, bar_w);
@@ -299,7 +301,7 @@ edge_net_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeTmaArgs
 #pragma unroll
         for (int k = 0; k < D / 16; ++k)                      // A = hidden in tensor memory, 8 packed columns per K = 16
           umma_ts(d1, hid + 8 * k, make_desc<KB>(w1_addr + k * 32), idesc, 1u);
-        issue_block<KB>(self_addr + se * BLK, id_addr, d1, idesc);
+        if (!a.enc) issue_block<KB>(self_addr + se * BLK, id_addr, d1, idesc);             // + old e (R14)
         umma_commit(&acc1_full[g]);
         PROF(2)
       };
@@ -322,7 +324,7 @@ edge_net_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeTmaArgs
         umma::umma<kBf16>(d0, ones_desc, b0_desc, idesc, 0u);
         issue_block<KB>(aux_addr + sh * 2 * BLK, w0_addr, d0, idesc);                      // h_src
         issue_block<KB>(aux_addr + sh * 2 * BLK + BLK, w0_addr + D * KB, d0, idesc);       // h_dst
-        issue_block<KB>(self_addr + se * BLK, w0_addr + 2 * D * KB, d0, idesc);            // e
+        if (!a.enc) issue_block<KB>(self_addr + se * BLK, w0_addr + 2 * D * KB, d0, idesc);   // e
         umma_commit(&acc0_full[g]);
         umma_commit(&aux_empty[sh]);                          // layer 0 was the gather slot's only reader
         PROF(4)
@@ -715,6 +717,8 @@ bool edge_tma_configure(etx_ctx* c) {
       if (!p) return false;
       c->edge_bias_img[2 * it + l] = p;
     }
+  c->eenc_b0_img = upload_bytes(c, pack_split_rows(c->layers[c->i_eenc].b));
+  if (!c->eenc_b0_img) return false;
   c->eenc_b1_img = upload_bytes(c, pack_split_rows(c->layers[c->i_eenc + 1].b));
   c->nenc_b1_img = upload_bytes(c, pack_split_rows(c->layers[c->i_nenc + 1].b));
   if (!c->eenc_b1_img || !c->nenc_b1_img) return false;
@@ -753,6 +757,25 @@ void launch_edge_net_tma(etx_ctx* c, int iter, int n_hits, bool do_head, cudaStr
   a.src = c->src; a.dst = c->dst; a.n_rows_ptr = c->n_edges;
   a.logit = c->logit; a.score = c->score_out; a.do_head = do_head ? 1 : 0;
   a.store_e = (do_head && !c->keep_final_state) ? 0 : 1;
+  a.enc = 0;
+  const long long max_rows_ll = (long long)n_hits * c->hp.k;
+  const int max_rows = (int)(max_rows_ll > 0x7fffffff ? 0x7fffffff : max_rows_ll);
+  if (c->hp.gnn_latent == 32) edge_tma_launch<32>(c, a, max_rows, s);
+  else edge_tma_launch<64>(c, a, max_rows, s);
+}
+
+// S4b with the paper's edge-encoder input (edge_enc_input == 1, L133): e0 = MLP([h0_src, h0_dst]).  The edge-network kernel
+// without an old state: nothing is loaded into the state slots, layer 0 has two K-blocks, layer 1 no identity block.
+void launch_edge_enc_h_tma(etx_ctx* c, int n_hits, bool do_head, cudaStream_t s) {
+  const int i0 = c->i_eenc;
+  EdgeTmaArgs a;
+  a.w0_img = c->layers[i0].dev.Wtc; a.w1_img = c->layers[i0 + 1].dev.Wtc; a.ident_img = c->ident_img;
+  a.b0_img = c->eenc_b0_img; a.b1_img = c->eenc_b1_img;
+  a.head_w = c->layers[c->i_head].dev.Wt; a.head_b = c->layers[c->i_head].dev.bias;
+  a.h = static_cast<const __nv_bfloat16*>(c->h);
+  a.src = c->src; a.dst = c->dst; a.n_rows_ptr = c->n_edges;
+  a.logit = c->logit; a.score = c->score_out; a.do_head = do_head ? 1 : 0;
+  a.store_e = 1; a.enc = 1;
   const long long max_rows_ll = (long long)n_hits * c->hp.k;
   const int max_rows = (int)(max_rows_ll > 0x7fffffff ? 0x7fffffff : max_rows_ll);
   if (c->hp.gnn_latent == 32) edge_tma_launch<32>(c, a, max_rows, s);

@@ -296,7 +296,7 @@ __global__ void __launch_bounds__(kWsThreads, 1) gnn_mlp_ws_kernel(GnnArgs a) {
           qv.x = pack_bf16x2(y[0], y[1]); qv.y = pack_bf16x2(y[2], y[3]);
           qv.z = pack_bf16x2(y[4], y[5]); qv.w = pack_bf16x2(y[6], y[7]);
           *reinterpret_cast<uint4*>(Hg + swz<KB>(r, c0 / 8 + ch)) = qv;        // staging (layer 1 has finished with Hg)
-          if (KIND == kEdgeNet && a.do_head) {                // the classifier sees the stored bf16 state (R20), ascending j (R16)
+          if (is_edge && a.do_head) {                         // the classifier sees the stored bf16 state (R20), ascending j (R16)
             const float* hw = headw + c0 + ch * 8;
             hacc = __fmaf_rn(bf16_lo(qv.x), hw[0], hacc); hacc = __fmaf_rn(bf16_hi(qv.x), hw[1], hacc);
             hacc = __fmaf_rn(bf16_lo(qv.y), hw[2], hacc); hacc = __fmaf_rn(bf16_hi(qv.y), hw[3], hacc);
@@ -316,7 +316,7 @@ __global__ void __launch_bounds__(kWsThreads, 1) gnn_mlp_ws_kernel(GnnArgs a) {
         if (grow < n_rows)
           *reinterpret_cast<uint4*>(state + (size_t)grow * D + piece * 8) = *reinterpret_cast<const uint4*>(Hg + swz<KB>(rr, piece));
       }
-      if (KIND == kEdgeNet && a.do_head && live) {
+      if (is_edge && a.do_head && live) {
         const float z = __fadd_rn(hacc, head_b);
         a.logit[row] = z;
         a.score[row] = 1.0f / (1.0f + expf(-z));

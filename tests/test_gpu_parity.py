@@ -337,6 +337,31 @@ def test_plain_run_skips_the_dead_final_edge_state_and_changes_nothing_else(name
     ctx.destroy()
 
 
+@pytest.mark.parametrize("d,eei,precision", [(32, 1, "bf16"), (64, 1, "bf16"), (64, 0, "bf16"), (32, 0, "bf16"),
+                                             (64, 0, "fp32"), (64, 1, "int8"), (64, 0, "int8")])
+def test_no_message_passing_steps_classifier_on_the_encoded_edges(d, eei, precision):
+    # degenerate case L = 0: the classifier reads e0 straight from the edge encoder (the head is fused into the encoder
+    # launch); with the paper's encoder input (L133) that is the edge-network kernel in its no-old-state mode
+    cfg = datagen.get_config("cfg1").replace(precision=precision, gnn_latent=d, gnn_iters=0, edge_enc_input=eei)
+    b = datagen.generate_batch(cfg, n_events=3)
+    W = centred_parity_weights(cfg.replace(precision="fp32") if precision == "int8" else cfg, b)
+    blob = _int8_blob(cfg, b, W) if precision == "int8" else datagen.pack_blob(cfg, W)
+    o, r = _oracle_all(cfg, b, blob, precision)
+    ctx = make_ctx(cfg, blob, b)
+    g = run_gpu(ctx, b, emb=r["emb"], src=r["src"], dst=r["dst"])
+    og = o.gnn(b.xyz, r["src"], r["dst"], want_states=True)
+    tol = 2e-2 if precision == "bf16" else 1e-4
+    assert np.abs(g["score"] - og["score"]).max() <= tol
+    assert np.mean((og["score"] > 0.01) & (og["score"] < 0.99)) > 0.3          # the comparison is informative
+    e = state(ctx, "e", r["src"].size, d)
+    assert np.abs(e - og["e"]).max() <= tol * max(1.0, float(np.abs(og["e"]).max()))
+    if precision == "int8":
+        assert np.array_equal(g["logit"], og["logit"])
+    g2 = run_gpu(ctx, b, debug=False)
+    assert np.array_equal(g2["track_id"], oracle.components(g2["src"], g2["dst"], g2["logit"], oracle.logit_threshold(cfg.threshold), b.n_hits))
+    ctx.destroy()
+
+
 def test_repeated_runs_on_one_handle_are_identical_and_smaller_batches_work():
     cfg, b, W = _setup("cfg1", 4, precision="fp32")
     blob = datagen.pack_blob(cfg, W)
