@@ -362,6 +362,28 @@ def test_no_message_passing_steps_classifier_on_the_encoded_edges(d, eei, precis
     ctx.destroy()
 
 
+@pytest.mark.parametrize("thr", [0.0, 1.0, 0.999, 1e-3])
+def test_threshold_extremes(thr):
+    # s_edge,min = 0 keeps every edge (components = those of the rough graph), 1 keeps none unless a score is exactly 1
+    # (every hit its own track on these weights); the decision is taken on the logit (R17)
+    cfg, b, W = _setup("cfg1", 3, precision="fp32")
+    cfg = cfg.replace(threshold=thr)
+    blob = datagen.pack_blob(cfg, W)
+    o, r = _oracle_all(cfg, b, blob, "fp32")
+    ctx = make_ctx(cfg, blob, b)
+    g = run_gpu(ctx, b, debug=False)
+    assert np.array_equal(g["src"], r["src"]) and np.array_equal(g["track_id"], r["track_id"])
+    n_tracks = np.unique(g["track_id"]).size
+    if thr == 0.0:
+        import scipy.sparse as sp
+        from scipy.sparse.csgraph import connected_components
+        A = sp.coo_matrix((np.ones(r["src"].size), (r["src"], r["dst"])), shape=(b.n_hits, b.n_hits))
+        assert n_tracks == connected_components(A, directed=False)[0]
+    if thr == 1.0:
+        assert n_tracks == b.n_hits
+    ctx.destroy()
+
+
 def test_repeated_runs_on_one_handle_are_identical_and_smaller_batches_work():
     cfg, b, W = _setup("cfg1", 4, precision="fp32")
     blob = datagen.pack_blob(cfg, W)
