@@ -431,11 +431,31 @@ __global__ void pack_edges_kernel(const int32_t* __restrict__ nbr, const int32_t
   }
 }
 
+// Large k with a radius cut leaves most of the k slots of a hit empty (cfg 5: ~15 of 50): sixteen lanes per hit walk
+// its deg[q] filled slots instead of one thread per slot.
+__global__ void pack_edges_sparse_kernel(const int32_t* __restrict__ nbr, const int32_t* __restrict__ deg,
+                                         const int32_t* __restrict__ row_ptr, int n_hits, int k,
+                                         int32_t* __restrict__ src, int32_t* __restrict__ dst) {
+  const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int q = (int)(t >> 4), l = (int)(t & 15);
+  if (q >= n_hits) return;
+  const int n = deg[q], base = row_ptr[q];
+  for (int sidx = l; sidx < n; sidx += 16) {
+    src[base + sidx] = q;
+    dst[base + sidx] = nbr[(size_t)q * k + sidx];
+  }
+}
+
 void launch_pack_edges(etx_ctx* c, int n_hits, cudaStream_t s) {
   exclusive_scan(c, c->deg, n_hits, c->row_ptr, c->n_edges, s);
   if (n_hits == 0) return;
-  size_t n = (size_t)n_hits * c->hp.k;
-  pack_edges_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(c->nbr, c->deg, c->row_ptr, n_hits, c->hp.k, c->src, c->dst);
+  if (c->hp.k > 16) {
+    const size_t n = (size_t)n_hits * 16;
+    pack_edges_sparse_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(c->nbr, c->deg, c->row_ptr, n_hits, c->hp.k, c->src, c->dst);
+  } else {
+    const size_t n = (size_t)n_hits * c->hp.k;
+    pack_edges_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(c->nbr, c->deg, c->row_ptr, n_hits, c->hp.k, c->src, c->dst);
+  }
   c->launches++;
 }
 
