@@ -170,7 +170,10 @@ def main():
         cfg = cfg.replace(n_events=args.events)
     config = {"workload": f"{cfg.name}: {cfg.n_events} synthetic VELO events/GPU, pile-up {cfg.mu_pv:g}, "
                           f"emb 3->{'->'.join([str(cfg.emb_hidden)] * cfg.emb_n_hidden_layers)}->4, k={cfg.k}, w={cfg.window}, "
-                          f"d={cfg.gnn_latent}, L={cfg.gnn_iters}, {cfg.precision}",
+                          f"d={cfg.gnn_latent}, L={cfg.gnn_iters}, {cfg.precision}"
+                          + (f", d2_max={cfg.d2_max:g}" if cfg.d2_max != float("inf") else "")
+                          + (", edge encoder on [h0_src,h0_dst]" if cfg.edge_enc_input else "")
+                          + (", cylindrical embedding input" if cfg.emb_input else ""),
               "events_per_gpu": cfg.n_events, "weights": "He-uniform seed 7, zero bias",
               "l2": "per-step working set (edge state alone > 1 GB) exceeds the 126 MB L2; no explicit flush"}
 
