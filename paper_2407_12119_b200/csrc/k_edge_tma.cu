@@ -420,13 +420,13 @@ edge_net_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeTmaArgs
 // ---------------------------------------------------------------------------------------------- S4b edge encoder
 // e0 = W1 relu(W0 |f_dst - f_src| + b0) + b1  (PAPER.md L133 with the configs' K = 3 input, R10 / R11).
 // The stage only WRITES the edge state (E * d * 2 bytes), so it is bound by that write plus the FFMA work of the
-// K = 3 layer, which stays on the fp32 pipe in the pinned order (R3, R20).  Four warpgroups each own the CTA's
-// tiles it = w (mod 4) from front to back: gather the two feature rows (prefetched one tile ahead, their indices
+// K = 3 layer, which stays on the fp32 pipe in the pinned order (R3, R20).  Five warpgroups each own the CTA's
+// tiles it = w (mod 5) from front to back (five is what tensor memory holds: 5 x (D + D/2) = 480 of 512 columns): gather the two feature rows (prefetched one tile ahead, their indices
 // two tiles ahead), layer 0 on the FFMA pipe, relu -> bf16 -> tensor memory (the A operand of layer 1), wait for
 // the MMA, TMEM -> bf16 -> the warpgroup's swizzled shared-memory slot, and one TMA store per tile.
-constexpr int kEncGroups = 4;
+constexpr int kEncGroups = 5;
 constexpr int kEncMmaWarp = kEncGroups * 4, kEncStoreWarp = kEncMmaWarp + 1;
-constexpr int kEncThreads = (kEncStoreWarp + 1) * 32;      // 576
+constexpr int kEncThreads = (kEncStoreWarp + 1) * 32;      // 704
 
 struct EncSmem { int out, w1, ones, b1, w3, bar, total; };
 template <int D>
@@ -459,7 +459,7 @@ __global__ void __launch_bounds__(kEncThreads, 1)
 edge_enc_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeEncArgs a) {
   constexpr int KB = D * 2, BLK = kRows * KB;
   constexpr EncSmem L = enc_layout<D>();
-  constexpr uint32_t TMEM_COLS = 8 * D;                      // acc[4] (D each) | hidden[4] (D/2 each), pow2
+  constexpr uint32_t TMEM_COLS = 8 * D;                      // acc[5] (D each) | hidden[5] (D/2 each) = 7.5 D, pow2
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + L.bar);
