@@ -130,10 +130,12 @@ def components_bfs(src, dst, keep, n):
     return lab
 
 
-def components_paper_sweeps(src, dst, keep, plane, n, n_planes=26, max_rounds=1000):
+def components_paper_sweeps(src, dst, keep, plane, n, n_planes=26, max_rounds=1000, stop_after=None):
     """PAPER.md L261 sec. 7.3: label = own index; forward sweep over planes taking the lowest label
     among left neighbours, then backward sweep over right neighbours; iterated to a fixed point.
-    Returns (labels, rounds)."""
+    Returns (labels, rounds), rounds = the number of forward + backward rounds that still changed a
+    label, plus the final one that changed nothing.  stop_after = r returns the labels after exactly r
+    rounds (the paper's own algorithm is stop_after = 1)."""
     lab = np.arange(n, dtype=np.int64)
     left = [[] for _ in range(n)]; right = [[] for _ in range(n)]
     for s, t, kk in zip(src, dst, keep):
@@ -152,7 +154,7 @@ def components_paper_sweeps(src, dst, keep, plane, n, n_planes=26, max_rounds=10
                 for u in right[v]:
                     if lab[u] < lab[v]:
                         lab[v] = lab[u]; changed = True
-        if not changed:
+        if not changed or (stop_after is not None and rnd >= stop_after):
             return lab.astype(np.int32), rnd
     raise RuntimeError("sweeps did not converge")
 
@@ -196,3 +198,77 @@ def centred_parity_weights(cfg, batch, seed=None):
     assert name == "head"
     layers[-1] = (name, W, (b - np.float32(med)).astype(np.float32))
     return layers
+
+
+# ---- the interaction network restated with explicit rounding points ------------------------
+def f32_chain(x, W, b):
+    """One Linear in the pinned fp32 order (R3): acc = 0; acc = fma(x[j], W[c][j], acc) for j
+    ascending; y = acc + b[c].  Each fma is emulated as an exact float64 product and sum rounded once to
+    fp32 (a 24 x 24 bit product is exact in float64)."""
+    x = np.asarray(x, np.float32); W = np.asarray(W, np.float32); b = np.asarray(b, np.float32)
+    acc = np.zeros((x.shape[0], W.shape[0]), np.float32)
+    for j in range(W.shape[1]):
+        acc = (x[:, j:j + 1].astype(np.float64) * W[None, :, j].astype(np.float64) + acc.astype(np.float64)).astype(np.float32)
+    return (acc + b[None, :]).astype(np.float32)
+
+
+def torch_bf16(x):
+    """RNE rounding to bfloat16 by torch's CPU conversion (not the oracle's bit manipulation)."""
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(x, np.float32)).to(torch.bfloat16).to(torch.float32).numpy()
+
+
+BF16_POINTS = ("weights", "enc_hidden", "enc_out", "msg", "node_hidden", "h_resid", "edge_hidden", "e_resid")
+
+
+def gnn_restated(cfg, layers, f, src, dst, points=(), on_linear_input=None):
+    """PAPER.md L133-142 (sec. 5.2) written out with numpy, one statement per step of the paper, every
+    Linear in the pinned fp32 order.  `points` names the places where a value is rounded to bfloat16
+    (R20): "weights" (Linears with K >= 16 except the head), hidden activations of the four
+    MLP kinds, encoder outputs, the message after its fp32 sum, h / e after the fp32 residual add.
+    `on_linear_input(name, x)` sees the input tensor of every Linear (used to recompute INT8 scales).
+    -> dict(h, e, logit)."""
+    lay = {n: (W.astype(np.float32), b.astype(np.float32)) for n, W, b in layers}
+    rnd = lambda x, p: torch_bf16(x) if p in points else x
+
+    def linear(name, x):
+        W, b = lay[name]
+        if on_linear_input is not None:
+            on_linear_input(name, x)
+        if W.shape[1] >= 16 and name != "head" and "weights" in points:
+            W = torch_bf16(W)
+        return f32_chain(x, W, b)
+
+    def mlp(n0, n1, x, hidden_point):
+        a = rnd(np.maximum(linear(n0, x), np.float32(0)), hidden_point)
+        return linear(n1, a)
+
+    f = np.asarray(f, np.float32)
+    n, E, d = f.shape[0], src.size, cfg.gnn_latent
+    h = rnd(mlp("nenc0", "nenc1", f, "enc_hidden"), "enc_out")                        # L133
+    x = np.abs(f[dst] - f[src]) if cfg.edge_enc_input == 0 else np.concatenate([h[src], h[dst]], 1)
+    e = rnd(mlp("eenc0", "eenc1", x, "enc_hidden"), "enc_out")
+    for it in range(cfg.gnn_iters):                                                   # L135-140
+        m = np.zeros((n, 2 * d), np.float32)
+        for i in range(E):                                                            # Eq.(4), ascending edge id
+            m[src[i], :d] = m[src[i], :d] + e[i]
+            m[dst[i], d:] = m[dst[i], d:] + e[i]
+        m = rnd(m, "msg")
+        h = rnd((h + mlp(f"node{it}_0", f"node{it}_1", np.concatenate([h, m], 1), "node_hidden")).astype(np.float32), "h_resid")
+        e = rnd((e + mlp(f"edge{it}_0", f"edge{it}_1", np.concatenate([h[src], h[dst], e], 1), "edge_hidden")).astype(np.float32), "e_resid")
+    logit = linear("head", e)[:, 0]                                                   # L142
+    return dict(h=h, e=e, logit=logit)
+
+
+def embed_restated(cfg, layers, f_emb, on_linear_input=None):
+    """PAPER.md L96 (sec. 5.1): the embedding MLP in the pinned fp32 order, ReLU after hidden layers."""
+    lay = {n: (W.astype(np.float32), b.astype(np.float32)) for n, W, b in layers}
+    a = np.asarray(f_emb, np.float32)
+    H = cfg.emb_n_hidden_layers
+    for l in range(H + 1):
+        if on_linear_input is not None:
+            on_linear_input(f"emb{l}", a)
+        a = f32_chain(a, *lay[f"emb{l}"])
+        if l < H:
+            a = np.maximum(a, np.float32(0))
+    return a

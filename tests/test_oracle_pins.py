@@ -513,15 +513,20 @@ def test_components_equal_bfs_scipy_and_iterated_paper_sweeps():
 
 
 def test_zigzag_component_needs_more_than_two_sweeps_but_oracle_is_exact():
-    # kept edges a->c, b->c, b->d with a<b on plane 0 and c<d on plane 1, plus d->f, g->f with g a
-    # low-plane, high-index... build a chain that two sweeps under-merge (documented in R18)
-    plane = np.array([0, 0, 1, 1], np.int32)
-    src = np.array([0, 1, 1], np.int32); dst = np.array([2, 2, 3], np.int32)
-    keep = np.ones(3, bool)
-    tid = oracle.components(src, dst, np.ones(3, F), 0.0, 4)
-    assert tid.tolist() == [0, 0, 0, 0]
-    sw, rounds = components_paper_sweeps(src, dst, keep, plane, 4)
-    assert sw.tolist() == [0, 0, 0, 0]
+    # R18: the paper's WCC is ONE forward and ONE backward sweep (L261).  A zig-zag component
+    # A -> B <- C -> D <- E -> F (A, C, E on plane 0; B, D, F on plane 1; edges always low plane -> high plane)
+    # is under-merged by it: the lowest label has to travel right, left, right, ... and each round of sweeps
+    # moves it by one zig-zag only.  The oracle labels exact components (the sweeps' fixed point).
+    plane = np.array([0, 0, 0, 1, 1, 1], np.int32)              # hits 0..2 = A, C, E ; 3..5 = B, D, F
+    src = np.array([0, 1, 1, 2, 2], np.int32); dst = np.array([3, 3, 4, 4, 5], np.int32)
+    keep = np.ones(5, bool)
+    tid = oracle.components(src, dst, np.ones(5, F), 0.0, 6)
+    assert tid.tolist() == [0] * 6
+    one, _ = components_paper_sweeps(src, dst, keep, plane, 6, stop_after=1)
+    assert one.tolist() == [0, 0, 1, 0, 1, 2]                  # the paper's two sweeps leave three labels
+    sw, rounds = components_paper_sweeps(src, dst, keep, plane, 6)
+    assert rounds > 2 and sw.tolist() == [0] * 6               # labels still change in the second round
+    assert np.array_equal(tid, components_bfs(src, dst, keep, 6))
 
 
 def test_truth_edges_on_noise_free_event_give_one_component_per_particle():
@@ -654,3 +659,82 @@ def test_oracle_bits_have_not_moved_since_the_stored_digests():
         pytest.skip("the seeded generator's float64 libm calls round differently on this machine: inputs differ, nothing to compare")
     for g, w in zip(got, want):
         assert g == w, (w["case"], {k: (g[k], w[k]) for k in w if g[k] != w[k]})
+
+
+# ------------------------------------------------------------------ bf16 rounding points inside the GNN (R20)
+def _bf16_gnn_case(eei):
+    from helpers import gnn_restated
+    cfg = toy_config(d=16, L=2, edge_enc_input=eei, precision="bf16")   # d = 16: every d-input Linear is a tensor layer
+    W = datagen.make_weights(cfg, "parity", seed=11)
+    xyz, src, dst = _tiny_graph(6, n=14, E=44)
+    blob = datagen.pack_blob(cfg, W)
+    out = oracle.Oracle(blob, "bf16").gnn(xyz, src, dst, want_states=True)
+    f = ((xyz + np.array(datagen.configs.NORM_OFFSET, F)) / np.array(datagen.configs.NORM_DIV, F)).astype(F)
+    return cfg, W, f, src, dst, out, gnn_restated
+
+
+@pytest.mark.parametrize("eei", [0, 1])
+def test_bf16_gnn_rounding_points_equal_a_torch_bfloat16_restatement_bit_for_bit(eei):
+    # PAPER.md L133-142 restated in numpy; the bf16 roundings are torch's bfloat16 conversion, placed at exactly the
+    # points of DESIGN.md R20: weights of the K >= 16 Linears (not the head, not the K = 3 layers), hidden
+    # activations, encoder outputs, the message after its fp32 sum, h / e after the fp32 residual add.
+    from helpers import BF16_POINTS
+    cfg, W, f, src, dst, out, gnn_restated = _bf16_gnn_case(eei)
+    ref = gnn_restated(cfg, W, f, src, dst, points=BF16_POINTS)
+    for key in ("h", "e", "logit"):
+        assert np.array_equal(out[key].view(np.uint32), ref[key].view(np.uint32)), key
+    # the stored states are bf16 numbers, the logits (fp32 head on the stored bf16 e) are not
+    assert np.array_equal(out["e"], torch.from_numpy(out["e"]).to(torch.bfloat16).to(torch.float32).numpy())
+    assert not np.array_equal(out["logit"], torch.from_numpy(out["logit"]).to(torch.bfloat16).to(torch.float32).numpy())
+
+
+def test_bf16_gnn_dropping_any_one_rounding_point_changes_the_result():
+    # the restatement is sensitive to every single rounding point: if the oracle missed or misplaced one of them
+    # the previous test could not pass
+    from helpers import BF16_POINTS
+    cfg, W, f, src, dst, out, gnn_restated = _bf16_gnn_case(0)
+    for drop in BF16_POINTS:
+        ref = gnn_restated(cfg, W, f, src, dst, points=tuple(p for p in BF16_POINTS if p != drop))
+        same = all(np.array_equal(out[k].view(np.uint32), ref[k].view(np.uint32)) for k in ("h", "e", "logit"))
+        assert not same, f"dropping the rounding point '{drop}' went unnoticed"
+    # and rounding somewhere R20 keeps fp32 (the K = 3 encoder weights) is noticed as well
+    W3 = [(n, torch.from_numpy(w).to(torch.bfloat16).to(torch.float32).numpy() if n in ("nenc0", "eenc0") else w, b) for n, w, b in W]
+    ref = gnn_restated(cfg, W3, f, src, dst, points=BF16_POINTS)
+    assert not np.array_equal(out["logit"], ref["logit"])
+
+
+# ------------------------------------------------------------------ INT8 calibration scales (R21)
+def test_int8_activation_scales_equal_an_independent_recomputation_bit_for_bit():
+    # s_x = max|x| / 127 over the INPUT tensor of every quantised Linear (a concatenated input is one tensor) in the
+    # fp32 forward of the calibration batch; recomputed here with the numpy restatement, not with the oracle's
+    # instrumentation.  The graph (k-NN edges) is taken from the oracle, whose k-NN is pinned above.
+    from helpers import embed_restated, gnn_restated
+    cfg = datagen.get_config("cfg0")
+    W = datagen.make_weights(cfg, "parity")
+    b = datagen.generate_batch(cfg, n_events=2, seed=datagen.configs.CALIBRATION_SEED)
+    blob = datagen.pack_blob(cfg, W)
+    got = oracle.calibrate_int8(blob, b.xyz, b.plane, b.event_offsets, cfg.k, cfg.window)
+    o = oracle.Oracle(blob, "fp32")
+    nbr, deg = oracle.knn(o.embed(b.xyz), b.plane, b.event_offsets, cfg.k, cfg.window)
+    src, dst, _ = oracle.build_edges(nbr, deg)
+    amax = {}
+    def see(name, x):
+        amax[name] = max(amax.get(name, 0.0), float(np.abs(x).max()))
+    f = ((b.xyz + np.array(datagen.configs.NORM_OFFSET, F)) / np.array(datagen.configs.NORM_DIV, F)).astype(F)
+    emb = embed_restated(cfg, W, f, on_linear_input=see)
+    assert np.array_equal(emb.view(np.uint32), o.embed(b.xyz).view(np.uint32))
+    gnn_restated(cfg, W, f, src, dst, points=(), on_linear_input=see)
+    names = datagen.weights.quantised_layer_names(cfg)
+    want = np.array([F(amax[n]) / F(127) for n in names], F)
+    assert got.size == len(names)
+    assert np.array_equal(got.view(np.uint32), want.view(np.uint32))
+    # the scale is taken over the whole concatenated input [h, m_out, m_in], whose message part dominates h here, and
+    # over inputs, not outputs: neither max|h| alone nor max|output| reproduces it
+    i = names.index("node0_0")
+    h_only = {}
+    gnn_restated(cfg, W, f, src, dst, points=(), on_linear_input=lambda n, x: h_only.setdefault(n, float(np.abs(x[:, :cfg.gnn_latent]).max())))
+    assert F(h_only["node0_0"]) / F(127) != got[i]
+    # a layer the calibration batch never excites keeps scale 1 (zero input -> s_x = 1)
+    Z = zero_layers(cfg)
+    z = oracle.calibrate_int8(datagen.pack_blob(cfg, Z), b.xyz, b.plane, b.event_offsets, cfg.k, cfg.window)
+    assert z[names.index("emb1")] == 1.0
