@@ -17,7 +17,9 @@
  * Readings of every point where the paper is silent are in DESIGN.md sec. 4
  * (R1..R26).  All pointers are plain pointers; "d_" = device memory on the
  * current CUDA device, "h_" = host memory.  No C++ or torch types cross this
- * boundary.  Every function returns an etx_status; nothing throws or aborts.
+ * boundary.  Every function returns an etx_status; nothing throws across the boundary.  One device-side guard
+ * exists: a kernel that waits more than ~20 s of wall-clock time on one mbarrier (a lost arrival, i.e. a bug)
+ * executes a trap instead of hanging the GPU, which surfaces as ETX_ERR_CUDA on the next call.
  * ==========================================================================*/
 #ifndef ETX_H_
 #define ETX_H_
@@ -37,7 +39,8 @@ typedef enum {
   ETX_ERR_ARG = -1,          /* null pointer, negative size, inconsistent offsets            */
   ETX_ERR_BLOB = -2,         /* weights blob: bad magic / version / shapes / size / scales   */
   ETX_ERR_CAPACITY = -3,     /* n_events > max_events or n_hits > max_hits                   */
-  ETX_ERR_INPUT_ORDER = -4,  /* device-side validation found hits not sorted by (event,plane)*/
+  ETX_ERR_INPUT_ORDER = -4,  /* device-side validation found hits not sorted by (event,plane),
+                                or a plane index outside [0, n_planes): see etx_input_status  */
   ETX_ERR_CUDA = -5,         /* a CUDA runtime call failed; see etx_last_error               */
   ETX_ERR_UNSUPPORTED = -6   /* shape / precision not built into this library                */
 } etx_status;
@@ -109,12 +112,21 @@ typedef struct {                     /* device pointers into the handle's worksp
 etx_status etx_create(const void* h_weights_blob, size_t blob_bytes, const etx_hyperparams* hp,
                       etx_handle* out);
 
-/* Enqueue the whole path S0..S5 for one packed batch on `stream` and return without synchronising.
+/* Enqueue the whole path S0..S5 for one packed batch on `stream` and return without synchronising the stream or
+ * the device.  (The one host-side wait: the event offsets travel through a pinned staging buffer of the handle, and
+ * the call blocks until the previous call's copy out of that buffer has been issued to the device -- microseconds.)
+ * The CUDA device that was current at etx_create must be current (ETX_ERR_ARG otherwise).
  *   d_xyz             [n_hits][3] fp32, millimetres, device; borrowed until the enqueued work is done
  *   d_plane           [n_hits] int32 in [0, n_planes), device; hits sorted by (event, plane)
  *   h_event_offsets   [n_events+1] int32, host; [0] = 0, non-decreasing, [n_events] = n_hits
  * Empty events / planes are legal; n_events = 0 is a no-op that reports 0 edges.
- * One handle serves one stream at a time; calls on one handle are not thread-safe. */
+ * One handle serves one stream at a time; calls on one handle are not thread-safe.
+ * Input validation (hyperparams.validate_input = 1) runs on the device as part of S0.  A batch that breaks the
+ * input contract is REJECTED on the device: its row offsets and edge count are forced to 0, so no later stage
+ * touches memory on its behalf, n_edges = 0 and track_id[h] = h.  etx_run itself still returns ETX_OK (it cannot
+ * know without synchronising); the verdict of the batch is read with etx_input_status after the stream has been
+ * synchronised.  A rejected batch never affects the calls that follow it.  Without validate_input an out-of-contract
+ * batch is the caller's responsibility (results undefined, memory accesses still bounded by the workspace). */
 etx_status etx_run(etx_handle h, const float* d_xyz, const int32_t* d_plane,
                    const int32_t* h_event_offsets, int32_t n_events, etx_stream stream,
                    etx_output* out);
@@ -125,10 +137,16 @@ etx_status etx_run(etx_handle h, const float* d_xyz, const int32_t* d_plane,
  * Pinned host memory makes the copies asynchronous (src / dst are copied under the GNN, and the scores
  * are written by the classifier straight into a pinned h_edge_score, which is device-addressable);
  * pageable memory works too.  *n_edges_out = E. */
+/* Returns ETX_ERR_INPUT_ORDER when validate_input is set and the batch was rejected (it synchronises anyway). */
 etx_status etx_run_host(etx_handle h, const float* h_xyz, const int32_t* h_plane,
                         const int32_t* h_event_offsets, int32_t n_events, etx_stream stream,
                         float* h_edge_score, int32_t* h_edge_src, int32_t* h_edge_dst,
                         int32_t* h_track_id, int32_t* n_edges_out);
+
+/* Verdict of the device-side input validation for the last etx_run / etx_dbg_run on this handle whose stream work
+ * has completed (the caller synchronises the stream first): ETX_OK, or ETX_ERR_INPUT_ORDER if that batch was
+ * rejected.  Always ETX_OK when validate_input = 0. */
+etx_status etx_input_status(etx_handle h);
 
 /* Track containers (L42: a particle is reconstructible with at least three VELO hits; L74, L82: the product of
  * the pipeline is the set of tracks, each a list of hits).  Enqueue on `stream`, after an etx_run on the same

@@ -87,6 +87,8 @@ def load_library():
     L.etx_run_host.argtypes = [vp, vp, vp, i32p, C.c_int32, vp, vp, vp, vp, vp, i32p]
     L.etx_destroy.restype = C.c_int
     L.etx_destroy.argtypes = [vp]
+    L.etx_input_status.restype = C.c_int
+    L.etx_input_status.argtypes = [vp]
     L.etx_tracks.restype = C.c_int
     L.etx_tracks.argtypes = [vp, C.c_int32, vp, C.POINTER(EtxTracks)]
     L.etx_workspace_bytes.restype = C.c_size_t
@@ -200,6 +202,10 @@ class Etx:
                              self._stream(), C.byref(out))
         self._check(st, "etx_run")
         return out
+
+    def input_status(self) -> int:
+        """etx_input_status: verdict of the device-side input validation of the last completed run (0 = ETX_OK)."""
+        return int(self._L.etx_input_status(self._h))
 
     def run_host(self, h_xyz, h_plane, event_offsets, h_score, h_src, h_dst, h_track_id) -> int:
         """etx_run_host: host (ideally pinned) tensors in and out; synchronises; returns E."""

@@ -159,7 +159,11 @@ etx_status run_impl(etx_ctx* c, const float* d_xyz, const int32_t* d_plane, cons
   const int n_hits = h_eo[n_events];
   if (n_hits > c->hp.max_hits) return fail(c, ETX_ERR_CAPACITY, "n_hits exceeds max_hits");
   if (n_hits > 0 && (!d_xyz || !d_plane)) return fail(c, ETX_ERR_ARG, "null hit arrays");
-  if (c->h_flags[0] & 1) { c->h_flags[0] = 0; return fail(c, ETX_ERR_INPUT_ORDER, "previous batch: hits not sorted by (event, plane) or plane out of range"); }
+  {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != c->device)
+      return fail(c, ETX_ERR_ARG, "the current CUDA device is not the one the handle was created on");
+  }
   const int last = inj ? (inj->last_stage > 0 ? inj->last_stage : 5) : 5;
   if (inj && ((inj->d_src == nullptr) != (inj->d_dst == nullptr))) return fail(c, ETX_ERR_ARG, "inject: src and dst go together");
   if (inj && inj->d_logit && !inj->d_src) return fail(c, ETX_ERR_ARG, "inject: logits need the edge list they belong to");
@@ -232,10 +236,8 @@ etx_status run_impl(etx_ctx* c, const float* d_xyz, const int32_t* d_plane, cons
             else if (kind == kEdgeEnc && c->edge_tma && c->hp.edge_enc_input == 1) launch_edge_enc_h_tma(c, n_hits, head, s);
             else if (kind == kNodeEnc && c->edge_tma) launch_edge_enc_tma(c, n_hits, true, s);
             else if (tensor_engine && c->precision == ETX_BF16 && c->engine != ETX_ENGINE_TC_SERIAL) launch_gnn_mlp_ws(c, kind, it, n_hits, head, s);
-            else if (kind == kEdgeNet && c->edge_i8 && c->tap_layer < 0)
-              launch_edge_net_i8(c, it, n_hits, head, s);
-            else if (kind == kNodeNet && c->edge_i8 && c->tap_layer < 0)
-              launch_node_net_i8(c, it, n_hits, s);
+            else if (kind == kEdgeNet && c->edge_i8) launch_edge_net_i8(c, it, n_hits, head, s);
+            else if (kind == kNodeNet && c->edge_i8) launch_node_net_i8(c, it, n_hits, s);
             else if (tensor_engine) launch_gnn_mlp_umma(c, kind, it, n_hits, head, s);
             else launch_gnn_mlp_simt(c, kind, it, n_hits, head, s);
           };
@@ -260,7 +262,7 @@ etx_status run_impl(etx_ctx* c, const float* d_xyz, const int32_t* d_plane, cons
       ETX_CUDA(cudaMemcpyAsync(c->h_n_edges, c->n_edges, sizeof(int32_t), cudaMemcpyDeviceToHost, s));
       ETX_CUDA(cudaEventRecord(c->edges_ready, s));
     }
-    if (c->hp.validate_input) {
+    if (c->hp.validate_input) {     // the verdict of THIS batch: readable through etx_input_status once the stream is synchronised
       ETX_CUDA(cudaMemcpyAsync(c->h_flags, c->flags, sizeof(int32_t), cudaMemcpyDeviceToHost, s));
       ETX_CUDA(cudaMemsetAsync(c->flags, 0, sizeof(int32_t), s));
     }
@@ -325,11 +327,18 @@ etx_status etx_create(const void* blob, size_t blob_bytes, const etx_hyperparams
   if (hp->threshold <= 0.0f) c->tau = -INFINITY;
   else if (hp->threshold >= 1.0f) c->tau = INFINITY;
   else c->tau = (float)log((double)hp->threshold / (1.0 - (double)hp->threshold));      // R17
-  etx_status st = parse_blob(c, static_cast<const uint8_t*>(blob), blob_bytes);
+  etx_status st = ETX_OK;
+  try {
+    st = parse_blob(c, static_cast<const uint8_t*>(blob), blob_bytes);
+  } catch (const std::bad_alloc&) {
+    c->error = "out of host memory while parsing the blob";
+    return bail(ETX_ERR_BLOB);
+  }
   if (st != ETX_OK) return bail(st);
   try {
     int dev = 0;
     ETX_CUDA(cudaGetDevice(&dev));
+    c->device = dev;
     ETX_CUDA(cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev));
     for (auto& l : c->layers) convert_layer(c, l);
     const size_t N = (size_t)hp->max_hits, E = (size_t)c->max_edges, B = (size_t)hp->max_events, d = hp->gnn_latent;
@@ -395,6 +404,8 @@ etx_status etx_create(const void* blob, size_t blob_bytes, const etx_hyperparams
   } catch (const CudaFail& f) {
     (void)f;
     return bail(ETX_ERR_CUDA);
+  } catch (const std::bad_alloc&) {
+    return bail(ETX_ERR_CUDA);
   }
   *out = c;
   return ETX_OK;
@@ -404,7 +415,6 @@ etx_status etx_destroy(etx_handle c) {
   if (!c) return ETX_OK;
   cudaDeviceSynchronize();
   for (void* p : c->allocs) { if (c->hp.alloc) { if (c->hp.dealloc) c->hp.dealloc(p, c->hp.alloc_ctx); } else cudaFree(p); }
-  if (c->tap) cudaFree(c->tap);
   if (c->h_event_off) cudaFreeHost(c->h_event_off);
   if (c->h_n_edges) cudaFreeHost(c->h_n_edges);
   if (c->h_n_tracks) cudaFreeHost(c->h_n_tracks);
@@ -490,6 +500,13 @@ etx_status etx_run_host(etx_handle c, const float* h_xyz, const int32_t* h_plane
   } catch (const CudaFail& f) {
     return fail(c, ETX_ERR_CUDA, std::string(f.what) + ": " + cudaGetErrorString(f.err));
   }
+  return etx_input_status(c);          // the stream is synchronised: the verdict of this very batch
+}
+
+etx_status etx_input_status(etx_handle c) {
+  if (!c) return ETX_ERR_ARG;
+  if (c->hp.validate_input && (c->h_flags[0] & 1))
+    return fail(c, ETX_ERR_INPUT_ORDER, "hits not sorted by (event, plane), or a plane index out of range: the batch was rejected (0 edges)");
   return ETX_OK;
 }
 
@@ -514,7 +531,7 @@ etx_status etx_dbg_buffer(etx_handle c, const char* name, const void** d_ptr, si
   if (!c || !name || !d_ptr || !bytes) return ETX_ERR_ARG;
   const size_t N = (size_t)c->last_n_hits, E = (size_t)c->h_n_edges[0], d = c->hp.gnn_latent, sb = c->state_bf16 ? 2 : 4;
   const std::string n(name);
-  if (n == "plane_off") { *d_ptr = c->plane_off; *bytes = 0; return ETX_OK; }
+  if (n == "plane_off") { *d_ptr = c->plane_off; *bytes = (size_t)c->last_n_events * (c->hp.n_planes + 1) * 4; return ETX_OK; }
   if (n == "emb") { *d_ptr = c->emb; *bytes = N * 16; return ETX_OK; }
   if (n == "feat") { *d_ptr = c->feat; *bytes = N * 16; return ETX_OK; }
   if (n == "feat_emb") { *d_ptr = c->feat_emb; *bytes = N * 16; return ETX_OK; }
@@ -541,7 +558,8 @@ etx_status etx_dbg_tap_layer(etx_handle c, int32_t layer_index) {
     const size_t width = (size_t)(c->hp.emb_hidden > c->hp.gnn_latent ? c->hp.emb_hidden : c->hp.gnn_latent);
     const size_t bytes = rows * width * 4;
     if (bytes > (size_t)4 << 30) return fail(c, ETX_ERR_CAPACITY, "tap buffer would exceed 4 GiB; use a smaller max_hits");
-    if (cudaMalloc(&c->tap, bytes ? bytes : 4) != cudaSuccess) return fail(c, ETX_ERR_CUDA, "cudaMalloc(tap)");
+    c->tap = static_cast<int32_t*>(etx::etx_device_alloc(c, bytes ? bytes : 4));   // through the handle's allocator, freed by etx_destroy
+    if (!c->tap) return fail(c, ETX_ERR_CUDA, "tap buffer allocation failed");
     c->tap_bytes = bytes;
   }
   c->tap_layer = layer_index;

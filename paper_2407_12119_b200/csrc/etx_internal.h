@@ -7,6 +7,7 @@
 #include <stdint.h>
 
 #include <string>
+#include <utility>
 #include <vector>
 
 #include "../../include/etx.h"
@@ -76,6 +77,8 @@ struct etx_ctx {
   bool state_bf16 = false;
   int max_edges = 0;
   int sm_count = 148;
+  int device = 0;                         // the CUDA device the handle was created on (tensor maps, sm_count, opt-ins)
+  std::vector<std::pair<const void*, int>> smem_opted;   // kernels whose dynamic shared-memory limit was raised for this handle
   std::string error;
   std::vector<etx::HostLayer> layers;     // blob order
   int i_emb0 = 0, i_nenc = 0, i_eenc = 0, i_iter0 = 0, i_head = 0;
@@ -139,6 +142,22 @@ struct etx_ctx {
 };
 
 namespace etx {
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a per-DEVICE setting, so the opt-in is remembered per handle (a handle
+// lives on one device), not per process; a larger request for the same kernel raises the limit again.
+template <typename K>
+inline void opt_in_smem(etx_ctx* c, K kern, int bytes) {
+  const void* f = reinterpret_cast<const void*>(kern);
+  for (auto& e : c->smem_opted)
+    if (e.first == f) {
+      if (e.second >= bytes) return;
+      cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+      e.second = bytes;
+      return;
+    }
+  cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  c->smem_opted.push_back({f, bytes});
+}
 
 // ---- launchers (each file owns its kernels) -------------------------------------------------------------
 // etx_api.cu: device memory through the handle's allocator (hp.alloc or cudaMalloc); nullptr on failure

@@ -244,11 +244,14 @@ __global__ void __launch_bounds__(kI8Threads, 1) edge_net_i8_kernel(const __grid
       // ---- epilogue 0: relu(fmaf(acc0, s_x s_w, b0)) -> int8 codes -> layer-1 operand (R21)
       mbar_wait(&acc0_full[g], j & 1);
       tc_fence_after();
+      // etx_dbg_tap_layer: the int32 accumulators of this very kernel, as the tests compare them with the oracle's
+      int32_t* tap0 = (a.tap && a.tap_layer == a.l0.index && live) ? a.tap + (size_t)row * D : nullptr;
+      int32_t* tap1 = (a.tap && a.tap_layer == a.l1.index && live) ? a.tap + (size_t)row * D : nullptr;
 #pragma unroll
       for (int c0 = 0; c0 < D; c0 += 32) {
         uint32_t v[32];
         tmem_ld32(tmem + lane_base + g * D + c0, v);
-        store_hidden32<kInt8, KB>(v, c0, scale0, bias0, inv_sx1, Hg, r, nullptr);
+        store_hidden32<kInt8, KB>(v, c0, scale0, bias0, inv_sx1, Hg, r, tap0);
       }
       tc_fence_before();
       fence_proxy_async();
@@ -261,6 +264,10 @@ __global__ void __launch_bounds__(kI8Threads, 1) edge_net_i8_kernel(const __grid
       for (int c0 = 0; c0 < D; c0 += 32) {
         uint32_t v[32];
         tmem_ld32(tmem + lane_base + 2 * D + g * D + c0, v);
+        if (tap1) {
+#pragma unroll
+          for (int jj = 0; jj < 32; ++jj) tap1[c0 + jj] = (int)v[jj];
+        }
 #pragma unroll
         for (int ch = 0; ch < 8; ++ch) {
           const int c = c0 + ch * 4;
@@ -301,8 +308,7 @@ template <int D, bool NODE>
 void edge_i8_launch(etx_ctx* c, const GnnArgs& a, int max_rows, cudaStream_t s) {
   auto kern = edge_net_i8_kernel<D, NODE>;
   constexpr int smem = i8_layout<D>().total + 1024;
-  static bool configured = false;
-  if (!configured) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); configured = true; }
+  opt_in_smem(c, kern, smem);
   const int tiles = (max_rows + kRows - 1) / kRows;
   const int grid = tiles < c->sm_count ? tiles : c->sm_count;     // one persistent CTA per SM
   if (grid <= 0) return;
@@ -337,7 +343,7 @@ bool edge_i8_configure(etx_ctx* c) {
   return true;
 }
 
-// INT8 mode, fp32 state, no accumulator tap requested (the tap stays with gnn_mlp_umma_kernel)
+// INT8 mode (AUTO engine): S4e; the accumulator tap of etx_dbg_tap_layer is served by this kernel itself
 void launch_edge_net_i8(etx_ctx* c, int iter, int n_hits, bool do_head, cudaStream_t s) {
   GnnArgs a;
   fill_gnn_args(c, kEdgeNet, iter, n_hits, do_head, a);

@@ -315,7 +315,7 @@ edge_net_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeTmaArgs
         for (uint32_t spins = 0;; ++spins) {
           if (pending >= 0 && mbar_test(&hid_full[pending & 1], (pending >> 1) & 1)) { layer1(pending); pending = -1; }
           if (mbar_test(&aux_full[sh], (it / kNH) & 1) && mbar_test(&self_full[se], (it / kNE) & 1)) break;
-          if (spins > (1u << 24)) __trap();
+          if ((spins & 0xfffffu) == 0xfffffu && mbar_stalled(spins)) __trap();
         }
         PROF(3)
         tc_fence_after();
@@ -676,8 +676,7 @@ template <int D>
 void edge_tma_launch(etx_ctx* c, const EdgeTmaArgs& a, int max_rows, cudaStream_t s) {
   auto kern = edge_net_tma_kernel<D>;
   constexpr int smem = et_layout<D>().total + 1024;
-  static bool configured = false;
-  if (!configured) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); configured = true; }
+  opt_in_smem(c, kern, smem);
   const int tiles = (max_rows + kRows - 1) / kRows;
   const int grid = tiles < c->sm_count ? tiles : c->sm_count;     // one persistent CTA per SM
   if (grid <= 0) return;
@@ -691,8 +690,7 @@ template <int D>
 void edge_enc_launch(etx_ctx* c, const EdgeEncArgs& a, const unsigned char* out_map, int max_rows, cudaStream_t s) {
   auto kern = edge_enc_tma_kernel<D>;
   constexpr int smem = enc_layout<D>().total + 1024;
-  static bool configured = false;
-  if (!configured) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); configured = true; }
+  opt_in_smem(c, kern, smem);
   const int tiles = (max_rows + kRows - 1) / kRows;
   const int grid = tiles < c->sm_count ? tiles : c->sm_count;     // one persistent CTA per SM (512 TMEM columns)
   if (grid <= 0) return;

@@ -114,7 +114,7 @@ __global__ void __launch_bounds__(kEmbThreads, 1) embed_ws_kernel(const EmbWsArg
             ++done[g]; --left; spins = 0;
           }
         }
-        if (spins > (1u << 26)) __trap();                    // never hang the GPU: a lost arrival becomes an error
+        if ((spins & 0xfffffu) == 0xfffffu && mbar_stalled(spins)) __trap();                 // never hang the GPU: a lost arrival becomes an error
       }
     }
   } else {
@@ -195,8 +195,7 @@ bool emb_ws_launch(etx_ctx* c, const EmbWsArgs& a, cudaStream_t s) {
   auto kern = embed_ws_kernel<D>;
   const int smem = emb_ws_smem<D>(a.n_mid) + 1024;
   if (smem > 227 * 1024) return false;
-  static int configured = 0;
-  if (configured < smem) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); configured = smem; }
+  opt_in_smem(c, kern, smem);
   const int tiles = (a.n_rows + kRows - 1) / kRows;
   const int grid = tiles < c->sm_count ? tiles : c->sm_count;     // one persistent CTA per SM
   if (grid <= 0) return true;

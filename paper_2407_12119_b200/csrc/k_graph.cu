@@ -35,9 +35,11 @@ __device__ __forceinline__ float atan2_r27(float y, float x) {
 
 template <bool CYL>
 __global__ void features_kernel(const float* __restrict__ xyz, float4* __restrict__ feat, float4* __restrict__ feat_emb,
-                                int n, FeatArgs a) {
+                                int32_t* __restrict__ deg, int n, FeatArgs a) {
   int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
+  deg[i] = 0;        // S2 writes the out-degree of every hit of every (event, plane) bucket; a hit of a rejected batch
+                     // (planes out of order / out of range) may belong to none and must not keep a stale value
   float x = xyz[3 * (size_t)i], y = xyz[3 * (size_t)i + 1], z = xyz[3 * (size_t)i + 2];
   feat[i] = make_float4(__fdiv_rn(__fadd_rn(x, a.o[0]), a.d[0]), __fdiv_rn(__fadd_rn(y, a.o[1]), a.d[1]),
                         __fdiv_rn(__fadd_rn(z, a.o[2]), a.d[2]), 0.0f);
@@ -56,8 +58,8 @@ void launch_features(etx_ctx* c, const float* xyz, int n_hits, cudaStream_t s) {
   for (int i = 0; i < 3; ++i) {
     a.o[i] = hp.norm_offset[i]; a.d[i] = hp.norm_div[i]; a.co[i] = hp.cyl_offset[i]; a.cd[i] = hp.cyl_div[i];
   }
-  if (hp.emb_input) features_kernel<true><<<(n_hits + 255) / 256, 256, 0, s>>>(xyz, c->feat, c->feat_emb, n_hits, a);
-  else features_kernel<false><<<(n_hits + 255) / 256, 256, 0, s>>>(xyz, c->feat, c->feat_emb, n_hits, a);
+  if (hp.emb_input) features_kernel<true><<<(n_hits + 255) / 256, 256, 0, s>>>(xyz, c->feat, c->feat_emb, c->deg, n_hits, a);
+  else features_kernel<false><<<(n_hits + 255) / 256, 256, 0, s>>>(xyz, c->feat, c->feat_emb, c->deg, n_hits, a);
   c->launches++;
 }
 
@@ -322,8 +324,7 @@ void launch_knn(etx_ctx* c, const int32_t* plane, int n_events, int n_hits, cuda
   const int32_t* only = nullptr;
   if (isfinite(hp.d2_max)) {
     constexpr int smem = kKnnCutTile * (int)sizeof(float4) + kKnnBuf * kKnnCutThreads * 8;
-    static bool configured = false;
-    if (!configured) { cudaFuncSetAttribute(knn_cut_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); configured = true; }
+    opt_in_smem(c, knn_cut_kernel, smem);
     knn_cut_kernel<<<nb, kKnnCutThreads, smem, s>>>(c->emb, c->plane_off, hp.n_planes, k, hp.window, hp.d2_max, c->nbr, c->deg, c->knn_redo);
     c->launches++;
     only = c->knn_redo;
@@ -386,8 +387,11 @@ __global__ void __launch_bounds__(kScanThreads) scan_bsum_kernel(int32_t* __rest
 
 __global__ void __launch_bounds__(kScanThreads) scan_write_kernel(const int32_t* __restrict__ in, int n,
                                                                  const int32_t* __restrict__ bsum,
-                                                                 int32_t* __restrict__ out, int32_t* __restrict__ total) {
+                                                                 int32_t* __restrict__ out, int32_t* __restrict__ total,
+                                                                 const int32_t* __restrict__ reject) {
   const int base = blockIdx.x * kScanChunk;
+  // validate_input found the batch out of contract: every prefix sum is 0, so E = 0 and no E-sized kernel runs
+  const bool rejected = reject != nullptr && reject[0] != 0;
   int vals[kScanItems], v = 0;
 #pragma unroll
   for (int j = 0; j < kScanItems; ++j) {
@@ -400,29 +404,30 @@ __global__ void __launch_bounds__(kScanThreads) scan_write_kernel(const int32_t*
 #pragma unroll
   for (int j = 0; j < kScanItems; ++j) {
     int i = base + threadIdx.x * kScanItems + j;
-    if (i < n) out[i] = ex;
+    if (i < n) out[i] = rejected ? 0 : ex;
     ex += vals[j];
-    if (i == n - 1) { out[n] = ex; if (total) *total = ex; }
+    if (i == n - 1) { out[n] = rejected ? 0 : ex; if (total) *total = rejected ? 0 : ex; }
   }
 }
 
 __global__ void scan_empty_kernel(int32_t* out, int32_t* total) { out[0] = 0; if (total) *total = 0; }
 
 // out[0..n] = exclusive prefix sums of in[0..n); *total = out[n]
-static void exclusive_scan(etx_ctx* c, const int32_t* in, int n, int32_t* out, int32_t* total, cudaStream_t s) {
+static void exclusive_scan(etx_ctx* c, const int32_t* in, int n, int32_t* out, int32_t* total, cudaStream_t s,
+                           const int32_t* reject = nullptr) {
   if (n == 0) { scan_empty_kernel<<<1, 1, 0, s>>>(out, total); c->launches++; return; }
   const int nb = (n + kScanChunk - 1) / kScanChunk;
   scan_reduce_kernel<<<nb, kScanThreads, 0, s>>>(in, n, c->scan_tmp);
   scan_bsum_kernel<<<1, kScanThreads, 0, s>>>(c->scan_tmp, nb);
-  scan_write_kernel<<<nb, kScanThreads, 0, s>>>(in, n, c->scan_tmp, out, total);
+  scan_write_kernel<<<nb, kScanThreads, 0, s>>>(in, n, c->scan_tmp, out, total, reject);
   c->launches += 3;
 }
 
 __global__ void pack_edges_kernel(const int32_t* __restrict__ nbr, const int32_t* __restrict__ deg,
                                   const int32_t* __restrict__ row_ptr, int n_hits, int k,
-                                  int32_t* __restrict__ src, int32_t* __restrict__ dst) {
+                                  int32_t* __restrict__ src, int32_t* __restrict__ dst, const int32_t* __restrict__ reject) {
   size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= (size_t)n_hits * k) return;
+  if (i >= (size_t)n_hits * k || reject[0] != 0) return;
   int q = (int)(i / k), sidx = (int)(i % k);
   if (sidx < deg[q]) {
     int pos = row_ptr[q] + sidx;
@@ -435,10 +440,10 @@ __global__ void pack_edges_kernel(const int32_t* __restrict__ nbr, const int32_t
 // its deg[q] filled slots instead of one thread per slot.
 __global__ void pack_edges_sparse_kernel(const int32_t* __restrict__ nbr, const int32_t* __restrict__ deg,
                                          const int32_t* __restrict__ row_ptr, int n_hits, int k,
-                                         int32_t* __restrict__ src, int32_t* __restrict__ dst) {
+                                         int32_t* __restrict__ src, int32_t* __restrict__ dst, const int32_t* __restrict__ reject) {
   const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   const int q = (int)(t >> 4), l = (int)(t & 15);
-  if (q >= n_hits) return;
+  if (q >= n_hits || reject[0] != 0) return;
   const int n = deg[q], base = row_ptr[q];
   for (int sidx = l; sidx < n; sidx += 16) {
     src[base + sidx] = q;
@@ -447,14 +452,14 @@ __global__ void pack_edges_sparse_kernel(const int32_t* __restrict__ nbr, const 
 }
 
 void launch_pack_edges(etx_ctx* c, int n_hits, cudaStream_t s) {
-  exclusive_scan(c, c->deg, n_hits, c->row_ptr, c->n_edges, s);
+  exclusive_scan(c, c->deg, n_hits, c->row_ptr, c->n_edges, s, c->flags);
   if (n_hits == 0) return;
   if (c->hp.k > 16) {
     const size_t n = (size_t)n_hits * 16;
-    pack_edges_sparse_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(c->nbr, c->deg, c->row_ptr, n_hits, c->hp.k, c->src, c->dst);
+    pack_edges_sparse_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(c->nbr, c->deg, c->row_ptr, n_hits, c->hp.k, c->src, c->dst, c->flags);
   } else {
     const size_t n = (size_t)n_hits * c->hp.k;
-    pack_edges_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(c->nbr, c->deg, c->row_ptr, n_hits, c->hp.k, c->src, c->dst);
+    pack_edges_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(c->nbr, c->deg, c->row_ptr, n_hits, c->hp.k, c->src, c->dst, c->flags);
   }
   c->launches++;
 }
@@ -504,7 +509,8 @@ __global__ void csc_sort_kernel(const int32_t* __restrict__ col_ptr, int n_hits,
 // so two lanes of a step can only meet on a dst if they belong to different src hits: the step is split into
 // phases, one per src it spans (at most a handful), and in a phase every lane of that src advances its dst's
 // cursor with a plain read-modify-write.  Phases and steps are sequential, so every dst group comes out in
-// ascending edge id (R9 / R22) by construction.  (match.any would rank the lanes of a step in one go, but costs
+// ascending edge id (R9 / R22) by construction.  A __syncwarp() separates them (shuffles and
+// reductions are no memory barrier).  (match.any would rank the lanes of a step in one go, but costs
 // ~1,400 cycles a step on this part.)  The cursors of a bucket are touched by this warp only (in shared memory, or
 // in the global scratch `cursor` for a bucket of more than kCscHits hits; initialised from col_ptr), so there is no
 // capacity limit and no atomic.
@@ -547,7 +553,8 @@ csc_bucket_kernel(const int32_t* __restrict__ src, const int32_t* __restrict__ d
       unsigned s_now = (unsigned)__shfl_sync(0xffffffffu, sq[u], 0);
       while (s_now < 0x7fffffffu) {                                  // one phase per src hit the step spans
         if (mine && (unsigned)sq[u] == s_now) { const int pos = cur[d]; cur[d] = pos + 1; in_edge[pos] = i; }
-        s_now = __reduce_min_sync(0xffffffffu, (unsigned)sq[u] > s_now ? (unsigned)sq[u] : 0x7fffffffu);   // also orders the phases
+        __syncwarp();                                                // the next phase (or step) reads these cursors
+        s_now = __reduce_min_sync(0xffffffffu, (unsigned)sq[u] > s_now ? (unsigned)sq[u] : 0x7fffffffu);
       }
     }
   }
@@ -660,9 +667,8 @@ uf_event_kernel(const int32_t* __restrict__ src, const int32_t* __restrict__ dst
 
 void launch_components(etx_ctx* c, const float* logit, int n_events, int n_hits, cudaStream_t s) {
   if (n_hits == 0 || n_events == 0) return;
-  static bool configured = false;
   constexpr int smem = kUfSmemHits * (int)sizeof(int32_t);
-  if (!configured) { cudaFuncSetAttribute(uf_event_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); configured = true; }
+  opt_in_smem(c, uf_event_kernel, smem);
   const int grid = n_events;                          // one CTA per event; the hardware balances them
   uf_event_kernel<<<grid, kUfThreads, smem, s>>>(c->src, c->dst, logit, c->row_ptr, c->event_off, n_events, c->tau, c->track_id);
   c->launches += 1;

@@ -357,8 +357,7 @@ template <int D> static size_t emb_smem() { return sizeof(float) * kTileRows * (
 template <int KIND, int MODE, typename ST, int D>
 static void gnn_launch_one(etx_ctx* c, const GnnArgs& a, int max_rows, cudaStream_t s) {
   auto kern = gnn_mlp_simt_kernel<KIND, MODE, ST, D>;
-  static bool configured = false;
-  if (!configured) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gnn_smem<D>()); configured = true; }
+  opt_in_smem(c, kern, (int)gnn_smem<D>());
   const int tiles = (max_rows + kTileRows - 1) / kTileRows;
   const int grid = tiles < c->sm_count * 3 ? tiles : c->sm_count * 3;
   if (grid <= 0) return;
@@ -415,8 +414,7 @@ void launch_gnn_mlp_simt(etx_ctx* c, int kind, int iter, int n_hits, bool do_hea
 template <int MODE, int D>
 static void emb_launch(etx_ctx* c, const EmbArgs& a, cudaStream_t s) {
   auto kern = embed_simt_kernel<MODE, D>;
-  static bool configured = false;
-  if (!configured) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)emb_smem<D>()); configured = true; }
+  opt_in_smem(c, kern, (int)emb_smem<D>());
   const int tiles = (a.n_rows + kTileRows - 1) / kTileRows;
   const int grid = tiles < c->sm_count * 3 ? tiles : c->sm_count * 3;
   if (grid <= 0) return;

@@ -446,8 +446,7 @@ template <int KIND, int PREC, int D>
 void gnn_umma_launch_one(etx_ctx* c, const GnnArgs& a, int max_rows, cudaStream_t s) {
   auto kern = gnn_mlp_umma_kernel<KIND, PREC, D>;
   constexpr int smem = gnn_smem_layout<PREC, D>().total + 1024;
-  static bool configured = false;
-  if (!configured) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); configured = true; }
+  opt_in_smem(c, kern, smem);
   const int tiles = (max_rows + kRows - 1) / kRows;
   int per_sm = (227 * 1024) / (smem + 1024);
   const int tmem_cols = 2 * D < 32 ? 32 : 2 * D;
@@ -473,7 +472,7 @@ template <int PREC, int D>
 void emb_umma_launch(etx_ctx* c, const EmbArgs& a, cudaStream_t s) {
   auto kern = embed_umma_kernel<PREC, D>;
   const int smem = emb_smem_layout<PREC, D>(a.n_layers - 2).total + 1024;
-  cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+  opt_in_smem(c, kern, smem);
   const int tiles = (a.n_rows + kRows - 1) / kRows;
   int per_sm = (227 * 1024) / (smem + 1024);
   if (per_sm > 2) per_sm = 2;                               // 256 TMEM columns per CTA

@@ -333,8 +333,7 @@ template <int KIND, bool L0T, int D>
 void ws_launch_one(etx_ctx* c, const GnnArgs& a, int max_rows, cudaStream_t s) {
   auto kern = gnn_mlp_ws_kernel<KIND, L0T, D>;
   constexpr int smem = ws_layout<D>().total + 1024;
-  static bool configured = false;
-  if (!configured) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); configured = true; }
+  opt_in_smem(c, kern, smem);
   const int tiles = (max_rows + kRows - 1) / kRows;
   const int grid = tiles < c->sm_count ? tiles : c->sm_count;     // one persistent CTA per SM
   if (grid <= 0) return;

@@ -20,6 +20,15 @@ __device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
 __device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
+// A wait is declared lost only by wall-clock time (about 20 s), never by a poll count: under a debugger, a sanitizer,
+// time-slicing or a throttled clock a healthy wait can take any number of polls.  Called every 2^20 polls.
+static __device__ __noinline__ bool mbar_stalled(uint32_t spins) {
+  unsigned long long now;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(now));
+  __shared__ unsigned long long first_seen;              // any waiter's first slow-path time stamp of this CTA
+  if (spins == 0xfffffu) { first_seen = now; return false; }
+  return now - first_seen > 20000000000ull;
+}
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
   const uint32_t addr = smem_u32(bar);
   uint32_t done = 0;
@@ -29,7 +38,7 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
         "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
         "selp.u32 %0, 1, 0, p;\n\t}"
         : "=r"(done) : "r"(addr), "r"(parity) : "memory");
-    if (!done && spins > (1u << 24)) __trap();       // never hang the GPU: a lost arrival becomes an error
+    if (!done && (spins & 0xfffffu) == 0xfffffu && mbar_stalled(spins)) __trap();   // never hang the GPU: a lost arrival becomes an error
   }
 }
 // one lane of the (converged) warp.  ptxas knows a region guarded by elect.sync runs single-threaded, so the

@@ -448,13 +448,27 @@ def test_error_codes_capacity_blob_order_unsupported():
     with pytest.raises(etx.EtxError) as ei:
         run_gpu(ctx, b, debug=False)
     assert ei.value.status == -3
-    # unsorted planes are detected on the device and reported by the next call
+    # unsorted planes are detected on the device; the batch is rejected THERE (no edges, every hit its own track),
+    # the verdict is read after synchronising, and the next (valid) batch runs normally
     ctx = make_ctx(cfg, blob, b, validate=True)
     bad = datagen.EventBatch(b.xyz, b.plane[::-1].copy(), b.event_offsets, b.particle)
-    run_gpu(ctx, bad, debug=False, ) if False else ctx.results(ctx.run(dev(bad.xyz), dev(bad.plane), bad.event_offsets))
+    r = ctx.results(ctx.run(dev(bad.xyz), dev(bad.plane), bad.event_offsets))
+    torch.cuda.synchronize()
+    assert ctx.input_status() == -4
+    assert r["n_edges"] == 0 and np.array_equal(r["track_id"].cpu().numpy(), np.arange(b.n_hits, dtype=np.int32))
+    oob = b.plane.copy(); oob[3] = 26                                      # a plane index out of range
+    ctx.results(ctx.run(dev(b.xyz), dev(oob), b.event_offsets))
+    torch.cuda.synchronize()
+    assert ctx.input_status() == -4
+    # etx_run_host synchronises and reports the same batch
+    cap = cfg.k * b.n_hits
+    hs = torch.empty(cap, dtype=torch.float32).pin_memory(); hi = torch.empty(cap, dtype=torch.int32).pin_memory()
+    hj = torch.empty(cap, dtype=torch.int32).pin_memory(); ht = torch.empty(b.n_hits, dtype=torch.int32).pin_memory()
     with pytest.raises(etx.EtxError) as ei:
-        ctx.run(dev(b.xyz), dev(b.plane), b.event_offsets)
+        ctx.run_host(torch.from_numpy(bad.xyz).pin_memory(), torch.from_numpy(bad.plane).pin_memory(), bad.event_offsets, hs, hi, hj, ht)
     assert ei.value.status == -4
+    E = ctx.run_host(torch.from_numpy(b.xyz).pin_memory(), torch.from_numpy(b.plane).pin_memory(), b.event_offsets, hs, hi, hj, ht)
+    assert E > 0 and ctx.input_status() == 0
     g = run_gpu(ctx, b, debug=False)                                       # the handle stays usable
     assert g["n_edges"] > 0
 
