@@ -45,6 +45,8 @@ class EtxConfig:
     edge_enc_input: int = 0     # 0: |f_dst - f_src| (configs), 1: [h0_src, h0_dst]
     emb_input: int = 0          # 0: the embedding reads the Cartesian features, 1: normalised (r, phi, z) (L96, R27)
     weights_seed: int = 7
+    triplets: int = 0           # 1: the blob also carries the two triplet classifiers (R28)
+    triplet_threshold: float = 0.5
 
     def replace(self, **kw) -> "EtxConfig":
         return dataclasses.replace(self, **kw)

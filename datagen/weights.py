@@ -9,11 +9,14 @@ Blob (little-endian):
     [0] magic 'ETXW' (0x57585445)  [1] version = 1
     [2] emb_hidden  [3] emb_n_hidden_layers  [4] emb_dim
     [5] gnn_latent  [6] gnn_iters            [7] edge_enc_input
-    [8] n_weight_floats  [9] n_act_scales    [10] emb_input   [11..15] zero
+    [8] n_weight_floats  [9] n_act_scales    [10] emb_input   [11] triplet classifiers present
+    [12..15] zero
   then fp32 tensors, each Linear as W[out][in] row-major followed by b[out], in
   this order: embedding layers 0..H; node encoder (2); edge encoder (2); for each
-  iteration: node net (2), edge net (2); head (1).  Concatenated inputs are
-  ordered [h, m_out, m_in] and [h_src, h_dst, e].
+  iteration: node net (2), edge net (2); head (1); with word 11 set, the
+  articulation classifier (2d -> d, d -> 1) and the elbow classifier (same
+  shapes).  Concatenated inputs are ordered [h, m_out, m_in], [h_src, h_dst, e]
+  and [e_first, e_second].
   then n_act_scales fp32 activation scales (INT8 only; one per quantised Linear,
   in layer order).
 """
@@ -45,13 +48,15 @@ def layer_shapes(cfg: EtxConfig) -> list[tuple[str, int, int]]:
         out += [(f"node{it}_0", d, 3 * d), (f"node{it}_1", d, d),
                 (f"edge{it}_0", d, 3 * d), (f"edge{it}_1", d, d)]
     out.append(("head", 1, d))
+    if getattr(cfg, "triplets", 0):           # articulation and elbow classifiers on [e_first, e_second] (L80, L160)
+        out += [("tart0", d, 2 * d), ("tart1", 1, d), ("telb0", d, 2 * d), ("telb1", 1, d)]
     return out
 
 
 def quantised_layer_names(cfg: EtxConfig) -> list[str]:
     """Linears that are quantised in INT8 mode: every Linear with in >= 16 except the
     d->1 head (reading R21), in blob order."""
-    return [n for (n, o, i) in layer_shapes(cfg) if i >= 16 and n != "head"]
+    return [n for (n, o, i) in layer_shapes(cfg) if i >= 16 and n not in ("head", "tart1", "telb1")]
 
 
 def n_act_scales(cfg: EtxConfig) -> int:
@@ -84,7 +89,7 @@ def make_weights(cfg: EtxConfig, preset: str = "he", seed: int | None = None
                 W[:, d:] *= np.float32(1.0 / (2.0 * cfg.k))
             if (name.startswith("node") or name.startswith("edge")) and name.endswith("_1"):
                 W *= np.float32(0.25)
-            if name == "head":
+            if name in ("head", "tart1", "telb1"):
                 W *= np.float32(2.0)
         elif preset != "he":
             raise ValueError(preset)
@@ -104,7 +109,8 @@ def pack_blob(cfg: EtxConfig, layers, act_scales: np.ndarray | None = None) -> b
     n_floats = len(body) // 4
     sc = np.zeros(0, "<f4") if act_scales is None else np.ascontiguousarray(act_scales, dtype="<f4")
     hdr = [BLOB_MAGIC, BLOB_VERSION, cfg.emb_hidden, cfg.emb_n_hidden_layers, cfg.emb_dim,
-           cfg.gnn_latent, cfg.gnn_iters, cfg.edge_enc_input, n_floats, int(sc.size), cfg.emb_input] + [0] * 5
+           cfg.gnn_latent, cfg.gnn_iters, cfg.edge_enc_input, n_floats, int(sc.size), cfg.emb_input,
+           int(getattr(cfg, "triplets", 0))] + [0] * 4
     return struct.pack("<16I", *hdr) + body + sc.tobytes()
 
 

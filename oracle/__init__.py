@@ -93,6 +93,18 @@ def lib():
         L.etxo_tracks.restype = C.c_int64
         L.etxo_tracks.argtypes = [C.POINTER(C.c_int32), C.c_int64, C.POINTER(C.c_int32), C.c_int64, C.c_int32,
                                   C.POINTER(C.c_int32), C.POINTER(C.c_int32), C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
+        u8p = C.POINTER(C.c_uint8)
+        L.etxo_triplets.restype = C.c_int64
+        L.etxo_triplets.argtypes = [C.POINTER(C.c_int32), C.POINTER(C.c_int32), u8p, C.c_int64, C.c_int64, C.c_int,
+                                    C.POINTER(C.c_int32), C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
+        L.etxo_triplet_scores.argtypes = [C.c_void_p, C.POINTER(C.c_float), C.POINTER(C.c_int32), C.POINTER(C.c_int32),
+                                          C.c_int64, C.c_int, C.POINTER(C.c_float), C.POINTER(C.c_float)]
+        L.etxo_has_triplets.restype = C.c_int
+        L.etxo_has_triplets.argtypes = [C.c_void_p]
+        L.etxo_tracks_from_triplets.restype = C.c_int64
+        L.etxo_tracks_from_triplets.argtypes = ([C.POINTER(C.c_int32), C.POINTER(C.c_int32), u8p, C.c_int64]
+                                                + [C.POINTER(C.c_int32), C.POINTER(C.c_int32), u8p, C.c_int64] * 3
+                                                + [C.c_int32, C.POINTER(C.c_int32), C.c_int64, C.POINTER(C.c_int32), C.c_int64])
         _lib = L
     return _lib
 
@@ -184,6 +196,51 @@ def tracks(track_id, event_offsets, min_hits=3):
                 event_track_offsets=ev)
 
 
+TRIPLET_KINDS = {"articulation": 0, "left_elbow": 1, "right_elbow": 2}
+
+
+def _u8(a):
+    return np.ascontiguousarray(a, dtype=np.uint8)
+
+
+def triplets(src, dst, keep, n, kind):
+    """Triplets of one kind on the purified hit graph (etxo_triplets).  -> (first [T], second [T], hit [T])."""
+    src, dst, keep = _i32(src), _i32(dst), _u8(keep)
+    k = TRIPLET_KINDS[kind] if isinstance(kind, str) else int(kind)
+    null = C.POINTER(C.c_int32)()
+    T = int(lib().etxo_triplets(_p(src, C.c_int32), _p(dst, C.c_int32), _p(keep, C.c_uint8), src.size, n, k, null, null, null))
+    a, b, h = (np.zeros(max(T, 1), np.int32) for _ in range(3))
+    lib().etxo_triplets(_p(src, C.c_int32), _p(dst, C.c_int32), _p(keep, C.c_uint8), src.size, n, k,
+                        _p(a, C.c_int32), _p(b, C.c_int32), _p(h, C.c_int32))
+    return a[:T].copy(), b[:T].copy(), h[:T].copy()
+
+
+def tracks_from_triplets(src, dst, keep, art, keep_art, left, keep_left, right, keep_right, min_hits=3):
+    """The four phases of PAPER.md sec. 5.4 (etxo_tracks_from_triplets).  art / left / right = (first, second) edge-id
+    arrays, keep_* their kept flags.  -> (track_offsets [T + 1], track_hits)."""
+    src, dst, keep = _i32(src), _i32(dst), _u8(keep)
+    E = src.size
+    args = []
+    n_shared_max = 0
+    for (f, s), kf in ((art, keep_art), (left, keep_left), (right, keep_right)):
+        f, s, kf = _i32(f), _i32(s), _u8(kf)
+        args += [f, s, kf]
+        n_shared_max = max(n_shared_max, f.size)
+    cap_tracks = E + int(np.asarray(art[0]).size) + 1
+    cap_hits = 2 * (E + 1) * 2 + 4 * int(np.asarray(art[0]).size) * 64 + 16
+    while True:
+        offs = np.zeros(cap_tracks + 1, np.int32); hits = np.zeros(cap_hits, np.int32)
+        T = int(lib().etxo_tracks_from_triplets(
+            _p(src, C.c_int32), _p(dst, C.c_int32), _p(keep, C.c_uint8), E,
+            _p(args[0], C.c_int32), _p(args[1], C.c_int32), _p(args[2], C.c_uint8), args[0].size,
+            _p(args[3], C.c_int32), _p(args[4], C.c_int32), _p(args[5], C.c_uint8), args[3].size,
+            _p(args[6], C.c_int32), _p(args[7], C.c_int32), _p(args[8], C.c_uint8), args[6].size,
+            int(min_hits), _p(offs, C.c_int32), cap_tracks, _p(hits, C.c_int32), cap_hits))
+        if T >= 0:
+            return offs[:T + 1].copy(), hits[:offs[T]].copy()
+        cap_hits *= 4
+
+
 class Oracle:
     """One model (weights blob + precision mode).  Methods mirror the stages of the hot path."""
 
@@ -251,6 +308,40 @@ class Oracle:
             out["m"] = m
         return out
 
+    def has_triplets(self) -> bool:
+        return bool(lib().etxo_has_triplets(self._h))
+
+    def triplet_scores(self, e_state, first, second, elbow: bool):
+        """Triplet classifier on pairs of final edge encodings (etxo_triplet_scores).  -> (logit [T], score [T])."""
+        e_state, first, second = _f32(e_state), _i32(first), _i32(second)
+        T = first.size
+        logit, score = np.zeros(max(T, 1), np.float32), np.zeros(max(T, 1), np.float32)
+        lib().etxo_triplet_scores(self._h, _p(e_state, C.c_float), _p(first, C.c_int32), _p(second, C.c_int32), T,
+                                  int(bool(elbow)), _p(logit, C.c_float), _p(score, C.c_float))
+        return logit[:T].copy(), score[:T].copy()
+
+    def run_triplets(self, xyz, src, dst, threshold=0.5, triplet_threshold=0.5, min_hits=3):
+        """Steps 4-7 of Figure 3 (L94) on a given rough graph: edge scores, purified hit graph, triplets of the
+        three kinds, their scores, purified edge graph, tracks.  -> dict."""
+        g = self.gnn(xyz, src, dst, want_states=True)
+        keep = (g["logit"] >= logit_threshold(threshold)).astype(np.uint8)
+        tau_t = logit_threshold(triplet_threshold)
+        n = np.asarray(xyz).shape[0]
+        out = dict(logit=g["logit"], keep=keep, e=g["e"])
+        kept = {}
+        for kind in ("articulation", "left_elbow", "right_elbow"):
+            f, s, h = triplets(src, dst, keep, n, kind)
+            z, sc = self.triplet_scores(g["e"], f, s, elbow=(kind != "articulation"))
+            out[kind] = dict(first=f, second=s, hit=h, logit=z, score=sc)
+            kept[kind] = (z >= tau_t).astype(np.uint8)
+        offs, hits = tracks_from_triplets(src, dst, keep,
+                                          (out["articulation"]["first"], out["articulation"]["second"]), kept["articulation"],
+                                          (out["left_elbow"]["first"], out["left_elbow"]["second"]), kept["left_elbow"],
+                                          (out["right_elbow"]["first"], out["right_elbow"]["second"]), kept["right_elbow"],
+                                          min_hits)
+        out["track_offsets"], out["track_hits"] = offs, hits
+        return out
+
     # --- instrumentation ---------------------------------------------------------------
     def n_layers(self) -> int:
         return int(lib().etxo_n_layers(self._h))
@@ -293,7 +384,7 @@ class Oracle:
                     logit=g["logit"], score=g["score"], track_id=tid)
 
 
-def calibrate_int8(blob_fp32: bytes, xyz, plane, event_offsets, k, window, d2_max=np.inf) -> np.ndarray:
+def calibrate_int8(blob_fp32: bytes, xyz, plane, event_offsets, k, window, d2_max=np.inf, threshold=0.5) -> np.ndarray:
     """Activation scales s_x = max|x|/127 per quantised Linear from the fp32 forward on a
     calibration batch (reading R21).  -> fp32 array in blob order."""
     o = Oracle(blob_fp32, "fp32")
@@ -301,7 +392,10 @@ def calibrate_int8(blob_fp32: bytes, xyz, plane, event_offsets, k, window, d2_ma
     emb = o.embed(xyz)
     nbr, deg = knn(emb, plane, event_offsets, k, window, d2_max)
     src, dst, _ = build_edges(nbr, deg)
-    o.gnn(xyz, src, dst)
+    if o.has_triplets():
+        o.run_triplets(xyz, src, dst, threshold, threshold)
+    else:
+        o.gnn(xyz, src, dst)
     o.record_absmax(False)
     return o.scales_from_absmax()
 

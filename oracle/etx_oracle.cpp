@@ -24,6 +24,13 @@
 //   head         : sigmoid closed forms, threshold boundary (L80)
 //   components   : scipy.sparse.csgraph + BFS + the paper's plane sweeps iterated
 //   tracks       : dictionary-based regrouping in Python, partition / ordering invariants, truth particles
+//   bf16 GNN     : a numpy restatement with torch.bfloat16 round trips at every R20 rounding point, bit for bit,
+//                  and shown to differ when any one point is dropped
+//   int8 scales  : every activation scale recomputed by an independent numpy forward, bit for bit
+//   triplets     : (tests/test_oracle_triplets.py) brute force over all pairs of edges, closed-form counts; the
+//                  classifier against float64 / pinned-fp32 / torch-bfloat16 restatements; track building against
+//                  a set + BFS formulation of the four phases, scipy components, hand-built e+e- and skipped-plane
+//                  fixtures, truth particles of a noise-free event
 //   The paper prints no worked numerical example, so no value
 //   here is pinned to a number printed by the paper.
 //
@@ -98,6 +105,8 @@ struct Model {
   Linear nenc[2], eenc[2];
   std::vector<Linear> node, edge;       // 2 per iteration
   Linear head;
+  int has_triplets = 0;                 // blob header word 11: the two triplet classifiers follow the head (L160)
+  Linear tart[2], telb[2];              // articulation / elbow classifier: 2d -> d -> 1
   std::vector<Linear*> all;             // blob order
   std::string error;
   // instrumentation (not part of the method)
@@ -205,6 +214,8 @@ bool parse_blob(Model& M, const uint8_t* blob, size_t bytes) {
   M.latent = (int)h[5]; M.iters = (int)h[6]; M.edge_enc_input = (int)h[7];
   M.emb_input = (int)h[10];
   if (M.emb_input != 0 && M.emb_input != 1) { M.error = "bad emb_input"; return false; }
+  M.has_triplets = (int)h[11];
+  if (M.has_triplets != 0 && M.has_triplets != 1) { M.error = "bad triplet flag"; return false; }
   const int D = M.emb_hidden, H = M.emb_layers_hidden, d = M.latent, L = M.iters;
   if (D < 1 || D > 256 || H < 1 || H > 8 || M.emb_dim < 1 || M.emb_dim > 16 || d < 1 || d > 85 ||
       L < 0 || L > 64) { M.error = "bad shapes"; return false; }
@@ -223,6 +234,10 @@ bool parse_blob(Model& M, const uint8_t* blob, size_t bytes) {
     set(M.edge[2 * it], d, 3 * d); set(M.edge[2 * it + 1], d, d);
   }
   set(M.head, 1, d, true);
+  if (M.has_triplets) {                 // L160: "an MLP ending with a layer with 1 unit" for articulations, one for elbows (R28)
+    set(M.tart[0], d, 2 * d); set(M.tart[1], 1, d, true);
+    set(M.telb[0], d, 2 * d); set(M.telb[1], 1, d, true);
+  }
   size_t need = 0; int nq = 0;
   for (Linear* l : M.all) { need += (size_t)l->out * l->in + l->out; nq += l->tensor; }
   if (h[8] != need) { M.error = "n_weight_floats mismatch"; return false; }
@@ -622,6 +637,157 @@ int64_t etxo_tracks(const int32_t* track_id, int64_t n, const int32_t* event_off
     event_track_off[e] = (int32_t)cnt;
   }
   return T;
+}
+
+// ---------------------------------------------------------------------------
+// Triplet stage (sec. 5.3, sec. 5.4).  The paper left it out of
+// its CUDA code (L238); readings R28-R31 in DESIGN.md say what is built where the text is silent.
+//
+// Triplet building (L152-158) on the purified hit graph (edges with keep[i] != 0, i.e. logit >= tau, L80 / L146).
+// A triplet is a pair of kept edges (first, second) with one common hit C:
+//   kind 0  articulation  A -> C, C -> B : first = the in-edge of C, second = the out-edge of C
+//   kind 1  left elbow    C -> A, C -> B : two distinct out-edges of C, first < second (edge id)
+//   kind 2  right elbow   A -> C, B -> C : two distinct in-edges of C,  first < second (edge id)
+// Order (R29): common hit C ascending, then first ascending, then second ascending.  Returns the number of
+// triplets; t_first / t_second / t_hit (each may be null: count only) receive the edge ids and the common hit.
+int64_t etxo_triplets(const int32_t* src, const int32_t* dst, const uint8_t* keep, int64_t E, int64_t n, int kind,
+                      int32_t* t_first, int32_t* t_second, int32_t* t_hit) {
+  std::vector<std::vector<int32_t>> out(n), in(n);               // kept edges per hit, ascending edge id
+  for (int64_t i = 0; i < E; ++i)
+    if (keep[i]) { out[src[i]].push_back((int32_t)i); in[dst[i]].push_back((int32_t)i); }
+  int64_t T = 0;
+  auto emit = [&](int32_t a, int32_t b, int64_t c) {
+    if (t_first) t_first[T] = a;
+    if (t_second) t_second[T] = b;
+    if (t_hit) t_hit[T] = (int32_t)c;
+    ++T;
+  };
+  for (int64_t c = 0; c < n; ++c) {
+    if (kind == 0) {
+      for (int32_t a : in[c]) for (int32_t b : out[c]) emit(a, b, c);
+    } else {
+      const std::vector<int32_t>& l = kind == 1 ? out[c] : in[c];
+      for (size_t i = 0; i < l.size(); ++i) for (size_t j = i + 1; j < l.size(); ++j) emit(l[i], l[j], c);
+    }
+  }
+  return T;
+}
+
+// Triplet classifier (L80: "transforms the pairs of edge encodings (triplets) into triplet scores"; L160: separate
+// classifiers for articulations and elbows, each "an MLP ending with a layer with 1 unit, and a sigmoid").
+// R28: input [e_first, e_second] (2d) of the FINAL edge encodings e^L, one hidden layer of width d with ReLU, then
+// d -> 1; z = logit, score = sigmoid(z).  `elbow` selects the classifier.  Precision modes as everywhere else
+// (R20 / R21): the 2d -> d layer is a tensor layer (bf16 weights / int8 codes, hidden activation rounded in bf16
+// mode), the d -> 1 layer is fp32 in the pinned order like the edge head.
+void etxo_triplet_scores(void* m, const float* e_state, const int32_t* t_first, const int32_t* t_second, int64_t T,
+                         int elbow, float* logit, float* score) {
+  Model& M = *static_cast<Model*>(m);
+  const int d = M.latent;
+  Linear* L = elbow ? M.telb : M.tart;
+#pragma omp parallel for schedule(static)
+  for (int64_t t = 0; t < T; ++t) {
+    float x[192], a[96], z;
+    std::memcpy(x, e_state + (size_t)t_first[t] * d, sizeof(float) * d);
+    std::memcpy(x + d, e_state + (size_t)t_second[t] * d, sizeof(float) * d);
+    linear(M, L[0], x, a, (size_t)t);
+    relu(a, d); state_round(M, a, d);
+    linear(M, L[1], a, &z, (size_t)t);
+    logit[t] = z;
+    score[t] = (float)(1.0 / (1.0 + std::exp(-(double)z)));
+  }
+}
+int etxo_has_triplets(void* m) { return static_cast<Model*>(m)->has_triplets; }
+
+// Track building from triplets (sec. 5.4, Figure 6), the four phases as read in R30:
+//  (1) "the left elbows and right elbows are connected": the two edges of every kept elbow are merged into one
+//      super-edge (union-find over edge ids, root = smallest id).  Articulations are mapped onto super-edges;
+//      "duplicate edges resulting from elbow connections are removed": equal (first, second) pairs collapse, and an
+//      articulation inside one super-edge disappears.
+//  (2) An articulation is SHARED when its first super-edge has two or more distinct successors or its second one
+//      two or more distinct predecessors ("two articulations sharing an edge").  WCC over the super-edges with the
+//      non-shared articulations only.
+//  (3) "a new track is formed for each remaining articulation, effectively duplicating the shared set": every shared
+//      articulation (X, Y) yields the track comp(X) u comp(Y); a component touched by no shared articulation is a
+//      track by itself.
+//  (4) edges -> hits: a track's hits are the end points of its edges, ascending.  Tracks with fewer than min_hits
+//      hits are dropped (L42), identical hit lists are kept once, and the result is ordered lexicographically by
+//      hit list (R31), so that it can be compared as arrays.
+// Only kept edges take part (an edge below the edge threshold is in no triplet, L146); a kept edge without any
+// kept triplet is a component of its own (two hits).  keepA / keepL / keepR flag the kept triplets of each kind.
+// Outputs: track_offsets[T + 1], track_hits[...] (capacities given by the caller: cap_tracks + 1, cap_hits);
+// returns T, or -1 if a capacity is too small.
+int64_t etxo_tracks_from_triplets(const int32_t* src, const int32_t* dst, const uint8_t* keep, int64_t E,
+                                  const int32_t* a_first, const int32_t* a_second, const uint8_t* keepA, int64_t TA,
+                                  const int32_t* l_first, const int32_t* l_second, const uint8_t* keepL, int64_t TL,
+                                  const int32_t* r_first, const int32_t* r_second, const uint8_t* keepR, int64_t TR,
+                                  int32_t min_hits, int32_t* track_offsets, int64_t cap_tracks,
+                                  int32_t* track_hits, int64_t cap_hits) {
+  std::vector<int32_t> sup(E);
+  for (int64_t i = 0; i < E; ++i) sup[i] = (int32_t)i;
+  auto find = [](std::vector<int32_t>& p, int32_t x) {
+    while (p[x] != x) { p[x] = p[p[x]]; x = p[x]; }
+    return x;
+  };
+  auto unite = [&](std::vector<int32_t>& p, int32_t a, int32_t b) {
+    a = find(p, a); b = find(p, b);
+    if (a == b) return;
+    if (a < b) p[b] = a; else p[a] = b;
+  };
+  // (1) elbows merge edges
+  for (int64_t t = 0; t < TL; ++t) if (keepL[t]) unite(sup, l_first[t], l_second[t]);
+  for (int64_t t = 0; t < TR; ++t) if (keepR[t]) unite(sup, r_first[t], r_second[t]);
+  std::vector<std::pair<int32_t, int32_t>> arts;
+  for (int64_t t = 0; t < TA; ++t)
+    if (keepA[t]) {
+      const int32_t x = find(sup, a_first[t]), y = find(sup, a_second[t]);
+      if (x != y) arts.push_back({x, y});
+    }
+  std::sort(arts.begin(), arts.end());
+  arts.erase(std::unique(arts.begin(), arts.end()), arts.end());
+  // (2) shared articulations, WCC over the rest
+  std::vector<int32_t> n_succ(E, 0), n_pred(E, 0);
+  for (auto& a : arts) { n_succ[a.first]++; n_pred[a.second]++; }      // arts are distinct pairs
+  std::vector<int32_t> comp(E);
+  for (int64_t i = 0; i < E; ++i) comp[i] = (int32_t)i;
+  std::vector<std::pair<int32_t, int32_t>> shared;
+  for (auto& a : arts) {
+    if (n_succ[a.first] >= 2 || n_pred[a.second] >= 2) shared.push_back(a);
+    else unite(comp, a.first, a.second);
+  }
+  // (3) tracks as sets of components
+  std::vector<uint8_t> touched(E, 0);
+  std::vector<std::vector<int32_t>> track_comps;
+  for (auto& a : shared) {
+    const int32_t p = find(comp, a.first), q = find(comp, a.second);
+    touched[p] = touched[q] = 1;
+    if (p == q) track_comps.push_back({p}); else track_comps.push_back({p, q});
+  }
+  for (int64_t i = 0; i < E; ++i)
+    if (keep[i] && find(sup, (int32_t)i) == i && find(comp, (int32_t)i) == i && !touched[i]) track_comps.push_back({(int32_t)i});
+  // members of every component: kept edges by the component of their super-edge
+  std::vector<std::vector<int32_t>> members(E);
+  for (int64_t i = 0; i < E; ++i)
+    if (keep[i]) members[find(comp, find(sup, (int32_t)i))].push_back((int32_t)i);
+  // (4) edges -> hits
+  std::vector<std::vector<int32_t>> tracks;
+  for (auto& tc : track_comps) {
+    std::vector<int32_t> hits;
+    for (int32_t c : tc) for (int32_t e : members[c]) { hits.push_back(src[e]); hits.push_back(dst[e]); }
+    std::sort(hits.begin(), hits.end());
+    hits.erase(std::unique(hits.begin(), hits.end()), hits.end());
+    if ((int32_t)hits.size() >= min_hits) tracks.push_back(hits);
+  }
+  std::sort(tracks.begin(), tracks.end());
+  tracks.erase(std::unique(tracks.begin(), tracks.end()), tracks.end());
+  if ((int64_t)tracks.size() > cap_tracks) return -1;
+  int64_t pos = 0;
+  track_offsets[0] = 0;
+  for (size_t t = 0; t < tracks.size(); ++t) {
+    if (pos + (int64_t)tracks[t].size() > cap_hits) return -1;
+    for (int32_t h : tracks[t]) track_hits[pos++] = h;
+    track_offsets[t + 1] = (int32_t)pos;
+  }
+  return (int64_t)tracks.size();
 }
 
 }  // extern "C"

@@ -194,9 +194,20 @@ def centred_parity_weights(cfg, batch, seed=None):
     o = oracle.Oracle(datagen.pack_blob(cfg, layers), "fp32")
     r = o.run(batch.xyz, batch.plane, batch.event_offsets, cfg.k, cfg.window, cfg.d2_max, cfg.threshold)
     med = float(np.median(r["logit"])) if r["logit"].size else 0.0
-    name, W, b = layers[-1]
-    assert name == "head"
-    layers[-1] = (name, W, (b - np.float32(med)).astype(np.float32))
+    names = [l[0] for l in layers]
+    ih = names.index("head")
+    name, W, b = layers[ih]
+    layers[ih] = (name, W, (b - np.float32(med)).astype(np.float32))
+    if getattr(cfg, "triplets", 0):
+        # the triplet classifiers likewise: biases moved so that about half of the triplets of each kind are kept
+        o = oracle.Oracle(datagen.pack_blob(cfg, layers), "fp32")
+        t = o.run_triplets(batch.xyz, r["src"], r["dst"], cfg.threshold, cfg.triplet_threshold)
+        za = t["articulation"]["logit"]
+        ze = np.concatenate([t["left_elbow"]["logit"], t["right_elbow"]["logit"]])
+        for lname, z in (("tart1", za), ("telb1", ze)):
+            i = names.index(lname)
+            name, W, b = layers[i]
+            layers[i] = (name, W, (b - np.float32(np.median(z) if z.size else 0.0)).astype(np.float32))
     return layers
 
 
