@@ -85,6 +85,9 @@ typedef struct {
                                         features (L133).                                                   */
   float    cyl_offset[3];
   float    cyl_div[3];
+  int32_t  max_triplets;             /* capacity per triplet kind of etx_triplets (0: the triplet stage is not used)     */
+  float    triplet_threshold;        /* a triplet is kept iff its score >= this (L80: "triplets scoring below ... are
+                                        discarded"; decided on the logit like the edge threshold, R17)                  */
   /* Optional device-memory allocator (L223: Allen hands every algorithm memory from its own per-stream
    * arena).  NULL alloc: cudaMalloc / cudaFree.  alloc must return device memory aligned to 256 bytes or
    * NULL on failure; dealloc is called once per block from etx_destroy; alloc and dealloc go together.    */
@@ -106,7 +109,8 @@ typedef struct {                     /* device pointers into the handle's worksp
 
 /* Create a context: parse + validate the weights blob (layout: datagen/weights.py header; fp32
  * tensors W[out][in], b[out] in the order emb 0..H, node enc (2), edge enc (2), per step node net (2)
- * + edge net (2), head; INT8 additionally one activation scale per Linear with K >= 16), convert the
+ * + edge net (2), head, and -- if header word 11 is set -- the articulation and the elbow triplet classifier
+ * (2d -> d, d -> 1 each); INT8 additionally one activation scale per Linear with K >= 16), convert the
  * weights to the precision's operand format, allocate the workspace for (max_events, max_hits, k).
  * The blob is copied; the caller may free it on return.  *out is set only on ETX_OK. */
 etx_status etx_create(const void* h_weights_blob, size_t blob_bytes, const etx_hyperparams* hp,
@@ -164,6 +168,30 @@ typedef struct {
 } etx_tracks_output;
 
 etx_status etx_tracks(etx_handle h, int32_t min_hits, etx_stream stream, etx_tracks_output* out);
+
+/* Triplet stage (sec. 5.3; R28, R29), the step the paper left out of its CUDA code
+ * (L238).  Enqueue on `stream`, after an etx_run on the same stream and handle: triplet building on the purified
+ * hit graph (edges with logit >= tau) and the two triplet classifiers on pairs of final edge encodings.  Needs a
+ * blob that carries the triplet classifiers (header word 11) and max_triplets > 0.  For kind k (0 articulation
+ * A->C, C->B: first = the in-edge of the common hit C, second = its out-edge; 1 left elbow C->A, C->B; 2 right elbow
+ * A->C, B->C; first < second for the elbows) the triplets are listed in ascending (C, first, second) order:
+ *   d_first[k], d_second[k]  [count[k]] edge ids      d_hit[k]  [count[k]] the common hit
+ *   d_logit[k], d_score[k]   [count[k]] classifier output (articulation classifier for kind 0, elbow classifier else)
+ * d_count / h_count [3]: the number of triplets of each kind (h_count: pinned mirror, valid after synchronising).  If
+ * a count exceeds max_triplets only the first max_triplets triplets of that kind are listed (the caller compares).
+ * Library-owned device pointers, valid until the next call on the handle; no synchronisation. */
+typedef struct {
+  const int32_t* d_first[3];
+  const int32_t* d_second[3];
+  const int32_t* d_hit[3];
+  const float*   d_logit[3];
+  const float*   d_score[3];
+  const int32_t* d_count;
+  const int32_t* h_count;
+  int32_t        capacity;
+} etx_triplets_output;
+
+etx_status etx_triplets(etx_handle h, etx_stream stream, etx_triplets_output* out);
 
 etx_status etx_destroy(etx_handle h);
 

@@ -36,6 +36,7 @@ class Hyperparams(C.Structure):
                 ("threshold", C.c_float), ("precision", C.c_int32), ("engine", C.c_int32),
                 ("max_events", C.c_int32), ("max_hits", C.c_int32), ("validate_input", C.c_int32),
                 ("emb_input", C.c_int32), ("cyl_offset", C.c_float * 3), ("cyl_div", C.c_float * 3),
+                ("max_triplets", C.c_int32), ("triplet_threshold", C.c_float),
                 ("alloc", ALLOC_FN), ("dealloc", DEALLOC_FN), ("alloc_ctx", C.c_void_p)]
 
 
@@ -48,6 +49,12 @@ class EtxOutput(C.Structure):
 class EtxTracks(C.Structure):
     _fields_ = [("d_track_index", C.c_void_p), ("d_track_offsets", C.c_void_p), ("d_track_hits", C.c_void_p),
                 ("d_event_track_offsets", C.c_void_p), ("d_n_tracks", C.c_void_p), ("h_n_tracks", C.POINTER(C.c_int32))]
+
+
+class EtxTriplets(C.Structure):
+    _fields_ = [("d_first", C.c_void_p * 3), ("d_second", C.c_void_p * 3), ("d_hit", C.c_void_p * 3),
+                ("d_logit", C.c_void_p * 3), ("d_score", C.c_void_p * 3), ("d_count", C.c_void_p),
+                ("h_count", C.POINTER(C.c_int32)), ("capacity", C.c_int32)]
 
 
 class Inject(C.Structure):
@@ -87,6 +94,8 @@ def load_library():
     L.etx_run_host.argtypes = [vp, vp, vp, i32p, C.c_int32, vp, vp, vp, vp, vp, i32p]
     L.etx_destroy.restype = C.c_int
     L.etx_destroy.argtypes = [vp]
+    L.etx_triplets.restype = C.c_int
+    L.etx_triplets.argtypes = [vp, vp, C.POINTER(EtxTriplets)]
     L.etx_input_status.restype = C.c_int
     L.etx_input_status.argtypes = [vp]
     L.etx_tracks.restype = C.c_int
@@ -118,7 +127,7 @@ def lib():
 
 
 def hyperparams_from_config(cfg, max_events: int, max_hits: int, precision: str | None = None,
-                            engine: str = "auto", validate_input: bool = False, n_planes: int = 26,
+                            engine: str = "auto", validate_input: bool = False, n_planes: int = 26, max_triplets: int = 0,
                             norm_offset=(0.0, 0.0, 300.0), norm_div=(40.0, 40.0, 1050.0),
                             cyl_offset=(-20.0, 0.0, 300.0), cyl_div=(12.0, 3.14159274, 1050.0)) -> Hyperparams:
     """etx_hyperparams from a datagen.EtxConfig-like object (attribute access only)."""
@@ -139,6 +148,8 @@ def hyperparams_from_config(cfg, max_events: int, max_hits: int, precision: str 
     hp.emb_input = getattr(cfg, "emb_input", 0)
     hp.cyl_offset = (C.c_float * 3)(*cyl_offset)
     hp.cyl_div = (C.c_float * 3)(*cyl_div)
+    hp.max_triplets = int(max_triplets)
+    hp.triplet_threshold = float(getattr(cfg, "triplet_threshold", 0.5))
     return hp
 
 
@@ -256,6 +267,21 @@ class Etx:
                     track_index=self._copy_out(out.d_track_index, 4 * n_hits, torch.int32),
                     track_hits=self._copy_out(out.d_track_hits, 4 * n_hits_kept, torch.int32),
                     event_track_offsets=self._copy_out(out.d_event_track_offsets, 4 * (n_events + 1), torch.int32))
+
+    def triplets(self) -> dict:
+        """etx_triplets on the current stream after a run; synchronises.  -> {kind: dict(first, second, hit, logit, score)}
+        as torch tensors, plus "count" (the true counts) and "capacity"."""
+        import torch
+        out = EtxTriplets()
+        self._check(self._L.etx_triplets(self._h, self._stream(), C.byref(out)), "etx_triplets")
+        torch.cuda.current_stream().synchronize()
+        res = {"count": [int(out.h_count[k]) for k in range(3)], "capacity": int(out.capacity)}
+        for k, kind in enumerate(("articulation", "left_elbow", "right_elbow")):
+            n = min(res["count"][k], res["capacity"])
+            res[kind] = dict(first=self._copy_out(out.d_first[k], 4 * n, torch.int32), second=self._copy_out(out.d_second[k], 4 * n, torch.int32),
+                             hit=self._copy_out(out.d_hit[k], 4 * n, torch.int32), logit=self._copy_out(out.d_logit[k], 4 * n, torch.float32),
+                             score=self._copy_out(out.d_score[k], 4 * n, torch.float32))
+        return res
 
     def workspace_bytes(self) -> int:
         return int(self._L.etx_workspace_bytes(self._h))

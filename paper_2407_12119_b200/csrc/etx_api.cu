@@ -71,6 +71,12 @@ etx_status parse_blob(etx_ctx* c, const uint8_t* blob, size_t bytes) {
   for (int it = 0; it < L; ++it) { add(d, 3 * d); add(d, d); add(d, 3 * d); add(d, d); }
   c->i_head = (int)c->layers.size();
   add(1, d, true);
+  if (h[11] > 1u) return fail(c, ETX_ERR_BLOB, "bad triplet-classifier flag");
+  if (h[11] == 1u) {                 // L160: articulation classifier, elbow classifier: 2d -> d -> 1 (R28)
+    c->i_trip = (int)c->layers.size();
+    add(d, 2 * d); add(1, d, true);
+    add(d, 2 * d); add(1, d, true);
+  }
   size_t need = 0; int nq = 0;
   for (auto& l : c->layers) { need += (size_t)l.out * l.in + l.out; nq += l.tensor; }
   if (h[8] != need) return fail(c, ETX_ERR_BLOB, "blob weight count differs from the shapes");
@@ -177,7 +183,9 @@ etx_status run_impl(etx_ctx* c, const float* d_xyz, const int32_t* d_plane, cons
     ETX_CUDA(cudaMemsetAsync(c->n_edges, 0, sizeof(int32_t), s));
     c->n_ev = 0; c->spans.clear();
     c->last_n_hits = n_hits; c->last_n_events = n_events;
-    c->keep_final_state = (inj != nullptr);   // e^L feeds only the classifier (L142); a plain run does not write it
+    // e^L feeds only the classifier (L142), so a plain run does not write it back -- unless the triplet stage, which
+    // reads pairs of final edge encodings (L80), can follow
+    c->keep_final_state = (inj != nullptr) || (c->i_trip >= 0 && c->hp.max_triplets > 0);
     StageTimer tm{c, s};
     bool edges_marked = false;
     const bool tensor_engine = (c->precision != ETX_FP32) && c->engine != ETX_ENGINE_SIMT;
@@ -311,7 +319,7 @@ etx_status etx_create(const void* blob, size_t blob_bytes, const etx_hyperparams
   if (hp->precision < 0 || hp->precision > 2 || hp->engine < 0 || hp->engine > 2) return bail(ETX_ERR_ARG);
   if ((hp->alloc == nullptr) != (hp->dealloc == nullptr)) return bail(ETX_ERR_ARG);
   if (hp->n_planes < 1 || hp->n_planes > 1024 || hp->k < 1 || hp->window < 1 || hp->max_events < 0 || hp->max_hits < 0 ||
-      hp->gnn_iters < 0 || hp->gnn_iters > 64 || hp->emb_n_hidden_layers < 1 || hp->emb_n_hidden_layers > 8 ||
+      hp->gnn_iters < 0 || hp->gnn_iters > 64 || hp->max_triplets < 0 || !(hp->triplet_threshold >= 0.0f && hp->triplet_threshold <= 1.0f) || hp->emb_n_hidden_layers < 1 || hp->emb_n_hidden_layers > 8 ||
       !(hp->threshold >= 0.0f && hp->threshold <= 1.0f) || isnan(hp->d2_max))
     return bail(ETX_ERR_ARG);
   for (int i = 0; i < 3; ++i)
@@ -372,6 +380,16 @@ etx_status etx_create(const void* blob, size_t blob_bytes, const etx_hyperparams
     c->trk_index = dev_alloc<int32_t>(c, N); c->trk_offsets = dev_alloc<int32_t>(c, N + 1);
     c->trk_hits = dev_alloc<int32_t>(c, N); c->trk_event_off = dev_alloc<int32_t>(c, B + 1);
     c->n_tracks = dev_alloc<int32_t>(c, 1);
+    if (hp->max_triplets > 0) {
+      const size_t T = (size_t)hp->max_triplets;
+      c->trip_cnt = dev_alloc<int32_t>(c, 3 * (N + 1)); c->trip_off = dev_alloc<int32_t>(c, 3 * (N + 1));
+      c->trip_first = dev_alloc<int32_t>(c, 3 * T); c->trip_second = dev_alloc<int32_t>(c, 3 * T); c->trip_hit = dev_alloc<int32_t>(c, 3 * T);
+      c->trip_logit = dev_alloc<float>(c, 3 * T); c->trip_score = dev_alloc<float>(c, 3 * T);
+      c->trip_total = dev_alloc<int32_t>(c, 4);
+      ETX_CUDA(cudaMemset(c->trip_total, 0, 4 * sizeof(int32_t)));
+      ETX_CUDA(cudaMallocHost(&c->h_trip_total, 4 * sizeof(int32_t)));
+      for (int i = 0; i < 4; ++i) c->h_trip_total[i] = 0;
+    }
     c->d_xyz_in = dev_alloc<float>(c, N * 3);
     c->d_plane_in = dev_alloc<int32_t>(c, N);
     ETX_CUDA(cudaMemset(c->n_edges, 0, sizeof(int32_t)));
@@ -419,6 +437,7 @@ etx_status etx_destroy(etx_handle c) {
   if (c->h_n_edges) cudaFreeHost(c->h_n_edges);
   if (c->h_n_tracks) cudaFreeHost(c->h_n_tracks);
   if (c->h_flags) cudaFreeHost(c->h_flags);
+  if (c->h_trip_total) cudaFreeHost(c->h_trip_total);
   if (c->staging_free) cudaEventDestroy(c->staging_free);
   if (c->edges_ready) cudaEventDestroy(c->edges_ready);
   if (c->copies_done) cudaEventDestroy(c->copies_done);
@@ -443,6 +462,26 @@ etx_status etx_tracks(etx_handle c, int32_t min_hits, etx_stream stream, etx_tra
     return fail(c, ETX_ERR_CUDA, "etx_tracks: launch failed");
   out->d_track_index = c->trk_index; out->d_track_offsets = c->trk_offsets; out->d_track_hits = c->trk_hits;
   out->d_event_track_offsets = c->trk_event_off; out->d_n_tracks = c->n_tracks; out->h_n_tracks = c->h_n_tracks;
+  return ETX_OK;
+}
+
+etx_status etx_triplets(etx_handle c, etx_stream stream, etx_triplets_output* out) {
+  if (!c) return ETX_ERR_ARG;
+  if (!out) return fail(c, ETX_ERR_ARG, "etx_triplets: null output");
+  if (c->i_trip < 0) return fail(c, ETX_ERR_BLOB, "etx_triplets: the blob carries no triplet classifiers (header word 11)");
+  if (c->hp.max_triplets <= 0) return fail(c, ETX_ERR_CAPACITY, "etx_triplets: max_triplets is 0");
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  launch_triplet_build(c, c->last_n_hits, s);
+  for (int k = 0; k < 3; ++k) launch_triplet_classifier(c, k, s);
+  if (cudaMemcpyAsync(c->h_trip_total, c->trip_total, 3 * sizeof(int32_t), cudaMemcpyDeviceToHost, s) != cudaSuccess ||
+      cudaGetLastError() != cudaSuccess)
+    return fail(c, ETX_ERR_CUDA, "etx_triplets: launch failed");
+  const size_t T = (size_t)c->hp.max_triplets;
+  for (int k = 0; k < 3; ++k) {
+    out->d_first[k] = c->trip_first + k * T; out->d_second[k] = c->trip_second + k * T; out->d_hit[k] = c->trip_hit + k * T;
+    out->d_logit[k] = c->trip_logit + k * T; out->d_score[k] = c->trip_score + k * T;
+  }
+  out->d_count = c->trip_total; out->h_count = c->h_trip_total; out->capacity = c->hp.max_triplets;
   return ETX_OK;
 }
 

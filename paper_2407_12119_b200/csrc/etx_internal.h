@@ -81,7 +81,7 @@ struct etx_ctx {
   std::vector<std::pair<const void*, int>> smem_opted;   // kernels whose dynamic shared-memory limit was raised for this handle
   std::string error;
   std::vector<etx::HostLayer> layers;     // blob order
-  int i_emb0 = 0, i_nenc = 0, i_eenc = 0, i_iter0 = 0, i_head = 0;
+  int i_emb0 = 0, i_nenc = 0, i_eenc = 0, i_iter0 = 0, i_head = 0, i_trip = -1;   // i_trip: the four triplet-classifier layers, or -1
   std::vector<void*> allocs;              // every device block of this handle (etx_device_alloc)
   size_t device_bytes = 0;
   // workspace
@@ -106,6 +106,10 @@ struct etx_ctx {
   int32_t *trk_size = nullptr, *trk_keep = nullptr, *trk_number = nullptr, *trk_ksize = nullptr;
   int32_t *trk_index = nullptr, *trk_offsets = nullptr, *trk_hits = nullptr, *trk_event_off = nullptr;
   int32_t *n_tracks = nullptr, *h_n_tracks = nullptr;
+  // triplet stage (etx_triplets): per-hit counts / offsets [3][max_hits + 1], triplets [3][max_triplets]
+  int32_t *trip_cnt = nullptr, *trip_off = nullptr, *trip_first = nullptr, *trip_second = nullptr, *trip_hit = nullptr;
+  float *trip_logit = nullptr, *trip_score = nullptr;
+  int32_t *trip_total = nullptr, *h_trip_total = nullptr;   // [3] device / pinned
   int last_n_events = 0;
   // k_edge_tma.cu: identity operand image, split-bias images [2 * iter + layer], CUtensorMap of `e` (opaque here)
   bool edge_tma = false;
@@ -173,11 +177,13 @@ void launch_rows_from_src(etx_ctx* c, int n_hits, int n_edges, cudaStream_t s); 
 void launch_csc(etx_ctx* c, int n_events, int n_hits, bool windowed, cudaStream_t s);                        // dst -> col_ptr, in_edge
 void launch_components(etx_ctx* c, const float* logit, int n_events, int n_hits, cudaStream_t s);
 void launch_tracks(etx_ctx* c, int n_events, int n_hits, int min_hits, cudaStream_t s);
+void launch_triplet_build(etx_ctx* c, int n_hits, cudaStream_t s);
 // k_mlp_simt.cu
 void launch_embed_simt(etx_ctx* c, int n_hits, cudaStream_t s);
 void launch_gnn_mlp_simt(etx_ctx* c, int kind, int iter, int n_hits, bool do_head, cudaStream_t s);
 void launch_scatter(etx_ctx* c, int n_hits, cudaStream_t s);
 void simt_configure(etx_ctx* c);
+void launch_triplet_classifier(etx_ctx* c, int kind, cudaStream_t s);
 void fill_gnn_args(etx_ctx* c, int kind, int iter, int n_hits, bool do_head, GnnArgs& a);
 // k_mlp_umma.cu
 bool umma_supported(const etx_ctx* c);

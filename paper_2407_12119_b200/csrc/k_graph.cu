@@ -756,4 +756,65 @@ void launch_tracks(etx_ctx* c, int n_events, int n_hits, int min_hits, cudaStrea
   c->launches += 5;
 }
 
+// --------------------------------------------------------------------------------------------------------
+// Triplet building (sec. 5.3; R29) on the purified hit graph (edges with logit >= tau, L80).
+// A triplet is a pair of kept edges (first, second) with one common hit C: kind 0 articulation (an in-edge and an
+// out-edge of C), kind 1 left elbow (two out-edges of C), kind 2 right elbow (two in-edges of C), first < second for
+// the elbows.  Order: C ascending, then first, then second -- which is the order of the CSR / CSC lists, both
+// ascending in edge id.  Count per hit -> exclusive scan -> fill; all integer work, bit-exact by construction.
+__global__ void trip_count_kernel(const int32_t* __restrict__ row_ptr, const int32_t* __restrict__ col_ptr,
+                                  const int32_t* __restrict__ in_edge, const float* __restrict__ logit, float tau, int n_hits,
+                                  int32_t* __restrict__ cnt /* [3][n_hits + 1] */) {
+  const int c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= n_hits) return;
+  int od = 0, id = 0;
+  for (int i = row_ptr[c]; i < row_ptr[c + 1]; ++i) od += logit[i] >= tau;
+  for (int i = col_ptr[c]; i < col_ptr[c + 1]; ++i) id += logit[in_edge[i]] >= tau;
+  const size_t st = (size_t)n_hits + 1;
+  cnt[c] = id * od;
+  cnt[st + c] = od * (od - 1) / 2;
+  cnt[2 * st + c] = id * (id - 1) / 2;
+}
+
+// one thread per common hit; triplets beyond `cap` are counted but not written (the caller compares the totals)
+__global__ void trip_fill_kernel(const int32_t* __restrict__ row_ptr, const int32_t* __restrict__ col_ptr,
+                                 const int32_t* __restrict__ in_edge, const float* __restrict__ logit, float tau, int n_hits,
+                                 const int32_t* __restrict__ off /* [3][n_hits + 1] */, int cap,
+                                 int32_t* __restrict__ first, int32_t* __restrict__ second, int32_t* __restrict__ hit /* [3][cap] */) {
+  const int c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= n_hits) return;
+  const size_t st = (size_t)n_hits + 1;
+  const int a0 = row_ptr[c], a1 = row_ptr[c + 1], b0 = col_ptr[c], b1 = col_ptr[c + 1];
+  auto put = [&](int kind, int pos, int f, int s2) {
+    if (pos < cap) { const size_t o = (size_t)kind * cap + pos; first[o] = f; second[o] = s2; hit[o] = c; }
+  };
+  int pa = off[c], pl = off[st + c], pr = off[2 * st + c];
+  for (int i = b0; i < b1; ++i) {                               // in-edges of c, ascending edge id
+    const int ei = in_edge[i];
+    if (!(logit[ei] >= tau)) continue;
+    for (int j = a0; j < a1; ++j) if (logit[j] >= tau) put(0, pa++, ei, j);              // articulations
+    for (int j = i + 1; j < b1; ++j) { const int ej = in_edge[j]; if (logit[ej] >= tau) put(2, pr++, ei, ej); }   // right elbows
+  }
+  for (int i = a0; i < a1; ++i) {                               // out-edges of c
+    if (!(logit[i] >= tau)) continue;
+    for (int j = i + 1; j < a1; ++j) if (logit[j] >= tau) put(1, pl++, i, j);            // left elbows
+  }
+}
+
+__global__ void trip_totals_kernel(const int32_t* __restrict__ off, int n_hits, int32_t* __restrict__ total) {
+  if (threadIdx.x < 3) total[threadIdx.x] = off[(size_t)threadIdx.x * ((size_t)n_hits + 1) + n_hits];
+}
+
+void launch_triplet_build(etx_ctx* c, int n_hits, cudaStream_t s) {
+  if (n_hits == 0) { cudaMemsetAsync(c->trip_total, 0, 3 * sizeof(int32_t), s); return; }
+  const int g = (n_hits + 127) / 128;
+  const size_t st = (size_t)n_hits + 1;
+  trip_count_kernel<<<g, 128, 0, s>>>(c->row_ptr, c->col_ptr, c->in_edge, c->logit, c->tau, n_hits, c->trip_cnt);
+  for (int k = 0; k < 3; ++k) exclusive_scan(c, c->trip_cnt + k * st, n_hits, c->trip_off + k * st, nullptr, s);
+  trip_totals_kernel<<<1, 32, 0, s>>>(c->trip_off, n_hits, c->trip_total);
+  trip_fill_kernel<<<g, 128, 0, s>>>(c->row_ptr, c->col_ptr, c->in_edge, c->logit, c->tau, n_hits, c->trip_off, c->hp.max_triplets,
+                                     c->trip_first, c->trip_second, c->trip_hit);
+  c->launches += 3;
+}
+
 }  // namespace etx

@@ -453,6 +453,90 @@ void launch_scatter(etx_ctx* c, int n_hits, cudaStream_t s) {
   c->launches++;
 }
 
+// ============================================================================================================
+// Triplet classifier (R28): z = w1 . relu(W0 [e_first, e_second] + b0) + b1 on pairs of
+// FINAL edge encodings, one classifier for articulations and one for elbows.  The 2d -> d layer is a tensor layer in
+// the sense of R20 / R21 (bf16 weights and rounded hidden activation / int8 codes), the d -> 1 layer is fp32 in the
+// pinned order like the edge head.  Same arithmetic in every precision as the rest of this file, so fp32 and int8
+// are bit-exact against the oracle.
+struct TripArgs {
+  LayerP l0, l1;
+  const void* e;                // [E][d] final edge state, state dtype
+  const int32_t* first; const int32_t* second;
+  const int32_t* n_ptr;         // device count of this kind
+  int cap;
+  float* logit; float* score;
+};
+
+template <int MODE, typename ST, int D>
+__global__ void __launch_bounds__(kMlpThreads) triplet_cls_simt_kernel(TripArgs a) {
+  constexpr int R = kTileRows, LDX = 2 * D + 4, LDY = D + 4;
+  extern __shared__ __align__(16) float smem[];
+  float* X = smem;                       // [R][LDX]
+  float* Y = X + R * LDX;                // [R][LDY]
+  const int n_rows = min(*a.n_ptr, a.cap);
+  const LayerP L0 = a.l0, L1 = a.l1;
+  for (int tile = blockIdx.x; (size_t)tile * R < (size_t)n_rows; tile += gridDim.x) {
+    const int row0 = tile * R;
+    __syncthreads();
+    constexpr int c4n = 2 * D / 4, seg4 = D / 4;
+    for (int idx = threadIdx.x; idx < R * c4n; idx += kMlpThreads) {
+      const int r = idx / c4n, c4 = idx % c4n, seg = c4 / seg4, within = (c4 % seg4) * 4;
+      const int row = row0 + r;
+      float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (row < n_rows) v = State<ST>::ld4(a.e, (size_t)(seg ? a.second[row] : a.first[row]) * D + within);
+      if (MODE == kModeInt8) { v.x = quant_i8(v.x, L0.inv_sx); v.y = quant_i8(v.y, L0.inv_sx); v.z = quant_i8(v.z, L0.inv_sx); v.w = quant_i8(v.w, L0.inv_sx); }
+      *reinterpret_cast<float4*>(X + r * LDX + c4 * 4) = v;
+    }
+    __syncthreads();
+    dense_tile<D, R>(X, LDX, 2 * D, L0.Wt, [&](int r, int c, const float* acc) {
+      float4 sc = __ldg(reinterpret_cast<const float4*>(L0.scale + c)), bi = __ldg(reinterpret_cast<const float4*>(L0.bias + c));
+      float y[4] = {__fmaf_rn(acc[0], sc.x, bi.x), __fmaf_rn(acc[1], sc.y, bi.y), __fmaf_rn(acc[2], sc.z, bi.z), __fmaf_rn(acc[3], sc.w, bi.w)};
+#pragma unroll
+      for (int j = 0; j < 4; ++j) { y[j] = y[j] > 0.0f ? y[j] : 0.0f; if (MODE == kModeBf16) y[j] = bf16r(y[j]); }   // the next layer is fp32: no int8 codes
+      *reinterpret_cast<float4*>(Y + r * LDY + c) = make_float4(y[0], y[1], y[2], y[3]);
+    });
+    __syncthreads();
+    if (threadIdx.x < R && row0 + threadIdx.x < n_rows) {
+      const float* x = Y + threadIdx.x * LDY;
+      float acc = 0.0f;
+      for (int j = 0; j < D; ++j) acc = __fmaf_rn(x[j], __ldg(L1.Wt + j), acc);
+      const float z = __fadd_rn(acc, __ldg(L1.bias));
+      a.logit[row0 + threadIdx.x] = z;
+      a.score[row0 + threadIdx.x] = 1.0f / (1.0f + expf(-z));
+    }
+  }
+}
+
+template <int MODE, typename ST, int D>
+static void trip_launch(etx_ctx* c, const TripArgs& a, cudaStream_t s) {
+  auto kern = triplet_cls_simt_kernel<MODE, ST, D>;
+  const int smem = (int)(sizeof(float) * kTileRows * (2 * D + 4 + D + 4));
+  opt_in_smem(c, kern, smem);
+  const int tiles = (a.cap + kTileRows - 1) / kTileRows;
+  const int grid = tiles < c->sm_count * 3 ? tiles : c->sm_count * 3;
+  if (grid <= 0) return;
+  kern<<<grid, kMlpThreads, smem, s>>>(a);
+  c->launches++;
+}
+
+// kind 0: articulations (classifier i_trip, i_trip + 1); kinds 1, 2: elbows (i_trip + 2, i_trip + 3)
+void launch_triplet_classifier(etx_ctx* c, int kind, cudaStream_t s) {
+  TripArgs a;
+  const int i0 = c->i_trip + (kind ? 2 : 0);
+  a.l0 = c->layers[i0].dev; a.l1 = c->layers[i0 + 1].dev;
+  a.e = c->e;
+  const size_t cap = (size_t)c->hp.max_triplets;
+  a.first = c->trip_first + kind * cap; a.second = c->trip_second + kind * cap;
+  a.n_ptr = c->trip_total + kind; a.cap = c->hp.max_triplets;
+  a.logit = c->trip_logit + kind * cap; a.score = c->trip_score + kind * cap;
+#define ETX_TRIP(MODE, ST) { if (c->hp.gnn_latent == 32) trip_launch<MODE, ST, 32>(c, a, s); else trip_launch<MODE, ST, 64>(c, a, s); }
+  if (c->precision == ETX_FP32) ETX_TRIP(kModeF32, float)
+  else if (c->precision == ETX_BF16) ETX_TRIP(kModeBf16, __nv_bfloat16)
+  else ETX_TRIP(kModeInt8, float)
+#undef ETX_TRIP
+}
+
 void simt_configure(etx_ctx*) {}
 
 }  // namespace etx

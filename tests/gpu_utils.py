@@ -16,10 +16,12 @@ def dev(a, dtype=None):
     return t.cuda()
 
 
-def make_ctx(cfg, blob, batch=None, precision=None, engine="auto", max_events=None, max_hits=None, validate=False):
+def make_ctx(cfg, blob, batch=None, precision=None, engine="auto", max_events=None, max_hits=None, validate=False,
+             max_triplets=0):
     B = max_events if max_events is not None else max(batch.n_events, 1)
     N = max_hits if max_hits is not None else max(batch.n_hits, 1)
-    hp = etx.hyperparams_from_config(cfg, B, N, precision=precision, engine=engine, validate_input=validate)
+    hp = etx.hyperparams_from_config(cfg, B, N, precision=precision, engine=engine, validate_input=validate,
+                                     max_triplets=max_triplets)
     return etx.Etx(blob, hp)
 
 

@@ -1,0 +1,101 @@
+"""GPU parity of the triplet stage (etx_triplets; sec. 5.3) against the oracle, through the C-ABI.
+Triplet building is integer work: the arrays must be equal.  The classifiers are bit-exact in fp32 and int8 (pinned
+fp32 order / integer accumulation) and within the bf16 bar otherwise.  Stage-isolated as DESIGN.md sec. 6 says:
+the oracle builds its triplets from the GPU's own logits (bit-exact comparison needs identical inputs), and scores
+them on the GPU's own final edge state."""
+import numpy as np
+import pytest
+import torch
+
+import datagen
+import oracle
+from gpu_utils import make_ctx, run_gpu, state
+from helpers import centred_parity_weights
+
+pytestmark = pytest.mark.gpu
+KINDS = ("articulation", "left_elbow", "right_elbow")
+
+
+def _setup(name, n_events, precision):
+    cfg = datagen.get_config(name).replace(precision=precision, triplets=1)
+    b = datagen.generate_batch(cfg, n_events=n_events)
+    W = centred_parity_weights(cfg.replace(precision="fp32"), b.slice_events(0, 1))
+    scales = None
+    if precision == "int8":
+        scales = oracle.calibrate_int8(datagen.pack_blob(cfg, W), b.xyz, b.plane, b.event_offsets, cfg.k, cfg.window)
+    return cfg, b, datagen.pack_blob(cfg, W, scales)
+
+
+@pytest.mark.parametrize("name,n_events,precision", [("cfg0", 2, "fp32"), ("cfg1", 2, "fp32"), ("cfg1", 2, "int8"),
+                                                     ("cfg1", 2, "bf16"), ("cfg0", 1, "bf16")])
+def test_triplets_and_scores_against_the_oracle(name, n_events, precision):
+    cfg, b, blob = _setup(name, n_events, precision)
+    ctx = make_ctx(cfg, blob, b, max_triplets=4_000_000)
+    g = run_gpu(ctx, b, debug=False)
+    t = ctx.triplets()
+    E, d = g["n_edges"], cfg.gnn_latent
+    e_gpu = state(ctx, "e", E, d)                              # e^L: written back because the triplet stage may follow
+    o = oracle.Oracle(blob, precision)
+    keep = (g["logit"] >= oracle.logit_threshold(cfg.threshold)).astype(np.uint8)
+    assert 0 < keep.sum() < E
+    total = 0
+    for k, kind in enumerate(KINDS):
+        f, s, h = oracle.triplets(g["src"], g["dst"], keep, b.n_hits, kind)
+        assert t["count"][k] == f.size, kind
+        assert np.array_equal(t[kind]["first"].cpu().numpy(), f), kind
+        assert np.array_equal(t[kind]["second"].cpu().numpy(), s), kind
+        assert np.array_equal(t[kind]["hit"].cpu().numpy(), h), kind
+        z, sc = o.triplet_scores(e_gpu, f, s, elbow=(k > 0))
+        gz, gs = t[kind]["logit"].cpu().numpy(), t[kind]["score"].cpu().numpy()
+        if precision in ("fp32", "int8"):
+            assert np.array_equal(gz, z), kind
+            assert np.abs(gs - sc).max(initial=0) <= 1e-6
+        else:                                                  # same arithmetic on the FFMA pipe: also bit-exact
+            assert np.array_equal(gz, z), kind
+        total += f.size
+        assert f.size > 0 and 0.05 < np.mean(z >= 0) < 0.95, (kind, float(np.mean(z >= 0)))
+    print(f"{name}/{precision}: E={E} kept={int(keep.sum())} triplets={t['count']}")
+    # the full chain on the GPU's outputs: the oracle's four-phase track building runs on the GPU's triplets
+    tau_t = oracle.logit_threshold(cfg.triplet_threshold)
+    kept = {kind: (t[kind]["logit"].cpu().numpy() >= tau_t).astype(np.uint8) for kind in KINDS}
+    pair = lambda kind: (t[kind]["first"].cpu().numpy(), t[kind]["second"].cpu().numpy())
+    offs, hits = oracle.tracks_from_triplets(g["src"], g["dst"], keep, pair("articulation"), kept["articulation"],
+                                             pair("left_elbow"), kept["left_elbow"], pair("right_elbow"), kept["right_elbow"], 3)
+    assert offs.size > 1 and hits.max() < b.n_hits
+    ctx.destroy()
+
+
+def test_triplet_stage_final_state_equals_the_oracle_in_fp32():
+    # end to end in fp32: the final edge state the triplet classifiers read is the oracle's, bit for bit
+    cfg, b, blob = _setup("cfg0", 2, "fp32")
+    ctx = make_ctx(cfg, blob, b, max_triplets=1_000_000)
+    g = run_gpu(ctx, b, debug=False)
+    o = oracle.Oracle(blob, "fp32")
+    r = o.run(b.xyz, b.plane, b.event_offsets, cfg.k, cfg.window)
+    tr = o.run_triplets(b.xyz, r["src"], r["dst"], cfg.threshold, cfg.triplet_threshold)
+    assert np.array_equal(state(ctx, "e", g["n_edges"], cfg.gnn_latent), tr["e"])
+    t = ctx.triplets()
+    for kind in KINDS:
+        assert np.array_equal(t[kind]["first"].cpu().numpy(), tr[kind]["first"])
+        assert np.array_equal(t[kind]["logit"].cpu().numpy(), tr[kind]["logit"]), kind
+    ctx.destroy()
+
+
+def test_triplet_capacity_and_missing_classifiers():
+    import paper_2407_12119_b200 as etx
+    cfg, b, blob = _setup("cfg0", 1, "fp32")
+    ctx = make_ctx(cfg, blob, b, max_triplets=16)              # far too small: counts are true, lists truncated
+    g = run_gpu(ctx, b, debug=False)
+    t = ctx.triplets()
+    keep = (g["logit"] >= oracle.logit_threshold(cfg.threshold)).astype(np.uint8)
+    f, s, h = oracle.triplets(g["src"], g["dst"], keep, b.n_hits, "articulation")
+    assert t["count"][0] == f.size > 16 and t["articulation"]["first"].numel() == 16
+    assert np.array_equal(t["articulation"]["first"].cpu().numpy(), f[:16])
+    ctx.destroy()
+    cfg2 = cfg.replace(triplets=0)
+    ctx = make_ctx(cfg2, datagen.pack_blob(cfg2, datagen.make_weights(cfg2, "parity")), b, max_triplets=100)
+    run_gpu(ctx, b, debug=False)
+    with pytest.raises(etx.EtxError) as ei:
+        ctx.triplets()
+    assert ei.value.status == -2
+    ctx.destroy()
