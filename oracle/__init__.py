@@ -22,6 +22,7 @@ _FLAGS = ["-O3", "-std=c++17", "-mavx2", "-mfma", "-ffp-contract=off", "-fno-fas
           "-shared", "-fPIC"]
 
 PRECISION = {"fp32": 0, "bf16": 1, "int8": 2}
+STATE_DTYPE = {"auto": 0, "fp32": 1, "bf16": 2}     # storage of h, e, m; "bf16" only changes int8 mode (R21)
 
 
 def build(force: bool = False) -> str:
@@ -35,7 +36,8 @@ def build(force: bool = False) -> str:
 
 class _Params(C.Structure):
     _fields_ = [("n_planes", C.c_int32), ("norm_offset", C.c_float * 3), ("norm_div", C.c_float * 3),
-                ("precision", C.c_int32), ("cyl_offset", C.c_float * 3), ("cyl_div", C.c_float * 3)]
+                ("precision", C.c_int32), ("cyl_offset", C.c_float * 3), ("cyl_div", C.c_float * 3),
+                ("state_dtype", C.c_int32)]
 
 
 _lib = None
@@ -246,9 +248,10 @@ class Oracle:
 
     def __init__(self, blob: bytes, precision: str = "fp32", n_planes: int = 26,
                  norm_offset=(0.0, 0.0, 300.0), norm_div=(40.0, 40.0, 1050.0),
-                 cyl_offset=(-20.0, 0.0, 300.0), cyl_div=(12.0, 3.14159274, 1050.0)):
+                 cyl_offset=(-20.0, 0.0, 300.0), cyl_div=(12.0, 3.14159274, 1050.0), state_dtype: str = "auto"):
         prm = _Params(n_planes, (C.c_float * 3)(*norm_offset), (C.c_float * 3)(*norm_div),
-                      PRECISION[precision], (C.c_float * 3)(*cyl_offset), (C.c_float * 3)(*cyl_div))
+                      PRECISION[precision], (C.c_float * 3)(*cyl_offset), (C.c_float * 3)(*cyl_div),
+                      STATE_DTYPE[state_dtype])
         self._blob = bytes(blob)
         self._h = lib().etxo_create(self._blob, len(self._blob), C.byref(prm))
         err = lib().etxo_error(self._h).decode()

@@ -101,6 +101,7 @@ struct Model {
   int emb_hidden = 0, emb_layers_hidden = 0, emb_dim = 4;
   int latent = 0, iters = 0, edge_enc_input = 0;
   int precision = P_FP32;
+  int state_bf16 = 0;                   // h, e, m stored as bf16: always in bf16 mode; optional in int8 mode (R21)
   std::vector<Linear> emb;              // H+1 layers
   Linear nenc[2], eenc[2];
   std::vector<Linear> node, edge;       // 2 per iteration
@@ -163,9 +164,15 @@ inline void linear(Model& M, const Linear& L, const float* x, float* y, size_t r
 }
 
 inline void relu(float* v, int n) { for (int i = 0; i < n; ++i) v[i] = v[i] > 0.0f ? v[i] : 0.0f; }
-// Rounding point of bf16 mode: every tensor the GPU stores or feeds to an MMA (R20).
-inline void state_round(const Model& M, float* v, int n) {
+// Rounding points (R20).  operand_round: a hidden activation fed to a bf16 MMA (bf16 mode only; in int8 mode the
+// operand is the int8 code, quantised from the fp32 value).  state_round: a stored state row h / e / m -- bf16 in
+// bf16 mode, and in int8 mode when the state dtype is bf16 (R21: "if bf16 is adopted for bandwidth, mirror the RNE
+// rounding in the oracle").
+inline void operand_round(const Model& M, float* v, int n) {
   if (M.precision == P_BF16) for (int i = 0; i < n; ++i) v[i] = bf16_round(v[i]);
+}
+inline void state_round(const Model& M, float* v, int n) {
+  if (M.state_bf16) for (int i = 0; i < n; ++i) v[i] = bf16_round(v[i]);
 }
 
 // f = ((x,y,z) + offset) / div : one fp32 add, one correctly rounded fp32 division (R1; L107 fn.5)
@@ -294,11 +301,13 @@ struct etxo_params {
   int32_t precision;   // 0 fp32, 1 bf16-emulated, 2 int8
   float cyl_offset[3]; // used when the blob says emb_input = 1 (R27)
   float cyl_div[3];
+  int32_t state_dtype; // 0: fp32 for fp32 / int8, bf16 for bf16 (the defaults); 1: fp32; 2: bf16 (int8 mode only)
 };
 
 void* etxo_create(const void* blob, uint64_t bytes, const etxo_params* prm) {
   Model* M = new Model();
   M->precision = prm->precision;
+  M->state_bf16 = (prm->precision == P_BF16) || (prm->precision == P_INT8 && prm->state_dtype == 2);
   M->n_planes = prm->n_planes;
   for (int i = 0; i < 3; ++i) { M->norm_off[i] = prm->norm_offset[i]; M->norm_div[i] = prm->norm_div[i]; }
   for (int i = 0; i < 3; ++i) { M->cyl_off[i] = prm->cyl_offset[i]; M->cyl_div[i] = prm->cyl_div[i]; }
@@ -397,10 +406,10 @@ void etxo_embed(void* m, const float* xyz, int64_t n, float* emb) {
     float a[256], t[256], f[3];
     features_emb(M, xyz + 3 * i, f);
     linear(M, M.emb[0], f, a, (size_t)i);
-    relu(a, M.emb[0].out); state_round(M, a, M.emb[0].out);
+    relu(a, M.emb[0].out); operand_round(M, a, M.emb[0].out);
     for (int l = 1; l < H; ++l) {
       linear(M, M.emb[l], a, t, (size_t)i);
-      relu(t, M.emb[l].out); state_round(M, t, M.emb[l].out);
+      relu(t, M.emb[l].out); operand_round(M, t, M.emb[l].out);
       std::memcpy(a, t, sizeof(float) * M.emb[l].out);
     }
     linear(M, M.emb[H], a, emb + (size_t)i * M.emb_dim, (size_t)i);
@@ -499,7 +508,7 @@ void etxo_gnn(void* m, const float* xyz, int64_t n, const int32_t* src, const in
   for (int64_t i = 0; i < n; ++i) {                       // node encoder
     float a[96], t[96];
     linear(M, M.nenc[0], &f[3 * i], a, (size_t)i);
-    relu(a, d); state_round(M, a, d);
+    relu(a, d); operand_round(M, a, d);
     linear(M, M.nenc[1], a, t, (size_t)i);
     state_round(M, t, d);
     std::memcpy(&h[(size_t)i * d], t, sizeof(float) * d);
@@ -514,7 +523,7 @@ void etxo_gnn(void* m, const float* xyz, int64_t n, const int32_t* src, const in
       std::memcpy(x + d, &h[(size_t)dst[i] * d], sizeof(float) * d);
     }
     linear(M, M.eenc[0], x, a, (size_t)i);
-    relu(a, d); state_round(M, a, d);
+    relu(a, d); operand_round(M, a, d);
     linear(M, M.eenc[1], a, t, (size_t)i);
     state_round(M, t, d);
     std::memcpy(&e[(size_t)i * d], t, sizeof(float) * d);
@@ -529,8 +538,8 @@ void etxo_gnn(void* m, const float* xyz, int64_t n, const int32_t* src, const in
       const float* ee = &e[(size_t)i * d];
       for (int c = 0; c < d; ++c) { mo[c] += ee[c]; mi[c] += ee[c]; }
     }
-    // bf16 mode: the message is a tensor-core operand, rounded once after the fp32 sum (R20)
-    if (M.precision == P_BF16) for (size_t i = 0; i < msg.size(); ++i) msg[i] = bf16_round(msg[i]);
+    // bf16 state: the message is stored (and is a tensor-core operand), rounded once after the fp32 sum (R20)
+    if (M.state_bf16) for (size_t i = 0; i < msg.size(); ++i) msg[i] = bf16_round(msg[i]);
     if (m_dump && it == m_iter) std::memcpy(m_dump, msg.data(), sizeof(float) * msg.size());
 
 #pragma omp parallel for schedule(static)
@@ -539,7 +548,7 @@ void etxo_gnn(void* m, const float* xyz, int64_t n, const int32_t* src, const in
       std::memcpy(x, &h[(size_t)i * d], sizeof(float) * d);
       std::memcpy(x + d, &msg[(size_t)i * 2 * d], sizeof(float) * 2 * d);
       linear(M, M.node[2 * it], x, a, (size_t)i);
-      relu(a, d); state_round(M, a, d);
+      relu(a, d); operand_round(M, a, d);
       linear(M, M.node[2 * it + 1], a, t, (size_t)i);
       float* hh = &h[(size_t)i * d];
       for (int c = 0; c < d; ++c) hh[c] = hh[c] + t[c];   // residual, fp32 add (R14)
@@ -552,7 +561,7 @@ void etxo_gnn(void* m, const float* xyz, int64_t n, const int32_t* src, const in
       std::memcpy(x + d, &h[(size_t)dst[i] * d], sizeof(float) * d);
       std::memcpy(x + 2 * d, &e[(size_t)i * d], sizeof(float) * d);
       linear(M, M.edge[2 * it], x, a, (size_t)i);
-      relu(a, d); state_round(M, a, d);
+      relu(a, d); operand_round(M, a, d);
       linear(M, M.edge[2 * it + 1], a, t, (size_t)i);
       float* ee = &e[(size_t)i * d];
       for (int c = 0; c < d; ++c) ee[c] = ee[c] + t[c];
@@ -690,7 +699,7 @@ void etxo_triplet_scores(void* m, const float* e_state, const int32_t* t_first, 
     std::memcpy(x, e_state + (size_t)t_first[t] * d, sizeof(float) * d);
     std::memcpy(x + d, e_state + (size_t)t_second[t] * d, sizeof(float) * d);
     linear(M, L[0], x, a, (size_t)t);
-    relu(a, d); state_round(M, a, d);
+    relu(a, d); operand_round(M, a, d);
     linear(M, L[1], a, &z, (size_t)t);
     logit[t] = z;
     score[t] = (float)(1.0 / (1.0 + std::exp(-(double)z)));

@@ -283,3 +283,46 @@ def embed_restated(cfg, layers, f_emb, on_linear_input=None):
         if l < H:
             a = np.maximum(a, np.float32(0))
     return a
+
+
+def gnn_restated_int8(cfg, layers, scales, f, src, dst, state_bf16):
+    """PAPER.md L133-142 in INT8 mode (R21) written out with numpy: every Linear with K >= 16 except the
+    head quantises its input tensor (q = clamp(rne(x * (1 / s_x)), +-127), one fp32 multiply), multiplies integer
+    codes (int64 matmul) and dequantises with y = fma((float) acc, s_x * s_w[c], b[c]); the K = 3 layers and the head
+    are the pinned fp32 chain.  state_bf16: h, e and the message are rounded to bfloat16 (torch) when stored.
+    -> dict(h, e, logit)."""
+    F = np.float32
+    lay = {n: (W.astype(F), b.astype(F)) for n, W, b in layers}
+    qnames = [n for n, W, b in layers if W.shape[1] >= 16 and n not in ("head", "tart1", "telb1")]
+    sx = {n: F(s) for n, s in zip(qnames, scales)}
+    st = (lambda x: torch_bf16(x)) if state_bf16 else (lambda x: x)
+
+    def linear(name, x):
+        W, b = lay[name]
+        if name not in sx:
+            return f32_chain(x, W, b)
+        inv = F(1.0) / sx[name]
+        q = np.clip(np.rint((x.astype(F) * inv).astype(F)), -127, 127).astype(np.int64)
+        amax = np.abs(W).max(1)
+        sw = np.where(amax > 0, (amax / F(127)).astype(F), F(1.0)).astype(F)
+        Wq = np.clip(np.rint((W / sw[:, None]).astype(F)), -127, 127).astype(np.int64)
+        acc = q @ Wq.T
+        scale = (sx[name] * sw).astype(F)
+        return (acc.astype(np.float64) * scale.astype(np.float64)[None, :] + b.astype(np.float64)[None, :]).astype(F)
+
+    mlp = lambda n0, n1, x: linear(n1, np.maximum(linear(n0, x), F(0)))
+    f = np.asarray(f, F)
+    n, E, d = f.shape[0], src.size, cfg.gnn_latent
+    h = st(mlp("nenc0", "nenc1", f))
+    x = np.abs(f[dst] - f[src]) if cfg.edge_enc_input == 0 else np.concatenate([h[src], h[dst]], 1)
+    e = st(mlp("eenc0", "eenc1", x))
+    for it in range(cfg.gnn_iters):
+        m = np.zeros((n, 2 * d), F)
+        for i in range(E):
+            m[src[i], :d] = m[src[i], :d] + e[i]
+            m[dst[i], d:] = m[dst[i], d:] + e[i]
+        m = st(m)
+        h = st((h + mlp(f"node{it}_0", f"node{it}_1", np.concatenate([h, m], 1))).astype(F))
+        e = st((e + mlp(f"edge{it}_0", f"edge{it}_1", np.concatenate([h[src], h[dst], e], 1))).astype(F))
+    logit = f32_chain(e, *lay["head"])[:, 0]
+    return dict(h=h, e=e, logit=logit)

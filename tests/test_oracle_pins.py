@@ -738,3 +738,29 @@ def test_int8_activation_scales_equal_an_independent_recomputation_bit_for_bit()
     Z = zero_layers(cfg)
     z = oracle.calibrate_int8(datagen.pack_blob(cfg, Z), b.xyz, b.plane, b.event_offsets, cfg.k, cfg.window)
     assert z[names.index("emb1")] == 1.0
+
+
+@pytest.mark.parametrize("state", ["fp32", "bf16"])
+def test_int8_gnn_forward_and_bf16_state_rounding_equal_an_integer_matmul_restatement(state):
+    # R21 with both state dtypes: quantiser, integer accumulation, fma dequantisation, and -- for state_dtype = bf16
+    # -- RNE rounding of h, e and the message where they are stored, nowhere else.  Bit for bit.
+    from helpers import gnn_restated_int8
+    cfg = toy_config(d=16, L=2, precision="int8")
+    W = datagen.make_weights(cfg, "parity", seed=13)
+    xyz, src, dst = _tiny_graph(8, n=14, E=44)
+    b = datagen.generate_batch(datagen.get_config("cfg0"))
+    scales = oracle.calibrate_int8(datagen.pack_blob(cfg, W), b.xyz, b.plane, b.event_offsets, cfg.k, cfg.window)
+    blob = datagen.pack_blob(cfg, W, scales)
+    out = oracle.Oracle(blob, "int8", state_dtype=state).gnn(xyz, src, dst, want_states=True)
+    f = ((xyz + np.array(datagen.configs.NORM_OFFSET, F)) / np.array(datagen.configs.NORM_DIV, F)).astype(F)
+    ref = gnn_restated_int8(cfg, W, scales, f, src, dst, state_bf16=(state == "bf16"))
+    for key in ("h", "e", "logit"):
+        assert np.array_equal(out[key].view(np.uint32), ref[key].view(np.uint32)), key
+    other = gnn_restated_int8(cfg, W, scales, f, src, dst, state_bf16=(state != "bf16"))
+    assert not np.array_equal(out["logit"], other["logit"])
+    is_bf16 = np.array_equal(out["e"], torch.from_numpy(out["e"]).to(torch.bfloat16).to(torch.float32).numpy())
+    assert is_bf16 == (state == "bf16")
+    # "auto" is fp32 state in int8 mode
+    if state == "fp32":
+        auto = oracle.Oracle(blob, "int8").gnn(xyz, src, dst)
+        assert np.array_equal(auto["logit"], out["logit"])
