@@ -118,7 +118,7 @@ def int8_scales(cfg, layers):
 def stage_model(cfg, N, E, pairs, peaks):
     """Algorithmic bytes / flops per step for every stage -> {stage: (bound, work, peak, unit)}."""
     D, H, d, L, k = cfg.emb_hidden, cfg.emb_n_hidden_layers, cfg.gnn_latent, cfg.gnn_iters, cfg.k
-    b = 2 if cfg.precision == "bf16" else 4
+    b = 2 if (cfg.precision == "bf16" or (cfg.precision == "int8" and getattr(cfg, "state_dtype", "auto") == "bf16")) else 4
     tens = peaks["bf16_sustained"] * (2.0 if cfg.precision == "int8" else 1.0)      # int8 nominal = 2x bf16
     ffma = 148 * 128 * 2 * 1.965e9 / 1e12                                           # TFLOP/s at max clock
     mlp_peak, mlp_bound = (ffma, "alu") if cfg.precision == "fp32" else (tens, "tensor")
@@ -142,7 +142,7 @@ def stage_model(cfg, N, E, pairs, peaks):
 def run_oracle_sample(cfg, batch, layers, n_events, scales=None):
     import oracle
     sub = batch.slice_events(0, min(n_events, batch.n_events))
-    o = oracle.Oracle(datagen.pack_blob(cfg, layers, scales), cfg.precision)
+    o = oracle.Oracle(datagen.pack_blob(cfg, layers, scales), cfg.precision, state_dtype=getattr(cfg, "state_dtype", "auto"))
     t0 = time.perf_counter()
     o.run(sub.xyz, sub.plane, sub.event_offsets, cfg.k, cfg.window, cfg.d2_max, cfg.threshold)
     dt = time.perf_counter() - t0

@@ -45,6 +45,7 @@ class EtxConfig:
     edge_enc_input: int = 0     # 0: |f_dst - f_src| (configs), 1: [h0_src, h0_dst]
     emb_input: int = 0          # 0: the embedding reads the Cartesian features, 1: normalised (r, phi, z) (L96, R27)
     weights_seed: int = 7
+    state_dtype: str = "auto"   # storage of h, e, m: "auto" (fp32 for fp32 / int8, bf16 for bf16), "fp32", "bf16" (int8 only; R21)
     triplets: int = 0           # 1: the blob also carries the two triplet classifiers (R28)
     triplet_threshold: float = 0.5
 
@@ -70,11 +71,12 @@ CONFIGS: dict[str, EtxConfig] = {
                       mu_tracks=40.0, noise_frac=0.02, events_seed=1002,
                       emb_hidden=128, emb_n_hidden_layers=3, k=10, window=2,
                       gnn_latent=64, gnn_iters=6, precision="bf16", **_COMMON),
-    # cfg 3: 1000 events, INT8 MLPs
+    # cfg 3: 1000 events, INT8 MLPs; h, e, m stored as bf16 (R21: the config text fixes the arithmetic --
+    # int8 operands, int32 accumulation, fp32 dequantisation -- not the storage of the state)
     "cfg3": EtxConfig(name="cfg3", n_events=1000, fixed_pv=None, mu_pv=5.0, fixed_tracks=None,
                       mu_tracks=40.0, noise_frac=0.02, events_seed=1003,
                       emb_hidden=128, emb_n_hidden_layers=3, k=10, window=2,
-                      gnn_latent=64, gnn_iters=6, precision="int8", **_COMMON),
+                      gnn_latent=64, gnn_iters=6, precision="int8", state_dtype="bf16", **_COMMON),
     # cfg 4: high-occupancy stress, bf16
     "cfg4": EtxConfig(name="cfg4", n_events=200, fixed_pv=None, mu_pv=20.0, fixed_tracks=None,
                       mu_tracks=40.0, noise_frac=0.02, events_seed=1004,

@@ -47,6 +47,11 @@ typedef enum {
 
 typedef enum { ETX_FP32 = 0, ETX_BF16 = 1, ETX_INT8 = 2 } etx_precision;
 
+/* Storage of the GNN state h, e, m (R20 / R21).  AUTO: fp32 for ETX_FP32 and ETX_INT8,
+ * bf16 for ETX_BF16.  ETX_INT8 may also store it in bf16 (RNE on store, fp32 arithmetic on the widened values): half
+ * the HBM bytes of the S4 loop.  Other combinations are ETX_ERR_UNSUPPORTED. */
+typedef enum { ETX_STATE_AUTO = 0, ETX_STATE_FP32 = 1, ETX_STATE_BF16 = 2 } etx_state_dtype;
+
 /* How the MLP layers with K >= 16 are executed (the K = 3 input layers and the d->1 head are
  * always fp32 FFMA in a pinned order, R4/R20/R21). */
 typedef enum {
@@ -85,6 +90,7 @@ typedef struct {
                                         features (L133).                                                   */
   float    cyl_offset[3];
   float    cyl_div[3];
+  int32_t  state_dtype;              /* etx_state_dtype                                                                  */
   int32_t  max_triplets;             /* capacity per triplet kind of etx_triplets (0: the triplet stage is not used)     */
   float    triplet_threshold;        /* a triplet is kept iff its score >= this (L80: "triplets scoring below ... are
                                         discarded"; decided on the logit like the edge threshold, R17)                  */
@@ -222,7 +228,7 @@ etx_status etx_dbg_run(etx_handle h, const float* d_xyz, const int32_t* d_plane,
 /* Device pointer + byte size of an internal buffer of the last run: "plane_off", "emb", "nbr", "deg",
  * "row_ptr", "col_ptr", "in_edge", "h", "e", "m", "logit", "tap", "feat", "feat_emb".  "nbr" is [n_hits][k]; only the
  * first deg[q] slots of a row are defined.  h / e / m are in the
- * state dtype (fp32 for ETX_FP32 and ETX_INT8, bf16 for ETX_BF16).  "e" holds the final edge state e^L only after
+ * state dtype (etx_state_dtype; by default fp32 for ETX_FP32 and ETX_INT8, bf16 for ETX_BF16).  "e" holds the final edge state e^L only after
  * etx_dbg_run: in etx_run the last edge network feeds the fused classifier and does not write e^L back (the
  * tensor-core kernels; after etx_run "e" is then e^(L-1)). */
 etx_status etx_dbg_buffer(etx_handle h, const char* name, const void** d_ptr, size_t* bytes);

@@ -12,6 +12,7 @@ _HEADER = os.path.join(HERE, "..", "include", "etx.h")
 
 PRECISION = {"fp32": 0, "bf16": 1, "int8": 2}
 ENGINE = {"auto": 0, "simt": 1, "tc_serial": 2}
+STATE_DTYPE = {"auto": 0, "fp32": 1, "bf16": 2}
 STAGE_NAMES = ["S0_plane_offsets", "S1_embedding", "S2_knn", "S3_compaction_csc", "S4_encoders",
                "S4c_scatter", "S4d_node_net", "S4e_edge_net_head", "S5_components"]
 STATUS = {0: "ETX_OK", -1: "ETX_ERR_ARG", -2: "ETX_ERR_BLOB", -3: "ETX_ERR_CAPACITY", -4: "ETX_ERR_INPUT_ORDER",
@@ -36,7 +37,7 @@ class Hyperparams(C.Structure):
                 ("threshold", C.c_float), ("precision", C.c_int32), ("engine", C.c_int32),
                 ("max_events", C.c_int32), ("max_hits", C.c_int32), ("validate_input", C.c_int32),
                 ("emb_input", C.c_int32), ("cyl_offset", C.c_float * 3), ("cyl_div", C.c_float * 3),
-                ("max_triplets", C.c_int32), ("triplet_threshold", C.c_float),
+                ("state_dtype", C.c_int32), ("max_triplets", C.c_int32), ("triplet_threshold", C.c_float),
                 ("alloc", ALLOC_FN), ("dealloc", DEALLOC_FN), ("alloc_ctx", C.c_void_p)]
 
 
@@ -127,7 +128,7 @@ def lib():
 
 
 def hyperparams_from_config(cfg, max_events: int, max_hits: int, precision: str | None = None,
-                            engine: str = "auto", validate_input: bool = False, n_planes: int = 26, max_triplets: int = 0,
+                            engine: str = "auto", validate_input: bool = False, n_planes: int = 26, max_triplets: int = 0, state_dtype: str | None = None,
                             norm_offset=(0.0, 0.0, 300.0), norm_div=(40.0, 40.0, 1050.0),
                             cyl_offset=(-20.0, 0.0, 300.0), cyl_div=(12.0, 3.14159274, 1050.0)) -> Hyperparams:
     """etx_hyperparams from a datagen.EtxConfig-like object (attribute access only)."""
@@ -148,6 +149,7 @@ def hyperparams_from_config(cfg, max_events: int, max_hits: int, precision: str 
     hp.emb_input = getattr(cfg, "emb_input", 0)
     hp.cyl_offset = (C.c_float * 3)(*cyl_offset)
     hp.cyl_div = (C.c_float * 3)(*cyl_div)
+    hp.state_dtype = STATE_DTYPE[state_dtype if state_dtype is not None else getattr(cfg, "state_dtype", "auto")]
     hp.max_triplets = int(max_triplets)
     hp.triplet_threshold = float(getattr(cfg, "triplet_threshold", 0.5))
     return hp

@@ -331,7 +331,10 @@ etx_status etx_create(const void* blob, size_t blob_bytes, const etx_hyperparams
     return bail(ETX_ERR_UNSUPPORTED);
   if ((long long)hp->k * hp->max_hits > 0x7fffffffLL) return bail(ETX_ERR_CAPACITY);
   c->max_edges = hp->k * hp->max_hits;
-  c->state_bf16 = (hp->precision == ETX_BF16);
+  if (hp->state_dtype < 0 || hp->state_dtype > 2) return bail(ETX_ERR_ARG);
+  if ((hp->precision == ETX_FP32 && hp->state_dtype == ETX_STATE_BF16) || (hp->precision == ETX_BF16 && hp->state_dtype == ETX_STATE_FP32))
+    return bail(ETX_ERR_UNSUPPORTED);
+  c->state_bf16 = (hp->precision == ETX_BF16) || (hp->precision == ETX_INT8 && hp->state_dtype == ETX_STATE_BF16);
   if (hp->threshold <= 0.0f) c->tau = -INFINITY;
   else if (hp->threshold >= 1.0f) c->tau = INFINITY;
   else c->tau = (float)log((double)hp->threshold / (1.0 - (double)hp->threshold));      // R17

@@ -25,7 +25,7 @@ namespace {
 
 using namespace umma;
 
-constexpr int kI8E = 4;                                    // ring of fp32 edge-state tiles
+constexpr int kI8E = 4;                                    // ring of fp32 edge-state tiles (6 when the state is bf16: half the bytes per tile)
 constexpr int kI8A = 2;                                    // ring of int8 operand tiles
 constexpr int kI8EpiWarps = 8, kI8ProdWarps = 8;
 constexpr int kI8MmaWarp = kI8EpiWarps + kI8ProdWarps, kI8LoadWarp = kI8MmaWarp + 1, kI8StoreWarp = kI8MmaWarp + 2;
@@ -51,11 +51,11 @@ __device__ __forceinline__ uint32_t e_off(uint32_t r, uint32_t c4) {
 }
 
 struct I8Smem { int e, a, h, w0, w1, par, bar, total; };
-template <int D>
+template <int D, bool SB>
 __host__ __device__ constexpr I8Smem i8_layout() {
   I8Smem s{};
-  s.e = 0;                                   // kI8E x [128][D] fp32, as D/32 boxes [128][128 B]
-  s.a = s.e + kI8E * kRows * D * 4;          // kI8A x 3 K-blocks [128][D] int8
+  s.e = 0;                                   // NE x [128][D] state tile: fp32 as D/32 boxes [128][128 B], bf16 as one box [128][2 D B]
+  s.a = s.e + (SB ? 6 : kI8E) * kRows * D * (SB ? 2 : 4);   // kI8A x 3 K-blocks [128][D] int8
   s.h = s.a + kI8A * 3 * kRows * D;          // 2 x [128][D]: layer-1 operand per epilogue warpgroup
   s.w0 = s.h + 2 * kRows * D;                // W0 image: 3 K-blocks [D][D]
   s.w1 = s.w0 + 3 * D * D;                   // W1 image
@@ -67,21 +67,25 @@ __host__ __device__ constexpr I8Smem i8_layout() {
 
 // NODE = false: S4e over edges (self state e, K-block 2; gathered h[src], h[dst]);  NODE = true: S4d over hits
 // (self state h, K-block 0; m_out, m_in of the same row).
-template <int D, bool NODE>
+// SB: the state rows (h, e, m) are bf16 (state_dtype = bf16, R21): one TMA box per tile, half the bytes, a deeper ring;
+// values are widened to fp32 before every arithmetic step and rounded (RNE) only when the new state is stored.
+template <int D, bool NODE, bool SB>
 __global__ void __launch_bounds__(kI8Threads, 1) edge_net_i8_kernel(const __grid_constant__ CUtensorMap e_map, GnnArgs a) {
   constexpr int KB = D;                                      // bytes per int8 segment row = swizzle width (32 / 64)
   constexpr int CPR = KB / 16;                               // 16-byte chunks per segment row
   constexpr int BLK = kRows * KB;
   constexpr int STAGE = 3 * BLK;
-  constexpr int ETILE = kRows * D * 4;
-  constexpr I8Smem L = i8_layout<D>();
+  constexpr int NE = SB ? 6 : kI8E;                          // depth of the state ring
+  constexpr int SROW = D * (SB ? 2 : 4);                     // bytes per state row
+  constexpr int ETILE = kRows * SROW;
+  constexpr I8Smem L = i8_layout<D, SB>();
   constexpr uint32_t TMEM_COLS = 4 * D;                      // acc0[2] | acc1[2]
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
   float* par = reinterpret_cast<float*>(smem + L.par);
   float *scale0 = par, *bias0 = par + D, *scale1 = par + 2 * D, *bias1 = par + 3 * D, *headw = par + 4 * D;
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + L.bar);
-  uint64_t *e_full = bars, *e_free = bars + kI8E, *out_ready = bars + 2 * kI8E, *a_full = bars + 3 * kI8E,
+  uint64_t *e_full = bars, *e_free = bars + NE, *out_ready = bars + 2 * NE, *a_full = bars + 3 * NE,
            *a_empty = a_full + kI8A, *acc0_full = a_empty + kI8A, *hid_full = acc0_full + 2, *acc1_full = acc0_full + 4,
            *bar_w = acc0_full + 6;
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc0_full + 7);
@@ -92,7 +96,7 @@ __global__ void __launch_bounds__(kI8Threads, 1) edge_net_i8_kernel(const __grid
   constexpr int SELF = NODE ? 0 : 2, AUX0 = NODE ? 1 : 0, AUX1 = NODE ? 2 : 1;   // K-blocks of the A tile
 
   if (tid == 0) {
-    for (int s = 0; s < kI8E; ++s) { mbar_init(&e_full[s], 1); mbar_init(&e_free[s], 1); mbar_init(&out_ready[s], 128); }
+    for (int s = 0; s < NE; ++s) { mbar_init(&e_full[s], 1); mbar_init(&e_free[s], 1); mbar_init(&out_ready[s], 128); }
     for (int s = 0; s < kI8A; ++s) { mbar_init(&a_full[s], kI8ProdThreads); mbar_init(&a_empty[s], 1); }
     for (int g = 0; g < 2; ++g) { mbar_init(&acc0_full[g], 1); mbar_init(&hid_full[g], 128); mbar_init(&acc1_full[g], 1); }
     mbar_init(bar_w, 1);
@@ -115,6 +119,7 @@ __global__ void __launch_bounds__(kI8Threads, 1) edge_net_i8_kernel(const __grid
     const int pt = tid - kI8EpiWarps * 32;                   // 0 .. 255
     const float inv_sx0 = a.l0.inv_sx;
     const float* hbase = static_cast<const float*>(a.h);
+    const __nv_bfloat16* hbase16 = static_cast<const __nv_bfloat16*>(a.h);
     auto quant16 = [&](const float4& f0, const float4& f1, const float4& f2, const float4& f3) {
       uint4 q;
       q.x = pack_i8x4(quant_i8(f0.x, inv_sx0), quant_i8(f0.y, inv_sx0), quant_i8(f0.z, inv_sx0), quant_i8(f0.w, inv_sx0));
@@ -123,13 +128,21 @@ __global__ void __launch_bounds__(kI8Threads, 1) edge_net_i8_kernel(const __grid
       q.w = pack_i8x4(quant_i8(f3.x, inv_sx0), quant_i8(f3.y, inv_sx0), quant_i8(f3.z, inv_sx0), quant_i8(f3.w, inv_sx0));
       return q;
     };
+    auto quant16b = [&](const uint4& u0, const uint4& u1) {     // 16 bf16 values, widened exactly
+      uint4 q;
+      q.x = pack_i8x4(quant_i8(bf16_lo(u0.x), inv_sx0), quant_i8(bf16_hi(u0.x), inv_sx0), quant_i8(bf16_lo(u0.y), inv_sx0), quant_i8(bf16_hi(u0.y), inv_sx0));
+      q.y = pack_i8x4(quant_i8(bf16_lo(u0.z), inv_sx0), quant_i8(bf16_hi(u0.z), inv_sx0), quant_i8(bf16_lo(u0.w), inv_sx0), quant_i8(bf16_hi(u0.w), inv_sx0));
+      q.z = pack_i8x4(quant_i8(bf16_lo(u1.x), inv_sx0), quant_i8(bf16_hi(u1.x), inv_sx0), quant_i8(bf16_lo(u1.y), inv_sx0), quant_i8(bf16_hi(u1.y), inv_sx0));
+      q.w = pack_i8x4(quant_i8(bf16_lo(u1.z), inv_sx0), quant_i8(bf16_hi(u1.z), inv_sx0), quant_i8(bf16_lo(u1.w), inv_sx0), quant_i8(bf16_hi(u1.w), inv_sx0));
+      return q;
+    };
     int it = 0;
     for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
-      const int sa = it % kI8A, se = it % kI8E;
+      const int sa = it % kI8A, se = it % NE;
       uint8_t* st = smem + L.a + sa * STAGE;
       const uint8_t* es = smem + L.e + se * ETILE;
       bool first = true;
-      // item c = (row r, 16-byte chunk `piece` of the int8 row) = 16 consecutive fp32 of the source row
+      // item c = (row r, 16-byte chunk `piece` of the int8 row) = 16 consecutive values of the source row
 #pragma unroll
       for (int i = 0; i < (kRows * CPR + kI8ProdThreads - 1) / kI8ProdThreads; ++i) {
         const int c = i * kI8ProdThreads + pt;
@@ -137,6 +150,28 @@ __global__ void __launch_bounds__(kI8Threads, 1) edge_net_i8_kernel(const __grid
           const int r = c / CPR, piece = c % CPR;
           int grow = tile * kRows + r;
           if (grow >= n_rows) grow = n_rows - 1;              // dead rows of the last tile: any valid row (never stored)
+          if (SB) {
+            const uint4 *ps, *pd;
+            if (NODE) {
+              ps = reinterpret_cast<const uint4*>(static_cast<const __nv_bfloat16*>(a.m) + (size_t)grow * 2 * D + piece * 16);
+              pd = ps + D / 8;
+            } else {
+              const int js = __ldg(a.src + grow), jd = __ldg(a.dst + grow);
+              ps = reinterpret_cast<const uint4*>(hbase16 + (size_t)js * D + piece * 16);
+              pd = reinterpret_cast<const uint4*>(hbase16 + (size_t)jd * D + piece * 16);
+            }
+            const uint4 s0 = __ldg(ps), s1 = __ldg(ps + 1), d0 = __ldg(pd), d1 = __ldg(pd + 1);
+            if (first) {                                      // the gathers are in flight while we wait for the slots
+              mbar_wait(&a_empty[sa], ((it / kI8A) & 1) ^ 1);
+              mbar_wait(&e_full[se], (it / NE) & 1);
+              first = false;
+            }
+            const uint4 e0 = *reinterpret_cast<const uint4*>(es + swz<SROW>(r, piece * 2 + 0));
+            const uint4 e1 = *reinterpret_cast<const uint4*>(es + swz<SROW>(r, piece * 2 + 1));
+            *reinterpret_cast<uint4*>(st + SELF * BLK + swz<KB>(r, piece)) = quant16b(e0, e1);
+            *reinterpret_cast<uint4*>(st + AUX0 * BLK + swz<KB>(r, piece)) = quant16b(s0, s1);
+            *reinterpret_cast<uint4*>(st + AUX1 * BLK + swz<KB>(r, piece)) = quant16b(d0, d1);
+          } else {
           const float4 *ps, *pd;
           if (NODE) {
             ps = reinterpret_cast<const float4*>(static_cast<const float*>(a.m) + (size_t)grow * 2 * D + piece * 16);
@@ -150,7 +185,7 @@ __global__ void __launch_bounds__(kI8Threads, 1) edge_net_i8_kernel(const __grid
           const float4 d0 = __ldg(pd), d1 = __ldg(pd + 1), d2 = __ldg(pd + 2), d3 = __ldg(pd + 3);
           if (first) {                                        // the gathers are in flight while we wait for the slots
             mbar_wait(&a_empty[sa], ((it / kI8A) & 1) ^ 1);
-            mbar_wait(&e_full[se], (it / kI8E) & 1);
+            mbar_wait(&e_full[se], (it / NE) & 1);
             first = false;
           }
           const float4 e0 = *reinterpret_cast<const float4*>(es + e_off(r, piece * 4 + 0));
@@ -160,9 +195,10 @@ __global__ void __launch_bounds__(kI8Threads, 1) edge_net_i8_kernel(const __grid
           *reinterpret_cast<uint4*>(st + SELF * BLK + swz<KB>(r, piece)) = quant16(e0, e1, e2, e3);
           *reinterpret_cast<uint4*>(st + AUX0 * BLK + swz<KB>(r, piece)) = quant16(s0, s1, s2, s3);
           *reinterpret_cast<uint4*>(st + AUX1 * BLK + swz<KB>(r, piece)) = quant16(d0, d1, d2, d3);
+          }
         }
       }
-      if (first) { mbar_wait(&a_empty[sa], ((it / kI8A) & 1) ^ 1); mbar_wait(&e_full[se], (it / kI8E) & 1); }
+      if (first) { mbar_wait(&a_empty[sa], ((it / kI8A) & 1) ^ 1); mbar_wait(&e_full[se], (it / NE) & 1); }
       fence_proxy_async();                                    // generic-proxy writes -> visible to the tensor core
       mbar_arrive(&a_full[sa]);
     }
@@ -171,11 +207,14 @@ __global__ void __launch_bounds__(kI8Threads, 1) edge_net_i8_kernel(const __grid
     if (lane == 0) {
       int it = 0;
       for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
-        const int s = it % kI8E;
-        mbar_wait(&e_free[s], ((it / kI8E) & 1) ^ 1);
+        const int s = it % NE;
+        mbar_wait(&e_free[s], ((it / NE) & 1) ^ 1);
         mbar_expect_tx(&e_full[s], ETILE);
+        if (SB) tma_load_2d(e_addr + s * ETILE, &e_map, 0, tile * kRows, &e_full[s]);
+        else {
 #pragma unroll
-        for (int b = 0; b < D / 32; ++b) tma_load_2d(e_addr + s * ETILE + b * kI8Sub, &e_map, 32 * b, tile * kRows, &e_full[s]);
+          for (int b = 0; b < D / 32; ++b) tma_load_2d(e_addr + s * ETILE + b * kI8Sub, &e_map, 32 * b, tile * kRows, &e_full[s]);
+        }
       }
     }
   } else if (warp == kI8StoreWarp) {
@@ -183,11 +222,14 @@ __global__ void __launch_bounds__(kI8Threads, 1) edge_net_i8_kernel(const __grid
     if (lane == 0) {
       int it = 0;
       for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
-        const int s = it % kI8E;
-        mbar_wait(&out_ready[s], (it / kI8E) & 1);
+        const int s = it % NE;
+        mbar_wait(&out_ready[s], (it / NE) & 1);
         if (a.do_head != 2) {                                 // 2: the new state is dead (last step of a plain etx_run)
+          if (SB) tma_store_2d(&e_map, e_addr + s * ETILE, 0, tile * kRows);
+          else {
 #pragma unroll
-          for (int b = 0; b < D / 32; ++b) tma_store_2d(&e_map, e_addr + s * ETILE + b * kI8Sub, 32 * b, tile * kRows);
+            for (int b = 0; b < D / 32; ++b) tma_store_2d(&e_map, e_addr + s * ETILE + b * kI8Sub, 32 * b, tile * kRows);
+          }
           asm volatile("cp.async.bulk.commit_group;" ::: "memory");
           asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
         }
@@ -240,7 +282,7 @@ __global__ void __launch_bounds__(kI8Threads, 1) edge_net_i8_kernel(const __grid
       const long long tile = blockIdx.x + (long long)it * gridDim.x;
       const long long row = tile * kRows + r;
       const bool live = row < n_rows;
-      uint8_t* es = smem + L.e + (it % kI8E) * ETILE;         // this tile's fp32 edge state, updated in place
+      uint8_t* es = smem + L.e + (it % NE) * ETILE;           // this tile's edge state, updated in place
       // ---- epilogue 0: relu(fmaf(acc0, s_x s_w, b0)) -> int8 codes -> layer-1 operand (R21)
       mbar_wait(&acc0_full[g], j & 1);
       tc_fence_after();
@@ -268,6 +310,29 @@ __global__ void __launch_bounds__(kI8Threads, 1) edge_net_i8_kernel(const __grid
 #pragma unroll
           for (int jj = 0; jj < 32; ++jj) tap1[c0 + jj] = (int)v[jj];
         }
+        if (SB) {
+#pragma unroll
+          for (int ch = 0; ch < 4; ++ch) {                    // 8 columns = one 16-byte chunk of the bf16 row
+            const int c = c0 + ch * 8;
+            uint4* p = reinterpret_cast<uint4*>(es + swz<SROW>(r, c / 8));
+            const uint4 o = *p;
+            float y[8];
+#pragma unroll
+            for (int jj = 0; jj < 8; ++jj) y[jj] = __fmaf_rn((float)(int)v[ch * 8 + jj], scale1[c + jj], bias1[c + jj]);
+            uint4 qv;                                         // fp32 residual add on the widened old state, RNE on store (R14, R21)
+            qv.x = pack_bf16x2(__fadd_rn(bf16_lo(o.x), y[0]), __fadd_rn(bf16_hi(o.x), y[1]));
+            qv.y = pack_bf16x2(__fadd_rn(bf16_lo(o.y), y[2]), __fadd_rn(bf16_hi(o.y), y[3]));
+            qv.z = pack_bf16x2(__fadd_rn(bf16_lo(o.z), y[4]), __fadd_rn(bf16_hi(o.z), y[5]));
+            qv.w = pack_bf16x2(__fadd_rn(bf16_lo(o.w), y[6]), __fadd_rn(bf16_hi(o.w), y[7]));
+            *p = qv;
+            if (!NODE && a.do_head) {                         // the classifier sees the stored (rounded) state, ascending j (R16)
+              hacc = __fmaf_rn(bf16_lo(qv.x), headw[c + 0], hacc); hacc = __fmaf_rn(bf16_hi(qv.x), headw[c + 1], hacc);
+              hacc = __fmaf_rn(bf16_lo(qv.y), headw[c + 2], hacc); hacc = __fmaf_rn(bf16_hi(qv.y), headw[c + 3], hacc);
+              hacc = __fmaf_rn(bf16_lo(qv.z), headw[c + 4], hacc); hacc = __fmaf_rn(bf16_hi(qv.z), headw[c + 5], hacc);
+              hacc = __fmaf_rn(bf16_lo(qv.w), headw[c + 6], hacc); hacc = __fmaf_rn(bf16_hi(qv.w), headw[c + 7], hacc);
+            }
+          }
+        } else
 #pragma unroll
         for (int ch = 0; ch < 8; ++ch) {
           const int c = c0 + ch * 4;
@@ -287,7 +352,7 @@ __global__ void __launch_bounds__(kI8Threads, 1) edge_net_i8_kernel(const __grid
       }
       tc_fence_before();                                      // acc1[g] may be overwritten after our next hid_full arrive
       fence_proxy_async();                                    // generic-proxy writes -> visible to the TMA store
-      mbar_arrive(&out_ready[it % kI8E]);
+      mbar_arrive(&out_ready[it % NE]);
       if (!NODE && a.do_head && live) {
         const float z = __fadd_rn(hacc, head_b);
         a.logit[row] = z;
@@ -304,10 +369,10 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
-template <int D, bool NODE>
+template <int D, bool NODE, bool SB>
 void edge_i8_launch(etx_ctx* c, const GnnArgs& a, int max_rows, cudaStream_t s) {
-  auto kern = edge_net_i8_kernel<D, NODE>;
-  constexpr int smem = i8_layout<D>().total + 1024;
+  auto kern = edge_net_i8_kernel<D, NODE, SB>;
+  constexpr int smem = i8_layout<D, SB>().total + 1024;
   opt_in_smem(c, kern, smem);
   const int tiles = (max_rows + kRows - 1) / kRows;
   const int grid = tiles < c->sm_count ? tiles : c->sm_count;     // one persistent CTA per SM
@@ -327,16 +392,18 @@ bool edge_i8_configure(etx_ctx* c) {
   cudaDriverEntryPointQueryResult qres;
   if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn) return false;
   const int D = c->hp.gnn_latent;
-  const cuuint64_t gstride[1] = {(cuuint64_t)D * 4};
-  const cuuint32_t box[2] = {32, (cuuint32_t)kRows};
+  const bool sb = c->state_bf16;
+  const cuuint64_t gstride[1] = {(cuuint64_t)D * (sb ? 2 : 4)};
+  const cuuint32_t box[2] = {sb ? (cuuint32_t)D : 32u, (cuuint32_t)kRows};   // fp32: boxes of 32 floats; bf16: the whole row
   const cuuint32_t estr[2] = {1, 1};
   for (int node = 0; node < 2; ++node) {
     const long long rows = node ? c->hp.max_hits : c->max_edges;
     const cuuint64_t gdim[2] = {(cuuint64_t)D, rows > 0 ? (cuuint64_t)rows : 1};
     CUtensorMap map;
     const CUresult r = reinterpret_cast<EncodeTiledFn>(fn)(
-        &map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, node ? c->h : c->e, gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-        CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        &map, sb ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, node ? c->h : c->e, gdim, gstride, box, estr,
+        CU_TENSOR_MAP_INTERLEAVE_NONE, (sb && D == 32) ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_128B,
+        CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return false;
     memcpy(node ? c->h_map : c->e_map, &map, sizeof(map));
   }
@@ -350,16 +417,16 @@ void launch_edge_net_i8(etx_ctx* c, int iter, int n_hits, bool do_head, cudaStre
   if (do_head && !c->keep_final_state) a.do_head = 2;        // e^L feeds only the classifier: do not write it back
   const long long max_rows_ll = (long long)n_hits * c->hp.k;
   const int max_rows = (int)(max_rows_ll > 0x7fffffff ? 0x7fffffff : max_rows_ll);
-  if (c->hp.gnn_latent == 32) edge_i8_launch<32, false>(c, a, max_rows, s);
-  else edge_i8_launch<64, false>(c, a, max_rows, s);
+  if (c->state_bf16) { if (c->hp.gnn_latent == 32) edge_i8_launch<32, false, true>(c, a, max_rows, s); else edge_i8_launch<64, false, true>(c, a, max_rows, s); }
+  else { if (c->hp.gnn_latent == 32) edge_i8_launch<32, false, false>(c, a, max_rows, s); else edge_i8_launch<64, false, false>(c, a, max_rows, s); }
 }
 
 // S4d in INT8 mode: the same kernel over hits (self state h, second and third segment m_out, m_in)
 void launch_node_net_i8(etx_ctx* c, int iter, int n_hits, cudaStream_t s) {
   GnnArgs a;
   fill_gnn_args(c, kNodeNet, iter, n_hits, false, a);
-  if (c->hp.gnn_latent == 32) edge_i8_launch<32, true>(c, a, n_hits, s);
-  else edge_i8_launch<64, true>(c, a, n_hits, s);
+  if (c->state_bf16) { if (c->hp.gnn_latent == 32) edge_i8_launch<32, true, true>(c, a, n_hits, s); else edge_i8_launch<64, true, true>(c, a, n_hits, s); }
+  else { if (c->hp.gnn_latent == 32) edge_i8_launch<32, true, false>(c, a, n_hits, s); else edge_i8_launch<64, true, false>(c, a, n_hits, s); }
 }
 
 }  // namespace etx

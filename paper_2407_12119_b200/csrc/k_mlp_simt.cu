@@ -379,6 +379,7 @@ template <int D>
 static void gnn_launch_d(etx_ctx* c, int kind, const GnnArgs& a, int max_rows, cudaStream_t s) {
   if (c->precision == ETX_FP32) gnn_launch_kind<kModeF32, float, D>(c, kind, a, max_rows, s);
   else if (c->precision == ETX_BF16) gnn_launch_kind<kModeBf16, __nv_bfloat16, D>(c, kind, a, max_rows, s);
+  else if (c->state_bf16) gnn_launch_kind<kModeInt8, __nv_bfloat16, D>(c, kind, a, max_rows, s);   // R21 with state_dtype = bf16
   else gnn_launch_kind<kModeInt8, float, D>(c, kind, a, max_rows, s);
 }
 
@@ -533,6 +534,7 @@ void launch_triplet_classifier(etx_ctx* c, int kind, cudaStream_t s) {
 #define ETX_TRIP(MODE, ST) { if (c->hp.gnn_latent == 32) trip_launch<MODE, ST, 32>(c, a, s); else trip_launch<MODE, ST, 64>(c, a, s); }
   if (c->precision == ETX_FP32) ETX_TRIP(kModeF32, float)
   else if (c->precision == ETX_BF16) ETX_TRIP(kModeBf16, __nv_bfloat16)
+  else if (c->state_bf16) ETX_TRIP(kModeInt8, __nv_bfloat16)
   else ETX_TRIP(kModeInt8, float)
 #undef ETX_TRIP
 }

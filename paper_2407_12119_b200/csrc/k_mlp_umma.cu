@@ -48,8 +48,10 @@ __host__ __device__ constexpr UmmaGnnSmem gnn_smem_layout() {
   return s;
 }
 
-template <int KIND, int PREC, int D>
+// SB: the state rows h / e / m are bf16 (always in bf16 mode; in int8 mode when state_dtype = bf16, R21)
+template <int KIND, int PREC, int D, bool SB>
 __global__ void __launch_bounds__(kUmmaThreads) gnn_mlp_umma_kernel(GnnArgs a) {
+  static_assert(PREC != kBf16 || SB, "bf16 precision stores bf16 state");
   constexpr int ESZ = PREC == kBf16 ? 2 : 1;
   constexpr int KB = D * ESZ;                                // swizzle width = segment bytes (32 / 64 / 128)
   constexpr int CPR = KB / 16;                               // 16-byte chunks per segment row
@@ -127,6 +129,27 @@ __global__ void __launch_bounds__(kUmmaThreads) gnn_mlp_umma_kernel(GnnArgs a) {
             uint4 v = make_uint4(0u, 0u, 0u, 0u);
             if (row0 + r < n_rows) v = __ldg(reinterpret_cast<const uint4*>(base + srow * stride_el + col0) + piece);
             *reinterpret_cast<uint4*>(blk + swz<KB>(r, piece)) = v;
+          }
+        } else if (SB) {
+          const __nv_bfloat16* base; int stride_el;          // state rows are bf16: widen, quantise while gathering
+#pragma unroll
+          for (int i = 0; i < CPR; ++i) {
+            const int c = i * kUmmaThreads + tid, r = c / CPR, piece = c % CPR;
+            size_t srow;
+            if (KIND == kNodeNet) { base = static_cast<const __nv_bfloat16*>(s == 0 ? a.h : a.m); stride_el = s == 0 ? D : 2 * D; srow = (size_t)(row0 + r); }
+            else if (s == 2) { base = static_cast<const __nv_bfloat16*>(a.e); stride_el = D; srow = (size_t)(row0 + r); }
+            else { base = static_cast<const __nv_bfloat16*>(a.h); stride_el = D; srow = (size_t)IDX[s * kRows + r]; }
+            const int col0 = (KIND == kNodeNet && s == 2) ? D : 0;
+            uint4 q = make_uint4(0u, 0u, 0u, 0u);
+            if (row0 + r < n_rows) {
+              const uint4* p = reinterpret_cast<const uint4*>(base + srow * stride_el + col0 + piece * 16);
+              const uint4 u0 = __ldg(p), u1 = __ldg(p + 1);
+              q.x = pack_i8x4(quant_i8(bf16_lo(u0.x), inv_sx0), quant_i8(bf16_hi(u0.x), inv_sx0), quant_i8(bf16_lo(u0.y), inv_sx0), quant_i8(bf16_hi(u0.y), inv_sx0));
+              q.y = pack_i8x4(quant_i8(bf16_lo(u0.z), inv_sx0), quant_i8(bf16_hi(u0.z), inv_sx0), quant_i8(bf16_lo(u0.w), inv_sx0), quant_i8(bf16_hi(u0.w), inv_sx0));
+              q.z = pack_i8x4(quant_i8(bf16_lo(u1.x), inv_sx0), quant_i8(bf16_hi(u1.x), inv_sx0), quant_i8(bf16_lo(u1.y), inv_sx0), quant_i8(bf16_hi(u1.y), inv_sx0));
+              q.w = pack_i8x4(quant_i8(bf16_lo(u1.z), inv_sx0), quant_i8(bf16_hi(u1.z), inv_sx0), quant_i8(bf16_lo(u1.w), inv_sx0), quant_i8(bf16_hi(u1.w), inv_sx0));
+            }
+            *reinterpret_cast<uint4*>(blk + swz<KB>(r, piece)) = q;
           }
         } else {
           const float* base; int stride_el;                  // state rows are fp32: quantise while gathering
@@ -226,13 +249,15 @@ __global__ void __launch_bounds__(kUmmaThreads) gnn_mlp_umma_kernel(GnnArgs a) {
           for (int j = 0; j < 32; ++j) tap_row[c0 + j] = (int)v[j];
         }
         if (live) {
-          if (PREC == kBf16) {
+          if (SB) {
             __nv_bfloat16* srow = static_cast<__nv_bfloat16*>(state) + (size_t)row * D + c0;
 #pragma unroll
             for (int ch = 0; ch < 4; ++ch) {
-              if (residual) {       // the old state row is the e / h segment of the A tile (already in shared memory)
+              if (residual) {       // bf16 precision: the old state row is the e / h segment of the A tile (already in
+                                    // shared memory); int8 precision: the A tile holds codes, re-read the row itself
                 const int sseg = (KIND == kNodeNet) ? 0 : 2;
-                const uint4 o = *reinterpret_cast<const uint4*>(A + sseg * (kRows * KB) + swz<KB>(tid, (c0 * 2) / 16 + ch));
+                const uint4 o = PREC == kBf16 ? *reinterpret_cast<const uint4*>(A + sseg * (kRows * KB) + swz<KB>(tid, (c0 * 2) / 16 + ch))
+                                              : *reinterpret_cast<const uint4*>(srow + ch * 8);
                 y[ch * 8 + 0] = __fadd_rn(bf16_lo(o.x), y[ch * 8 + 0]); y[ch * 8 + 1] = __fadd_rn(bf16_hi(o.x), y[ch * 8 + 1]);
                 y[ch * 8 + 2] = __fadd_rn(bf16_lo(o.y), y[ch * 8 + 2]); y[ch * 8 + 3] = __fadd_rn(bf16_hi(o.y), y[ch * 8 + 3]);
                 y[ch * 8 + 4] = __fadd_rn(bf16_lo(o.z), y[ch * 8 + 4]); y[ch * 8 + 5] = __fadd_rn(bf16_hi(o.z), y[ch * 8 + 5]);
@@ -442,9 +467,9 @@ std::vector<uint8_t> pack_weight_image(const std::vector<float>& w, int N, int K
   return img;
 }
 
-template <int KIND, int PREC, int D>
+template <int KIND, int PREC, int D, bool SB>
 void gnn_umma_launch_one(etx_ctx* c, const GnnArgs& a, int max_rows, cudaStream_t s) {
-  auto kern = gnn_mlp_umma_kernel<KIND, PREC, D>;
+  auto kern = gnn_mlp_umma_kernel<KIND, PREC, D, SB>;
   constexpr int smem = gnn_smem_layout<PREC, D>().total + 1024;
   opt_in_smem(c, kern, smem);
   const int tiles = (max_rows + kRows - 1) / kRows;
@@ -458,13 +483,13 @@ void gnn_umma_launch_one(etx_ctx* c, const GnnArgs& a, int max_rows, cudaStream_
   c->launches++;
 }
 
-template <int PREC, int D>
+template <int PREC, int D, bool SB>
 void gnn_umma_launch_kind(etx_ctx* c, int kind, const GnnArgs& a, int max_rows, cudaStream_t s) {
   switch (kind) {
-    case kNodeEnc: gnn_umma_launch_one<kNodeEnc, PREC, D>(c, a, max_rows, s); break;
-    case kEdgeEnc: gnn_umma_launch_one<kEdgeEnc, PREC, D>(c, a, max_rows, s); break;
-    case kNodeNet: gnn_umma_launch_one<kNodeNet, PREC, D>(c, a, max_rows, s); break;
-    default:       gnn_umma_launch_one<kEdgeNet, PREC, D>(c, a, max_rows, s); break;
+    case kNodeEnc: gnn_umma_launch_one<kNodeEnc, PREC, D, SB>(c, a, max_rows, s); break;
+    case kEdgeEnc: gnn_umma_launch_one<kEdgeEnc, PREC, D, SB>(c, a, max_rows, s); break;
+    case kNodeNet: gnn_umma_launch_one<kNodeNet, PREC, D, SB>(c, a, max_rows, s); break;
+    default:       gnn_umma_launch_one<kEdgeNet, PREC, D, SB>(c, a, max_rows, s); break;
   }
 }
 
@@ -528,8 +553,9 @@ void launch_gnn_mlp_umma(etx_ctx* c, int kind, int iter, int n_hits, bool do_hea
   const long long max_rows_ll = is_edge ? (long long)n_hits * c->hp.k : n_hits;
   const int max_rows = (int)(max_rows_ll > 0x7fffffff ? 0x7fffffff : max_rows_ll);
   const int d = c->hp.gnn_latent;
-  if (c->precision == ETX_BF16) { if (d == 32) gnn_umma_launch_kind<kBf16, 32>(c, kind, a, max_rows, s); else gnn_umma_launch_kind<kBf16, 64>(c, kind, a, max_rows, s); }
-  else { if (d == 32) gnn_umma_launch_kind<kInt8, 32>(c, kind, a, max_rows, s); else gnn_umma_launch_kind<kInt8, 64>(c, kind, a, max_rows, s); }
+  if (c->precision == ETX_BF16) { if (d == 32) gnn_umma_launch_kind<kBf16, 32, true>(c, kind, a, max_rows, s); else gnn_umma_launch_kind<kBf16, 64, true>(c, kind, a, max_rows, s); }
+  else if (c->state_bf16) { if (d == 32) gnn_umma_launch_kind<kInt8, 32, true>(c, kind, a, max_rows, s); else gnn_umma_launch_kind<kInt8, 64, true>(c, kind, a, max_rows, s); }
+  else { if (d == 32) gnn_umma_launch_kind<kInt8, 32, false>(c, kind, a, max_rows, s); else gnn_umma_launch_kind<kInt8, 64, false>(c, kind, a, max_rows, s); }
 }
 
 }  // namespace etx

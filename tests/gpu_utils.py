@@ -52,6 +52,6 @@ def run_gpu(ctx, batch, emb=None, src=None, dst=None, logit=None, last_stage=5, 
 
 def state(ctx, name, rows, d):
     """h / e / m as float32 numpy [rows, d] whatever the state dtype."""
-    bf16 = ctx.hp.precision == 1
+    bf16 = ctx.hp.precision == 1 or (ctx.hp.precision == 2 and ctx.hp.state_dtype == 2)
     t = ctx.buffer(name, torch.bfloat16 if bf16 else torch.float32)
     return t.float().cpu().numpy().reshape(rows, d)

@@ -139,7 +139,7 @@ def test_full_size_int8_cfg3_bit_exact_on_sampled_events():
     ctx = make_ctx(cfg, blob, b)
     g = run_gpu(ctx, b, debug=False)
     _whole_batch_invariants(cfg, b, g)
-    o = oracle.Oracle(blob, "int8")
+    o = oracle.Oracle(blob, "int8", state_dtype=cfg.state_dtype)      # cfg 3 stores the state as bf16 (R21)
     eo, rp = b.event_offsets, g["row_ptr"]
     events = _sample_events(b, n_random=2)
     for ev in events:

@@ -25,7 +25,7 @@ def _setup(name, n_events=None, preset="parity", precision=None, seed=None):
 
 
 def _oracle_all(cfg, b, blob, precision):
-    o = oracle.Oracle(blob, precision)
+    o = oracle.Oracle(blob, precision, state_dtype=cfg.state_dtype)
     r = o.run(b.xyz, b.plane, b.event_offsets, cfg.k, cfg.window, cfg.d2_max, cfg.threshold)
     r["col_ptr"], r["in_edge"] = oracle.csc(r["dst"], b.n_hits)
     return o, r
@@ -522,6 +522,48 @@ def test_int8_tensor_core_path_is_bit_exact_end_to_end(name, n_events):
     g2 = run_gpu(ctx, b)
     assert np.array_equal(state(ctx, "e", r["src"].size, cfg.gnn_latent), og["e"])
     assert np.array_equal(g2["logit"], g["logit"]) and np.array_equal(g2["track_id"], g["track_id"])
+
+
+@pytest.mark.parametrize("name,n_events,engine", [("cfg1", 3, "auto"), ("cfg0", 1, "auto"), ("cfg1", 2, "simt"), ("cfg1", 2, "tc_serial"),
+                                                  ("cfg5", 1, "auto")])
+def test_int8_with_bf16_state_is_bit_exact_end_to_end(name, n_events, engine):
+    # state_dtype = bf16 in INT8 mode (R21 / SURVEY A21): h, e, m are stored as bf16 (RNE), every arithmetic step is
+    # still the pinned fp32 / integer one, so all three engines must reproduce the oracle bit for bit
+    cfg, b, W = _setup(name, n_events, precision="int8")
+    cfg = cfg.replace(state_dtype="bf16")
+    scales = oracle.calibrate_int8(datagen.pack_blob(cfg, W), b.xyz, b.plane, b.event_offsets, cfg.k, cfg.window, cfg.d2_max)
+    blob = datagen.pack_blob(cfg, W, scales)
+    o, r = _oracle_all(cfg, b, blob, "int8")
+    og = o.gnn(b.xyz, r["src"], r["dst"], want_states=True)
+    ctx = make_ctx(cfg, blob, b, engine=engine)
+    g = run_gpu(ctx, b, debug=False)
+    assert np.array_equal(g["emb"], r["emb"])
+    assert np.array_equal(g["src"], r["src"]) and np.array_equal(g["dst"], r["dst"])
+    assert np.array_equal(state(ctx, "h", b.n_hits, cfg.gnn_latent), og["h"])
+    assert np.array_equal(g["logit"], r["logit"])
+    assert np.array_equal(g["track_id"], r["track_id"])
+    g2 = run_gpu(ctx, b)                                           # etx_dbg_run writes e^L back
+    assert np.array_equal(state(ctx, "e", r["src"].size, cfg.gnn_latent), og["e"])
+    assert np.array_equal(state(ctx, "m", b.n_hits, 2 * cfg.gnn_latent),
+                          o.gnn(b.xyz, r["src"], r["dst"], m_iter=cfg.gnn_iters - 1)["m"])
+    assert np.array_equal(g2["logit"], g["logit"])
+    # the stored state really is bf16, and it differs from the fp32-state result
+    e = state(ctx, "e", r["src"].size, cfg.gnn_latent)
+    assert np.array_equal(e, torch.from_numpy(e).to(torch.bfloat16).float().numpy())
+    r32 = oracle.Oracle(blob, "int8").run(b.xyz, b.plane, b.event_offsets, cfg.k, cfg.window, cfg.d2_max, cfg.threshold)
+    assert not np.array_equal(r32["logit"], r["logit"])
+    # int32 accumulators of the production kernels (AUTO engine) with the bf16 state
+    if engine == "auto" and name == "cfg1":
+        names = [n for n, _, _ in datagen.layer_shapes(cfg)]
+        for lname, rows in (("node1_0", b.n_hits), ("edge2_0", r["src"].size), ("edge5_1", r["src"].size), ("eenc1", r["src"].size)):
+            li = names.index(lname)
+            tap = np.zeros((rows, cfg.gnn_latent), np.int32)
+            o.set_tap(li, tap); o.gnn(b.xyz, r["src"], r["dst"]); o.set_tap(-1, None)
+            ctx.tap_layer(li)
+            run_gpu(ctx, b, debug=False)
+            got = ctx.buffer("tap", torch.int32).cpu().numpy()[: rows * cfg.gnn_latent].reshape(rows, cfg.gnn_latent)
+            ctx.tap_layer(-1)
+            assert np.array_equal(got, tap), lname
 
 
 def test_int8_tensor_core_accumulators_bit_exact():

@@ -20,7 +20,7 @@ def test_library_builds_loads_and_exports_every_declared_symbol():
         assert hasattr(lib, n), n
     L = etx.load_library()
     assert L.etx_status_string(0) == b"ETX_OK" and L.etx_status_string(-3) == b"ETX_ERR_CAPACITY"
-    assert ctypes.sizeof(etx.Hyperparams) == 4 * 32 + 3 * 8       # 32 four-byte fields, three pointers
+    assert ctypes.sizeof(etx.Hyperparams) == 4 * 33 + 4 + 3 * 8   # 33 four-byte fields, padding, three pointers
 
 
 def test_host_side_argument_checks_need_no_gpu():
