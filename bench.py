@@ -30,8 +30,8 @@ import datagen  # noqa: E402
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel (S4e edge network): the mean over the
 # six launches of one pass (five write e back, the last does not) from the `ncu --set full` capture summarised in
-# profiles/r1h_launches_s4e_traffic.md, per workload; bench.py cannot run ncu itself.
-NCU_TRAFFIC_BYTES = {("cfg2", 500): 2.5150e9}
+# profiles/r2_launches_cfg2.md, per workload; bench.py cannot run ncu itself.
+NCU_TRAFFIC_BYTES = {("cfg2", 500): 2.5139e9}
 METRIC = "events_per_s"
 UNIT = "events/s"
 DTYPE = {"fp32": "f32", "bf16": "bf16", "int8": "int8"}
@@ -128,7 +128,9 @@ def stage_model(cfg, N, E, pairs, peaks):
         "S1_embedding": (mlp_bound, N * 2.0 * (3 * D + (H - 1) * D * D + 4 * D), mlp_peak, "TFLOP/s"),
         "S2_knn": ("alu", pairs * 12.0, alu_lane, "lane-instr/s"),
         "S3_compaction_csc": ("hbm", 4.0 * k * N + 12.0 * E + 8.0 * E + 16.0 * N, peaks["hbm"], "GB/s"),
-        "S4_encoders": (mlp_bound, 2.0 * (3 * d + d * d) * (N + E), mlp_peak, "TFLOP/s"),
+        # the stage only writes the state: bound by the (N + E) d b bytes of h0 / e0 (profiles/r1f), not by its FLOPs
+        "S4_encoders": ("hbm", 1.0 * (N + E) * d * b + 16.0 * N + 8.0 * E, peaks["hbm"], "GB/s") if cfg.precision != "fp32"
+                       else (mlp_bound, 2.0 * (3 * d + d * d) * (N + E), mlp_peak, "TFLOP/s"),
         # e is read from HBM once (the second direction finds its rows in L2: ncu, profiles/r1f_stage_rooflines.md)
         "S4c_scatter": ("hbm", L * (1.0 * E * d * b + 2.0 * N * d * b + 4.0 * E + 8.0 * N), peaks["hbm"], "GB/s"),
         "S4d_node_net": ("hbm", L * (4.0 * N * d * b), peaks["hbm"], "GB/s"),
@@ -231,7 +233,6 @@ def main():
         out = ctx.run(d_xyz, d_plane, batch.event_offsets)
     torch.cuda.synchronize()
     E = int(out.h_n_edges[0]); N = batch.n_hits
-    ctx.enable_timing(True)
     sampler = ClockSampler(local_rank); sampler.start()
     launches0 = ctx.launch_count()
     barrier()
@@ -244,7 +245,12 @@ def main():
     ms = ev0.elapsed_time(ev1)
     clocks = sampler.stop()
     launches = ctx.launch_count() - launches0
-    stage_ms = ctx.stage_times()                      # CUDA events of the last timed step, on the launching stream
+    # per-stage times: ONE extra pass with the library's stage events switched on (CUDA events on the launching
+    # stream between the stages); the headline above is the plain etx_run path without them
+    ctx.enable_timing(True)
+    ctx.run(d_xyz, d_plane, batch.event_offsets)
+    torch.cuda.synchronize()
+    stage_ms = ctx.stage_times()
     ctx.enable_timing(False)
     from paper_2407_12119_b200.sharding import whole_job
     ms, (tot_events, tot_hits, _) = whole_job(ms, [batch.n_events, N, E], dist, "cuda")
@@ -295,6 +301,10 @@ def main():
                 "achieved": dom_bytes / (dom_ms * 1e-3) / 1e9 if dom_ms > 0 else None, "peak": peaks["hbm"], "unit": "GB/s",
                 "frac": (dom_bytes / (dom_ms * 1e-3) / 1e9 / peaks["hbm"]) if dom_ms > 0 else None,
                 "traffic": NCU_TRAFFIC_BYTES.get((cfg.name, cfg.n_events)),
+                "traffic_source": "recorded: ncu --set full capture of this kernel at this workload, profiles/r2_launches_cfg2.md "
+                                  "(bench.py cannot run ncu; null for other workloads)",
+                "note": "S4e moves its algorithmic bytes once (traffic / algorithmic = 0.98); what holds it below the copy peak is "
+                        "on-chip: shared-memory bandwidth and the cp.async gather of h[src], h[dst] (profiles/r2_s4e_ablation.md)",
                 "peak_source": peaks["source"], "avg_launch_ms": dom_ms, "algorithmic_bytes_per_launch": dom_bytes,
                 "share_of_step": stage_ms[dom] / (ms / args.steps) if ms > 0 else None}
     cpu_baseline = None
@@ -302,9 +312,14 @@ def main():
         v, dt, n, cores = run_oracle_sample(cfg, batch, layers, args.cpu_events, scales)
         cpu_baseline = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
                         "sample": f"first {n} events of the same batch, whole path S0..S5, {dt:.1f} s"}
+        import oracle
+        oracle.set_threads(1)                             # also once single-threaded, on a smaller sample
+        v1, dt1, n1, _ = run_oracle_sample(cfg, batch, layers, max(1, args.cpu_events // 32), scales)
+        oracle.set_threads(cores)
+        cpu_baseline["single_thread"] = {"value": v1, "unit": UNIT, "cores": 1, "sample": f"first {n1} events, {dt1:.1f} s"}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": DTYPE[cfg.precision], "data": "synthetic", "config": dict(config, engine=args.engine),
+            "dtype": DTYPE[cfg.precision], "data": "synthetic", "config": config, "engine": args.engine,
             "hits_per_s": tot_hits * args.steps / (ms * 1e-3), "n_hits": N, "n_edges": E, "clocks": clocks, "e2e": e2e,
             "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu_baseline, "stages": stages}
     print(json.dumps(line))

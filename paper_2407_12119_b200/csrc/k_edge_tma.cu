@@ -100,17 +100,6 @@ __device__ __forceinline__ void umma_ts(uint32_t tmem_d, uint32_t tmem_a, uint64
                ::"r"(tmem_d), "r"(tmem_a), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
 }
 
-// Developer profiling (build with ETX_NVCC_EXTRA=-DETX_EDGE_PROF): per-role cycle counts of CTA 0, printed at exit.
-#ifdef ETX_EDGE_PROF
-#define PROF_DECL long long pt_[6] = {0, 0, 0, 0, 0, 0}; long long pc_ = clock64();
-#define PROF(i) { const long long n_ = clock64(); pt_[i] += n_ - pc_; pc_ = n_; }
-#define PROF_OUT(name) if (blockIdx.x == 0 && lane == 0) printf("%s w%d: %lld %lld %lld %lld %lld %lld\n", name, warp, pt_[0], pt_[1], pt_[2], pt_[3], pt_[4], pt_[5]);
-#else
-#define PROF_DECL
-#define PROF(i)
-#define PROF_OUT(name)
-#endif
-
 struct EtSmem { int self, aux, w0, w1, ident, ones, b0, b1, headw, bar, total; };
 template <int D>
 __host__ __device__ constexpr EtSmem et_layout() {
@@ -202,7 +191,6 @@ edge_net_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeTmaArgs
     // most one mbarrier phase ahead, which the parity wait requires; the warpgroup's fourth warp only donates its
     // registers.)
     const int pw = warp - kEpiWarps;
-    PROF_DECL
     for (int it = pw; pw < kNH && blockIdx.x + (long long)it * gridDim.x < n_tiles; it += kNH) {
       const int tile = blockIdx.x + it * gridDim.x;
       const int s = it % kNH;
@@ -213,9 +201,7 @@ edge_net_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeTmaArgs
         if (row >= n_rows) row = n_rows - 1;                  // dead rows of the last tile: any valid row
         isv[j] = __ldg(a.src + row); idv[j] = __ldg(a.dst + row);
       }
-      PROF(0)
       mbar_wait(&aux_empty[s], ((it / kNH) & 1) ^ 1);
-      PROF(1)
       const uint32_t st = aux_addr + s * 2 * BLK;
 #pragma unroll
       for (int j = 0; j < 4; ++j) {
@@ -230,49 +216,37 @@ edge_net_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeTmaArgs
         }
       }
       cp_async_commit();
-      PROF(2)
       cp_async_wait<0>();
       fence_proxy_async();                                    // generic-proxy writes -> visible to the tensor core
       mbar_arrive(&aux_full[s]);
-      PROF(3)
     }
-    PROF_OUT("gather[idx,empty,issue,land]")
   } else if (warp == kLoadWarp) {
     // ================================================================================================ TMA loads
     if (lane == 0) {
-      PROF_DECL
       int it = 0;
       for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
         const int s = it % kNE;
-        PROF(0)
         mbar_wait(&self_empty[s], ((it / kNE) & 1) ^ 1);
-        PROF(1)
         if (a.enc) { mbar_arrive(&self_full[s]); continue; }  // no old state: the slot is only the output staging
         mbar_expect_tx(&self_full[s], BLK);
         tma_load_2d(self_addr + s * BLK, &e_map, 0, tile * kRows, &self_full[s]);
       }
-      PROF_OUT("loader[-,empty]")
     }
   } else if (warp == kStoreWarp) {
     // ================================================================================================ TMA stores
     if (lane == 0) {
-      PROF_DECL
       int it = 0;
       for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
         const int s = it % kNE;
-        PROF(0)
         mbar_wait(&out_ready[s], (it / kNE) & 1);
-        PROF(1)
         if (a.store_e) {
           tma_store_2d(&e_map, self_addr + s * BLK, 0, tile * kRows);
           bulk_commit();
           bulk_wait_read0();                                  // the slot has been read: hand it back to the loader
         }
         mbar_arrive(&self_empty[s]);
-        PROF(2)
       }
       bulk_wait0();
-      PROF_OUT("store[-,ready,read]")
     }
   } else if (warp == kMmaWarp) {
     // ================================================================================================ MMA issuer
@@ -289,12 +263,9 @@ edge_net_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeTmaArgs
       const uint32_t w0_addr = smem_u32(smem + L.w0), w1_addr = smem_u32(smem + L.w1), id_addr = smem_u32(smem + L.ident);
       const uint64_t ones_desc = make_desc<32>(smem_u32(smem + L.ones));
       const uint64_t b0_desc = make_desc<32>(smem_u32(smem + L.b0)), b1_desc = make_desc<32>(smem_u32(smem + L.b1));
-      PROF_DECL
       auto layer1 = [&](int j) {                              // acc1 = 1*b1' + hidden*W1^T + e*I   (tile j of this CTA)
         const int g = j & 1, se = j % kNE;
-        PROF(0)
         mbar_wait(&hid_full[g], (j >> 1) & 1);
-        PROF(1)
         tc_fence_after();
         const uint32_t d1 = tmem + 2 * D + g * D, hid = tmem + 4 * D + g * (D / 2);
         umma::umma<kBf16>(d1, ones_desc, b1_desc, idesc, 0u);
@@ -303,7 +274,6 @@ edge_net_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeTmaArgs
           umma_ts(d1, hid + 8 * k, make_desc<KB>(w1_addr + k * 32), idesc, 1u);
         if (!a.enc) issue_block<KB>(self_addr + se * BLK, id_addr, d1, idesc);             // + old e (R14)
         umma_commit(&acc1_full[g]);
-        PROF(2)
       };
       // Issue order: layer 0 of tile it, then layer 1 of tile it-1 (so the tensor pipe always has the next tile's
       // big layer queued) -- but while tile it's operands are still in flight, a layer 1 that has become ready
@@ -311,13 +281,11 @@ edge_net_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeTmaArgs
       int it = 0, pending = -1;                               // pending: tile whose layer 1 has not been issued yet
       for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
         const int g = it & 1, se = it % kNE, sh = it % kNH;
-        PROF(0)
         for (uint32_t spins = 0;; ++spins) {
           if (pending >= 0 && mbar_test(&hid_full[pending & 1], (pending >> 1) & 1)) { layer1(pending); pending = -1; }
           if (mbar_test(&aux_full[sh], (it / kNH) & 1) && mbar_test(&self_full[se], (it / kNE) & 1)) break;
           if ((spins & 0xfffffu) == 0xfffffu && mbar_stalled(spins)) __trap();
         }
-        PROF(3)
         tc_fence_after();
         // acc0[g] was drained by epilogue 0 of tile it-2: hid_full, waited on for layer 1 of it-2, covers it
         const uint32_t d0 = tmem + g * D;
@@ -327,12 +295,10 @@ edge_net_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeTmaArgs
         if (!a.enc) issue_block<KB>(self_addr + se * BLK, w0_addr + 2 * D * KB, d0, idesc);   // e
         umma_commit(&acc0_full[g]);
         umma_commit(&aux_empty[sh]);                          // layer 0 was the gather slot's only reader
-        PROF(4)
         if (pending >= 0) layer1(pending);
         pending = it;
       }
       if (pending >= 0) layer1(pending);
-      PROF_OUT("mma[-,wait_hid,issue1,wait_ops,issue0]")
     }
   } else {
     // ================================================================================================ epilogue
@@ -342,16 +308,13 @@ edge_net_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeTmaArgs
     const uint32_t lane_base = (uint32_t)(q * 32) << 16;
     const float head_b = a.head_b[0];
     int j = 0;
-    PROF_DECL
     for (int it = g; blockIdx.x + (long long)it * gridDim.x < n_tiles; it += 2, ++j) {
       const int tile = blockIdx.x + it * gridDim.x;
       const int row = tile * kRows + r;
       uint8_t* out = smem + L.self + (it % kNE) * BLK;        // the e tile, updated in place
       // ---- epilogue 0: relu(acc0) -> bf16, packed two per column -> tensor memory, the A operand of layer 1 (R3, R20);
       //      the bias is already in acc0
-      PROF(0)
       mbar_wait(&acc0_full[g], j & 1);
-      PROF(1)
       tc_fence_after();
 #pragma unroll
       for (int c0 = 0; c0 < D; c0 += 64) {
@@ -372,10 +335,8 @@ edge_net_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeTmaArgs
       tmem_st_wait();
       tc_fence_before();
       mbar_arrive(&hid_full[g]);
-      PROF(2)
       // ---- epilogue 1: acc1 (= b1 + W1 hidden + old e) -> bf16 -> the slot, optional classifier (R14, R16, R20)
       mbar_wait(&acc1_full[g], j & 1);
-      PROF(3)
       tc_fence_after();
       float hacc = 0.0f;
 #pragma unroll
@@ -403,14 +364,12 @@ edge_net_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeTmaArgs
       tc_fence_before();                                      // acc1[g] may be overwritten after our next hid_full arrive
       fence_proxy_async();                                    // generic-proxy writes -> visible to the TMA store
       mbar_arrive(&out_ready[it % kNE]);
-      PROF(4)
       if (a.do_head && row < n_rows) {
         const float z = __fadd_rn(hacc, head_b);
         a.logit[row] = z;
         a.score[row] = 1.0f / (1.0f + expf(-z));
       }
     }
-    PROF_OUT("epi[tail,wait_acc0,ep0,wait_acc1,ep1]")
   }
   tc_fence_before();
   __syncthreads();
@@ -494,6 +453,9 @@ edge_enc_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeEncArgs
 
   if (warp == kEncStoreWarp) {
     // ================================================================================================ TMA stores
+    // One TMA store per tile.  (Measured alternatives, both without gain: two stores in flight per SM -- the stage
+    // stays at 0.34 ms, the TMA unit reads a 16 KB tile out of shared memory at ~17 bytes per cycle whatever the depth;
+    // the store warp copying the tile out with 16-byte plain stores -- 1.02 ms.)
     if (lane == 0) {
       int it = 0;
       for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
@@ -554,17 +516,14 @@ edge_enc_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeEncArgs
       load_idx(1, is_n, id_n);
       fs = __ldg(a.feat + is0); fd = __ldg(a.feat + id0);
     }
-    PROF_DECL
     for (int j = 0; tile_of(j) < n_tiles; ++j) {
       const long long tile = tile_of(j);
-      PROF(0)
       // R11: component-wise |f_dst - f_src| of the normalised features
       float fx = fabsf(__fsub_rn(fd.x, fs.x)), fy = fabsf(__fsub_rn(fd.y, fs.y)), fz = fabsf(__fsub_rn(fd.z, fs.z));
       if (a.node) { fx = fs.x; fy = fs.y; fz = fs.z; }        // S4a: the hit's own normalised features
       // prefetch: features of tile j + 1 (their indices are here), indices of tile j + 2
       fs = __ldg(a.feat + is_n); fd = __ldg(a.feat + id_n);
       load_idx(j + 2, is_n, id_n);
-      PROF(1)
       // ---- layer 0 on the FFMA pipe, pinned order (R3); relu -> bf16 -> tensor memory
 #pragma unroll
       for (int c0 = 0; c0 < D; c0 += 64) {
@@ -588,13 +547,11 @@ edge_enc_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeEncArgs
       tmem_st_wait();
       tc_fence_before();
       mbar_arrive(&hid_full[g]);
-      PROF(2)
       // ---- layer 1 result (bias already inside): TMEM -> bf16 -> the group's slot -> TMA store (R20)
       const int sl = 2 * g + (j & 1);
       uint8_t* out = smem + L.out + sl * BLK;
       mbar_wait(&slot_free[sl], ((j >> 1) & 1) ^ 1);          // the store of tile j - 2 has read the slot
       mbar_wait(&acc_full[g], j & 1);
-      PROF(3)
       tc_fence_after();
 #pragma unroll
       for (int c0 = 0; c0 < D; c0 += 32) {
@@ -615,9 +572,7 @@ edge_enc_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeEncArgs
       fence_proxy_async();
       mbar_arrive(&out_ready[sl]);
       (void)tile;
-      PROF(4)
     }
-    PROF_OUT("enc[tail,feat,ffma,wait_acc,epi]")
   }
   tc_fence_before();
   __syncthreads();
