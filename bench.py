@@ -133,10 +133,13 @@ def stage_model(cfg, N, E, pairs, peaks):
                        else (mlp_bound, 2.0 * (3 * d + d * d) * (N + E), mlp_peak, "TFLOP/s"),
         # e is read from HBM once (the second direction finds its rows in L2: ncu, profiles/r1f_stage_rooflines.md)
         "S4c_scatter": ("hbm", L * (1.0 * E * d * b + 2.0 * N * d * b + 4.0 * E + 8.0 * N), peaks["hbm"], "GB/s"),
-        "S4d_node_net": ("hbm", L * (4.0 * N * d * b), peaks["hbm"], "GB/s"),
+        # fp32 mode runs the networks on the FFMA pipe in the pinned order: bound by their FLOPs, not by bytes
+        "S4d_node_net": ("hbm", L * (4.0 * N * d * b), peaks["hbm"], "GB/s") if cfg.precision != "fp32"
+                        else ("alu", L * 2.0 * (3 * d * d + d * d) * N, ffma, "TFLOP/s"),
         # e is read by every step and written by all but the last (e^L feeds only the classifier, which is fused)
         "S4e_edge_net_head": ("hbm", L * ((2.0 * d * b + 8.0) * E + N * d * b) + 8.0 * E - (E * d * b if L else 0.0),
-                              peaks["hbm"], "GB/s"),
+                              peaks["hbm"], "GB/s") if cfg.precision != "fp32"
+                             else ("alu", (L * 2.0 * (3 * d * d + d * d) + 2.0 * d) * E, ffma, "TFLOP/s"),
         "S5_components": ("hbm", 12.0 * E + 8.0 * N, peaks["hbm"], "GB/s"),
     }
 
@@ -297,15 +300,18 @@ def main():
     L = max(cfg.gnn_iters, 1)
     dom_ms = stage_ms[dom] / L
     dom_bytes = model[dom][1] / L
-    roofline = {"kernel": "edge network MLP (S4e), one launch per message-passing step", "bound": "hbm",
-                "achieved": dom_bytes / (dom_ms * 1e-3) / 1e9 if dom_ms > 0 else None, "peak": peaks["hbm"], "unit": "GB/s",
-                "frac": (dom_bytes / (dom_ms * 1e-3) / 1e9 / peaks["hbm"]) if dom_ms > 0 else None,
+    dom_bound, _, dom_peak, dom_unit = model[dom]
+    dom_div = 1e12 if dom_unit == "TFLOP/s" else 1e9
+    roofline = {"kernel": "edge network MLP (S4e), one launch per message-passing step", "bound": dom_bound,
+                "achieved": dom_bytes / (dom_ms * 1e-3) / dom_div if dom_ms > 0 else None, "peak": dom_peak, "unit": dom_unit,
+                "frac": (dom_bytes / (dom_ms * 1e-3) / dom_div / dom_peak) if dom_ms > 0 else None,
                 "traffic": NCU_TRAFFIC_BYTES.get((cfg.name, cfg.n_events)),
                 "traffic_source": "recorded: ncu --set full capture of this kernel at this workload, profiles/r2_launches_cfg2.md "
                                   "(bench.py cannot run ncu; null for other workloads)",
                 "note": "S4e moves its algorithmic bytes once (traffic / algorithmic = 0.98); what holds it below the copy peak is "
                         "on-chip: shared-memory bandwidth and the cp.async gather of h[src], h[dst] (profiles/r2_s4e_ablation.md)",
-                "peak_source": peaks["source"], "avg_launch_ms": dom_ms, "algorithmic_bytes_per_launch": dom_bytes,
+                "peak_source": peaks["source"] if dom_bound == "hbm" else "derived: 148 SM x 128 lanes x 2 x 1.965 GHz (DESIGN.md sec. 3)",
+                "avg_launch_ms": dom_ms, "algorithmic_work_per_launch": dom_bytes,
                 "share_of_step": stage_ms[dom] / (ms / args.steps) if ms > 0 else None}
     cpu_baseline = None
     if not args.no_cpu_baseline:
