@@ -153,6 +153,23 @@ etx_status etx_run_host(etx_handle h, const float* h_xyz, const int32_t* h_plane
                         float* h_edge_score, int32_t* h_edge_src, int32_t* h_edge_dst,
                         int32_t* h_track_id, int32_t* n_edges_out);
 
+/* The same work as etx_run_host, asynchronously and pipelined (Allen keeps several streams of events
+ * in flight so that copies hide under compute): etx_submit_host enqueues the H2D copy of the inputs (on the handle's
+ * copy stream, under the previous batch's compute), S0..S5 on `stream`, and the D2H of the results, and returns
+ * without synchronising; etx_wait_host(ticket) blocks until that submission has completed and returns its status
+ * (ETX_ERR_INPUT_ORDER for a rejected batch).  At most TWO submissions may be in flight per handle: wait for
+ * submission i before submitting i + 2, and give the two in-flight submissions different output buffers.  All output
+ * buffers must be pinned (page-locked) host memory.  The edge list and the scores of submission i are copied out, at
+ * their exact size, by the next call on the handle -- the submission of i + 1 or the wait for i -- once the host has
+ * learnt E, which S3 produced long before: the edge list under batch i's own GNN, the scores under batch i + 1 (each
+ * slot has its own device score buffer).  *h_n_edges (plain host int32) receives E and is valid after etx_wait_host.  The h_* input arrays and
+ * h_event_offsets must stay valid until the submission has completed (h_event_offsets: until the call returns). */
+etx_status etx_submit_host(etx_handle h, const float* h_xyz, const int32_t* h_plane,
+                           const int32_t* h_event_offsets, int32_t n_events, etx_stream stream,
+                           float* h_edge_score, int32_t* h_edge_src, int32_t* h_edge_dst,
+                           int32_t* h_track_id, int32_t* h_n_edges, int32_t* ticket);
+etx_status etx_wait_host(etx_handle h, int32_t ticket);
+
 /* Verdict of the device-side input validation for the last etx_run / etx_dbg_run on this handle whose stream work
  * has completed (the caller synchronises the stream first): ETX_OK, or ETX_ERR_INPUT_ORDER if that batch was
  * rejected.  Always ETX_OK when validate_input = 0. */

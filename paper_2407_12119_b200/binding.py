@@ -95,6 +95,10 @@ def load_library():
     L.etx_run_host.argtypes = [vp, vp, vp, i32p, C.c_int32, vp, vp, vp, vp, vp, i32p]
     L.etx_destroy.restype = C.c_int
     L.etx_destroy.argtypes = [vp]
+    L.etx_submit_host.restype = C.c_int
+    L.etx_submit_host.argtypes = [vp, vp, vp, i32p, C.c_int32, vp, vp, vp, vp, vp, vp, i32p]
+    L.etx_wait_host.restype = C.c_int
+    L.etx_wait_host.argtypes = [vp, C.c_int32]
     L.etx_triplets.restype = C.c_int
     L.etx_triplets.argtypes = [vp, vp, C.POINTER(EtxTriplets)]
     L.etx_input_status.restype = C.c_int
@@ -229,6 +233,20 @@ class Etx:
                                   ptr(h_src), ptr(h_dst), ptr(h_track_id), C.byref(E))
         self._check(st, "etx_run_host")
         return int(E.value)
+
+    def submit_host(self, h_xyz, h_plane, event_offsets, h_score, h_src, h_dst, h_track_id, h_n_edges) -> int:
+        """etx_submit_host: pinned host tensors in and out, returns at once with a ticket (two may be in flight)."""
+        eo, eop, B = self._offsets(event_offsets)
+        t = C.c_int32(0)
+        ptr = lambda x: C.c_void_p(x.data_ptr()) if x is not None else C.c_void_p()
+        self._keep_async = getattr(self, "_keep_async", [])[-3:] + [(h_xyz, h_plane, eo, h_score, h_src, h_dst, h_track_id, h_n_edges)]
+        st = self._L.etx_submit_host(self._h, ptr(h_xyz), ptr(h_plane), eop, B, self._stream(), ptr(h_score), ptr(h_src),
+                                     ptr(h_dst), ptr(h_track_id), ptr(h_n_edges), C.byref(t))
+        self._check(st, "etx_submit_host")
+        return int(t.value)
+
+    def wait_host(self, ticket: int):
+        self._check(self._L.etx_wait_host(self._h, int(ticket)), "etx_wait_host")
 
     # -- debug entry points ----------------------------------------------------------------------
     def dbg_run(self, d_xyz, d_plane, event_offsets, emb=None, src=None, dst=None, logit=None,

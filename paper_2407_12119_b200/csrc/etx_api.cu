@@ -195,6 +195,7 @@ etx_status run_impl(etx_ctx* c, const float* d_xyz, const int32_t* d_plane, cons
       launch_features(c, d_xyz, n_hits, s);
       launch_plane_offsets(c, d_plane, n_events, s);
       if (c->hp.validate_input) launch_validate(c, d_plane, n_events, n_hits, s);
+      if (c->inputs_read_cur) ETX_CUDA(cudaEventRecord(c->inputs_read_cur, s));   // S0 is the only reader of xyz / plane
       tm.end();
       // ---- S1
       tm.begin(1);
@@ -223,8 +224,8 @@ etx_status run_impl(etx_ctx* c, const float* d_xyz, const int32_t* d_plane, cons
         }
         // E and the edge list are final here: mirror E to the host and mark the point (etx_run_host starts the
         // D2H copy of src / dst on its copy stream from this event, under the GNN)
-        ETX_CUDA(cudaMemcpyAsync(c->h_n_edges, c->n_edges, sizeof(int32_t), cudaMemcpyDeviceToHost, s));
-        ETX_CUDA(cudaEventRecord(c->edges_ready, s));
+        ETX_CUDA(cudaMemcpyAsync(c->h_n_edges_cur ? c->h_n_edges_cur : c->h_n_edges, c->n_edges, sizeof(int32_t), cudaMemcpyDeviceToHost, s));
+        ETX_CUDA(cudaEventRecord(c->edges_ready_cur ? c->edges_ready_cur : c->edges_ready, s));
         edges_marked = true;
         if (last >= 3) launch_csc(c, n_events, n_hits, !(inj && inj->d_src), s);
         tm.end();
@@ -267,11 +268,11 @@ etx_status run_impl(etx_ctx* c, const float* d_xyz, const int32_t* d_plane, cons
       }
     }
     if (!edges_marked) {
-      ETX_CUDA(cudaMemcpyAsync(c->h_n_edges, c->n_edges, sizeof(int32_t), cudaMemcpyDeviceToHost, s));
-      ETX_CUDA(cudaEventRecord(c->edges_ready, s));
+      ETX_CUDA(cudaMemcpyAsync(c->h_n_edges_cur ? c->h_n_edges_cur : c->h_n_edges, c->n_edges, sizeof(int32_t), cudaMemcpyDeviceToHost, s));
+      ETX_CUDA(cudaEventRecord(c->edges_ready_cur ? c->edges_ready_cur : c->edges_ready, s));
     }
     if (c->hp.validate_input) {     // the verdict of THIS batch: readable through etx_input_status once the stream is synchronised
-      ETX_CUDA(cudaMemcpyAsync(c->h_flags, c->flags, sizeof(int32_t), cudaMemcpyDeviceToHost, s));
+      ETX_CUDA(cudaMemcpyAsync(c->h_flags_cur ? c->h_flags_cur : c->h_flags, c->flags, sizeof(int32_t), cudaMemcpyDeviceToHost, s));
       ETX_CUDA(cudaMemsetAsync(c->flags, 0, sizeof(int32_t), s));
     }
     ETX_CUDA(cudaGetLastError());
@@ -441,10 +442,21 @@ etx_status etx_destroy(etx_handle c) {
   if (c->h_n_tracks) cudaFreeHost(c->h_n_tracks);
   if (c->h_flags) cudaFreeHost(c->h_flags);
   if (c->h_trip_total) cudaFreeHost(c->h_trip_total);
+  if (c->h_slot_flags) cudaFreeHost(c->h_slot_flags);
+  if (c->h_slot_n_edges) cudaFreeHost(c->h_slot_n_edges);
+  for (int i = 0; i < 2; ++i) {
+    if (c->slot_edges_ready[i]) cudaEventDestroy(c->slot_edges_ready[i]);
+    if (c->slot_edges_copied[i]) cudaEventDestroy(c->slot_edges_copied[i]);
+    if (c->slot_copies_done[i]) cudaEventDestroy(c->slot_copies_done[i]);
+    if (c->slot_done[i]) cudaEventDestroy(c->slot_done[i]);
+    if (c->slot_inputs_read[i]) cudaEventDestroy(c->slot_inputs_read[i]);
+    if (c->slot_h2d[i]) cudaEventDestroy(c->slot_h2d[i]);
+  }
   if (c->staging_free) cudaEventDestroy(c->staging_free);
   if (c->edges_ready) cudaEventDestroy(c->edges_ready);
   if (c->copies_done) cudaEventDestroy(c->copies_done);
   if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+  if (c->h2d_stream) cudaStreamDestroy(c->h2d_stream);
   for (int i = 0; i < 256; ++i) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
   delete c;
   return ETX_OK;
@@ -548,6 +560,127 @@ etx_status etx_run_host(etx_handle c, const float* h_xyz, const int32_t* h_plane
 etx_status etx_input_status(etx_handle c) {
   if (!c) return ETX_ERR_ARG;
   if (c->hp.validate_input && (c->h_flags[0] & 1))
+    return fail(c, ETX_ERR_INPUT_ORDER, "hits not sorted by (event, plane), or a plane index out of range: the batch was rejected (0 edges)");
+  return ETX_OK;
+}
+
+static void* mapped_ptr(void* host) {
+  if (!host) return nullptr;
+  cudaPointerAttributes attr;
+  if (cudaPointerGetAttributes(&attr, host) == cudaSuccess && attr.type == cudaMemoryTypeHost && attr.devicePointer) return attr.devicePointer;
+  (void)cudaGetLastError();
+  return nullptr;
+}
+
+// The edge list of a submission can only be copied out once the host knows E.  That is learnt without stalling the
+// pipeline: the copy of submission i is issued by the NEXT call on the handle (etx_submit_host of i + 1, or
+// etx_wait_host of i), by which time S3 of batch i -- an early stage -- has long passed while its GNN still runs.
+static void flush_edge_copy(etx_ctx* c, int slot) {
+  etx_ctx::PendingCopy& pc = c->slot_copy[slot];
+  if (!pc.pending) return;
+  pc.pending = false;
+  ETX_CUDA(cudaEventSynchronize(c->slot_edges_ready[slot]));
+  const int E = c->h_slot_n_edges[slot];
+  *pc.h_n = E;
+  ETX_CUDA(cudaStreamWaitEvent(c->copy_stream, c->slot_edges_ready[slot], 0));
+  if (E > 0 && pc.h_src) ETX_CUDA(cudaMemcpyAsync(pc.h_src, c->src, sizeof(int32_t) * (size_t)E, cudaMemcpyDeviceToHost, c->copy_stream));
+  if (E > 0 && pc.h_dst) ETX_CUDA(cudaMemcpyAsync(pc.h_dst, c->dst, sizeof(int32_t) * (size_t)E, cudaMemcpyDeviceToHost, c->copy_stream));
+  ETX_CUDA(cudaEventRecord(c->slot_edges_copied[slot], c->copy_stream));
+  // the scores leave once the batch's last kernel has written them -- under the next batch's compute, from this slot's
+  // own score buffer
+  ETX_CUDA(cudaStreamWaitEvent(c->copy_stream, c->slot_done[slot], 0));
+  if (E > 0 && pc.h_score) ETX_CUDA(cudaMemcpyAsync(pc.h_score, pc.d_score, sizeof(float) * (size_t)E, cudaMemcpyDeviceToHost, c->copy_stream));
+  ETX_CUDA(cudaEventRecord(c->slot_copies_done[slot], c->copy_stream));
+}
+
+etx_status etx_submit_host(etx_handle c, const float* h_xyz, const int32_t* h_plane, const int32_t* h_event_offsets,
+                           int32_t n_events, etx_stream stream, float* h_edge_score, int32_t* h_edge_src,
+                           int32_t* h_edge_dst, int32_t* h_track_id, int32_t* h_n_edges, int32_t* ticket) {
+  if (!c) return ETX_ERR_ARG;
+  if (!h_event_offsets || n_events < 0 || !h_n_edges || !ticket) return fail(c, ETX_ERR_ARG, "null argument");
+  if (n_events > c->hp.max_events) return fail(c, ETX_ERR_CAPACITY, "n_events exceeds max_events");
+  const int n_hits = h_event_offsets[n_events];
+  if (n_hits < 0 || n_hits > c->hp.max_hits) return fail(c, ETX_ERR_CAPACITY, "n_hits exceeds max_hits");
+  if (n_hits > 0 && (!h_xyz || !h_plane)) return fail(c, ETX_ERR_ARG, "null hit arrays");
+  // pinned output buffers: the copies must be truly asynchronous
+  if ((h_edge_score && !mapped_ptr(h_edge_score)) || (h_edge_src && !mapped_ptr(h_edge_src)) || (h_edge_dst && !mapped_ptr(h_edge_dst)) ||
+      (h_track_id && !mapped_ptr(h_track_id)))
+    return fail(c, ETX_ERR_ARG, "etx_submit_host needs pinned (page-locked) output buffers");
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  const int slot = (int)(c->n_submitted & 1), prev = slot ^ 1;
+  try {
+    if (!c->d_xyz_in2) {                                   // first use: the second staging set and the per-slot events
+      c->d_xyz_in2 = dev_alloc<float>(c, (size_t)c->hp.max_hits * 3);
+      c->d_plane_in2 = dev_alloc<int32_t>(c, (size_t)c->hp.max_hits);
+      c->score2 = dev_alloc<float>(c, (size_t)c->max_edges);
+      ETX_CUDA(cudaStreamCreateWithFlags(&c->h2d_stream, cudaStreamNonBlocking));
+      ETX_CUDA(cudaMallocHost(&c->h_slot_flags, 2 * sizeof(int32_t)));
+      ETX_CUDA(cudaMallocHost(&c->h_slot_n_edges, 2 * sizeof(int32_t)));
+      for (int i = 0; i < 2; ++i) {
+        c->h_slot_flags[i] = 0; c->h_slot_n_edges[i] = 0;
+        ETX_CUDA(cudaEventCreateWithFlags(&c->slot_done[i], cudaEventDisableTiming));
+        ETX_CUDA(cudaEventCreateWithFlags(&c->slot_inputs_read[i], cudaEventDisableTiming));
+        ETX_CUDA(cudaEventCreateWithFlags(&c->slot_h2d[i], cudaEventDisableTiming));
+        ETX_CUDA(cudaEventCreateWithFlags(&c->slot_edges_ready[i], cudaEventDisableTiming));
+        ETX_CUDA(cudaEventCreateWithFlags(&c->slot_copies_done[i], cudaEventDisableTiming));
+        ETX_CUDA(cudaEventCreateWithFlags(&c->slot_edges_copied[i], cudaEventDisableTiming));
+      }
+    }
+    if (c->slot_copy[slot].pending) return fail(c, ETX_ERR_ARG, "etx_submit_host: wait for submission i before submitting i + 2");
+    // the previous submission's edge list: issue its copy now, and keep this batch's S3 from overwriting src / dst early
+    if (c->n_submitted >= 1) {
+      flush_edge_copy(c, prev);
+      ETX_CUDA(cudaStreamWaitEvent(s, c->slot_edges_copied[prev], 0));
+    }
+    float* dx = slot ? c->d_xyz_in2 : c->d_xyz_in;
+    int32_t* dp = slot ? c->d_plane_in2 : c->d_plane_in;
+    // H2D on its own stream, under the previous batch's compute; the staging set was last read by S0 two submissions ago
+    if (c->n_submitted >= 2) ETX_CUDA(cudaStreamWaitEvent(c->h2d_stream, c->slot_inputs_read[slot], 0));
+    if (n_hits > 0) {
+      ETX_CUDA(cudaMemcpyAsync(dx, h_xyz, sizeof(float) * 3 * (size_t)n_hits, cudaMemcpyHostToDevice, c->h2d_stream));
+      ETX_CUDA(cudaMemcpyAsync(dp, h_plane, sizeof(int32_t) * (size_t)n_hits, cudaMemcpyHostToDevice, c->h2d_stream));
+    }
+    ETX_CUDA(cudaEventRecord(c->slot_h2d[slot], c->h2d_stream));
+    ETX_CUDA(cudaStreamWaitEvent(s, c->slot_h2d[slot], 0));
+    c->score_out = slot ? c->score2 : c->score;
+    c->h_flags_cur = &c->h_slot_flags[slot];
+    c->inputs_read_cur = c->slot_inputs_read[slot];
+    c->edges_ready_cur = c->slot_edges_ready[slot];
+    c->h_n_edges_cur = &c->h_slot_n_edges[slot];
+    etx_output o;
+    const etx_status st = run_impl(c, dx, dp, h_event_offsets, n_events, s, nullptr, &o);
+    c->score_out = c->score; c->h_flags_cur = nullptr; c->inputs_read_cur = nullptr; c->edges_ready_cur = nullptr; c->h_n_edges_cur = nullptr;
+    if (st != ETX_OK) return st;
+    if (h_track_id && n_hits > 0)
+      ETX_CUDA(cudaMemcpyAsync(h_track_id, c->track_id, sizeof(int32_t) * (size_t)n_hits, cudaMemcpyDeviceToHost, s));
+    ETX_CUDA(cudaEventRecord(c->slot_done[slot], s));
+    c->slot_copy[slot].h_src = h_edge_src; c->slot_copy[slot].h_dst = h_edge_dst; c->slot_copy[slot].h_n = h_n_edges;
+    c->slot_copy[slot].h_score = h_edge_score; c->slot_copy[slot].d_score = slot ? c->score2 : c->score;
+    c->slot_copy[slot].pending = true;
+    ETX_CUDA(cudaGetLastError());
+  } catch (const CudaFail& f) {
+    return fail(c, ETX_ERR_CUDA, std::string(f.what) + ": " + cudaGetErrorString(f.err));
+  }
+  *ticket = (int32_t)(c->n_submitted & 0x7fffffff);
+  c->n_submitted++;
+  return ETX_OK;
+}
+
+etx_status etx_wait_host(etx_handle c, int32_t ticket) {
+  if (!c) return ETX_ERR_ARG;
+  const long long newest = (c->n_submitted - 1) & 0x7fffffff;
+  const long long t = (long long)ticket;
+  if (c->n_submitted == 0 || t > newest || newest - t > 1)
+    return fail(c, ETX_ERR_ARG, "etx_wait_host: unknown ticket (only the last two submissions can be waited for)");
+  const int slot = (int)(t & 1);
+  try {
+    flush_edge_copy(c, slot);
+    ETX_CUDA(cudaEventSynchronize(c->slot_copies_done[slot]));
+    ETX_CUDA(cudaEventSynchronize(c->slot_done[slot]));
+  } catch (const CudaFail& f) {
+    return fail(c, ETX_ERR_CUDA, std::string(f.what) + ": " + cudaGetErrorString(f.err));
+  }
+  if (c->hp.validate_input && (c->h_slot_flags[slot] & 1))
     return fail(c, ETX_ERR_INPUT_ORDER, "hits not sorted by (event, plane), or a plane index out of range: the batch was rejected (0 edges)");
   return ETX_OK;
 }

@@ -134,6 +134,24 @@ struct etx_ctx {
   // staging for etx_run_host
   float* d_xyz_in = nullptr;
   int32_t* d_plane_in = nullptr;
+  // etx_submit_host / etx_wait_host: a second input staging set, one completion event, "inputs consumed" event and
+  // validation flag per slot (two submissions may be in flight)
+  float* d_xyz_in2 = nullptr;
+  int32_t* d_plane_in2 = nullptr;
+  cudaEvent_t slot_done[2] = {nullptr, nullptr}, slot_inputs_read[2] = {nullptr, nullptr}, slot_h2d[2] = {nullptr, nullptr};
+  int32_t* h_slot_flags = nullptr;        // pinned [2]
+  int32_t* h_flags_cur = nullptr;         // where run_impl mirrors the validation flag of the batch it enqueues
+  cudaEvent_t inputs_read_cur = nullptr;  // recorded by run_impl once S0 has read xyz / plane (or nullptr)
+  cudaEvent_t edges_ready_cur = nullptr;  // run_impl records this instead of edges_ready when set
+  int32_t* h_n_edges_cur = nullptr;       // ... and mirrors E here instead of h_n_edges
+  cudaEvent_t slot_edges_ready[2] = {nullptr, nullptr}, slot_copies_done[2] = {nullptr, nullptr};
+  int32_t* h_slot_n_edges = nullptr;      // pinned [2]
+  struct PendingCopy { int32_t* h_src = nullptr; int32_t* h_dst = nullptr; int32_t* h_n = nullptr; float* h_score = nullptr;
+                       const float* d_score = nullptr; bool pending = false; } slot_copy[2];
+  cudaEvent_t slot_edges_copied[2] = {nullptr, nullptr};
+  float* score2 = nullptr;                // second score buffer: the scores of submission i are copied out under batch i + 1
+  cudaStream_t h2d_stream = nullptr;      // inputs of the next submission (PCIe is full duplex: D2H runs on copy_stream)
+  long long n_submitted = 0;
   // timing
   bool timing = false;
   cudaEvent_t ev[256] = {};

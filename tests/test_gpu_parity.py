@@ -496,6 +496,56 @@ def test_run_host_matches_device_run(precision, pinned):
     assert np.array_equal(g2["score"], g["score"])
 
 
+@pytest.mark.parametrize("precision", ["fp32", "bf16"])
+def test_submit_host_pipelined_matches_run_host(precision):
+    import paper_2407_12119_b200 as etx
+    # etx_submit_host / etx_wait_host: two submissions in flight, inputs copied under the previous batch's compute, the
+    # edge list written to the host by the device itself.  Different batches alternate, so any cross-talk between the
+    # two staging sets or output buffers would show.
+    cfg, b, W = _setup("cfg1", 4, precision=precision)
+    blob = datagen.pack_blob(cfg, W)
+    batches = [b.slice_events(0, 2), b.slice_events(1, 4), b.slice_events(2, 3), b, b.slice_events(0, 1)]
+    ctx = make_ctx(cfg, blob, b, validate=True)
+    want = [run_gpu(ctx, x, debug=False) for x in batches]
+    cap = cfg.k * b.n_hits
+    pin = lambda *shape, dtype: torch.empty(*shape, dtype=dtype).pin_memory()
+    bufs = [dict(sc=pin(cap, dtype=torch.float32), s=pin(cap, dtype=torch.int32), d=pin(cap, dtype=torch.int32),
+                 t=pin(b.n_hits, dtype=torch.int32), n=torch.zeros(1, dtype=torch.int32)) for _ in range(2)]
+    hx = [torch.from_numpy(x.xyz).pin_memory() for x in batches]; hp = [torch.from_numpy(x.plane).pin_memory() for x in batches]
+    tickets = []
+
+    def check(i):
+        ctx.wait_host(tickets[i])
+        o, w = bufs[i & 1], want[i]
+        E = int(o["n"][0])
+        assert E == w["n_edges"], i
+        assert np.array_equal(o["s"].numpy()[:E], w["src"]) and np.array_equal(o["d"].numpy()[:E], w["dst"]), i
+        assert np.array_equal(o["sc"].numpy()[:E], w["score"]), i
+        assert np.array_equal(o["t"].numpy()[:batches[i].n_hits], w["track_id"]), i
+
+    for rep in range(2):
+        tickets.clear()
+        for i, x in enumerate(batches):
+            o = bufs[i & 1]
+            tickets.append(ctx.submit_host(hx[i], hp[i], x.event_offsets, o["sc"], o["s"], o["d"], o["t"], o["n"]))
+            if i >= 1:
+                check(i - 1)
+        check(len(batches) - 1)
+    # pageable output buffers are refused (the device writes them itself); a rejected batch reports on ITS ticket
+    with pytest.raises(etx.EtxError) as ei:
+        ctx.submit_host(hx[0], hp[0], batches[0].event_offsets, torch.empty(cap), bufs[0]["s"], bufs[0]["d"], bufs[0]["t"], bufs[0]["n"])
+    assert ei.value.status == -1
+    bad = torch.from_numpy(batches[0].plane[::-1].copy()).pin_memory()
+    t_bad = ctx.submit_host(hx[0], bad, batches[0].event_offsets, bufs[0]["sc"], bufs[0]["s"], bufs[0]["d"], bufs[0]["t"], bufs[0]["n"])
+    t_ok = ctx.submit_host(hx[1], hp[1], batches[1].event_offsets, bufs[1]["sc"], bufs[1]["s"], bufs[1]["d"], bufs[1]["t"], bufs[1]["n"])
+    with pytest.raises(etx.EtxError) as ei:
+        ctx.wait_host(t_bad)
+    assert ei.value.status == -4 and int(bufs[0]["n"][0]) == 0
+    ctx.wait_host(t_ok)
+    assert int(bufs[1]["n"][0]) == want[1]["n_edges"]
+    ctx.destroy()
+
+
 # ================================================================================== tcgen05 engine (bf16 / int8)
 def _int8_blob(cfg, b, W):
     scales = oracle.calibrate_int8(datagen.pack_blob(cfg, W), b.xyz, b.plane, b.event_offsets, cfg.k, cfg.window)
