@@ -162,7 +162,9 @@ etx_status etx_run_host(etx_handle h, const float* h_xyz, const int32_t* h_plane
  * buffers must be pinned (page-locked) host memory.  The edge list and the scores of submission i are copied out, at
  * their exact size, by the next call on the handle -- the submission of i + 1 or the wait for i -- once the host has
  * learnt E, which S3 produced long before: the edge list under batch i's own GNN, the scores under batch i + 1 (each
- * slot has its own device score buffer).  *h_n_edges (plain host int32) receives E and is valid after etx_wait_host.  The h_* input arrays and
+ * slot has its own device score buffer).  *h_n_edges (plain host int32) receives E and is valid after etx_wait_host.
+ * While a submission has not been waited for, etx_run / etx_run_host / etx_dbg_run on the same handle return
+ * ETX_ERR_ARG (they would overwrite its results).  The h_* input arrays and
  * h_event_offsets must stay valid until the submission has completed (h_event_offsets: until the call returns). */
 etx_status etx_submit_host(etx_handle h, const float* h_xyz, const int32_t* h_plane,
                            const int32_t* h_event_offsets, int32_t n_events, etx_stream stream,

@@ -464,6 +464,8 @@ etx_status etx_destroy(etx_handle c) {
 
 etx_status etx_run(etx_handle c, const float* d_xyz, const int32_t* d_plane, const int32_t* h_event_offsets,
                    int32_t n_events, etx_stream stream, etx_output* out) {
+  if (c && (c->slot_copy[0].pending || c->slot_copy[1].pending))
+    return fail(c, ETX_ERR_ARG, "a submission of etx_submit_host has not been waited for yet (etx_wait_host)");
   return run_impl(c, d_xyz, d_plane, h_event_offsets, n_events, static_cast<cudaStream_t>(stream), nullptr, out);
 }
 
@@ -502,6 +504,8 @@ etx_status etx_triplets(etx_handle c, etx_stream stream, etx_triplets_output* ou
 
 etx_status etx_dbg_run(etx_handle c, const float* d_xyz, const int32_t* d_plane, const int32_t* h_event_offsets,
                        int32_t n_events, etx_stream stream, const etx_inject* inj, etx_output* out) {
+  if (c && (c->slot_copy[0].pending || c->slot_copy[1].pending))
+    return fail(c, ETX_ERR_ARG, "a submission of etx_submit_host has not been waited for yet (etx_wait_host)");
   return run_impl(c, d_xyz, d_plane, h_event_offsets, n_events, static_cast<cudaStream_t>(stream), inj, out);
 }
 
@@ -509,6 +513,8 @@ etx_status etx_run_host(etx_handle c, const float* h_xyz, const int32_t* h_plane
                         int32_t n_events, etx_stream stream, float* h_edge_score, int32_t* h_edge_src,
                         int32_t* h_edge_dst, int32_t* h_track_id, int32_t* n_edges_out) {
   if (!c) return ETX_ERR_ARG;
+  if (c && (c->slot_copy[0].pending || c->slot_copy[1].pending))
+    return fail(c, ETX_ERR_ARG, "a submission of etx_submit_host has not been waited for yet (etx_wait_host)");
   if (!h_event_offsets || n_events < 0 || !n_edges_out) return fail(c, ETX_ERR_ARG, "null argument");
   if (n_events > c->hp.max_events) return fail(c, ETX_ERR_CAPACITY, "n_events exceeds max_events");
   const int n_hits = h_event_offsets[n_events];

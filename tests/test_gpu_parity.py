@@ -541,8 +541,19 @@ def test_submit_host_pipelined_matches_run_host(precision):
     with pytest.raises(etx.EtxError) as ei:
         ctx.wait_host(t_bad)
     assert ei.value.status == -4 and int(bufs[0]["n"][0]) == 0
+    # other calls on the handle are refused while a submission is outstanding, and work again afterwards
+    with pytest.raises(etx.EtxError) as ei:
+        run_gpu(ctx, batches[0], debug=False)
+    assert ei.value.status == -1
     ctx.wait_host(t_ok)
     assert int(bufs[1]["n"][0]) == want[1]["n_edges"]
+    g = run_gpu(ctx, batches[0], debug=False)
+    assert np.array_equal(g["score"], want[0]["score"])
+    # an empty batch goes through the pipeline too
+    empty = b.slice_events(0, 0)
+    t = ctx.submit_host(hx[0], hp[0], np.zeros(1, np.int32), bufs[0]["sc"], bufs[0]["s"], bufs[0]["d"], bufs[0]["t"], bufs[0]["n"])
+    ctx.wait_host(t)
+    assert int(bufs[0]["n"][0]) == 0
     ctx.destroy()
 
 
