@@ -49,6 +49,12 @@ struct GnnArgs {
   int edge_enc_input;
   int32_t* tap;              // int32 accumulators of layer tap_layer, or nullptr
   int tap_layer;
+  // INT8, warp-specialised kernels: the node network also stores the int8 codes of the new h under the NEXT edge
+  // network's input scale (hq_out, hq_inv_sx); the edge network gathers those codes (hq_in) instead of re-quantising
+  // h[src] / h[dst] for every edge.  nullptr: quantise on the fly.
+  int8_t* hq_out = nullptr;
+  float hq_inv_sx = 1.0f;
+  const int8_t* hq_in = nullptr;
 };
 
 struct EmbArgs {
@@ -121,6 +127,7 @@ struct etx_ctx {
   std::vector<void*> edge_bias_img;
   alignas(64) unsigned char e_map[128] = {};
   alignas(64) unsigned char h_map[128] = {};   // CUtensorMap of `h` (node encoder output)
+  int8_t* hq = nullptr;                   // [max_hits][d] int8 codes of h for the edge network (INT8, AUTO engine)
   int32_t* tap = nullptr;
   size_t tap_bytes = 0;
   int tap_layer = -1;

@@ -137,6 +137,73 @@ __global__ void __launch_bounds__(kI8Threads, 1) edge_net_i8_kernel(const __grid
       return q;
     };
     int it = 0;
+    if (!NODE && a.hq_in != nullptr) {
+      // h[src], h[dst] arrive as int8 codes (written by the node network under this layer's input scale): the producers
+      // only move them.  The gather is a dependent chain (index -> code row) of L2 round trips, so it is software-
+      // pipelined in registers: codes one tile ahead, indices two tiles ahead; the only values quantised here are the
+      // tile's own state rows.
+      constexpr int ITEMS = (kRows * CPR + kI8ProdThreads - 1) / kI8ProdThreads;
+      auto load_idx = [&](long long tile, int (&js)[ITEMS], int (&jd)[ITEMS]) {
+#pragma unroll
+        for (int i = 0; i < ITEMS; ++i) {
+          const int c = i * kI8ProdThreads + pt;
+          js[i] = 0; jd[i] = 0;
+          if (tile < n_tiles && c < kRows * CPR) {
+            long long grow = tile * kRows + c / CPR;
+            if (grow >= n_rows) grow = n_rows - 1;
+            js[i] = __ldg(a.src + grow); jd[i] = __ldg(a.dst + grow);
+          }
+        }
+      };
+      auto load_codes = [&](const int (&js)[ITEMS], const int (&jd)[ITEMS], uint4 (&cs)[ITEMS], uint4 (&cd)[ITEMS]) {
+#pragma unroll
+        for (int i = 0; i < ITEMS; ++i) {
+          const int piece = (i * kI8ProdThreads + pt) % CPR;
+          cs[i] = __ldg(reinterpret_cast<const uint4*>(a.hq_in + (size_t)js[i] * D) + piece);
+          cd[i] = __ldg(reinterpret_cast<const uint4*>(a.hq_in + (size_t)jd[i] * D) + piece);
+        }
+      };
+      int js1[ITEMS], jd1[ITEMS], js2[ITEMS], jd2[ITEMS];
+      uint4 cs0[ITEMS], cd0[ITEMS], cs1[ITEMS], cd1[ITEMS];
+      load_idx(blockIdx.x, js1, jd1);
+      load_codes(js1, jd1, cs0, cd0);                                // codes of the first tile
+      load_idx((long long)blockIdx.x + gridDim.x, js1, jd1);         // indices of the second
+      for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
+        const int sa = it % kI8A, se = it % NE;
+        uint8_t* st = smem + L.a + sa * STAGE;
+        const uint8_t* es = smem + L.e + se * ETILE;
+        if (tile + gridDim.x < n_tiles) load_codes(js1, jd1, cs1, cd1);   // next tile's codes: in flight under this tile
+        load_idx(tile + 2LL * gridDim.x, js2, jd2);
+        mbar_wait(&a_empty[sa], ((it / kI8A) & 1) ^ 1);
+        mbar_wait(&e_full[se], (it / NE) & 1);
+#pragma unroll
+        for (int i = 0; i < ITEMS; ++i) {
+          const int c = i * kI8ProdThreads + pt;
+          if (c < kRows * CPR) {
+            const int r = c / CPR, piece = c % CPR;
+            uint4 q;
+            if (SB) {
+              const uint4 e0 = *reinterpret_cast<const uint4*>(es + swz<SROW>(r, piece * 2 + 0));
+              const uint4 e1 = *reinterpret_cast<const uint4*>(es + swz<SROW>(r, piece * 2 + 1));
+              q = quant16b(e0, e1);
+            } else {
+              const float4 e0 = *reinterpret_cast<const float4*>(es + e_off(r, piece * 4 + 0));
+              const float4 e1 = *reinterpret_cast<const float4*>(es + e_off(r, piece * 4 + 1));
+              const float4 e2 = *reinterpret_cast<const float4*>(es + e_off(r, piece * 4 + 2));
+              const float4 e3 = *reinterpret_cast<const float4*>(es + e_off(r, piece * 4 + 3));
+              q = quant16(e0, e1, e2, e3);
+            }
+            *reinterpret_cast<uint4*>(st + SELF * BLK + swz<KB>(r, piece)) = q;
+            *reinterpret_cast<uint4*>(st + AUX0 * BLK + swz<KB>(r, piece)) = cs0[i];
+            *reinterpret_cast<uint4*>(st + AUX1 * BLK + swz<KB>(r, piece)) = cd0[i];
+          }
+        }
+        fence_proxy_async();                                    // generic-proxy writes -> visible to the tensor core
+        mbar_arrive(&a_full[sa]);
+#pragma unroll
+        for (int i = 0; i < ITEMS; ++i) { cs0[i] = cs1[i]; cd0[i] = cd1[i]; js1[i] = js2[i]; jd1[i] = jd2[i]; }
+      }
+    } else
     for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
       const int sa = it % kI8A, se = it % NE;
       uint8_t* st = smem + L.a + sa * STAGE;
@@ -302,6 +369,7 @@ __global__ void __launch_bounds__(kI8Threads, 1) edge_net_i8_kernel(const __grid
       mbar_wait(&acc1_full[g], j & 1);
       tc_fence_after();
       float hacc = 0.0f;
+      uint32_t hq_w[4] = {0u, 0u, 0u, 0u};
 #pragma unroll
       for (int c0 = 0; c0 < D; c0 += 32) {
         uint32_t v[32];
@@ -325,6 +393,12 @@ __global__ void __launch_bounds__(kI8Threads, 1) edge_net_i8_kernel(const __grid
             qv.z = pack_bf16x2(__fadd_rn(bf16_lo(o.z), y[4]), __fadd_rn(bf16_hi(o.z), y[5]));
             qv.w = pack_bf16x2(__fadd_rn(bf16_lo(o.w), y[6]), __fadd_rn(bf16_hi(o.w), y[7]));
             *p = qv;
+            if (NODE && a.hq_out && live) {                   // codes of the stored h for the edge network that follows
+              const float is = a.hq_inv_sx;
+              hq_w[(ch & 1) * 2 + 0] = pack_i8x4(quant_i8(bf16_lo(qv.x), is), quant_i8(bf16_hi(qv.x), is), quant_i8(bf16_lo(qv.y), is), quant_i8(bf16_hi(qv.y), is));
+              hq_w[(ch & 1) * 2 + 1] = pack_i8x4(quant_i8(bf16_lo(qv.z), is), quant_i8(bf16_hi(qv.z), is), quant_i8(bf16_lo(qv.w), is), quant_i8(bf16_hi(qv.w), is));
+              if (ch & 1) *reinterpret_cast<uint4*>(a.hq_out + (size_t)row * D + c - 8) = make_uint4(hq_w[0], hq_w[1], hq_w[2], hq_w[3]);
+            }
             if (!NODE && a.do_head) {                         // the classifier sees the stored (rounded) state, ascending j (R16)
               hacc = __fmaf_rn(bf16_lo(qv.x), headw[c + 0], hacc); hacc = __fmaf_rn(bf16_hi(qv.x), headw[c + 1], hacc);
               hacc = __fmaf_rn(bf16_lo(qv.y), headw[c + 2], hacc); hacc = __fmaf_rn(bf16_hi(qv.y), headw[c + 3], hacc);
@@ -344,6 +418,11 @@ __global__ void __launch_bounds__(kI8Threads, 1) edge_net_i8_kernel(const __grid
           y.z = __fadd_rn(o.z, __fmaf_rn((float)(int)v[ch * 4 + 2], scale1[c + 2], bias1[c + 2]));
           y.w = __fadd_rn(o.w, __fmaf_rn((float)(int)v[ch * 4 + 3], scale1[c + 3], bias1[c + 3]));
           *p = y;
+          if (NODE && a.hq_out && live) {
+            const float is = a.hq_inv_sx;
+            hq_w[ch & 3] = pack_i8x4(quant_i8(y.x, is), quant_i8(y.y, is), quant_i8(y.z, is), quant_i8(y.w, is));
+            if ((ch & 3) == 3) *reinterpret_cast<uint4*>(a.hq_out + (size_t)row * D + c - 12) = make_uint4(hq_w[0], hq_w[1], hq_w[2], hq_w[3]);
+          }
           if (!NODE && a.do_head) {                           // ascending j (R16)
             hacc = __fmaf_rn(y.x, headw[c + 0], hacc); hacc = __fmaf_rn(y.y, headw[c + 1], hacc);
             hacc = __fmaf_rn(y.z, headw[c + 2], hacc); hacc = __fmaf_rn(y.w, headw[c + 3], hacc);
@@ -387,6 +466,8 @@ void edge_i8_launch(etx_ctx* c, const GnnArgs& a, int max_rows, cudaStream_t s) 
 
 // INT8 mode: tensor map of the fp32 edge state (boxes of 128 rows x 32 floats, 128B swizzle)
 bool edge_i8_configure(etx_ctx* c) {
+  c->hq = static_cast<int8_t*>(etx_device_alloc(c, (size_t)(c->hp.max_hits > 0 ? c->hp.max_hits : 1) * c->hp.gnn_latent + 256));
+  if (!c->hq) return false;
   static_assert(sizeof(CUtensorMap) == sizeof(c->e_map), "etx_ctx::e_map must hold a CUtensorMap");
   void* fn = nullptr;
   cudaDriverEntryPointQueryResult qres;
@@ -415,6 +496,7 @@ void launch_edge_net_i8(etx_ctx* c, int iter, int n_hits, bool do_head, cudaStre
   GnnArgs a;
   fill_gnn_args(c, kEdgeNet, iter, n_hits, do_head, a);
   if (do_head && !c->keep_final_state) a.do_head = 2;        // e^L feeds only the classifier: do not write it back
+  a.hq_in = c->hq;                                           // written by this iteration's node network (launch_node_net_i8)
   const long long max_rows_ll = (long long)n_hits * c->hp.k;
   const int max_rows = (int)(max_rows_ll > 0x7fffffff ? 0x7fffffff : max_rows_ll);
   if (c->state_bf16) { if (c->hp.gnn_latent == 32) edge_i8_launch<32, false, true>(c, a, max_rows, s); else edge_i8_launch<64, false, true>(c, a, max_rows, s); }
@@ -425,6 +507,8 @@ void launch_edge_net_i8(etx_ctx* c, int iter, int n_hits, bool do_head, cudaStre
 void launch_node_net_i8(etx_ctx* c, int iter, int n_hits, cudaStream_t s) {
   GnnArgs a;
   fill_gnn_args(c, kNodeNet, iter, n_hits, false, a);
+  a.hq_out = c->hq;                                          // codes of the new h under the input scale of this iteration's edge network
+  a.hq_inv_sx = c->layers[c->i_iter0 + 4 * iter + 2].dev.inv_sx;
   if (c->state_bf16) { if (c->hp.gnn_latent == 32) edge_i8_launch<32, true, true>(c, a, n_hits, s); else edge_i8_launch<64, true, true>(c, a, n_hits, s); }
   else { if (c->hp.gnn_latent == 32) edge_i8_launch<32, true, false>(c, a, n_hits, s); else edge_i8_launch<64, true, false>(c, a, n_hits, s); }
 }
