@@ -107,6 +107,13 @@ def lib():
         L.etxo_tracks_from_triplets.argtypes = ([C.POINTER(C.c_int32), C.POINTER(C.c_int32), u8p, C.c_int64]
                                                 + [C.POINTER(C.c_int32), C.POINTER(C.c_int32), u8p, C.c_int64] * 3
                                                 + [C.c_int32, C.POINTER(C.c_int32), C.c_int64, C.POINTER(C.c_int32), C.c_int64])
+        L.etxo_triplet_components.restype = C.c_int64
+        L.etxo_triplet_components.argtypes = ([u8p, C.c_int64] + [C.POINTER(C.c_int32), C.POINTER(C.c_int32), u8p, C.c_int64] * 3
+                                              + [C.POINTER(C.c_int32)] * 3)
+        L.etxo_tracks_from_components.restype = C.c_int64
+        L.etxo_tracks_from_components.argtypes = [C.POINTER(C.c_int32), C.POINTER(C.c_int32), C.POINTER(C.c_int32), C.c_int64,
+                                                  C.POINTER(C.c_int32), C.POINTER(C.c_int32), C.c_int64, C.c_int32,
+                                                  C.POINTER(C.c_int32), C.c_int64, C.POINTER(C.c_int32), C.c_int64]
         _lib = L
     return _lib
 
@@ -238,6 +245,42 @@ def tracks_from_triplets(src, dst, keep, art, keep_art, left, keep_left, right, 
             _p(args[3], C.c_int32), _p(args[4], C.c_int32), _p(args[5], C.c_uint8), args[3].size,
             _p(args[6], C.c_int32), _p(args[7], C.c_int32), _p(args[8], C.c_uint8), args[6].size,
             int(min_hits), _p(offs, C.c_int32), cap_tracks, _p(hits, C.c_int32), cap_hits))
+        if T >= 0:
+            return offs[:T + 1].copy(), hits[:offs[T]].copy()
+        cap_hits *= 4
+
+
+def triplet_components(keep, art, keep_art, left, keep_left, right, keep_right):
+    """Phases (1)-(2) of sec. 5.4 (etxo_triplet_components).  -> (edge_comp [E], shared [n, 2] sorted, unique)."""
+    keep = _u8(keep)
+    E = keep.size
+    args = []
+    for (f, s), kf in ((art, keep_art), (left, keep_left), (right, keep_right)):
+        args += [_i32(f), _i32(s), _u8(kf)]
+    TA = args[0].size
+    comp = np.zeros(max(E, 1), np.int32); sx = np.zeros(max(TA, 1), np.int32); sy = np.zeros(max(TA, 1), np.int32)
+    n = int(lib().etxo_triplet_components(
+        _p(keep, C.c_uint8), E,
+        _p(args[0], C.c_int32), _p(args[1], C.c_int32), _p(args[2], C.c_uint8), args[0].size,
+        _p(args[3], C.c_int32), _p(args[4], C.c_int32), _p(args[5], C.c_uint8), args[3].size,
+        _p(args[6], C.c_int32), _p(args[7], C.c_int32), _p(args[8], C.c_uint8), args[6].size,
+        _p(comp, C.c_int32), _p(sx, C.c_int32), _p(sy, C.c_int32)))
+    return comp[:E].copy(), np.stack([sx[:n], sy[:n]], axis=1).astype(np.int32)
+
+
+def tracks_from_components(src, dst, edge_comp, shared, min_hits=3):
+    """Phases (3)-(4) of sec. 5.4 (etxo_tracks_from_components).  -> (track_offsets [T + 1], track_hits)."""
+    src, dst, comp = _i32(src), _i32(dst), _i32(edge_comp)
+    shared = np.asarray(shared, np.int32).reshape(-1, 2)
+    sx, sy = _i32(shared[:, 0]), _i32(shared[:, 1])
+    E = src.size
+    cap_tracks = E + shared.shape[0] + 1
+    cap_hits = 4 * (E + 1) + 16
+    while True:
+        offs = np.zeros(cap_tracks + 1, np.int32); hits = np.zeros(cap_hits, np.int32)
+        T = int(lib().etxo_tracks_from_components(_p(src, C.c_int32), _p(dst, C.c_int32), _p(comp, C.c_int32), E,
+                                                  _p(sx, C.c_int32), _p(sy, C.c_int32), shared.shape[0], int(min_hits),
+                                                  _p(offs, C.c_int32), cap_tracks, _p(hits, C.c_int32), cap_hits))
         if T >= 0:
             return offs[:T + 1].copy(), hits[:offs[T]].copy()
         cap_hits *= 4

@@ -723,14 +723,19 @@ int etxo_has_triplets(void* m) { return static_cast<Model*>(m)->has_triplets; }
 //      hit list (R31), so that it can be compared as arrays.
 // Only kept edges take part (an edge below the edge threshold is in no triplet, L146); a kept edge without any
 // kept triplet is a component of its own (two hits).  keepA / keepL / keepR flag the kept triplets of each kind.
-// Outputs: track_offsets[T + 1], track_hits[...] (capacities given by the caller: cap_tracks + 1, cap_hits);
-// returns T, or -1 if a capacity is too small.
-int64_t etxo_tracks_from_triplets(const int32_t* src, const int32_t* dst, const uint8_t* keep, int64_t E,
-                                  const int32_t* a_first, const int32_t* a_second, const uint8_t* keepA, int64_t TA,
-                                  const int32_t* l_first, const int32_t* l_second, const uint8_t* keepL, int64_t TL,
-                                  const int32_t* r_first, const int32_t* r_second, const uint8_t* keepR, int64_t TR,
-                                  int32_t min_hits, int32_t* track_offsets, int64_t cap_tracks,
-                                  int32_t* track_hits, int64_t cap_hits) {
+//
+// The work is split in two so that the first half can be compared with the CUDA path, which stops there:
+//   etxo_triplet_components  phases (1)-(2): edge_comp[e] = the component of kept edge e, named by the smallest edge
+//                            id in it (-1 for an edge that is not kept), and the shared articulations as pairs of
+//                            component names, sorted and without repeats (a pair with equal names is kept: it still
+//                            marks its component as part of a shared structure).  Returns the number of pairs
+//                            (capacity TA).
+//   etxo_tracks_from_components  phases (3)-(4).
+int64_t etxo_triplet_components(const uint8_t* keep, int64_t E,
+                                const int32_t* a_first, const int32_t* a_second, const uint8_t* keepA, int64_t TA,
+                                const int32_t* l_first, const int32_t* l_second, const uint8_t* keepL, int64_t TL,
+                                const int32_t* r_first, const int32_t* r_second, const uint8_t* keepR, int64_t TR,
+                                int32_t* edge_comp, int32_t* shared_x, int32_t* shared_y) {
   std::vector<int32_t> sup(E);
   for (int64_t i = 0; i < E; ++i) sup[i] = (int32_t)i;
   auto find = [](std::vector<int32_t>& p, int32_t x) {
@@ -763,20 +768,31 @@ int64_t etxo_tracks_from_triplets(const int32_t* src, const int32_t* dst, const 
     if (n_succ[a.first] >= 2 || n_pred[a.second] >= 2) shared.push_back(a);
     else unite(comp, a.first, a.second);
   }
+  for (int64_t i = 0; i < E; ++i) edge_comp[i] = keep[i] ? find(comp, find(sup, (int32_t)i)) : -1;
+  for (auto& a : shared) { a.first = find(comp, a.first); a.second = find(comp, a.second); }
+  std::sort(shared.begin(), shared.end());
+  shared.erase(std::unique(shared.begin(), shared.end()), shared.end());
+  for (size_t i = 0; i < shared.size(); ++i) { shared_x[i] = shared[i].first; shared_y[i] = shared[i].second; }
+  return (int64_t)shared.size();
+}
+
+// Outputs: track_offsets[T + 1], track_hits[...] (capacities given by the caller: cap_tracks + 1, cap_hits);
+// returns T, or -1 if a capacity is too small.
+int64_t etxo_tracks_from_components(const int32_t* src, const int32_t* dst, const int32_t* edge_comp, int64_t E,
+                                    const int32_t* shared_x, const int32_t* shared_y, int64_t n_shared,
+                                    int32_t min_hits, int32_t* track_offsets, int64_t cap_tracks,
+                                    int32_t* track_hits, int64_t cap_hits) {
   // (3) tracks as sets of components
   std::vector<uint8_t> touched(E, 0);
   std::vector<std::vector<int32_t>> track_comps;
-  for (auto& a : shared) {
-    const int32_t p = find(comp, a.first), q = find(comp, a.second);
+  for (int64_t i = 0; i < n_shared; ++i) {
+    const int32_t p = shared_x[i], q = shared_y[i];
     touched[p] = touched[q] = 1;
     if (p == q) track_comps.push_back({p}); else track_comps.push_back({p, q});
   }
-  for (int64_t i = 0; i < E; ++i)
-    if (keep[i] && find(sup, (int32_t)i) == i && find(comp, (int32_t)i) == i && !touched[i]) track_comps.push_back({(int32_t)i});
-  // members of every component: kept edges by the component of their super-edge
-  std::vector<std::vector<int32_t>> members(E);
-  for (int64_t i = 0; i < E; ++i)
-    if (keep[i]) members[find(comp, find(sup, (int32_t)i))].push_back((int32_t)i);
+  std::vector<std::vector<int32_t>> members(E);                       // kept edges by component name
+  for (int64_t i = 0; i < E; ++i) if (edge_comp[i] >= 0) members[edge_comp[i]].push_back((int32_t)i);
+  for (int64_t i = 0; i < E; ++i) if (!members[i].empty() && !touched[i]) track_comps.push_back({(int32_t)i});
   // (4) edges -> hits
   std::vector<std::vector<int32_t>> tracks;
   for (auto& tc : track_comps) {
@@ -797,6 +813,19 @@ int64_t etxo_tracks_from_triplets(const int32_t* src, const int32_t* dst, const 
     track_offsets[t + 1] = (int32_t)pos;
   }
   return (int64_t)tracks.size();
+}
+
+int64_t etxo_tracks_from_triplets(const int32_t* src, const int32_t* dst, const uint8_t* keep, int64_t E,
+                                  const int32_t* a_first, const int32_t* a_second, const uint8_t* keepA, int64_t TA,
+                                  const int32_t* l_first, const int32_t* l_second, const uint8_t* keepL, int64_t TL,
+                                  const int32_t* r_first, const int32_t* r_second, const uint8_t* keepR, int64_t TR,
+                                  int32_t min_hits, int32_t* track_offsets, int64_t cap_tracks,
+                                  int32_t* track_hits, int64_t cap_hits) {
+  std::vector<int32_t> edge_comp(E > 0 ? E : 1), sx(TA > 0 ? TA : 1), sy(TA > 0 ? TA : 1);
+  const int64_t ns = etxo_triplet_components(keep, E, a_first, a_second, keepA, TA, l_first, l_second, keepL, TL,
+                                             r_first, r_second, keepR, TR, edge_comp.data(), sx.data(), sy.data());
+  return etxo_tracks_from_components(src, dst, edge_comp.data(), E, sx.data(), sy.data(), ns, min_hits,
+                                     track_offsets, cap_tracks, track_hits, cap_hits);
 }
 
 }  // extern "C"

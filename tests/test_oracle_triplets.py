@@ -323,3 +323,22 @@ def test_run_triplets_end_to_end_shapes_and_thresholds():
     assert t["track_offsets"][0] == 0 and (np.diff(t["track_offsets"]) >= 3).all()
     # every hit of every track is a hit of the event; tracks may share hits (that is the point of sec. 5.4)
     assert t["track_hits"].max(initial=0) < b.n_hits
+
+
+@pytest.mark.parametrize("seed", [0, 3, 5])
+def test_components_then_tracks_equals_the_one_call_and_component_names_are_minimum_edge_ids(seed):
+    plane, src, dst, keep = _random_graph(seed, n=16, E=34)
+    rng = np.random.default_rng(200 + seed)
+    trip = {k: oracle.triplets(src, dst, keep, plane.size, k)[:2] for k in ("articulation", "left_elbow", "right_elbow")}
+    ka = (rng.random(trip["articulation"][0].size) < 0.7).astype(np.uint8)
+    kl = (rng.random(trip["left_elbow"][0].size) < 0.3).astype(np.uint8)
+    kr = (rng.random(trip["right_elbow"][0].size) < 0.3).astype(np.uint8)
+    comp, shared = oracle.triplet_components(keep, trip["articulation"], ka, trip["left_elbow"], kl, trip["right_elbow"], kr)
+    assert np.array_equal(comp >= 0, keep > 0)
+    for c in np.unique(comp[comp >= 0]):
+        assert c == np.flatnonzero(comp == c).min()              # a component is named by its smallest edge id
+    assert shared.shape[0] > 0 and np.array_equal(shared, np.unique(shared, axis=0))
+    assert set(shared.reshape(-1).tolist()) <= set(comp[comp >= 0].tolist())
+    a = oracle.tracks_from_components(src, dst, comp, shared, 3)
+    b = oracle.tracks_from_triplets(src, dst, keep, trip["articulation"], ka, trip["left_elbow"], kl, trip["right_elbow"], kr, 3)
+    assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
