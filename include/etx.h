@@ -218,6 +218,27 @@ typedef struct {
 
 etx_status etx_triplets(etx_handle h, etx_stream stream, etx_triplets_output* out);
 
+/* Track building from triplets, phases (1)-(2) (sec. 5.4; R30).  Enqueue after
+ * etx_triplets on the same stream and handle.  Triplets are kept iff logit >= tau_t (triplet_threshold).  The two
+ * edges of every kept elbow are merged into a super-edge; kept articulations are mapped onto super-edges (duplicates
+ * collapse); an articulation is SHARED iff its first super-edge has >= 2 distinct successors or its second >= 2
+ * distinct predecessors; the other articulations connect their super-edges.  Results:
+ *   d_edge_component [n_edges]  for a kept edge the name of its set of connected edges = the smallest edge id in it,
+ *                               -1 for an edge below the edge threshold
+ *   d_shared [n_shared][2]      the shared articulations as (component of first, component of second); unordered and
+ *                               possibly repeated -- a set (each yields the track "union of the two components",
+ *                               phase 3; the expansion into hit lists, phases 3-4, is a host-side listing)
+ * Exact only if no triplet count exceeded max_triplets (compare etx_triplets' counts).  No synchronisation. */
+typedef struct {
+  const int32_t* d_edge_component;
+  const int32_t* d_shared;
+  const int32_t* d_n_shared;
+  const int32_t* h_n_shared;             /* pinned mirror; valid once the stream has been synchronised */
+  int32_t        capacity;               /* pairs d_shared can hold (= max_triplets)                    */
+} etx_triplet_components_output;
+
+etx_status etx_triplet_components(etx_handle h, etx_stream stream, etx_triplet_components_output* out);
+
 etx_status etx_destroy(etx_handle h);
 
 /* Device bytes held by the handle (workspace + converted weights), as requested from the allocator. */

@@ -58,6 +58,11 @@ class EtxTriplets(C.Structure):
                 ("h_count", C.POINTER(C.c_int32)), ("capacity", C.c_int32)]
 
 
+class EtxTripletComponents(C.Structure):
+    _fields_ = [("d_edge_component", C.c_void_p), ("d_shared", C.c_void_p), ("d_n_shared", C.c_void_p),
+                ("h_n_shared", C.POINTER(C.c_int32)), ("capacity", C.c_int32)]
+
+
 class Inject(C.Structure):
     _fields_ = [("d_emb", C.c_void_p), ("d_src", C.c_void_p), ("d_dst", C.c_void_p), ("n_edges", C.c_int32),
                 ("d_logit", C.c_void_p), ("last_stage", C.c_int32)]
@@ -101,6 +106,8 @@ def load_library():
     L.etx_wait_host.argtypes = [vp, C.c_int32]
     L.etx_triplets.restype = C.c_int
     L.etx_triplets.argtypes = [vp, vp, C.POINTER(EtxTriplets)]
+    L.etx_triplet_components.restype = C.c_int
+    L.etx_triplet_components.argtypes = [vp, vp, C.POINTER(EtxTripletComponents)]
     L.etx_input_status.restype = C.c_int
     L.etx_input_status.argtypes = [vp]
     L.etx_tracks.restype = C.c_int
@@ -302,6 +309,16 @@ class Etx:
                              hit=self._copy_out(out.d_hit[k], 4 * n, torch.int32), logit=self._copy_out(out.d_logit[k], 4 * n, torch.float32),
                              score=self._copy_out(out.d_score[k], 4 * n, torch.float32))
         return res
+
+    def triplet_components(self, n_edges: int) -> dict:
+        """etx_triplet_components after triplets(); synchronises.  -> dict(edge_component [E], shared [n, 2])."""
+        import torch
+        out = EtxTripletComponents()
+        self._check(self._L.etx_triplet_components(self._h, self._stream(), C.byref(out)), "etx_triplet_components")
+        torch.cuda.current_stream().synchronize()
+        n = min(int(out.h_n_shared[0]), int(out.capacity))
+        return dict(edge_component=self._copy_out(out.d_edge_component, 4 * n_edges, torch.int32),
+                    shared=self._copy_out(out.d_shared, 8 * n, torch.int32).reshape(-1, 2), n_shared=int(out.h_n_shared[0]))
 
     def workspace_bytes(self) -> int:
         return int(self._L.etx_workspace_bytes(self._h))

@@ -339,6 +339,9 @@ etx_status etx_create(const void* blob, size_t blob_bytes, const etx_hyperparams
   if (hp->threshold <= 0.0f) c->tau = -INFINITY;
   else if (hp->threshold >= 1.0f) c->tau = INFINITY;
   else c->tau = (float)log((double)hp->threshold / (1.0 - (double)hp->threshold));      // R17
+  if (hp->triplet_threshold <= 0.0f) c->tau_t = -INFINITY;
+  else if (hp->triplet_threshold >= 1.0f) c->tau_t = INFINITY;
+  else c->tau_t = (float)log((double)hp->triplet_threshold / (1.0 - (double)hp->triplet_threshold));
   etx_status st = ETX_OK;
   try {
     st = parse_blob(c, static_cast<const uint8_t*>(blob), blob_bytes);
@@ -390,6 +393,15 @@ etx_status etx_create(const void* blob, size_t blob_bytes, const etx_hyperparams
       c->trip_first = dev_alloc<int32_t>(c, 3 * T); c->trip_second = dev_alloc<int32_t>(c, 3 * T); c->trip_hit = dev_alloc<int32_t>(c, 3 * T);
       c->trip_logit = dev_alloc<float>(c, 3 * T); c->trip_score = dev_alloc<float>(c, 3 * T);
       c->trip_total = dev_alloc<int32_t>(c, 4);
+      c->tc_par1 = dev_alloc<int32_t>(c, E); c->tc_par2 = dev_alloc<int32_t>(c, E);
+      c->tc_succ = dev_alloc<int32_t>(c, E); c->tc_pred = dev_alloc<int32_t>(c, E); c->tc_comp = dev_alloc<int32_t>(c, E);
+      c->tc_shared = dev_alloc<int32_t>(c, 2 * T);
+      c->tc_tab_size = 1024; while (c->tc_tab_size < 2 * T) c->tc_tab_size <<= 1;
+      c->tc_tab = dev_alloc<unsigned long long>(c, c->tc_tab_size);
+      c->tc_n_shared = dev_alloc<int32_t>(c, 1);
+      ETX_CUDA(cudaMemset(c->tc_n_shared, 0, sizeof(int32_t)));
+      ETX_CUDA(cudaMallocHost(&c->h_tc_n_shared, sizeof(int32_t)));
+      c->h_tc_n_shared[0] = 0;
       ETX_CUDA(cudaMemset(c->trip_total, 0, 4 * sizeof(int32_t)));
       ETX_CUDA(cudaMallocHost(&c->h_trip_total, 4 * sizeof(int32_t)));
       for (int i = 0; i < 4; ++i) c->h_trip_total[i] = 0;
@@ -442,6 +454,7 @@ etx_status etx_destroy(etx_handle c) {
   if (c->h_n_tracks) cudaFreeHost(c->h_n_tracks);
   if (c->h_flags) cudaFreeHost(c->h_flags);
   if (c->h_trip_total) cudaFreeHost(c->h_trip_total);
+  if (c->h_tc_n_shared) cudaFreeHost(c->h_tc_n_shared);
   if (c->h_slot_flags) cudaFreeHost(c->h_slot_flags);
   if (c->h_slot_n_edges) cudaFreeHost(c->h_slot_n_edges);
   for (int i = 0; i < 2; ++i) {
@@ -499,6 +512,20 @@ etx_status etx_triplets(etx_handle c, etx_stream stream, etx_triplets_output* ou
     out->d_logit[k] = c->trip_logit + k * T; out->d_score[k] = c->trip_score + k * T;
   }
   out->d_count = c->trip_total; out->h_count = c->h_trip_total; out->capacity = c->hp.max_triplets;
+  return ETX_OK;
+}
+
+etx_status etx_triplet_components(etx_handle c, etx_stream stream, etx_triplet_components_output* out) {
+  if (!c) return ETX_ERR_ARG;
+  if (!out) return fail(c, ETX_ERR_ARG, "etx_triplet_components: null output");
+  if (c->i_trip < 0 || c->hp.max_triplets <= 0) return fail(c, ETX_ERR_CAPACITY, "etx_triplet_components: the triplet stage is not configured");
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  launch_triplet_components(c, s);
+  if (cudaMemcpyAsync(c->h_tc_n_shared, c->tc_n_shared, sizeof(int32_t), cudaMemcpyDeviceToHost, s) != cudaSuccess ||
+      cudaGetLastError() != cudaSuccess)
+    return fail(c, ETX_ERR_CUDA, "etx_triplet_components: launch failed");
+  out->d_edge_component = c->tc_comp; out->d_shared = c->tc_shared; out->d_n_shared = c->tc_n_shared;
+  out->h_n_shared = c->h_tc_n_shared; out->capacity = c->hp.max_triplets;
   return ETX_OK;
 }
 

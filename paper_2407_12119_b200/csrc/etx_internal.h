@@ -116,6 +116,13 @@ struct etx_ctx {
   int32_t *trip_cnt = nullptr, *trip_off = nullptr, *trip_first = nullptr, *trip_second = nullptr, *trip_hit = nullptr;
   float *trip_logit = nullptr, *trip_score = nullptr;
   int32_t *trip_total = nullptr, *h_trip_total = nullptr;   // [3] device / pinned
+  // etx_triplet_components: union-find parents over edges (elbows; non-shared articulations), distinct successor /
+  // predecessor counts, hash set of (super-edge, super-edge) pairs, outputs
+  int32_t *tc_par1 = nullptr, *tc_par2 = nullptr, *tc_succ = nullptr, *tc_pred = nullptr, *tc_comp = nullptr, *tc_shared = nullptr;
+  unsigned long long* tc_tab = nullptr;
+  size_t tc_tab_size = 0;
+  int32_t *tc_n_shared = nullptr, *h_tc_n_shared = nullptr;
+  float tau_t = 0.0f;
   int last_n_events = 0;
   // k_edge_tma.cu: identity operand image, split-bias images [2 * iter + layer], CUtensorMap of `e` (opaque here)
   bool edge_tma = false;
@@ -203,6 +210,7 @@ void launch_csc(etx_ctx* c, int n_events, int n_hits, bool windowed, cudaStream_
 void launch_components(etx_ctx* c, const float* logit, int n_events, int n_hits, cudaStream_t s);
 void launch_tracks(etx_ctx* c, int n_events, int n_hits, int min_hits, cudaStream_t s);
 void launch_triplet_build(etx_ctx* c, int n_hits, cudaStream_t s);
+void launch_triplet_components(etx_ctx* c, cudaStream_t s);
 // k_mlp_simt.cu
 void launch_embed_simt(etx_ctx* c, int n_hits, cudaStream_t s);
 void launch_gnn_mlp_simt(etx_ctx* c, int kind, int iter, int n_hits, bool do_head, cudaStream_t s);

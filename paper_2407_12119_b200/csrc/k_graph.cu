@@ -817,4 +817,98 @@ void launch_triplet_build(etx_ctx* c, int n_hits, cudaStream_t s) {
   c->launches += 3;
 }
 
+// --------------------------------------------------------------------------------------------------------
+// Track building from triplets, phases (1)-(2) (sec. 5.4; R30): which kept edges end up
+// in one set of connected edges, and which articulations are shared.  Same lock-free union-find as S5 (roots only
+// ever move to a smaller index, so a set is named by its smallest edge id whatever the interleaving); the distinct
+// (super-edge, super-edge) articulation pairs are collected in an open-addressing hash set, the first inserter of a
+// pair counting it as a successor / predecessor.  All outputs are sets or minima: deterministic.
+constexpr unsigned long long kTcEmpty = 0xffffffffffffffffull;
+
+__global__ void tc_init_kernel(int32_t* __restrict__ par1, int32_t* __restrict__ par2, int32_t* __restrict__ n_succ,
+                               int32_t* __restrict__ n_pred, const int32_t* __restrict__ n_edges,
+                               unsigned long long* __restrict__ tab, size_t tab_size, int32_t* __restrict__ n_shared) {
+  const int E = *n_edges;
+  const size_t stride = (size_t)gridDim.x * blockDim.x, t0 = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  for (size_t i = t0; i < (size_t)E; i += stride) { par1[i] = (int32_t)i; par2[i] = (int32_t)i; n_succ[i] = 0; n_pred[i] = 0; }
+  for (size_t i = t0; i < tab_size; i += stride) tab[i] = kTcEmpty;
+  if (t0 == 0) *n_shared = 0;
+}
+
+// (1) the two edges of every kept elbow (kinds 1 and 2) become one super-edge
+__global__ void tc_elbows_kernel(const int32_t* __restrict__ first, const int32_t* __restrict__ second, const float* __restrict__ logit,
+                                 const int32_t* __restrict__ total, int cap, float tau_t, int32_t* par1) {
+  const size_t stride = (size_t)gridDim.x * blockDim.x;
+  for (int kind = 1; kind <= 2; ++kind) {
+    const int n = min(total[kind], cap);
+    const size_t o = (size_t)kind * cap;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < (size_t)n; i += stride)
+      if (logit[o + i] >= tau_t) uf_union(par1, first[o + i], second[o + i]);
+  }
+}
+
+__device__ __forceinline__ size_t tc_hash(unsigned long long k, size_t mask) {
+  k ^= k >> 33; k *= 0xff51afd7ed558ccdull; k ^= k >> 33; k *= 0xc4ceb9fe1a85ec53ull; k ^= k >> 33;
+  return (size_t)k & mask;
+}
+
+// kept articulations mapped onto super-edges; duplicates collapse, one inside a super-edge disappears
+__global__ void tc_arts_kernel(const int32_t* __restrict__ first, const int32_t* __restrict__ second, const float* __restrict__ logit,
+                               const int32_t* __restrict__ total, int cap, float tau_t, int32_t* par1,
+                               unsigned long long* tab, size_t mask, int32_t* n_succ, int32_t* n_pred) {
+  const int n = min(total[0], cap);
+  const size_t stride = (size_t)gridDim.x * blockDim.x;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < (size_t)n; i += stride) {
+    if (!(logit[i] >= tau_t)) continue;
+    const int x = uf_find(par1, first[i]), y = uf_find(par1, second[i]);
+    if (x == y) continue;
+    const unsigned long long key = ((unsigned long long)(unsigned)x << 32) | (unsigned)y;
+    size_t slot = tc_hash(key, mask);
+    while (true) {
+      const unsigned long long old = atomicCAS(&tab[slot], kTcEmpty, key);
+      if (old == kTcEmpty) { atomicAdd(&n_succ[x], 1); atomicAdd(&n_pred[y], 1); break; }
+      if (old == key) break;
+      slot = (slot + 1) & mask;
+    }
+  }
+}
+
+// (2) a pair is shared iff its first super-edge has >= 2 distinct successors or its second >= 2 distinct predecessors;
+// the others connect their super-edges
+__global__ void tc_link_kernel(const unsigned long long* __restrict__ tab, size_t tab_size, const int32_t* __restrict__ n_succ,
+                               const int32_t* __restrict__ n_pred, int32_t* par2, int32_t* __restrict__ shared, int32_t* n_shared, int cap) {
+  const size_t stride = (size_t)gridDim.x * blockDim.x;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < tab_size; i += stride) {
+    const unsigned long long key = tab[i];
+    if (key == kTcEmpty) continue;
+    const int x = (int)(key >> 32), y = (int)(key & 0xffffffffu);
+    if (n_succ[x] >= 2 || n_pred[y] >= 2) {
+      const int p = atomicAdd(n_shared, 1);
+      if (p < cap) { shared[2 * (size_t)p] = x; shared[2 * (size_t)p + 1] = y; }
+    } else {
+      uf_union(par2, x, y);
+    }
+  }
+}
+
+__global__ void tc_label_kernel(const float* __restrict__ edge_logit, float tau, const int32_t* __restrict__ n_edges, int32_t* par1,
+                                int32_t* par2, int32_t* __restrict__ edge_comp, int32_t* __restrict__ shared,
+                                const int32_t* __restrict__ n_shared, int cap) {
+  const int E = *n_edges, ns = min(*n_shared, cap);
+  const size_t stride = (size_t)gridDim.x * blockDim.x, t0 = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  for (size_t i = t0; i < (size_t)E; i += stride) edge_comp[i] = edge_logit[i] >= tau ? uf_find(par2, uf_find(par1, (int)i)) : -1;
+  for (size_t i = t0; i < 2 * (size_t)ns; i += stride) shared[i] = uf_find(par2, shared[i]);
+}
+
+void launch_triplet_components(etx_ctx* c, cudaStream_t s) {
+  const int g = c->sm_count * 8, cap = c->hp.max_triplets;
+  tc_init_kernel<<<g, 256, 0, s>>>(c->tc_par1, c->tc_par2, c->tc_succ, c->tc_pred, c->n_edges, c->tc_tab, c->tc_tab_size, c->tc_n_shared);
+  tc_elbows_kernel<<<g, 256, 0, s>>>(c->trip_first, c->trip_second, c->trip_logit, c->trip_total, cap, c->tau_t, c->tc_par1);
+  tc_arts_kernel<<<g, 256, 0, s>>>(c->trip_first, c->trip_second, c->trip_logit, c->trip_total, cap, c->tau_t, c->tc_par1,
+                                   c->tc_tab, c->tc_tab_size - 1, c->tc_succ, c->tc_pred);
+  tc_link_kernel<<<g, 256, 0, s>>>(c->tc_tab, c->tc_tab_size, c->tc_succ, c->tc_pred, c->tc_par2, c->tc_shared, c->tc_n_shared, cap);
+  tc_label_kernel<<<g, 256, 0, s>>>(c->logit, c->tau, c->n_edges, c->tc_par1, c->tc_par2, c->tc_comp, c->tc_shared, c->tc_n_shared, cap);
+  c->launches += 5;
+}
+
 }  // namespace etx

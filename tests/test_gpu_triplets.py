@@ -62,6 +62,18 @@ def test_triplets_and_scores_against_the_oracle(name, n_events, precision):
     offs, hits = oracle.tracks_from_triplets(g["src"], g["dst"], keep, pair("articulation"), kept["articulation"],
                                              pair("left_elbow"), kept["left_elbow"], pair("right_elbow"), kept["right_elbow"], 3)
     assert offs.size > 1 and hits.max() < b.n_hits
+    # phases (1)-(2) of the track building on the GPU (etx_triplet_components): component names and the set of shared
+    # articulations equal the oracle's; the tracks listed from the GPU's components equal the oracle's tracks
+    tc = ctx.triplet_components(E)
+    comp, shared = oracle.triplet_components(keep, pair("articulation"), kept["articulation"], pair("left_elbow"), kept["left_elbow"],
+                                             pair("right_elbow"), kept["right_elbow"])
+    assert np.array_equal(tc["edge_component"].cpu().numpy(), comp)
+    got_shared = tc["shared"].cpu().numpy()
+    got_shared = np.unique(got_shared, axis=0) if got_shared.size else got_shared.reshape(0, 2)
+    assert np.array_equal(got_shared, shared) and shared.shape[0] > 0
+    o2, h2 = oracle.tracks_from_components(g["src"], g["dst"], tc["edge_component"].cpu().numpy(), got_shared, 3)
+    assert np.array_equal(o2, offs) and np.array_equal(h2, hits)
+    print(f"   components: {np.unique(comp[comp >= 0]).size}, shared articulations: {shared.shape[0]}, tracks: {offs.size - 1}")
     ctx.destroy()
 
 
