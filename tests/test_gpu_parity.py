@@ -440,6 +440,11 @@ def test_error_codes_capacity_blob_order_unsupported():
     with pytest.raises(etx.EtxError) as ei:
         make_ctx(cfg.replace(gnn_latent=48), datagen.pack_blob(cfg.replace(gnn_latent=48), datagen.make_weights(cfg.replace(gnn_latent=48))), b)
     assert ei.value.status == -6
+    # state_dtype: bf16 state needs bf16 or int8 precision, fp32 state fp32 or int8 (include/etx.h)
+    for prec, st in (("fp32", "bf16"), ("bf16", "fp32")):
+        with pytest.raises(etx.EtxError) as ei:
+            make_ctx(cfg.replace(precision=prec, state_dtype=st), blob, b)
+        assert ei.value.status == -6
     ctx = make_ctx(cfg, blob, b, max_events=1, max_hits=b.n_hits, validate=True)
     with pytest.raises(etx.EtxError) as ei:
         run_gpu(ctx, b, debug=False)

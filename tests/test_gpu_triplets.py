@@ -16,8 +16,8 @@ pytestmark = pytest.mark.gpu
 KINDS = ("articulation", "left_elbow", "right_elbow")
 
 
-def _setup(name, n_events, precision):
-    cfg = datagen.get_config(name).replace(precision=precision, triplets=1)
+def _setup(name, n_events, precision, state_dtype="auto"):
+    cfg = datagen.get_config(name).replace(precision=precision, triplets=1, state_dtype=state_dtype)
     b = datagen.generate_batch(cfg, n_events=n_events)
     W = centred_parity_weights(cfg.replace(precision="fp32"), b.slice_events(0, 1))
     scales = None
@@ -26,16 +26,16 @@ def _setup(name, n_events, precision):
     return cfg, b, datagen.pack_blob(cfg, W, scales)
 
 
-@pytest.mark.parametrize("name,n_events,precision", [("cfg0", 2, "fp32"), ("cfg1", 2, "fp32"), ("cfg1", 2, "int8"),
-                                                     ("cfg1", 2, "bf16"), ("cfg0", 1, "bf16")])
-def test_triplets_and_scores_against_the_oracle(name, n_events, precision):
-    cfg, b, blob = _setup(name, n_events, precision)
+@pytest.mark.parametrize("name,n_events,precision,sdt", [("cfg0", 2, "fp32", "auto"), ("cfg1", 2, "fp32", "auto"), ("cfg1", 2, "int8", "auto"),
+                                                           ("cfg1", 2, "int8", "bf16"), ("cfg1", 2, "bf16", "auto"), ("cfg0", 1, "bf16", "auto")])
+def test_triplets_and_scores_against_the_oracle(name, n_events, precision, sdt):
+    cfg, b, blob = _setup(name, n_events, precision, sdt)
     ctx = make_ctx(cfg, blob, b, max_triplets=4_000_000)
     g = run_gpu(ctx, b, debug=False)
     t = ctx.triplets()
     E, d = g["n_edges"], cfg.gnn_latent
     e_gpu = state(ctx, "e", E, d)                              # e^L: written back because the triplet stage may follow
-    o = oracle.Oracle(blob, precision)
+    o = oracle.Oracle(blob, precision, state_dtype=cfg.state_dtype)
     keep = (g["logit"] >= oracle.logit_threshold(cfg.threshold)).astype(np.uint8)
     assert 0 < keep.sum() < E
     total = 0
