@@ -13,9 +13,11 @@
  *   S4 interaction net    encoders, L x (Eq.(4) messages, node net,
  *                         edge net, residual), edge classifier        L133-148 sec. 5.2
  *   S5 threshold + WCC    discard score < s_edge,min; components      L80, L82, L206, L261 sec. 7.3
+ *   (separate calls, not part of the timed path: etx_tracks -- track containers, L42 / L74 / L82;
+ *    etx_triplets, etx_triplet_components -- the triplet stage, L150-176 sec. 5.3-5.4)
  *
  * Readings of every point where the paper is silent are in DESIGN.md sec. 4
- * (R1..R26).  All pointers are plain pointers; "d_" = device memory on the
+ * (R1..R31).  All pointers are plain pointers; "d_" = device memory on the
  * current CUDA device, "h_" = host memory.  No C++ or torch types cross this
  * boundary.  Every function returns an etx_status; nothing throws across the boundary.  One device-side guard
  * exists: a kernel that waits more than ~20 s of wall-clock time on one mbarrier (a lost arrival, i.e. a bug)
