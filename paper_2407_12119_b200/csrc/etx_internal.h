@@ -15,7 +15,9 @@
 namespace etx {
 
 constexpr int kMaxEmbLayers = 9;     // H + 1, H <= 8
-constexpr int kTileRows = 64;        // rows (hits / edges) per CTA tile of the FFMA MLP kernels
+constexpr int kTileRows = 64;        // rows (hits / edges) per CTA tile of the FFMA embedding / triplet kernels
+constexpr int kGnnRows = 128;        // rows per CTA tile of the FFMA interaction-network kernels
+constexpr int kGnnThreads = 512;     // ... and their threads (one CTA per SM at d = 64: 16 warps hide the FFMA / LDS latencies)
 constexpr int kMlpThreads = 256;
 
 // One Linear, as the kernels see it.  W is stored transposed ([K][N], N contiguous) in fp32 holding the

@@ -56,26 +56,31 @@ __device__ __forceinline__ float to_operand(float v, float inv_sx_next) {
 }
 
 // ---- one dense layer over a tile of R rows held in shared memory -----------------------------------------
-// 256 threads; thread (rg, cg) owns TM consecutive rows x 4 consecutive output columns.  X: [R][ldx] fp32 in
-// shared memory (ldx % 4 == 0), Wt: [K][N] in global memory (L1-resident).  epi(row_in_tile, col, acc[4]).
-template <int N, int R, typename Epi>
+// 256 threads; thread (rg, cg) owns the TM rows rg, rg + RG, rg + 2 RG, ... x 4 consecutive output columns (rows
+// interleaved, so the two row groups of a warp read neighbouring rows of X: different banks whatever TM is).
+// X: [R][ldx] fp32 in shared memory (ldx % 4 == 0), Wt: [K][N] in shared memory (the GNN kernels stage both weight
+// matrices once per CTA) or in global memory (L1-resident: embedding, triplet classifiers).
+// epi(row_in_tile, col, acc[4]).  Blocking over rows and output channels only changes which thread owns an output:
+// each output is still ONE ascending-k fmaf chain (R3), so the result does not depend on the tile shape.
+template <int N, int R, int NT = kMlpThreads, typename Epi>
 __device__ __forceinline__ void dense_tile(const float* __restrict__ X, int ldx, int K,
                                            const float* __restrict__ Wt, Epi epi) {
-  constexpr int CG = N / 4, RG = kMlpThreads / CG, TM = R / RG;
+  constexpr int CG = N / 4, RG = NT / CG, TM = R / RG;
   static_assert(TM >= 1 && RG * TM == R, "tile shape");
   const int cg = threadIdx.x % CG, rg = threadIdx.x / CG;
   float acc[TM][4];
 #pragma unroll
   for (int i = 0; i < TM; ++i) acc[i][0] = acc[i][1] = acc[i][2] = acc[i][3] = 0.0f;
-  const float* xr = X + (size_t)(rg * TM) * ldx;
+  const float* xr = X + (size_t)rg * ldx;
+  const int rstep = RG * ldx;
   const float4* w4 = reinterpret_cast<const float4*>(Wt) + cg;
   int k = 0;
   for (; k + 4 <= K; k += 4) {
-    const float4 w0 = __ldg(w4 + (size_t)(k + 0) * CG), w1 = __ldg(w4 + (size_t)(k + 1) * CG),
-                 w2 = __ldg(w4 + (size_t)(k + 2) * CG), w3 = __ldg(w4 + (size_t)(k + 3) * CG);
+    const float4 w0 = w4[(size_t)(k + 0) * CG], w1 = w4[(size_t)(k + 1) * CG],
+                 w2 = w4[(size_t)(k + 2) * CG], w3 = w4[(size_t)(k + 3) * CG];
 #pragma unroll
     for (int i = 0; i < TM; ++i) {
-      const float4 x = *reinterpret_cast<const float4*>(xr + i * ldx + k);
+      const float4 x = *reinterpret_cast<const float4*>(xr + i * rstep + k);
       acc[i][0] = __fmaf_rn(x.x, w0.x, acc[i][0]); acc[i][1] = __fmaf_rn(x.x, w0.y, acc[i][1]);
       acc[i][2] = __fmaf_rn(x.x, w0.z, acc[i][2]); acc[i][3] = __fmaf_rn(x.x, w0.w, acc[i][3]);
       acc[i][0] = __fmaf_rn(x.y, w1.x, acc[i][0]); acc[i][1] = __fmaf_rn(x.y, w1.y, acc[i][1]);
@@ -87,24 +92,24 @@ __device__ __forceinline__ void dense_tile(const float* __restrict__ X, int ldx,
     }
   }
   for (; k < K; ++k) {
-    const float4 w0 = __ldg(w4 + (size_t)k * CG);
+    const float4 w0 = w4[(size_t)k * CG];
 #pragma unroll
     for (int i = 0; i < TM; ++i) {
-      const float x = xr[i * ldx + k];
+      const float x = xr[i * rstep + k];
       acc[i][0] = __fmaf_rn(x, w0.x, acc[i][0]); acc[i][1] = __fmaf_rn(x, w0.y, acc[i][1]);
       acc[i][2] = __fmaf_rn(x, w0.z, acc[i][2]); acc[i][3] = __fmaf_rn(x, w0.w, acc[i][3]);
     }
   }
 #pragma unroll
-  for (int i = 0; i < TM; ++i) epi(rg * TM + i, cg * 4, acc[i]);
+  for (int i = 0; i < TM; ++i) epi(rg + i * RG, cg * 4, acc[i]);
 }
 
 // K = 3 input layer (never a tensor layer): out[r][c] = relu(fmaf chain + b), converted for the next layer.
-template <int MODE, int R>
+template <int MODE, int R, int NT = kMlpThreads>
 __device__ __forceinline__ void input_layer3(const float* __restrict__ F /*[R][4] smem*/, const LayerP& L,
                                              float inv_sx_next, float* __restrict__ Y, int ldy) {
   const int N = L.N;
-  for (int idx = threadIdx.x; idx < R * N; idx += kMlpThreads) {
+  for (int idx = threadIdx.x; idx < R * N; idx += NT) {
     const int r = idx / N, c = idx % N;
     float acc = 0.0f;
     acc = __fmaf_rn(F[r * 4 + 0], __ldg(L.Wt + c), acc);
@@ -177,17 +182,25 @@ __global__ void __launch_bounds__(kMlpThreads) embed_simt_kernel(EmbArgs a) {
 //   node network  h <- h + MLP([h, m_out, m_in])                (L140, R12, R14)
 //   edge network  e <- e + MLP([h_src, h_dst, e]), updated h    (L140, R13); optional head z = w.e + b (R16)
 template <int KIND, int MODE, typename ST, int D>
-__global__ void __launch_bounds__(kMlpThreads) gnn_mlp_simt_kernel(GnnArgs a) {
-  constexpr int R = kTileRows;
+__global__ void __launch_bounds__(kGnnThreads) gnn_mlp_simt_kernel(GnnArgs a) {
+  // 128-row tiles, 8 rows x 4 output channels per thread, both weight matrices resident in shared memory (128 FFMA per
+  // 12 conflict-free shared-memory loads), and the gather of the input rows issued eight loads deep per thread.  The
+  // 64-row kernel with weights read through L1 ran at 30 % of the FFMA pipe; what held it back was the gather, one
+  // dependent load per loop iteration (profiles/r2_kernels_full.md).
+  constexpr int R = kGnnRows;
   constexpr int K0MAX = 3 * D, LDX = K0MAX + 4, LDY = D + 4;
   extern __shared__ __align__(16) float smem[];
   float* X = smem;                       // [R][LDX]
   float* Y = X + R * LDX;                // [R][LDY]
-  int* IDX = reinterpret_cast<int*>(Y + R * LDY);   // [2][R] src, dst
+  float* W0s = Y + R * LDY;              // [K0][D]   layer-0 weights (tensor layers; a K = 3 layer reads its own through L1)
+  float* W1s = W0s + K0MAX * D;          // [D][D]
+  int* IDX = reinterpret_cast<int*>(W1s + D * D);   // [2][R] src, dst
   const int n_rows = a.n_rows_ptr ? *a.n_rows_ptr : a.n_rows;
   const bool is_edge = (KIND == kEdgeEnc || KIND == kEdgeNet);
   const LayerP L0 = a.l0, L1 = a.l1;
   const bool quant_in = (MODE == kModeInt8) && L0.tensor;
+  if (L0.K > 3) for (int i = threadIdx.x; i < L0.K * D / 4; i += kGnnThreads) reinterpret_cast<float4*>(W0s)[i] = __ldg(reinterpret_cast<const float4*>(L0.Wt) + i);
+  for (int i = threadIdx.x; i < D * D / 4; i += kGnnThreads) reinterpret_cast<float4*>(W1s)[i] = __ldg(reinterpret_cast<const float4*>(L1.Wt) + i);
 
   for (int tile = blockIdx.x; (size_t)tile * R < (size_t)n_rows; tile += gridDim.x) {
     const int row0 = tile * R;
@@ -214,32 +227,47 @@ __global__ void __launch_bounds__(kMlpThreads) gnn_mlp_simt_kernel(GnnArgs a) {
       }
       __syncthreads();
       // layer 0 (K = 3) writes its output (the layer-1 operand) into X, then Y is free again
-      input_layer3<MODE, R>(Y, L0, L1.inv_sx, X, LDX);
+      input_layer3<MODE, R, kGnnThreads>(Y, L0, L1.inv_sx, X, LDX);
       __syncthreads();
     } else {
       const int K0 = L0.K;                               // 2D (paper's edge encoder) or 3D
       const int c4n = K0 / 4, seg4 = D / 4;
-      for (int idx = threadIdx.x; idx < R * c4n; idx += kMlpThreads) {
-        const int r = idx / c4n, c4 = idx % c4n, seg = c4 / seg4, within = (c4 % seg4) * 4;
-        const int row = row0 + r;
-        float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (row < n_rows) {
-          if (KIND == kNodeNet) {
-            v = seg == 0 ? State<ST>::ld4(a.h, (size_t)row * D + within)
-                         : State<ST>::ld4(a.m, (size_t)row * 2 * D + (size_t)(seg - 1) * D + within);
-          } else {
-            if (seg == 0) v = State<ST>::ld4(a.h, (size_t)IDX[r] * D + within);
-            else if (seg == 1) v = State<ST>::ld4(a.h, (size_t)IDX[R + r] * D + within);
-            else v = State<ST>::ld4(a.e, (size_t)row * D + within);
+      constexpr int GB = 8;                              // loads in flight per thread
+      for (int base = 0; base < R * c4n; base += kGnnThreads * GB) {
+        float4 v[GB];
+#pragma unroll
+        for (int u = 0; u < GB; ++u) {
+          const int idx = base + u * kGnnThreads + threadIdx.x;
+          v[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+          if (idx < R * c4n) {
+            const int r = idx / c4n, c4 = idx % c4n, seg = c4 / seg4, within = (c4 % seg4) * 4;
+            const int row = row0 + r;
+            if (row < n_rows) {
+              if (KIND == kNodeNet) {
+                v[u] = seg == 0 ? State<ST>::ld4(a.h, (size_t)row * D + within)
+                                : State<ST>::ld4(a.m, (size_t)row * 2 * D + (size_t)(seg - 1) * D + within);
+              } else {
+                if (seg == 0) v[u] = State<ST>::ld4(a.h, (size_t)IDX[r] * D + within);
+                else if (seg == 1) v[u] = State<ST>::ld4(a.h, (size_t)IDX[R + r] * D + within);
+                else v[u] = State<ST>::ld4(a.e, (size_t)row * D + within);
+              }
+            }
           }
         }
-        if (quant_in) { v.x = quant_i8(v.x, L0.inv_sx); v.y = quant_i8(v.y, L0.inv_sx); v.z = quant_i8(v.z, L0.inv_sx); v.w = quant_i8(v.w, L0.inv_sx); }
-        *reinterpret_cast<float4*>(X + r * LDX + c4 * 4) = v;
+#pragma unroll
+        for (int u = 0; u < GB; ++u) {
+          const int idx = base + u * kGnnThreads + threadIdx.x;
+          if (idx < R * c4n) {
+            float4 w = v[u];
+            if (quant_in) { w.x = quant_i8(w.x, L0.inv_sx); w.y = quant_i8(w.y, L0.inv_sx); w.z = quant_i8(w.z, L0.inv_sx); w.w = quant_i8(w.w, L0.inv_sx); }
+            *reinterpret_cast<float4*>(X + (idx / c4n) * LDX + (idx % c4n) * 4) = w;
+          }
+        }
       }
       __syncthreads();
       // layer 0: K0 -> D, ReLU, operand conversion for layer 1
       int32_t* tap0 = (a.tap && a.tap_layer == L0.index) ? a.tap : nullptr;
-      dense_tile<D, R>(X, LDX, K0, L0.Wt, [&](int r, int c, const float* acc) {
+      dense_tile<D, R, kGnnThreads>(X, LDX, K0, W0s, [&](int r, int c, const float* acc) {
         float4 sc = __ldg(reinterpret_cast<const float4*>(L0.scale + c)), bi = __ldg(reinterpret_cast<const float4*>(L0.bias + c));
         float y[4] = {__fmaf_rn(acc[0], sc.x, bi.x), __fmaf_rn(acc[1], sc.y, bi.y), __fmaf_rn(acc[2], sc.z, bi.z), __fmaf_rn(acc[3], sc.w, bi.w)};
 #pragma unroll
@@ -258,7 +286,7 @@ __global__ void __launch_bounds__(kMlpThreads) gnn_mlp_simt_kernel(GnnArgs a) {
     // ---- layer 1: D -> D, linear; residual for the networks; store the state --------------------------------
     int32_t* tap1 = (a.tap && a.tap_layer == L1.index) ? a.tap : nullptr;
     void* state = is_edge ? a.e : a.h;
-    dense_tile<D, R>(HID, ldh, D, L1.Wt, [&](int r, int c, const float* acc) {
+    dense_tile<D, R, kGnnThreads>(HID, ldh, D, W1s, [&](int r, int c, const float* acc) {
       const int row = row0 + r;
       float4 sc = __ldg(reinterpret_cast<const float4*>(L1.scale + c)), bi = __ldg(reinterpret_cast<const float4*>(L1.bias + c));
       float4 y = make_float4(__fmaf_rn(acc[0], sc.x, bi.x), __fmaf_rn(acc[1], sc.y, bi.y), __fmaf_rn(acc[2], sc.z, bi.z), __fmaf_rn(acc[3], sc.w, bi.w));
@@ -351,17 +379,21 @@ __global__ void __launch_bounds__(256) scatter_kernel(const void* __restrict__ e
 }
 
 // ------------------------------------------------------------------------------------------------------------
-template <int D> static size_t gnn_smem() { return sizeof(float) * kTileRows * ((3 * D + 4) + (D + 4)) + sizeof(int) * 2 * kTileRows; }
+template <int D> static size_t gnn_smem() {
+  return sizeof(float) * (kGnnRows * ((3 * D + 4) + (D + 4)) + 3 * D * D + D * D) + sizeof(int) * 2 * kGnnRows;
+}
 template <int D> static size_t emb_smem() { return sizeof(float) * kTileRows * (2 * (D + 4) + 4); }
 
 template <int KIND, int MODE, typename ST, int D>
 static void gnn_launch_one(etx_ctx* c, const GnnArgs& a, int max_rows, cudaStream_t s) {
   auto kern = gnn_mlp_simt_kernel<KIND, MODE, ST, D>;
   opt_in_smem(c, kern, (int)gnn_smem<D>());
-  const int tiles = (max_rows + kTileRows - 1) / kTileRows;
-  const int grid = tiles < c->sm_count * 3 ? tiles : c->sm_count * 3;
+  const int tiles = (max_rows + kGnnRows - 1) / kGnnRows;
+  int per_sm = (int)((227 * 1024) / (gnn_smem<D>() + 1024));
+  if (per_sm < 1) per_sm = 1;
+  const int grid = tiles < c->sm_count * per_sm ? tiles : c->sm_count * per_sm;
   if (grid <= 0) return;
-  kern<<<grid, kMlpThreads, gnn_smem<D>(), s>>>(a);
+  kern<<<grid, kGnnThreads, gnn_smem<D>(), s>>>(a);
   c->launches++;
 }
 
