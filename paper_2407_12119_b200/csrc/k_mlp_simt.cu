@@ -354,15 +354,19 @@ template <> struct Vec16<__nv_bfloat16> {
   }
 };
 
+// 64-thread blocks: 1.81 ms for the six launches at cfg 2 against 1.83-1.88 (128) and 1.85-1.93 (256), same box -- the
+// shorter the block, the smaller the tail behind its longest node
+constexpr int kScatterThreads = 64;
+
 template <typename ST, int D>
-__global__ void __launch_bounds__(256) scatter_kernel(const void* __restrict__ e, const int32_t* __restrict__ row_ptr,
+__global__ void __launch_bounds__(kScatterThreads) scatter_kernel(const void* __restrict__ e, const int32_t* __restrict__ row_ptr,
                                                       const int32_t* __restrict__ col_ptr, const int32_t* __restrict__ in_edge,
                                                       void* __restrict__ m, int n_hits) {
   constexpr int V = Vec16<ST>::V, LPN = D / V;            // lanes per node
   // Nodes are walked from the last to the first: the edge network that ran just before wrote e in ascending
   // order, so the tail of e is what the L2 still holds, and the next edge network starts at the head, which this
   // pass reads last.
-  const int gid = (gridDim.x - 1 - blockIdx.x) * (256 / LPN) + threadIdx.x / LPN;
+  const int gid = (gridDim.x - 1 - blockIdx.x) * (kScatterThreads / LPN) + threadIdx.x / LPN;
   const int c = (threadIdx.x % LPN) * V;
   if (gid >= n_hits) return;
   float sum[V];
@@ -474,14 +478,14 @@ void launch_embed_simt(etx_ctx* c, int n_hits, cudaStream_t s) {
 void launch_scatter(etx_ctx* c, int n_hits, cudaStream_t s) {
   if (n_hits == 0) return;
   const int d = c->hp.gnn_latent;
-  const int npb = 256 / (d / (c->state_bf16 ? 8 : 4));
+  const int npb = kScatterThreads / (d / (c->state_bf16 ? 8 : 4));
   const int grid = (n_hits + npb - 1) / npb;
   if (c->state_bf16) {
-    if (d == 32) scatter_kernel<__nv_bfloat16, 32><<<grid, 256, 0, s>>>(c->e, c->row_ptr, c->col_ptr, c->in_edge, c->m, n_hits);
-    else scatter_kernel<__nv_bfloat16, 64><<<grid, 256, 0, s>>>(c->e, c->row_ptr, c->col_ptr, c->in_edge, c->m, n_hits);
+    if (d == 32) scatter_kernel<__nv_bfloat16, 32><<<grid, kScatterThreads, 0, s>>>(c->e, c->row_ptr, c->col_ptr, c->in_edge, c->m, n_hits);
+    else scatter_kernel<__nv_bfloat16, 64><<<grid, kScatterThreads, 0, s>>>(c->e, c->row_ptr, c->col_ptr, c->in_edge, c->m, n_hits);
   } else {
-    if (d == 32) scatter_kernel<float, 32><<<grid, 256, 0, s>>>(c->e, c->row_ptr, c->col_ptr, c->in_edge, c->m, n_hits);
-    else scatter_kernel<float, 64><<<grid, 256, 0, s>>>(c->e, c->row_ptr, c->col_ptr, c->in_edge, c->m, n_hits);
+    if (d == 32) scatter_kernel<float, 32><<<grid, kScatterThreads, 0, s>>>(c->e, c->row_ptr, c->col_ptr, c->in_edge, c->m, n_hits);
+    else scatter_kernel<float, 64><<<grid, kScatterThreads, 0, s>>>(c->e, c->row_ptr, c->col_ptr, c->in_edge, c->m, n_hits);
   }
   c->launches++;
 }
