@@ -133,6 +133,8 @@ struct etx_ctx {
   void* eenc_b0_img = nullptr;
   void* eenc_b1_img = nullptr;
   void* nenc_b1_img = nullptr;
+  void* trip_b0_img[2] = {nullptr, nullptr};   // split-bias images of the two triplet classifiers' first layer
+  void* zero_bias_img = nullptr;
   std::vector<void*> edge_bias_img;
   alignas(64) unsigned char e_map[128] = {};
   alignas(64) unsigned char h_map[128] = {};   // CUtensorMap of `h` (node encoder output)
@@ -238,5 +240,6 @@ bool launch_embed_ws(etx_ctx* c, int n_hits, cudaStream_t s);
 bool edge_tma_configure(etx_ctx* c);
 void launch_edge_net_tma(etx_ctx* c, int iter, int n_hits, bool do_head, cudaStream_t s);
 void launch_edge_enc_tma(etx_ctx* c, int n_hits, bool node, cudaStream_t s);
+void launch_triplet_cls_tma(etx_ctx* c, int kind, cudaStream_t s);
 
 }  // namespace etx

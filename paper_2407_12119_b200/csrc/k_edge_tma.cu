@@ -125,6 +125,7 @@ struct EdgeTmaArgs {
   const __nv_bfloat16* h;
   const int32_t* src; const int32_t* dst;
   const int32_t* n_rows_ptr;
+  int max_rows;                // > 0: rows beyond this are not processed (triplet lists are capped at max_triplets)
   float* logit; float* score;
   int do_head;
   int store_e;                 // 0: the new edge state is dead (last step of a plain etx_run: only the classifier reads it)
@@ -157,7 +158,7 @@ edge_net_tma_kernel(const __grid_constant__ CUtensorMap e_map, const EdgeTmaArgs
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc0_full + 7);
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int n_rows = *a.n_rows_ptr;
+  const int n_rows = a.max_rows > 0 ? min(*a.n_rows_ptr, a.max_rows) : *a.n_rows_ptr;
   const int n_tiles = (n_rows + kRows - 1) / kRows;
 
   if (tid == 0) {
@@ -675,6 +676,12 @@ bool edge_tma_configure(etx_ctx* c) {
   c->eenc_b1_img = upload_bytes(c, pack_split_rows(c->layers[c->i_eenc + 1].b));
   c->nenc_b1_img = upload_bytes(c, pack_split_rows(c->layers[c->i_nenc + 1].b));
   if (!c->eenc_b1_img || !c->nenc_b1_img) return false;
+  if (c->i_trip >= 0) {
+    c->trip_b0_img[0] = upload_bytes(c, pack_split_rows(c->layers[c->i_trip].b));
+    c->trip_b0_img[1] = upload_bytes(c, pack_split_rows(c->layers[c->i_trip + 2].b));
+    c->zero_bias_img = upload_bytes(c, pack_split_rows(std::vector<float>((size_t)D, 0.0f)));
+    if (!c->trip_b0_img[0] || !c->trip_b0_img[1] || !c->zero_bias_img) return false;
+  }
   void* fn = nullptr;
   cudaDriverEntryPointQueryResult qres;
   if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn) return false;
@@ -710,7 +717,7 @@ void launch_edge_net_tma(etx_ctx* c, int iter, int n_hits, bool do_head, cudaStr
   a.src = c->src; a.dst = c->dst; a.n_rows_ptr = c->n_edges;
   a.logit = c->logit; a.score = c->score_out; a.do_head = do_head ? 1 : 0;
   a.store_e = (do_head && !c->keep_final_state) ? 0 : 1;
-  a.enc = 0;
+  a.enc = 0; a.max_rows = 0;
   const long long max_rows_ll = (long long)n_hits * c->hp.k;
   const int max_rows = (int)(max_rows_ll > 0x7fffffff ? 0x7fffffff : max_rows_ll);
   if (c->hp.gnn_latent == 32) edge_tma_launch<32>(c, a, max_rows, s);
@@ -728,11 +735,33 @@ void launch_edge_enc_h_tma(etx_ctx* c, int n_hits, bool do_head, cudaStream_t s)
   a.h = static_cast<const __nv_bfloat16*>(c->h);
   a.src = c->src; a.dst = c->dst; a.n_rows_ptr = c->n_edges;
   a.logit = c->logit; a.score = c->score_out; a.do_head = do_head ? 1 : 0;
-  a.store_e = 1; a.enc = 1;
+  a.store_e = 1; a.enc = 1; a.max_rows = 0;
   const long long max_rows_ll = (long long)n_hits * c->hp.k;
   const int max_rows = (int)(max_rows_ll > 0x7fffffff ? 0x7fffffff : max_rows_ll);
   if (c->hp.gnn_latent == 32) edge_tma_launch<32>(c, a, max_rows, s);
   else edge_tma_launch<64>(c, a, max_rows, s);
+}
+
+// Triplet classifier (R28) on the tensor cores: the edge-network kernel in its
+// no-old-state mode gathers the two final edge encodings of a triplet (rows of e, by the triplet's edge ids) as the two
+// K-blocks of layer 0 (W0 = the classifier's 2d -> d layer, bias inside the MMA), rounds relu(acc0) to bf16 -- R20's
+// operand rounding -- and runs a "layer 1" whose weight is the identity and whose bias is zero, which hands the bf16
+// hidden activations through exactly; the fused head then IS the classifier's d -> 1 layer: an fp32 chain in ascending
+// j over the bf16 hidden values, plus bias, and the sigmoid.  Nothing is stored but logit and score.
+void launch_triplet_cls_tma(etx_ctx* c, int kind, cudaStream_t s) {
+  const int i0 = c->i_trip + (kind ? 2 : 0);
+  const size_t cap = (size_t)c->hp.max_triplets;
+  EdgeTmaArgs a;
+  a.w0_img = c->layers[i0].dev.Wtc; a.w1_img = c->ident_img; a.ident_img = c->ident_img;
+  a.b0_img = c->trip_b0_img[kind ? 1 : 0]; a.b1_img = c->zero_bias_img;
+  a.head_w = c->layers[i0 + 1].dev.Wt; a.head_b = c->layers[i0 + 1].dev.bias;
+  a.h = static_cast<const __nv_bfloat16*>(c->e);
+  a.src = c->trip_first + kind * cap; a.dst = c->trip_second + kind * cap;
+  a.n_rows_ptr = c->trip_total + kind; a.max_rows = c->hp.max_triplets;
+  a.logit = c->trip_logit + kind * cap; a.score = c->trip_score + kind * cap;
+  a.do_head = 1; a.store_e = 0; a.enc = 1;
+  if (c->hp.gnn_latent == 32) edge_tma_launch<32>(c, a, c->hp.max_triplets, s);
+  else edge_tma_launch<64>(c, a, c->hp.max_triplets, s);
 }
 
 // S4b with the configs' K = 3 edge-encoder input (edge_enc_input == 0), or S4a (node = true): the same kernel over hits

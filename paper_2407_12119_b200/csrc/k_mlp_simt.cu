@@ -559,6 +559,7 @@ static void trip_launch(etx_ctx* c, const TripArgs& a, cudaStream_t s) {
 
 // kind 0: articulations (classifier i_trip, i_trip + 1); kinds 1, 2: elbows (i_trip + 2, i_trip + 3)
 void launch_triplet_classifier(etx_ctx* c, int kind, cudaStream_t s) {
+  if (c->edge_tma) { launch_triplet_cls_tma(c, kind, s); return; }     // bf16, AUTO engine: the tcgen05 tile code
   TripArgs a;
   const int i0 = c->i_trip + (kind ? 2 : 0);
   a.l0 = c->layers[i0].dev; a.l1 = c->layers[i0 + 1].dev;

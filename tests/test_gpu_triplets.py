@@ -50,8 +50,9 @@ def test_triplets_and_scores_against_the_oracle(name, n_events, precision, sdt):
         if precision in ("fp32", "int8"):
             assert np.array_equal(gz, z), kind
             assert np.abs(gs - sc).max(initial=0) <= 1e-6
-        else:                                                  # same arithmetic on the FFMA pipe: also bit-exact
-            assert np.array_equal(gz, z), kind
+        else:                                                  # bf16, AUTO engine: layer 0 on the tensor cores (accumulation
+            assert np.abs(gs - sc).max(initial=0) <= 2e-2, kind    # order not reproducible on a CPU): the bf16 score bar
+            assert np.abs(gz - z).max(initial=0) <= 2e-2 * max(1.0, float(np.abs(z).max(initial=0))), kind
         total += f.size
         assert f.size > 0 and 0.05 < np.mean(z >= 0) < 0.95, (kind, float(np.mean(z >= 0)))
     print(f"{name}/{precision}: E={E} kept={int(keep.sum())} triplets={t['count']}")
@@ -74,6 +75,21 @@ def test_triplets_and_scores_against_the_oracle(name, n_events, precision, sdt):
     o2, h2 = oracle.tracks_from_components(g["src"], g["dst"], tc["edge_component"].cpu().numpy(), got_shared, 3)
     assert np.array_equal(o2, offs) and np.array_equal(h2, hits)
     print(f"   components: {np.unique(comp[comp >= 0]).size}, shared articulations: {shared.shape[0]}, tracks: {offs.size - 1}")
+    ctx.destroy()
+
+
+def test_triplet_classifier_bf16_on_the_ffma_engine_is_bit_exact():
+    # ETX_ENGINE_SIMT reproduces the oracle's rounding points and order exactly, also in bf16 (the debugging reference of
+    # the tensor-core classifier)
+    cfg, b, blob = _setup("cfg1", 2, "bf16")
+    ctx = make_ctx(cfg, blob, b, max_triplets=1_000_000, engine="simt")
+    g = run_gpu(ctx, b, debug=False)
+    t = ctx.triplets()
+    e_gpu = state(ctx, "e", g["n_edges"], cfg.gnn_latent)
+    o = oracle.Oracle(blob, "bf16")
+    for k, kind in enumerate(KINDS):
+        z, _ = o.triplet_scores(e_gpu, t[kind]["first"].cpu().numpy(), t[kind]["second"].cpu().numpy(), elbow=(k > 0))
+        assert np.array_equal(t[kind]["logit"].cpu().numpy(), z), kind
     ctx.destroy()
 
 
