@@ -196,6 +196,40 @@ typedef struct {
 
 etx_status etx_tracks(etx_handle h, int32_t min_hits, etx_stream stream, etx_tracks_output* out);
 
+/* The same regrouping for callers that are not allowed to allocate device memory: no handle, no workspace, and the
+ * call itself never calls cudaMalloc / cudaFree or any routine that allocates -- it only enqueues kernels and
+ * cudaMemsetAsync on `stream`.  It is meant for code that runs inside a host framework which owns all device memory and
+ * forbids allocation in its event loop (Allen, hands every algorithm slices of a per-stream arena
+ * sized in advance: cudaMalloc / cudaFree there would take the device-wide allocator lock and can stall the other
+ * streams of events), and for plug-ins that are given raw device pointers and nothing else.
+ *   inputs  (device, borrowed)  d_track_id [n_hits]         as etx_output.d_track_id: the smallest hit index of the
+ *                                                           hit's component (values in [0, n_hits), track_id[r] == r
+ *                                                           for that smallest hit, a component inside one event)
+ *                               d_event_offsets [n_events+1] [0] = 0, non-decreasing, [n_events] = n_hits -- on the
+ *                                                           DEVICE here (etx_run takes them from the host)
+ *   outputs (device, caller's)  d_track_index [n_hits], d_track_offsets [n_hits + 1] (entries [0 .. n_tracks] are the
+ *                               CSR offsets, later entries repeat the total), d_track_hits [n_hits] (the first
+ *                               offsets[n_tracks] entries are written), d_event_track_offsets [n_events + 1],
+ *                               d_n_tracks [1].  Same meaning and same values as etx_tracks_output.
+ * Its work arrays live in a fixed array inside the library image instead: about 16 MiB of device memory on every GPU
+ * that loads libetx.so, held until the process exits.  What follows from that:
+ *   - n_hits > ETX_TRACKS_STATIC_MAX_HITS returns ETX_ERR_CAPACITY and launches nothing (split the batch at an event
+ *     boundary, or use etx_tracks).  n_events is not limited.
+ *   - The first call on each device resolves the array's device address (cudaGetSymbolAddress, once per device, with
+ *     that device current, return code checked).  Make that first call before any stream capture is begun.
+ *   - Every call on a GPU uses the same array and finds the previous call's contents in it; the call zeroes what it
+ *     needs zeroed.  Calls whose device work can overlap on one GPU (two streams, two threads) race on it: keep them on
+ *     one stream or order them with events.  Calls on different GPUs are independent.
+ * No synchronisation; results are valid once `stream` has reached the end of the enqueued work.  Returns ETX_ERR_ARG
+ * for null pointers, negative sizes or min_hits < 1, ETX_ERR_CUDA if a launch fails; etx_tracks_static_error() gives
+ * the message of the last failing call on the calling thread ("" if the last call succeeded). */
+#define ETX_TRACKS_STATIC_MAX_HITS (1 << 20)
+etx_status etx_tracks_static(const int32_t* d_track_id, const int32_t* d_event_offsets, int32_t n_hits,
+                             int32_t n_events, int32_t min_hits, etx_stream stream, int32_t* d_track_index,
+                             int32_t* d_track_offsets, int32_t* d_track_hits, int32_t* d_event_track_offsets,
+                             int32_t* d_n_tracks);
+const char* etx_tracks_static_error(void);
+
 /* Triplet stage (sec. 5.3; R28, R29), the step the paper left out of its CUDA code
  * (L238).  Enqueue on `stream`, after an etx_run on the same stream and handle: triplet building on the purified
  * hit graph (edges with logit >= tau) and the two triplet classifiers on pairs of final edge encodings.  Needs a

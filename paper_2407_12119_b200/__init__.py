@@ -7,4 +7,4 @@ kernels; PyTorch is used only for device memory and streams.  There is no CPU fa
 package without the built library, or without a CUDA device, raises.
 """
 from .binding import (Etx, EtxError, EtxOutput, Hyperparams, Inject, STAGE_NAMES, hyperparams_from_config,  # noqa: F401
-                      lib, lib_path, load_library, declared_symbols)
+                      lib, lib_path, load_library, declared_symbols, tracks_static, TRACKS_STATIC_MAX_HITS)

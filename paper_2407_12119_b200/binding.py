@@ -112,6 +112,10 @@ def load_library():
     L.etx_input_status.argtypes = [vp]
     L.etx_tracks.restype = C.c_int
     L.etx_tracks.argtypes = [vp, C.c_int32, vp, C.POINTER(EtxTracks)]
+    L.etx_tracks_static.restype = C.c_int
+    L.etx_tracks_static.argtypes = [vp, vp, C.c_int32, C.c_int32, C.c_int32, vp, vp, vp, vp, vp, vp]
+    L.etx_tracks_static_error.restype = C.c_char_p
+    L.etx_tracks_static_error.argtypes = []
     L.etx_workspace_bytes.restype = C.c_size_t
     L.etx_workspace_bytes.argtypes = [vp]
     L.etx_status_string.restype = C.c_char_p
@@ -136,6 +140,33 @@ def load_library():
 
 def lib():
     return load_library()
+
+
+TRACKS_STATIC_MAX_HITS = 1 << 20        # ETX_TRACKS_STATIC_MAX_HITS of include/etx.h
+
+
+def tracks_static(d_track_id, d_event_offsets, min_hits: int, out: dict) -> None:
+    """etx_tracks_static on the current stream: the regrouping of `Etx.tracks` without a handle, for callers that may
+    not allocate device memory (the library takes its work arrays from a fixed array inside libetx.so, see
+    include/etx.h).  Every tensor is the caller's: `d_track_id` [n_hits] and `d_event_offsets` [n_events + 1] are int32
+    CUDA tensors, `out` holds int32 CUDA tensors track_index [n_hits], track_offsets [n_hits + 1], track_hits [n_hits],
+    event_track_offsets [n_events + 1] and n_tracks [1], which the call fills.  Nothing is allocated here either and
+    nothing is synchronised.  Calls that could overlap on one GPU must be ordered by the caller."""
+    import torch
+    L = load_library()
+    n_hits, n_events = int(d_track_id.numel()), int(d_event_offsets.numel()) - 1
+    for name, t, n in (("track_id", d_track_id, n_hits), ("event_offsets", d_event_offsets, n_events + 1),
+                       ("track_index", out["track_index"], n_hits), ("track_offsets", out["track_offsets"], n_hits + 1),
+                       ("track_hits", out["track_hits"], n_hits), ("event_track_offsets", out["event_track_offsets"], n_events + 1),
+                       ("n_tracks", out["n_tracks"], 1)):
+        if not (t.is_cuda and t.dtype == torch.int32 and t.is_contiguous() and t.numel() >= n):
+            raise ValueError(f"tracks_static: {name} must be a contiguous int32 CUDA tensor with at least {n} elements")
+    st = L.etx_tracks_static(d_track_id.data_ptr(), d_event_offsets.data_ptr(), n_hits, n_events, int(min_hits),
+                             C.c_void_p(torch.cuda.current_stream().cuda_stream), out["track_index"].data_ptr(),
+                             out["track_offsets"].data_ptr(), out["track_hits"].data_ptr(),
+                             out["event_track_offsets"].data_ptr(), out["n_tracks"].data_ptr())
+    if st != 0:
+        raise EtxError(st, L.etx_tracks_static_error().decode())
 
 
 def hyperparams_from_config(cfg, max_events: int, max_hits: int, precision: str | None = None,
