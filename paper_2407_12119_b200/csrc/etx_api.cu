@@ -477,7 +477,7 @@ etx_status etx_destroy(etx_handle c) {
 
 etx_status etx_run(etx_handle c, const float* d_xyz, const int32_t* d_plane, const int32_t* h_event_offsets,
                    int32_t n_events, etx_stream stream, etx_output* out) {
-  if (c && (c->slot_copy[0].pending || c->slot_copy[1].pending))
+  if (c && (c->slot_unwaited[0] || c->slot_unwaited[1]))
     return fail(c, ETX_ERR_ARG, "a submission of etx_submit_host has not been waited for yet (etx_wait_host)");
   return run_impl(c, d_xyz, d_plane, h_event_offsets, n_events, static_cast<cudaStream_t>(stream), nullptr, out);
 }
@@ -531,7 +531,7 @@ etx_status etx_triplet_components(etx_handle c, etx_stream stream, etx_triplet_c
 
 etx_status etx_dbg_run(etx_handle c, const float* d_xyz, const int32_t* d_plane, const int32_t* h_event_offsets,
                        int32_t n_events, etx_stream stream, const etx_inject* inj, etx_output* out) {
-  if (c && (c->slot_copy[0].pending || c->slot_copy[1].pending))
+  if (c && (c->slot_unwaited[0] || c->slot_unwaited[1]))
     return fail(c, ETX_ERR_ARG, "a submission of etx_submit_host has not been waited for yet (etx_wait_host)");
   return run_impl(c, d_xyz, d_plane, h_event_offsets, n_events, static_cast<cudaStream_t>(stream), inj, out);
 }
@@ -540,7 +540,7 @@ etx_status etx_run_host(etx_handle c, const float* h_xyz, const int32_t* h_plane
                         int32_t n_events, etx_stream stream, float* h_edge_score, int32_t* h_edge_src,
                         int32_t* h_edge_dst, int32_t* h_track_id, int32_t* n_edges_out) {
   if (!c) return ETX_ERR_ARG;
-  if (c && (c->slot_copy[0].pending || c->slot_copy[1].pending))
+  if (c && (c->slot_unwaited[0] || c->slot_unwaited[1]))
     return fail(c, ETX_ERR_ARG, "a submission of etx_submit_host has not been waited for yet (etx_wait_host)");
   if (!h_event_offsets || n_events < 0 || !n_edges_out) return fail(c, ETX_ERR_ARG, "null argument");
   if (n_events > c->hp.max_events) return fail(c, ETX_ERR_CAPACITY, "n_events exceeds max_events");
@@ -642,24 +642,29 @@ etx_status etx_submit_host(etx_handle c, const float* h_xyz, const int32_t* h_pl
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   const int slot = (int)(c->n_submitted & 1), prev = slot ^ 1;
   try {
-    if (!c->d_xyz_in2) {                                   // first use: the second staging set and the per-slot events
-      c->d_xyz_in2 = dev_alloc<float>(c, (size_t)c->hp.max_hits * 3);
-      c->d_plane_in2 = dev_alloc<int32_t>(c, (size_t)c->hp.max_hits);
-      c->score2 = dev_alloc<float>(c, (size_t)c->max_edges);
-      ETX_CUDA(cudaStreamCreateWithFlags(&c->h2d_stream, cudaStreamNonBlocking));
-      ETX_CUDA(cudaMallocHost(&c->h_slot_flags, 2 * sizeof(int32_t)));
-      ETX_CUDA(cudaMallocHost(&c->h_slot_n_edges, 2 * sizeof(int32_t)));
-      for (int i = 0; i < 2; ++i) {
-        c->h_slot_flags[i] = 0; c->h_slot_n_edges[i] = 0;
-        ETX_CUDA(cudaEventCreateWithFlags(&c->slot_done[i], cudaEventDisableTiming));
-        ETX_CUDA(cudaEventCreateWithFlags(&c->slot_inputs_read[i], cudaEventDisableTiming));
-        ETX_CUDA(cudaEventCreateWithFlags(&c->slot_h2d[i], cudaEventDisableTiming));
-        ETX_CUDA(cudaEventCreateWithFlags(&c->slot_edges_ready[i], cudaEventDisableTiming));
-        ETX_CUDA(cudaEventCreateWithFlags(&c->slot_copies_done[i], cudaEventDisableTiming));
-        ETX_CUDA(cudaEventCreateWithFlags(&c->slot_edges_copied[i], cudaEventDisableTiming));
-      }
+    if (!c->submit_ready) {
+      // first use: the second staging set, the second score buffer and the per-slot events.  Every resource is created
+      // only if it does not exist yet and the flag is set last, so a call that failed half-way is completed by the next
+      // one instead of leaving null events behind.  (These blocks add to etx_workspace_bytes.)
+      if (!c->d_xyz_in2) c->d_xyz_in2 = dev_alloc<float>(c, (size_t)c->hp.max_hits * 3);
+      if (!c->d_plane_in2) c->d_plane_in2 = dev_alloc<int32_t>(c, (size_t)c->hp.max_hits);
+      if (!c->score2) c->score2 = dev_alloc<float>(c, (size_t)c->max_edges);
+      if (!c->h2d_stream) ETX_CUDA(cudaStreamCreateWithFlags(&c->h2d_stream, cudaStreamNonBlocking));
+      if (!c->h_slot_flags) { ETX_CUDA(cudaMallocHost(&c->h_slot_flags, 2 * sizeof(int32_t))); c->h_slot_flags[0] = c->h_slot_flags[1] = 0; }
+      if (!c->h_slot_n_edges) { ETX_CUDA(cudaMallocHost(&c->h_slot_n_edges, 2 * sizeof(int32_t))); c->h_slot_n_edges[0] = c->h_slot_n_edges[1] = 0; }
+      for (int i = 0; i < 2; ++i)
+        for (cudaEvent_t* ev : {&c->slot_done[i], &c->slot_inputs_read[i], &c->slot_h2d[i], &c->slot_edges_ready[i],
+                                &c->slot_copies_done[i], &c->slot_edges_copied[i]})
+          if (!*ev) ETX_CUDA(cudaEventCreateWithFlags(ev, cudaEventDisableTiming));
+      c->submit_ready = true;
     }
-    if (c->slot_copy[slot].pending) return fail(c, ETX_ERR_ARG, "etx_submit_host: wait for submission i before submitting i + 2");
+    // Submission i - 2 used this slot: its results (validation verdict, E, device score buffer, the caller's output
+    // buffers) are released by etx_wait_host and by nothing else -- the edge-list copy that submission i - 1 issued on
+    // its behalf does not count.
+    if (c->slot_unwaited[slot]) return fail(c, ETX_ERR_ARG, "etx_submit_host: wait for submission i before submitting i + 2");
+    // belt and braces for the slot's score buffer: this batch's classifier must not write it before the D2H of the
+    // scores of submission i - 2 has finished (etx_wait_host has synchronised on that event already)
+    if (c->n_submitted >= 2) ETX_CUDA(cudaStreamWaitEvent(s, c->slot_copies_done[slot], 0));
     // the previous submission's edge list: issue its copy now, and keep this batch's S3 from overwriting src / dst early
     if (c->n_submitted >= 1) {
       flush_edge_copy(c, prev);
@@ -690,6 +695,7 @@ etx_status etx_submit_host(etx_handle c, const float* h_xyz, const int32_t* h_pl
     c->slot_copy[slot].h_src = h_edge_src; c->slot_copy[slot].h_dst = h_edge_dst; c->slot_copy[slot].h_n = h_n_edges;
     c->slot_copy[slot].h_score = h_edge_score; c->slot_copy[slot].d_score = slot ? c->score2 : c->score;
     c->slot_copy[slot].pending = true;
+    c->slot_unwaited[slot] = true;
     ETX_CUDA(cudaGetLastError());
   } catch (const CudaFail& f) {
     return fail(c, ETX_ERR_CUDA, std::string(f.what) + ": " + cudaGetErrorString(f.err));
@@ -713,6 +719,7 @@ etx_status etx_wait_host(etx_handle c, int32_t ticket) {
   } catch (const CudaFail& f) {
     return fail(c, ETX_ERR_CUDA, std::string(f.what) + ": " + cudaGetErrorString(f.err));
   }
+  c->slot_unwaited[slot] = false;
   if (c->hp.validate_input && (c->h_slot_flags[slot] & 1))
     return fail(c, ETX_ERR_INPUT_ORDER, "hits not sorted by (event, plane), or a plane index out of range: the batch was rejected (0 edges)");
   return ETX_OK;

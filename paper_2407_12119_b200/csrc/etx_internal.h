@@ -170,6 +170,8 @@ struct etx_ctx {
   float* score2 = nullptr;                // second score buffer: the scores of submission i are copied out under batch i + 1
   cudaStream_t h2d_stream = nullptr;      // inputs of the next submission (PCIe is full duplex: D2H runs on copy_stream)
   long long n_submitted = 0;
+  bool slot_unwaited[2] = {false, false}; // set by etx_submit_host, cleared by etx_wait_host only (not by the edge-list flush)
+  bool submit_ready = false;              // the lazily created submit resources all exist
   // timing
   bool timing = false;
   cudaEvent_t ev[256] = {};

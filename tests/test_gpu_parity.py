@@ -559,6 +559,19 @@ def test_submit_host_pipelined_matches_run_host(precision):
     t = ctx.submit_host(hx[0], hp[0], np.zeros(1, np.int32), bufs[0]["sc"], bufs[0]["s"], bufs[0]["d"], bufs[0]["t"], bufs[0]["n"])
     ctx.wait_host(t)
     assert int(bufs[0]["n"][0]) == 0
+    # a third submission while neither of the first two has been waited for is refused (it would reuse the first one's
+    # slot: verdict, E, device score buffer); the two in flight are unharmed, and the slot is free again after its wait
+    tickets.clear()
+    for i in (0, 1):
+        o = bufs[i]
+        tickets.append(ctx.submit_host(hx[i], hp[i], batches[i].event_offsets, o["sc"], o["s"], o["d"], o["t"], o["n"]))
+    with pytest.raises(etx.EtxError) as ei:
+        ctx.submit_host(hx[2], hp[2], batches[2].event_offsets, bufs[0]["sc"], bufs[0]["s"], bufs[0]["d"], bufs[0]["t"], bufs[0]["n"])
+    assert ei.value.status == -1
+    check(0)
+    tickets.append(ctx.submit_host(hx[2], hp[2], batches[2].event_offsets, bufs[0]["sc"], bufs[0]["s"], bufs[0]["d"], bufs[0]["t"], bufs[0]["n"]))
+    check(1)
+    check(2)
     ctx.destroy()
 
 
