@@ -27,7 +27,10 @@ static __device__ __noinline__ bool mbar_stalled(uint32_t spins) {
   asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(now));
   __shared__ unsigned long long first_seen;              // any waiter's first slow-path time stamp of this CTA
   if (spins == 0xfffffu) { first_seen = now; return false; }
-  return now - first_seen > 20000000000ull;
+  // another waiter may have stored a LATER first_seen between this thread's clock read and this load: the unsigned
+  // difference would wrap and read as a stall, so a time stamp that is not in the past never counts
+  const unsigned long long t0 = first_seen;
+  return now > t0 && now - t0 > 20000000000ull;
 }
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
   const uint32_t addr = smem_u32(bar);
