@@ -240,6 +240,7 @@ const char* etx_tracks_static_error(void);
  *   d_logit[k], d_score[k]   [count[k]] classifier output (articulation classifier for kind 0, elbow classifier else)
  * d_count / h_count [3]: the number of triplets of each kind (h_count: pinned mirror, valid after synchronising).  If
  * a count exceeds max_triplets only the first max_triplets triplets of that kind are listed (the caller compares).
+ * Counts are int32 and saturate: 2^31 - 1 means "at least 2^31 - 1" (they never wrap to a negative number).
  * Library-owned device pointers, valid until the next call on the handle; no synchronisation. */
 typedef struct {
   const int32_t* d_first[3];

@@ -762,6 +762,80 @@ void launch_tracks(etx_ctx* c, int n_events, int n_hits, int min_hits, cudaStrea
 // out-edge of C), kind 1 left elbow (two out-edges of C), kind 2 right elbow (two in-edges of C), first < second for
 // the elbows.  Order: C ascending, then first, then second -- which is the order of the CSR / CSC lists, both
 // ascending in edge id.  Count per hit -> exclusive scan -> fill; all integer work, bit-exact by construction.
+// Counts, offsets and totals of triplets are int32 and SATURATE at kTripSat = 2^31 - 1 instead of wrapping (threshold
+// near 0, large k and a large batch can exceed it): a saturated offset is >= any capacity, so nothing is written for it,
+// and a total of 2^31 - 1 reads "at least that many".  Saturating addition of non-negative numbers is associative, so
+// the block-wise prefix sum below is exact up to the limit.  (S3's own scan stays the plain one: E <= k * max_hits.)
+constexpr int32_t kTripSat = 0x7fffffff;
+__device__ __forceinline__ int sat_add(int a, int b) {          // a, b in [0, kTripSat]
+  const unsigned s = (unsigned)a + (unsigned)b;
+  return s > (unsigned)kTripSat ? kTripSat : (int)s;
+}
+// exclusive saturating prefix sum of one value per thread over the block (blockDim = kScanThreads); *total = block sum
+__device__ __forceinline__ int block_exclusive_sat_scan(int v, int* total) {
+  __shared__ int warp_incl[kScanThreads / 32];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  int x = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { const int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x = sat_add(x, y); }
+  int excl = __shfl_up_sync(0xffffffffu, x, 1);                 // the exclusive value is shuffled, not "inclusive - v"
+  if (lane == 0) excl = 0;
+  if (lane == 31) warp_incl[wid] = x;
+  __syncthreads();
+  int base = 0, all = 0;
+#pragma unroll
+  for (int i = 0; i < kScanThreads / 32; ++i) { const int s = warp_incl[i]; if (i < wid) base = sat_add(base, s); all = sat_add(all, s); }
+  __syncthreads();
+  *total = all;
+  return sat_add(base, excl);
+}
+__global__ void __launch_bounds__(kScanThreads) sat_scan_reduce_kernel(const int32_t* __restrict__ in, int n, int32_t* __restrict__ bsum) {
+  const int base = blockIdx.x * kScanChunk;
+  int v = 0;
+#pragma unroll
+  for (int j = 0; j < kScanItems; ++j) { const int i = base + threadIdx.x * kScanItems + j; if (i < n) v = sat_add(v, in[i]); }
+  int tot; block_exclusive_sat_scan(v, &tot);
+  if (threadIdx.x == 0) bsum[blockIdx.x] = tot;
+}
+__global__ void __launch_bounds__(kScanThreads) sat_scan_bsum_kernel(int32_t* __restrict__ bsum, int nb) {
+  int carry = 0;                                   // single block, sequential over chunks of 256
+  for (int b0 = 0; b0 < nb; b0 += kScanThreads) {
+    const int i = b0 + threadIdx.x;
+    int tot;
+    const int ex = block_exclusive_sat_scan(i < nb ? bsum[i] : 0, &tot);
+    if (i < nb) bsum[i] = sat_add(carry, ex);
+    carry = sat_add(carry, tot);
+  }
+}
+__global__ void __launch_bounds__(kScanThreads) sat_scan_write_kernel(const int32_t* __restrict__ in, int n, const int32_t* __restrict__ bsum,
+                                                                     int32_t* __restrict__ out) {
+  const int base = blockIdx.x * kScanChunk;
+  int vals[kScanItems], v = 0;
+#pragma unroll
+  for (int j = 0; j < kScanItems; ++j) {
+    const int i = base + threadIdx.x * kScanItems + j;
+    vals[j] = i < n ? in[i] : 0;
+    v = sat_add(v, vals[j]);
+  }
+  int tot;
+  int ex = sat_add(block_exclusive_sat_scan(v, &tot), bsum[blockIdx.x]);
+#pragma unroll
+  for (int j = 0; j < kScanItems; ++j) {
+    const int i = base + threadIdx.x * kScanItems + j;
+    if (i < n) out[i] = ex;
+    ex = sat_add(ex, vals[j]);
+    if (i == n - 1) out[n] = ex;
+  }
+}
+// out[0..n] = exclusive saturating prefix sums of in[0..n), n >= 1
+static void exclusive_sat_scan(etx_ctx* c, const int32_t* in, int n, int32_t* out, cudaStream_t s) {
+  const int nb = (n + kScanChunk - 1) / kScanChunk;
+  sat_scan_reduce_kernel<<<nb, kScanThreads, 0, s>>>(in, n, c->scan_tmp);
+  sat_scan_bsum_kernel<<<1, kScanThreads, 0, s>>>(c->scan_tmp, nb);
+  sat_scan_write_kernel<<<nb, kScanThreads, 0, s>>>(in, n, c->scan_tmp, out);
+  c->launches += 3;
+}
+
 __global__ void trip_count_kernel(const int32_t* __restrict__ row_ptr, const int32_t* __restrict__ col_ptr,
                                   const int32_t* __restrict__ in_edge, const float* __restrict__ logit, float tau, int n_hits,
                                   int32_t* __restrict__ cnt /* [3][n_hits + 1] */) {
@@ -771,9 +845,10 @@ __global__ void trip_count_kernel(const int32_t* __restrict__ row_ptr, const int
   for (int i = row_ptr[c]; i < row_ptr[c + 1]; ++i) od += logit[i] >= tau;
   for (int i = col_ptr[c]; i < col_ptr[c + 1]; ++i) id += logit[in_edge[i]] >= tau;
   const size_t st = (size_t)n_hits + 1;
-  cnt[c] = id * od;
-  cnt[st + c] = od * (od - 1) / 2;
-  cnt[2 * st + c] = id * (id - 1) / 2;
+  const long long lid = id, lod = od;                           // an in-degree of 65,536 already overflows id * (id - 1) in 32 bits
+  cnt[c] = (int32_t)min(lid * lod, (long long)kTripSat);
+  cnt[st + c] = (int32_t)min(lod * (lod - 1) / 2, (long long)kTripSat);
+  cnt[2 * st + c] = (int32_t)min(lid * (lid - 1) / 2, (long long)kTripSat);
 }
 
 // one thread per common hit; triplets beyond `cap` are counted but not written (the caller compares the totals)
@@ -786,18 +861,19 @@ __global__ void trip_fill_kernel(const int32_t* __restrict__ row_ptr, const int3
   const size_t st = (size_t)n_hits + 1;
   const int a0 = row_ptr[c], a1 = row_ptr[c + 1], b0 = col_ptr[c], b1 = col_ptr[c + 1];
   auto put = [&](int kind, int pos, int f, int s2) {
-    if (pos < cap) { const size_t o = (size_t)kind * cap + pos; first[o] = f; second[o] = s2; hit[o] = c; }
+    if (pos >= 0 && pos < cap) { const size_t o = (size_t)kind * cap + pos; first[o] = f; second[o] = s2; hit[o] = c; }
   };
+  auto next = [](int& p) { const int q = p; if (p < kTripSat) ++p; return q; };     // a saturated offset stays saturated
   int pa = off[c], pl = off[st + c], pr = off[2 * st + c];
   for (int i = b0; i < b1; ++i) {                               // in-edges of c, ascending edge id
     const int ei = in_edge[i];
     if (!(logit[ei] >= tau)) continue;
-    for (int j = a0; j < a1; ++j) if (logit[j] >= tau) put(0, pa++, ei, j);              // articulations
-    for (int j = i + 1; j < b1; ++j) { const int ej = in_edge[j]; if (logit[ej] >= tau) put(2, pr++, ei, ej); }   // right elbows
+    for (int j = a0; j < a1; ++j) if (logit[j] >= tau) put(0, next(pa), ei, j);              // articulations
+    for (int j = i + 1; j < b1; ++j) { const int ej = in_edge[j]; if (logit[ej] >= tau) put(2, next(pr), ei, ej); }   // right elbows
   }
   for (int i = a0; i < a1; ++i) {                               // out-edges of c
     if (!(logit[i] >= tau)) continue;
-    for (int j = i + 1; j < a1; ++j) if (logit[j] >= tau) put(1, pl++, i, j);            // left elbows
+    for (int j = i + 1; j < a1; ++j) if (logit[j] >= tau) put(1, next(pl), i, j);            // left elbows
   }
 }
 
@@ -810,7 +886,7 @@ void launch_triplet_build(etx_ctx* c, int n_hits, cudaStream_t s) {
   const int g = (n_hits + 127) / 128;
   const size_t st = (size_t)n_hits + 1;
   trip_count_kernel<<<g, 128, 0, s>>>(c->row_ptr, c->col_ptr, c->in_edge, c->logit, c->tau, n_hits, c->trip_cnt);
-  for (int k = 0; k < 3; ++k) exclusive_scan(c, c->trip_cnt + k * st, n_hits, c->trip_off + k * st, nullptr, s);
+  for (int k = 0; k < 3; ++k) exclusive_sat_scan(c, c->trip_cnt + k * st, n_hits, c->trip_off + k * st, s);
   trip_totals_kernel<<<1, 32, 0, s>>>(c->trip_off, n_hits, c->trip_total);
   trip_fill_kernel<<<g, 128, 0, s>>>(c->row_ptr, c->col_ptr, c->in_edge, c->logit, c->tau, n_hits, c->trip_off, c->hp.max_triplets,
                                      c->trip_first, c->trip_second, c->trip_hit);
@@ -840,7 +916,7 @@ __global__ void tc_elbows_kernel(const int32_t* __restrict__ first, const int32_
                                  const int32_t* __restrict__ total, int cap, float tau_t, int32_t* par1) {
   const size_t stride = (size_t)gridDim.x * blockDim.x;
   for (int kind = 1; kind <= 2; ++kind) {
-    const int n = min(total[kind], cap);
+    const int n = max(0, min(total[kind], cap));
     const size_t o = (size_t)kind * cap;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < (size_t)n; i += stride)
       if (logit[o + i] >= tau_t) uf_union(par1, first[o + i], second[o + i]);
@@ -856,7 +932,7 @@ __device__ __forceinline__ size_t tc_hash(unsigned long long k, size_t mask) {
 __global__ void tc_arts_kernel(const int32_t* __restrict__ first, const int32_t* __restrict__ second, const float* __restrict__ logit,
                                const int32_t* __restrict__ total, int cap, float tau_t, int32_t* par1,
                                unsigned long long* tab, size_t mask, int32_t* n_succ, int32_t* n_pred) {
-  const int n = min(total[0], cap);
+  const int n = max(0, min(total[0], cap));
   const size_t stride = (size_t)gridDim.x * blockDim.x;
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < (size_t)n; i += stride) {
     if (!(logit[i] >= tau_t)) continue;
@@ -894,7 +970,7 @@ __global__ void tc_link_kernel(const unsigned long long* __restrict__ tab, size_
 __global__ void tc_label_kernel(const float* __restrict__ edge_logit, float tau, const int32_t* __restrict__ n_edges, int32_t* par1,
                                 int32_t* par2, int32_t* __restrict__ edge_comp, int32_t* __restrict__ shared,
                                 const int32_t* __restrict__ n_shared, int cap) {
-  const int E = *n_edges, ns = min(*n_shared, cap);
+  const int E = *n_edges, ns = max(0, min(*n_shared, cap));
   const size_t stride = (size_t)gridDim.x * blockDim.x, t0 = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   for (size_t i = t0; i < (size_t)E; i += stride) edge_comp[i] = edge_logit[i] >= tau ? uf_find(par2, uf_find(par1, (int)i)) : -1;
   for (size_t i = t0; i < 2 * (size_t)ns; i += stride) shared[i] = uf_find(par2, shared[i]);

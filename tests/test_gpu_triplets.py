@@ -127,3 +127,39 @@ def test_triplet_capacity_and_missing_classifiers():
         ctx.triplets()
     assert ei.value.status == -2
     ctx.destroy()
+
+
+def test_triplet_counts_saturate_instead_of_wrapping():
+    # 46,368 hits on plane 0 with 64 out-edges each onto 2,048 hits of plane 1 (in-degree 1,449), every edge kept:
+    # 2048 * C(1449, 2) = 2,148,507,648 right elbows, more than int32 holds.  The count must read 2^31 - 1 ("at least"),
+    # not a negative number; the list keeps its first max_triplets entries, nothing is written out of bounds, and the
+    # kinds that fit are still counted exactly.
+    import paper_2407_12119_b200 as etx
+    from gpu_utils import dev
+    S, T, k = 32 * 1449, 2048, 64
+    cfg = datagen.get_config("cfg0").replace(precision="fp32", triplets=1, k=k)
+    n = S + T
+    rng = np.random.default_rng(3)
+    xyz = rng.normal(0, 10, (n, 3)).astype(np.float32)
+    plane = np.concatenate([np.zeros(S, np.int32), np.ones(T, np.int32)])
+    b = datagen.EventBatch(xyz, plane, np.array([0, n], np.int32), np.full(n, -1, np.int64))
+    s_idx = np.repeat(np.arange(S, dtype=np.int32), k)
+    d_idx = (S + (np.arange(S, dtype=np.int32)[:, None] % 32) * 64 + np.arange(k, dtype=np.int32)[None, :]).reshape(-1).astype(np.int32)
+    blob = datagen.pack_blob(cfg, datagen.make_weights(cfg, "parity"))
+    ctx = make_ctx(cfg, blob, b, max_triplets=16)
+    out = ctx.dbg_run(dev(xyz), dev(plane), b.event_offsets, src=dev(s_idx), dst=dev(d_idx),
+                      logit=dev(np.full(s_idx.size, 10.0, np.float32)))
+    r = ctx.results(out)
+    assert r["n_edges"] == S * k
+    t = ctx.triplets()
+    assert t["count"] == [0, S * (k * (k - 1) // 2), 2**31 - 1], t["count"]
+    # right elbows of the first plane-1 hit: its in-edges are edge 64 * s of the sources s = 0, 32, 64, ...
+    re = t["right_elbow"]
+    assert np.array_equal(re["first"].cpu().numpy(), np.zeros(16, np.int32))
+    assert np.array_equal(re["second"].cpu().numpy(), 2048 * np.arange(1, 17, dtype=np.int32))
+    assert np.array_equal(re["hit"].cpu().numpy(), np.full(16, S, np.int32))
+    le = t["left_elbow"]
+    assert np.array_equal(le["first"].cpu().numpy(), np.zeros(16, np.int32)) and np.array_equal(le["second"].cpu().numpy(), np.arange(1, 17, dtype=np.int32))
+    c = ctx.triplet_components(r["n_edges"])                    # reads min(count, capacity) triplets: must stay in bounds
+    assert c["edge_component"].numel() == r["n_edges"]
+    ctx.destroy()
