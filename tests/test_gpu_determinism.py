@@ -25,7 +25,7 @@ def _digest(ctx, out, n_hits, extra=("row_ptr", "col_ptr", "in_edge")):
     return h.hexdigest(), r
 
 
-@pytest.mark.parametrize("name,precision,n_events,reps", [("cfg2", "bf16", 500, 12), ("cfg1", "fp32", 8, 60), ("cfg3", "int8", 40, 25),
+@pytest.mark.parametrize("name,precision,n_events,reps", [("cfg2", "bf16", 500, 12), ("cfg1", "fp32", 8, 60), ("cfg3", "int8", 40, 25), ("cfg3b", "int8", 40, 25),
                                                           ("cfg5", "bf16", 60, 25), ("cfg4", "bf16", 6, 25)])
 def test_repeated_runs_are_bit_identical(name, precision, n_events, reps):
     cfg = datagen.get_config(name).replace(precision=precision)

@@ -126,10 +126,11 @@ def test_full_size_fp32_cfg1_end_to_end_sampled_events():
     ctx.destroy()
 
 
-def test_full_size_int8_cfg3_bit_exact_on_sampled_events():
+@pytest.mark.parametrize("name", ["cfg3", "cfg3b"])          # state stored as fp32 (cfg 3) and as bf16 (cfg 3b)
+def test_full_size_int8_cfg3_bit_exact_on_sampled_events(name):
     # 1000 events, INT8 MLPs (R21): integer accumulation is order-free and every other op is a single pinned fp32
     # op, so on sampled events the embedding, the edges, the logits and the track ids must equal the oracle's bits
-    cfg = datagen.get_config("cfg3")
+    cfg = datagen.get_config(name)
     b = datagen.generate_batch(cfg)
     W = centred_parity_weights(cfg.replace(precision="fp32"), b.slice_events(0, 2))
     cal = datagen.generate_batch(datagen.get_config("cfg1"), n_events=datagen.configs.CALIBRATION_EVENTS,
@@ -139,7 +140,7 @@ def test_full_size_int8_cfg3_bit_exact_on_sampled_events():
     ctx = make_ctx(cfg, blob, b)
     g = run_gpu(ctx, b, debug=False)
     _whole_batch_invariants(cfg, b, g)
-    o = oracle.Oracle(blob, "int8", state_dtype=cfg.state_dtype)      # cfg 3 stores the state as bf16 (R21)
+    o = oracle.Oracle(blob, "int8", state_dtype=cfg.state_dtype)      # cfg 3b stores the state as bf16 (R21)
     eo, rp = b.event_offsets, g["row_ptr"]
     events = _sample_events(b, n_random=2)
     for ev in events:
@@ -152,5 +153,5 @@ def test_full_size_int8_cfg3_bit_exact_on_sampled_events():
         assert np.array_equal(g["logit"][e0:e1], r["logit"]), ev
         assert np.abs(g["score"][e0:e1] - r["score"]).max(initial=0.0) <= 1e-4
         assert np.array_equal(g["track_id"][h0:h1] - h0, r["track_id"]), ev
-    print(f"cfg3/int8: N={b.n_hits} E={g['n_edges']} sampled events {events} bit-exact")
+    print(f"{name}/int8 (state {cfg.state_dtype}): N={b.n_hits} E={g['n_edges']} sampled events {events} bit-exact")
     ctx.destroy()
