@@ -165,6 +165,9 @@ def main():
     ap.add_argument("--engine", default="auto", choices=["auto", "simt", "tc_serial"])
     ap.add_argument("--cpu-events", type=int, default=500, help="oracle sample size for cpu_baseline (about 10 s of CPU work at cfg2)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--streams", type=int, default=1, help="handles on that many CUDA streams, each running the whole batch per step "
+                    "(PAPER.md L223: Allen keeps several streams of 500 events in flight)")
+    ap.add_argument("--stage-passes", type=int, default=5, help="instrumented passes the per-stage times are averaged over")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -179,8 +182,7 @@ def main():
                           + (f", d2_max={cfg.d2_max:g}" if cfg.d2_max != float("inf") else "")
                           + (", edge encoder on [h0_src,h0_dst]" if cfg.edge_enc_input else "")
                           + (", cylindrical embedding input" if cfg.emb_input else ""),
-              "events_per_gpu": cfg.n_events, "weights": "He-uniform seed 7, zero bias",
-              "l2": "per-step working set (edge state alone > 1 GB) exceeds the 126 MB L2; no explicit flush"}
+              "events_per_gpu": cfg.n_events, "weights": "He-uniform seed 7, zero bias"}
 
     # ------------------------------------------------------------------ reference arm = the CPU oracle
     if args.impl == "reference":
@@ -232,31 +234,87 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
+    # further handles on their own streams (--streams): each runs the whole batch every step, concurrently
+    extra = [(etx.Etx(blob, hp), torch.cuda.Stream()) for _ in range(max(args.streams, 1) - 1)]
+
+    def one_step():
+        o = ctx.run(d_xyz, d_plane, batch.event_offsets)
+        for c2, s2 in extra:
+            with torch.cuda.stream(s2):
+                c2.run(d_xyz, d_plane, batch.event_offsets)
+        return o
+
+    def fork():                                    # the side streams start after everything already on the main stream
+        for _, s2 in extra:
+            s2.wait_stream(stream)
+
+    def join():                                    # ... and the main stream ends after all of them
+        for _, s2 in extra:
+            stream.wait_stream(s2)
+
+    fork()
     for _ in range(max(args.warmup, 3)):
-        out = ctx.run(d_xyz, d_plane, batch.event_offsets)
+        out = one_step()
+    join()
     torch.cuda.synchronize()
     E = int(out.h_n_edges[0]); N = batch.n_hits
+    d_, L_ = cfg.gnn_latent, cfg.gnn_iters
+    sb = 2 if (cfg.precision == "bf16" or (cfg.precision == "int8" and getattr(cfg, "state_dtype", "auto") == "bf16")) else 4
+    working_set = (E * d_ + 3 * N * d_) * sb + 12 * E + 32 * N           # e, h, m, edge list + scores, hit arrays
+    L2_BYTES = 126e6
+    flush_l2 = working_set < 2 * L2_BYTES
+    if flush_l2:
+        # the batch would stay (partly) resident in the 126 MB L2 from one step to the next: every step is timed on its
+        # own and a 512 MB write in between evicts it (the write itself is outside the timed spans)
+        flush_buf = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")
+        config["l2"] = (f"per-step working set {working_set / 1e6:.0f} MB would fit the 126 MB L2: flushed between timed steps "
+                        "(512 MB write, untimed; steps timed one by one)")
+    else:
+        config["l2"] = (f"per-step working set {working_set / 1e6:.0f} MB (edge state alone {E * d_ * sb / 1e6:.0f} MB) exceeds the "
+                        "126 MB L2; no explicit flush")
+    config["streams"] = max(args.streams, 1)
     sampler = ClockSampler(local_rank); sampler.start()
-    launches0 = ctx.launch_count()
+    launches0 = ctx.launch_count() + sum(c2.launch_count() for c2, _ in extra)
     barrier()
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    ev0.record(stream)
-    for _ in range(args.steps):
-        out = ctx.run(d_xyz, d_plane, batch.event_offsets)
-    ev1.record(stream)
-    barrier()
-    ms = ev0.elapsed_time(ev1)
+    if flush_l2:
+        pairs_ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+        for a, b_ in pairs_ev:
+            flush_buf.fill_(1)
+            a.record(stream); fork()
+            out = one_step()
+            join(); b_.record(stream)
+        barrier()
+        ms = sum(a.elapsed_time(b_) for a, b_ in pairs_ev)
+    else:
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record(stream); fork()
+        for _ in range(args.steps):
+            out = one_step()
+        join(); ev1.record(stream)
+        barrier()
+        ms = ev0.elapsed_time(ev1)
     clocks = sampler.stop()
-    launches = ctx.launch_count() - launches0
-    # per-stage times: ONE extra pass with the library's stage events switched on (CUDA events on the launching
-    # stream between the stages); the headline above is the plain etx_run path without them
+    launches = ctx.launch_count() + sum(c2.launch_count() for c2, _ in extra) - launches0
+    for c2, _ in extra:
+        c2.destroy()
+    # per-stage times: extra passes of ONE handle with the library's stage events switched on (CUDA events on the
+    # launching stream between the stages), averaged; the headline above is the plain etx_run path without them
     ctx.enable_timing(True)
-    ctx.run(d_xyz, d_plane, batch.event_offsets)
-    torch.cuda.synchronize()
-    stage_ms = ctx.stage_times()
+    acc = {}
+    n_pass = max(args.stage_passes, 1)
+    for _ in range(n_pass):
+        if flush_l2:
+            flush_buf.fill_(1)
+        ctx.run(d_xyz, d_plane, batch.event_offsets)
+        torch.cuda.synchronize()
+        for name, v in ctx.stage_times().items():
+            acc.setdefault(name, []).append(v)
+    stage_ms = {name: float(np.mean(v)) for name, v in acc.items()}
+    stage_ms_spread = {name: [float(np.min(v)), float(np.max(v))] for name, v in acc.items()}
     ctx.enable_timing(False)
     from paper_2407_12119_b200.sharding import whole_job
-    ms, (tot_events, tot_hits, _) = whole_job(ms, [batch.n_events, N, E], dist, "cuda")
+    n_str = max(args.streams, 1)
+    ms, (tot_events, tot_hits, _) = whole_job(ms, [batch.n_events * n_str, N * n_str, E], dist, "cuda")
     value = tot_events * args.steps / (ms * 1e-3)
 
     # ---- end to end through etx_run_host: pinned host buffers, H2D + D2H inside the timed region
@@ -295,10 +353,11 @@ def main():
     e2e_s = time.perf_counter() - t0
     e2e_s, _ = whole_job(e2e_s, [], dist, "cuda")
     assert int(outs[(args.steps - 1) & 1][4][0]) == E2
-    e2e = {"value": tot_events * args.steps / e2e_s, "unit": UNIT,
+    e2e_events = tot_events / n_str                       # the end-to-end legs run one handle
+    e2e = {"value": e2e_events * args.steps / e2e_s, "unit": UNIT,
            "h2d_bytes_per_step": int(16 * N + 4 * (batch.n_events + 1)), "d2h_bytes_per_step": int(12 * E2 + 4 * N + 4),
            "api": "etx_submit_host / etx_wait_host, two batches in flight (pinned host buffers; each step copies its inputs in and its results out)",
-           "synchronous": {"value": tot_events * args.steps / e2e_sync_s, "unit": UNIT, "api": "etx_run_host, one batch at a time"}}
+           "synchronous": {"value": e2e_events * args.steps / e2e_sync_s, "unit": UNIT, "api": "etx_run_host, one batch at a time"}}
 
     if rank != 0:
         if dist is not None:
@@ -318,25 +377,42 @@ def main():
     for name, (bound, work, peak, unit) in model.items():
         t = stage_ms.get(name, 0.0) * 1e-3
         ach = (work / t / (1e12 if unit == "TFLOP/s" else 1e9 if unit == "GB/s" else 1.0)) if t > 0 else None
-        stages[name] = {"ms": stage_ms.get(name, 0.0), "bound": bound, "achieved": ach, "peak": peak, "unit": unit,
-                        "frac": (ach / peak) if ach else None}
+        stages[name] = {"ms": stage_ms.get(name, 0.0), "ms_min_max": stage_ms_spread.get(name), "bound": bound, "achieved": ach,
+                        "peak": peak, "unit": unit, "frac": (ach / peak) if ach else None}
     dom = "S4e_edge_net_head"
     L = max(cfg.gnn_iters, 1)
     dom_ms = stage_ms[dom] / L
-    dom_bytes = model[dom][1] / L
     dom_bound, _, dom_peak, dom_unit = model[dom]
     dom_div = 1e12 if dom_unit == "TFLOP/s" else 1e9
+    wide = model[dom][1] / L                                  # every compulsory byte (or, fp32: the flops) per launch
+    if dom_bound == "hbm":
+        # e read + e write = 2 d b per edge, the h gathers L2-resident; the last launch of a pass
+        # feeds only the fused classifier and does not write e back.  `frac` is quoted on THIS count; the wider one
+        # (+ src / dst, h once per node, logit / score) is reported beside it.
+        dom_bytes = (2 * L - 1) * d_ * sb * E / L
+    else:
+        dom_bytes = wide
+    rate = lambda work: work / (dom_ms * 1e-3) / dom_div if dom_ms > 0 else None
+    hbm_note = ("S4e moves its bytes once (ncu traffic / compulsory bytes = 0.98 at cfg2); what holds it below the copy peak is on chip: "
+                "shared-memory bandwidth and the cp.async gather of h[src], h[dst] (profiles/r2_s4e_ablation.md)")
     roofline = {"kernel": "edge network MLP (S4e), one launch per message-passing step", "bound": dom_bound,
-                "achieved": dom_bytes / (dom_ms * 1e-3) / dom_div if dom_ms > 0 else None, "peak": dom_peak, "unit": dom_unit,
-                "frac": (dom_bytes / (dom_ms * 1e-3) / dom_div / dom_peak) if dom_ms > 0 else None,
-                "traffic": NCU_TRAFFIC_BYTES.get((cfg.name, cfg.n_events)),
-                "traffic_source": "recorded: ncu --set full capture of this kernel at this workload, profiles/r2_launches_cfg2.md "
-                                  "(bench.py cannot run ncu; null for other workloads)",
-                "note": "S4e moves its algorithmic bytes once (traffic / algorithmic = 0.98); what holds it below the copy peak is "
-                        "on-chip: shared-memory bandwidth and the cp.async gather of h[src], h[dst] (profiles/r2_s4e_ablation.md)",
+                "achieved": rate(dom_bytes), "peak": dom_peak, "unit": dom_unit,
+                "frac": rate(dom_bytes) / dom_peak if dom_ms > 0 else None,
+                "algorithmic_work_per_launch": dom_bytes,
+                "algorithmic_count": "SURVEY.md sec. 8(d): 2 d b per edge (e read + e write), last launch of a pass writes no e"
+                                     if dom_bound == "hbm" else "2 (3 d d + d d) flops per edge (+ 2 d for the head)",
+                "compulsory": {"work_per_launch": wide, "achieved": rate(wide), "frac": rate(wide) / dom_peak if dom_ms > 0 else None,
+                               "count": "algorithmic + src / dst (8 E) + h once per node (N d b) + logit and score writes"}
+                              if dom_bound == "hbm" else None,
+                "traffic": NCU_TRAFFIC_BYTES.get((cfg.name, cfg.n_events)) if n_str == 1 and args.engine == "auto" else None,
+                "traffic_source": ("recorded: ncu --set full capture of this kernel at this workload (profiles/r2_launches_cfg2.md); "
+                                   "bench.py cannot run ncu") if (cfg.name, cfg.n_events) in NCU_TRAFFIC_BYTES
+                                  else "no ncu capture recorded for this workload",
+                "note": hbm_note if dom_bound == "hbm" else "fp32 mode runs the networks on the FFMA pipe in the oracle's pinned order (DESIGN.md R4)",
+                "l2": "flushed between steps" if flush_l2 else "working set exceeds L2",
                 "peak_source": peaks["source"] if dom_bound == "hbm" else "derived: 148 SM x 128 lanes x 2 x 1.965 GHz (DESIGN.md sec. 3)",
-                "avg_launch_ms": dom_ms, "algorithmic_work_per_launch": dom_bytes,
-                "share_of_step": stage_ms[dom] / (ms / args.steps) if ms > 0 else None}
+                "avg_launch_ms": dom_ms, "stage_passes": n_pass,
+                "share_of_step": stage_ms[dom] / (ms / args.steps / 1.0) if (ms > 0 and n_str == 1) else None}
     cpu_baseline = None
     if not args.no_cpu_baseline:
         v, dt, n, cores = run_oracle_sample(cfg, batch, layers, args.cpu_events, scales)

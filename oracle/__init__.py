@@ -20,6 +20,13 @@ _LIB = os.path.join(_HERE, "libetx_oracle.so")
 # -ffp-contract=off: no silent fusion; fused multiply-adds are explicit std::fmaf (hardware FMA via -mfma).
 _FLAGS = ["-O3", "-std=c++17", "-mavx2", "-mfma", "-ffp-contract=off", "-fno-fast-math", "-fopenmp",
           "-shared", "-fPIC"]
+# ETX_ORACLE_SANITIZE=1: the same source under AddressSanitizer + UndefinedBehaviorSanitizer, as a library of its own
+# (DESIGN.md sec. 5).  Python is not built with ASan, so its runtime has to be preloaded:
+#   ETX_ORACLE_SANITIZE=1 LD_PRELOAD=$(gcc -print-file-name=libasan.so) ASAN_OPTIONS=detect_leaks=0 \
+#       python -m pytest tests/test_oracle_pins.py tests/test_oracle_triplets.py -q
+if os.environ.get("ETX_ORACLE_SANITIZE") == "1":
+    _LIB = os.path.join(_HERE, "libetx_oracle_san.so")
+    _FLAGS = ["-O1", "-g", "-fno-omit-frame-pointer", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined"] + _FLAGS[1:]
 
 PRECISION = {"fp32": 0, "bf16": 1, "int8": 2}
 STATE_DTYPE = {"auto": 0, "fp32": 1, "bf16": 2}     # storage of h, e, m; "bf16" only changes int8 mode (R21)

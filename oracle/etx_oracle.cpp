@@ -10,7 +10,7 @@
 // is never a fallback for it.
 //
 // Every function cites the passage it follows.  Where the paper is silent the
-// reading is the one listed in DESIGN.md section 4 ("Readings"), numbered R1..R27.
+// reading is the one listed in DESIGN.md section 4 ("Readings"), numbered R1..R31.
 //
 // Pins (tests/test_oracle_pins.py, run with -m "not gpu"):
 //   features/MLP : closed forms on hand-made weights, float64 matmul bound; cylindrical input (R27): float64

@@ -113,6 +113,45 @@ def test_full_size_bf16_invariants_and_sampled_events(name, preset):
     ctx.destroy()
 
 
+@pytest.mark.parametrize("preset", ["parity", "he"])
+def test_full_size_cfg2_every_event_chained(preset):
+    # The sampled-events test above would miss a tile-scheduling fault that hits one mid-batch event, so here the
+    # chained protocol runs over ALL 500 events of the headline batch at once -- the oracle is
+    # OpenMP-parallel over hits / edges and needs about ten seconds: oracle S2 + S3 on the GPU's embedding == the GPU's
+    # edge list; oracle S4 on those edges against every score (parity weights, 2e-2) or every logit relative to its
+    # own magnitude (He weights, 0.02; R24); oracle S5 on the GPU's logits == every track id.
+    cfg = datagen.get_config("cfg2")
+    b = datagen.generate_batch(cfg)
+    W = datagen.make_weights(cfg, "he") if preset == "he" else centred_parity_weights(cfg, b.slice_events(0, 2))
+    blob = datagen.pack_blob(cfg, W)
+    ctx = make_ctx(cfg, blob, b)
+    g = run_gpu(ctx, b, debug=False)
+    ctx.destroy()
+    nbr, deg = oracle.knn(g["emb"], b.plane, b.event_offsets, cfg.k, cfg.window, cfg.d2_max)
+    src, dst, _ = oracle.build_edges(nbr, deg)
+    assert src.size == g["n_edges"]
+    assert np.array_equal(g["src"], src) and np.array_equal(g["dst"], dst)
+    o = oracle.Oracle(blob, "bf16")
+    og = o.gnn(b.xyz, src, dst, want_states=(preset == "he"))
+    if preset == "parity":
+        err = np.abs(g["score"] - og["score"])
+        worst, what = float(err.max()), "max |score err|"
+        assert worst <= 2e-2, worst
+        assert np.mean((g["score"] > 0.01) & (g["score"] < 0.99)) > 0.3
+    else:
+        _, head_w, head_b = datagen.unpack_blob(cfg, blob)[0][-1]
+        assert np.isfinite(g["logit"]).all()
+        mag = np.abs(og["e"]).astype(np.float32) @ np.abs(head_w[0]).astype(np.float32) + abs(float(head_b[0]))
+        ratio = np.abs(g["logit"].astype(np.float64) - og["logit"]) / np.maximum(mag.astype(np.float64), 1e-30)
+        worst, what = float(ratio.max()), "max |logit err| / (|w|.|e| + |b|)"
+        assert worst <= 0.02, worst
+    tid = oracle.components(src, dst, g["logit"], oracle.logit_threshold(cfg.threshold), b.n_hits)
+    assert np.array_equal(g["track_id"], tid)
+    ev_of_edge = np.searchsorted(b.event_offsets, src, side="right") - 1
+    print(f"cfg2/{preset}: {b.n_events}/{b.n_events} events compared element by element (N={b.n_hits}, E={src.size}, "
+          f"{np.unique(ev_of_edge).size} events with edges): edges and track ids equal, {what} = {worst:.3e}")
+
+
 def test_full_size_fp32_cfg1_end_to_end_sampled_events():
     cfg = datagen.get_config("cfg1")                            # 64 events, fp32 throughout
     b = datagen.generate_batch(cfg)
