@@ -14,7 +14,7 @@
  *                         edge net, residual), edge classifier        L133-148 sec. 5.2
  *   S5 threshold + WCC    discard score < s_edge,min; components      L80, L82, L206, L261 sec. 7.3
  *   (separate calls, not part of the timed path: etx_tracks -- track containers, L42 / L74 / L82;
- *    etx_triplets, etx_triplet_components -- the triplet stage, L150-176 sec. 5.3-5.4)
+ *    etx_triplets, etx_triplet_components, etx_triplet_tracks -- the triplet stage, L150-176 sec. 5.3-5.4)
  *
  * Readings of every point where the paper is silent are in DESIGN.md sec. 4
  * (R1..R31).  All pointers are plain pointers; "d_" = device memory on the
@@ -264,7 +264,7 @@ etx_status etx_triplets(etx_handle h, etx_stream stream, etx_triplets_output* ou
  *                               -1 for an edge below the edge threshold
  *   d_shared [n_shared][2]      the shared articulations as (component of first, component of second); unordered and
  *                               possibly repeated -- a set (each yields the track "union of the two components",
- *                               phase 3; the expansion into hit lists, phases 3-4, is a host-side listing)
+ *                               phase 3; etx_triplet_tracks lists the tracks, phases 3-4)
  * Exact only if no triplet count exceeded max_triplets (compare etx_triplets' counts).  No synchronisation. */
 typedef struct {
   const int32_t* d_edge_component;
@@ -275,6 +275,33 @@ typedef struct {
 } etx_triplet_components_output;
 
 etx_status etx_triplet_components(etx_handle h, etx_stream stream, etx_triplet_components_output* out);
+
+/* Track building from triplets, phases (3)-(4) (sec. 5.4: "a new track is formed for each remaining
+ * articulation, effectively duplicating the shared set of connected edges.  Finally, edges are replaced by their
+ * corresponding hits"; Fig. 6; R30, R31).  Enqueue after etx_triplet_components on the same stream and
+ * handle.  Every shared articulation (X, Y) gives the track "hits of set X and of set Y"; a set of connected edges that
+ * no shared articulation touches is a track by itself; a track's hits are the end points of its edges.  Hits ascend
+ * inside a track; tracks with fewer than min_hits hits are dropped (L42: 3); identical hit lists are kept once; tracks
+ * are ordered lexicographically by hit list -- so tracks may share hits, which is the point of the triplet stage (e+e-
+ * pairs, L166).  Results (library-owned device memory, valid until the next call on the handle; no synchronisation):
+ *   d_track_offsets [n_tracks + 1]  CSR offsets into d_track_hits          d_track_hits [offsets[n_tracks]]
+ *   d_counts / h_counts [3]         n_tracks, total number of listed hits, overflow flag (h_counts: pinned mirror,
+ *                                   valid once the stream has been synchronised)
+ * Capacities: track_capacity = max_triplets + k * max_hits tracks (never exceeded: at most one track per shared
+ * articulation and per set) and hit_capacity = 2 * track_capacity listed hits (a shared set is listed once per
+ * articulation that shares it, so there is no bound in terms of n_hits); if the latter is exceeded the
+ * overflow flag is 1, the counts are the true ones and the lists are cut there.  Exact only if etx_triplets' counts
+ * stayed within max_triplets.  Needs max_triplets + k * max_hits < 2^31 (ETX_ERR_UNSUPPORTED otherwise). */
+typedef struct {
+  const int32_t* d_track_offsets;
+  const int32_t* d_track_hits;
+  const int32_t* d_counts;
+  const int32_t* h_counts;
+  int32_t        track_capacity;
+  int32_t        hit_capacity;
+} etx_triplet_tracks_output;
+
+etx_status etx_triplet_tracks(etx_handle h, int32_t min_hits, etx_stream stream, etx_triplet_tracks_output* out);
 
 etx_status etx_destroy(etx_handle h);
 
@@ -303,7 +330,8 @@ etx_status etx_dbg_run(etx_handle h, const float* d_xyz, const int32_t* d_plane,
                        const etx_inject* inj, etx_output* out);
 
 /* Device pointer + byte size of an internal buffer of the last run: "plane_off", "emb", "nbr", "deg",
- * "row_ptr", "col_ptr", "in_edge", "h", "e", "m", "logit", "tap", "feat", "feat_emb".  "nbr" is [n_hits][k]; only the
+ * "row_ptr", "col_ptr", "in_edge", "h", "e", "m", "logit", "tap", "feat", "feat_emb", "trip_logit" ([3][max_triplets]
+ * classifier outputs of etx_triplets; the fixture tests overwrite them to choose which triplets are kept).  "nbr" is [n_hits][k]; only the
  * first deg[q] slots of a row are defined.  h / e / m are in the
  * state dtype (etx_state_dtype; by default fp32 for ETX_FP32 and ETX_INT8, bf16 for ETX_BF16).  "e" holds the final edge state e^L only after
  * etx_dbg_run: in etx_run the last edge network feeds the fused classifier and does not write e^L back (the

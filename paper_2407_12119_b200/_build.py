@@ -15,7 +15,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libetx.so")
 SOURCES = ["etx_api.cu", "k_graph.cu", "k_mlp_simt.cu", "k_mlp_umma.cu", "k_mlp_ws.cu", "k_edge_tma.cu", "k_embed_ws.cu", "k_edge_i8.cu",
-           "k_tracks_static.cu"]
+           "k_tracks_static.cu", "k_triplet_tracks.cu"]
 HEADERS = [os.path.join(CSRC, "etx_internal.h"), os.path.join(CSRC, "umma_common.cuh"), os.path.join(HERE, "..", "include", "etx.h")]
 # no fast-math, no FTZ, no implicit contraction: every fp32 op is the one written (R4)
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "--extended-lambda",

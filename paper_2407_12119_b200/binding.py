@@ -63,6 +63,11 @@ class EtxTripletComponents(C.Structure):
                 ("h_n_shared", C.POINTER(C.c_int32)), ("capacity", C.c_int32)]
 
 
+class EtxTripletTracks(C.Structure):
+    _fields_ = [("d_track_offsets", C.c_void_p), ("d_track_hits", C.c_void_p), ("d_counts", C.c_void_p),
+                ("h_counts", C.POINTER(C.c_int32)), ("track_capacity", C.c_int32), ("hit_capacity", C.c_int32)]
+
+
 class Inject(C.Structure):
     _fields_ = [("d_emb", C.c_void_p), ("d_src", C.c_void_p), ("d_dst", C.c_void_p), ("n_edges", C.c_int32),
                 ("d_logit", C.c_void_p), ("last_stage", C.c_int32)]
@@ -108,6 +113,8 @@ def load_library():
     L.etx_triplets.argtypes = [vp, vp, C.POINTER(EtxTriplets)]
     L.etx_triplet_components.restype = C.c_int
     L.etx_triplet_components.argtypes = [vp, vp, C.POINTER(EtxTripletComponents)]
+    L.etx_triplet_tracks.restype = C.c_int
+    L.etx_triplet_tracks.argtypes = [vp, C.c_int32, vp, C.POINTER(EtxTripletTracks)]
     L.etx_input_status.restype = C.c_int
     L.etx_input_status.argtypes = [vp]
     L.etx_tracks.restype = C.c_int
@@ -351,6 +358,19 @@ class Etx:
         return dict(edge_component=self._copy_out(out.d_edge_component, 4 * n_edges, torch.int32),
                     shared=self._copy_out(out.d_shared, 8 * n, torch.int32).reshape(-1, 2), n_shared=int(out.h_n_shared[0]))
 
+    def triplet_tracks(self, min_hits: int = 3) -> dict:
+        """etx_triplet_tracks after triplet_components(); synchronises.  -> dict(track_offsets [T + 1], track_hits,
+        n_tracks, n_listed_hits, overflow); the lists are cut at the capacities when overflow is set."""
+        import torch
+        out = EtxTripletTracks()
+        self._check(self._L.etx_triplet_tracks(self._h, int(min_hits), self._stream(), C.byref(out)), "etx_triplet_tracks")
+        torch.cuda.current_stream().synchronize()
+        T, H, ovf = int(out.h_counts[0]), int(out.h_counts[1]), int(out.h_counts[2])
+        Tl, Hl = min(T, int(out.track_capacity)), min(H, int(out.hit_capacity))
+        return dict(n_tracks=T, n_listed_hits=H, overflow=ovf,
+                    track_offsets=self._copy_out(out.d_track_offsets, 4 * (Tl + 1), torch.int32),
+                    track_hits=self._copy_out(out.d_track_hits, 4 * Hl, torch.int32))
+
     def workspace_bytes(self) -> int:
         return int(self._L.etx_workspace_bytes(self._h))
 
@@ -364,6 +384,18 @@ class Etx:
         p, n = C.c_void_p(), C.c_size_t()
         self._check(self._L.etx_dbg_buffer(self._h, name.encode(), C.byref(p), C.byref(n)), "etx_dbg_buffer")
         return self._copy_out(p.value, n.value, dtype, shape)
+
+    def buffer_view(self, name: str, dtype):
+        """A zero-copy, WRITABLE torch view of an internal device buffer (etx_dbg_buffer).  For fault-injection and
+        fixture tests only: it aliases library-owned memory."""
+        import torch
+        torch.cuda.current_stream().synchronize()
+        p, n = C.c_void_p(), C.c_size_t()
+        self._check(self._L.etx_dbg_buffer(self._h, name.encode(), C.byref(p), C.byref(n)), "etx_dbg_buffer")
+
+        class _Raw:
+            __cuda_array_interface__ = {"shape": (int(n.value),), "typestr": "|u1", "data": (int(p.value), False), "version": 2}
+        return torch.as_tensor(_Raw(), device="cuda").view(dtype)
 
     @staticmethod
     def _copy_out(ptr, nbytes: int, dtype, shape=None):

@@ -6,6 +6,8 @@
 
 #include <new>
 
+#include <algorithm>
+
 #include "etx_internal.h"
 
 using namespace etx;
@@ -402,6 +404,23 @@ etx_status etx_create(const void* blob, size_t blob_bytes, const etx_hyperparams
       ETX_CUDA(cudaMemset(c->tc_n_shared, 0, sizeof(int32_t)));
       ETX_CUDA(cudaMallocHost(&c->h_tc_n_shared, sizeof(int32_t)));
       c->h_tc_n_shared[0] = 0;
+      // etx_triplet_tracks: a hit is listed once per set it touches (at most once per kept incident edge: 2 E in all)
+      c->tt_set_off = dev_alloc<int32_t>(c, E + 1);
+      c->tt_set_hits = dev_alloc<int32_t>(c, 2 * E);
+      c->tt_bucket_cand = dev_alloc<int32_t>(c, T + E);
+      c->tt_scan_tmp = dev_alloc<int32_t>(c, (E > N ? E : N) / 2048 + 2);
+      // at most one track per shared articulation plus one per set of connected edges: T + E can never overflow; the
+      // listed hits have no such bound (a shared set is listed once per articulation that shares it)
+      c->tt_track_cap = (int)std::min<size_t>(T + E, 0x7ffffff0);
+      c->tt_hit_cap = (int)std::min<size_t>(2 * (T + E), 0x7ffffff0);
+      c->tt_track_len = dev_alloc<int32_t>(c, (size_t)c->tt_track_cap + 1);
+      c->tt_track_off = dev_alloc<int32_t>(c, (size_t)c->tt_track_cap + 1);
+      c->tt_track_hits = dev_alloc<int32_t>(c, (size_t)c->tt_hit_cap);
+      c->tt_counts = dev_alloc<int32_t>(c, 4);
+      ETX_CUDA(cudaMemset(c->tt_counts, 0, 4 * sizeof(int32_t)));
+      ETX_CUDA(cudaMemset(c->tt_track_off, 0, sizeof(int32_t)));
+      ETX_CUDA(cudaMallocHost(&c->h_tt_counts, 4 * sizeof(int32_t)));
+      for (int i = 0; i < 4; ++i) c->h_tt_counts[i] = 0;
       ETX_CUDA(cudaMemset(c->trip_total, 0, 4 * sizeof(int32_t)));
       ETX_CUDA(cudaMallocHost(&c->h_trip_total, 4 * sizeof(int32_t)));
       for (int i = 0; i < 4; ++i) c->h_trip_total[i] = 0;
@@ -455,6 +474,7 @@ etx_status etx_destroy(etx_handle c) {
   if (c->h_flags) cudaFreeHost(c->h_flags);
   if (c->h_trip_total) cudaFreeHost(c->h_trip_total);
   if (c->h_tc_n_shared) cudaFreeHost(c->h_tc_n_shared);
+  if (c->h_tt_counts) cudaFreeHost(c->h_tt_counts);
   if (c->h_slot_flags) cudaFreeHost(c->h_slot_flags);
   if (c->h_slot_n_edges) cudaFreeHost(c->h_slot_n_edges);
   for (int i = 0; i < 2; ++i) {
@@ -526,6 +546,22 @@ etx_status etx_triplet_components(etx_handle c, etx_stream stream, etx_triplet_c
     return fail(c, ETX_ERR_CUDA, "etx_triplet_components: launch failed");
   out->d_edge_component = c->tc_comp; out->d_shared = c->tc_shared; out->d_n_shared = c->tc_n_shared;
   out->h_n_shared = c->h_tc_n_shared; out->capacity = c->hp.max_triplets;
+  return ETX_OK;
+}
+
+etx_status etx_triplet_tracks(etx_handle c, int32_t min_hits, etx_stream stream, etx_triplet_tracks_output* out) {
+  if (!c) return ETX_ERR_ARG;
+  if (!out || min_hits < 1) return fail(c, ETX_ERR_ARG, "etx_triplet_tracks: null output or min_hits < 1");
+  if (c->i_trip < 0 || c->hp.max_triplets <= 0) return fail(c, ETX_ERR_CAPACITY, "etx_triplet_tracks: the triplet stage is not configured");
+  if ((long long)c->hp.max_triplets + c->max_edges > 0x7fffffffLL)
+    return fail(c, ETX_ERR_UNSUPPORTED, "etx_triplet_tracks: max_triplets + k * max_hits must stay below 2^31");
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  launch_triplet_tracks(c, c->last_n_events, c->last_n_hits, min_hits, s);
+  if (cudaMemcpyAsync(c->h_tt_counts, c->tt_counts, 4 * sizeof(int32_t), cudaMemcpyDeviceToHost, s) != cudaSuccess ||
+      cudaGetLastError() != cudaSuccess)
+    return fail(c, ETX_ERR_CUDA, "etx_triplet_tracks: launch failed");
+  out->d_track_offsets = c->tt_track_off; out->d_track_hits = c->tt_track_hits; out->d_counts = c->tt_counts;
+  out->h_counts = c->h_tt_counts; out->track_capacity = c->tt_track_cap; out->hit_capacity = c->tt_hit_cap;
   return ETX_OK;
 }
 
@@ -760,6 +796,7 @@ etx_status etx_dbg_buffer(etx_handle c, const char* name, const void** d_ptr, si
   if (n == "e") { *d_ptr = c->e; *bytes = E * d * sb; return ETX_OK; }
   if (n == "logit") { *d_ptr = c->logit; *bytes = E * 4; return ETX_OK; }
   if (n == "tap") { *d_ptr = c->tap; *bytes = c->tap_bytes; return ETX_OK; }
+  if (n == "trip_logit") { *d_ptr = c->trip_logit; *bytes = c->trip_logit ? 3 * (size_t)c->hp.max_triplets * 4 : 0; return ETX_OK; }
   return fail(c, ETX_ERR_ARG, "unknown buffer name");
 }
 

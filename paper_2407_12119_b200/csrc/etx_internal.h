@@ -125,6 +125,11 @@ struct etx_ctx {
   size_t tc_tab_size = 0;
   int32_t *tc_n_shared = nullptr, *h_tc_n_shared = nullptr;
   float tau_t = 0.0f;
+  // etx_triplet_tracks (k_triplet_tracks.cu): hit lists of the sets of connected edges (CSR by set name), candidate
+  // numbers bucketed by first hit, the track list, {n_tracks, total hits, overflow} device / pinned
+  int32_t *tt_set_off = nullptr, *tt_set_hits = nullptr, *tt_bucket_cand = nullptr, *tt_scan_tmp = nullptr;
+  int32_t *tt_track_len = nullptr, *tt_track_off = nullptr, *tt_track_hits = nullptr, *tt_counts = nullptr, *h_tt_counts = nullptr;
+  int tt_hit_cap = 0, tt_track_cap = 0;
   int last_n_events = 0;
   // k_edge_tma.cu: identity operand image, split-bias images [2 * iter + layer], CUtensorMap of `e` (opaque here)
   bool edge_tma = false;
@@ -217,6 +222,8 @@ void launch_components(etx_ctx* c, const float* logit, int n_events, int n_hits,
 void launch_tracks(etx_ctx* c, int n_events, int n_hits, int min_hits, cudaStream_t s);
 void launch_triplet_build(etx_ctx* c, int n_hits, cudaStream_t s);
 void launch_triplet_components(etx_ctx* c, cudaStream_t s);
+// k_triplet_tracks.cu
+void launch_triplet_tracks(etx_ctx* c, int n_events, int n_hits, int min_hits, cudaStream_t s);
 // k_mlp_simt.cu
 void launch_embed_simt(etx_ctx* c, int n_hits, cudaStream_t s);
 void launch_gnn_mlp_simt(etx_ctx* c, int kind, int iter, int n_hits, bool do_head, cudaStream_t s);

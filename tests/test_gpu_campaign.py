@@ -111,4 +111,10 @@ def test_campaign_triplet_stage(seed):
     got = tc["shared"].cpu().numpy()
     got = np.unique(got, axis=0) if got.size else got.reshape(0, 2)
     assert np.array_equal(got, shared), cfg
+    # phases (3)-(4) in the product: the track list equals the oracle's four-phase result as arrays
+    offs, hits = oracle.tracks_from_triplets(g["src"], g["dst"], keep, pairs["articulation"], kept["articulation"], pairs["left_elbow"],
+                                             kept["left_elbow"], pairs["right_elbow"], kept["right_elbow"], 3)
+    tt = ctx.triplet_tracks(3)
+    assert tt["overflow"] == 0 and np.array_equal(tt["track_offsets"].cpu().numpy(), offs), cfg
+    assert np.array_equal(tt["track_hits"].cpu().numpy(), hits), cfg
     ctx.destroy()

@@ -74,6 +74,19 @@ def test_triplets_and_scores_against_the_oracle(name, n_events, precision, sdt):
     assert np.array_equal(got_shared, shared) and shared.shape[0] > 0
     o2, h2 = oracle.tracks_from_components(g["src"], g["dst"], tc["edge_component"].cpu().numpy(), got_shared, 3)
     assert np.array_equal(o2, offs) and np.array_equal(h2, hits)
+    # phases (3)-(4) on the GPU (etx_triplet_tracks): the track list equals the oracle's one-call result as arrays -- no
+    # oracle function is left inside the chain under test; a second call with another filter on the same handle
+    for min_hits in (3, 1, 5):
+        tt = ctx.triplet_tracks(min_hits)
+        if min_hits != 3:
+            offs_m, hits_m = oracle.tracks_from_triplets(g["src"], g["dst"], keep, pair("articulation"), kept["articulation"],
+                                                         pair("left_elbow"), kept["left_elbow"], pair("right_elbow"), kept["right_elbow"], min_hits)
+        else:
+            offs_m, hits_m = offs, hits
+        assert tt["overflow"] == 0 and tt["n_tracks"] == offs_m.size - 1 and tt["n_listed_hits"] == hits_m.size, min_hits
+        assert np.array_equal(tt["track_offsets"].cpu().numpy(), offs_m), min_hits
+        assert np.array_equal(tt["track_hits"].cpu().numpy(), hits_m), min_hits
+    assert np.bincount(hits, minlength=b.n_hits).max() >= 2                  # some hit is in more than one track
     print(f"   components: {np.unique(comp[comp >= 0]).size}, shared articulations: {shared.shape[0]}, tracks: {offs.size - 1}")
     ctx.destroy()
 
@@ -163,3 +176,54 @@ def test_triplet_counts_saturate_instead_of_wrapping():
     c = ctx.triplet_components(r["n_edges"])                    # reads min(count, capacity) triplets: must stay in bounds
     assert c["edge_component"].numel() == r["n_edges"]
     ctx.destroy()
+
+
+def _tracks_on_gpu_with_chosen_triplets(src, dst, planes, reject, min_hits=3):
+    """Hand-built hit graph through the product's triplet chain: edges injected (all kept), triplets built on the device,
+    their classifier outputs overwritten so that exactly the (kind, first, second) in `reject` fall below the threshold,
+    then etx_triplet_components + etx_triplet_tracks.  -> (triplet lists, list of tracks as tuples)."""
+    from gpu_utils import dev
+    n = len(planes)
+    cfg = datagen.get_config("cfg0").replace(precision="fp32", triplets=1, k=4)
+    b = datagen.hand_batch([[(float(i), 0.0, int(p)) for i, p in enumerate(planes)]])
+    blob = datagen.pack_blob(cfg, datagen.make_weights(cfg, "parity"))
+    ctx = make_ctx(cfg, blob, b, max_triplets=64)
+    src, dst = np.asarray(src, np.int32), np.asarray(dst, np.int32)
+    ctx.dbg_run(dev(b.xyz), dev(b.plane), b.event_offsets, src=dev(src), dst=dev(dst), logit=dev(np.full(src.size, 10.0, np.float32)))
+    t = ctx.triplets()
+    z = ctx.buffer_view("trip_logit", torch.float32).view(3, -1)
+    lists = {}
+    for k, kind in enumerate(KINDS):
+        f, s = t[kind]["first"].cpu().numpy(), t[kind]["second"].cpu().numpy()
+        lists[kind] = list(zip(f.tolist(), s.tolist()))
+        vals = [-10.0 if (kind, a, c) in reject else 10.0 for a, c in lists[kind]]
+        if vals:
+            z[k, :len(vals)] = torch.tensor(vals, dtype=torch.float32, device="cuda")
+    torch.cuda.synchronize()
+    ctx.triplet_components(src.size)
+    tt = ctx.triplet_tracks(min_hits)
+    offs, hits = tt["track_offsets"].cpu().numpy(), tt["track_hits"].cpu().numpy()
+    ctx.destroy()
+    assert tt["overflow"] == 0 and offs.size == tt["n_tracks"] + 1
+    return lists, [tuple(hits[offs[i]:offs[i + 1]].tolist()) for i in range(tt["n_tracks"])]
+
+
+def test_electron_pair_fixture_through_the_product_chain():
+    # PAPER.md L168-170 / Fig. 6: an e+e- pair shares hits 0, 1 and separates, 1 -> 2 -> 4 and 1 -> 3 -> 5.  With the left
+    # elbow (1 -> 2, 1 -> 3) rejected and all four articulations kept, the shared edge 0 -> 1 is duplicated: two tracks
+    # with hits 0 and 1 in both.  (Expected lists written out by hand; tests/test_oracle_triplets.py pins the oracle to
+    # the same ones.)
+    src, dst, planes = [0, 1, 1, 2, 3], [1, 2, 3, 4, 5], [0, 1, 2, 2, 3, 3]
+    lists, tracks = _tracks_on_gpu_with_chosen_triplets(src, dst, planes, {("left_elbow", 1, 2)})
+    assert lists["articulation"] == [(0, 1), (0, 2), (1, 3), (2, 4)] and lists["left_elbow"] == [(1, 2)] and lists["right_elbow"] == []
+    assert tracks == [(0, 1, 2, 4), (0, 1, 3, 5)]
+    # elbow accepted: 1 -> 2 and 1 -> 3 are one super-edge with two successors, the sharing moves one step down
+    _, tracks = _tracks_on_gpu_with_chosen_triplets(src, dst, planes, set())
+    assert tracks == [(0, 1, 2, 3, 4), (0, 1, 2, 3, 5)]
+    # a rejected articulation splits a chain; min_hits = 2 keeps the two-hit piece
+    _, tracks = _tracks_on_gpu_with_chosen_triplets([0, 1, 2, 4, 5, 7], [1, 2, 3, 5, 6, 8], [0, 1, 2, 3, 4, 5, 6, 7, 8],
+                                                    {("articulation", 0, 1)}, min_hits=2)
+    assert tracks == [(0, 1), (1, 2, 3), (4, 5, 6), (7, 8)]
+    # skipped plane: 0 -> 1, 0 -> 2, 1 -> 2, 2 -> 3 with both elbows accepted is one track
+    _, tracks = _tracks_on_gpu_with_chosen_triplets([0, 0, 1, 2], [1, 2, 2, 3], [0, 1, 2, 3], set())
+    assert tracks == [(0, 1, 2, 3)]
