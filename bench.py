@@ -108,10 +108,29 @@ def workload(cfg, rank: int, world: int = 1):
     return batch, layers
 
 
+def calibration_batch():
+    return datagen.generate_batch(datagen.get_config("cfg1"), n_events=datagen.configs.CALIBRATION_EVENTS,
+                                  seed=datagen.configs.CALIBRATION_SEED)
+
+
 def int8_scales(cfg, layers):
-    import oracle  # calibration is part of producing the blob, not of the timed path (R21)
-    cal = datagen.generate_batch(datagen.get_config("cfg1"), n_events=datagen.configs.CALIBRATION_EVENTS,
-                                 seed=datagen.configs.CALIBRATION_SEED)
+    """INT8 activation scales from the library's own calibration call (etx_calibrate: the fp32 FFMA engine over the
+    16-event calibration batch); part of producing the blob, not of the timed path (R21)."""
+    import torch
+    import paper_2407_12119_b200 as etx
+    cal = calibration_batch()
+    cfg32 = cfg.replace(precision="fp32", state_dtype="auto")
+    hp = etx.hyperparams_from_config(cfg32, cal.n_events, cal.n_hits)
+    ctx = etx.Etx(datagen.pack_blob(cfg32, layers), hp)
+    scales = ctx.calibrate(torch.from_numpy(cal.xyz).cuda(), torch.from_numpy(cal.plane).cuda(), cal.event_offsets)
+    ctx.destroy()
+    return scales
+
+
+def int8_scales_reference(cfg, layers):
+    """The reference arm has no GPU library: the oracle's own calibration (the same definition, R21)."""
+    import oracle
+    cal = calibration_batch()
     return oracle.calibrate_int8(datagen.pack_blob(cfg, layers), cal.xyz, cal.plane, cal.event_offsets, cfg.k, cfg.window)
 
 
@@ -189,7 +208,7 @@ def main():
         if rank != 0:
             return 0
         batch, layers = workload(cfg, 0)
-        scales = int8_scales(cfg, layers) if cfg.precision == "int8" else None
+        scales = int8_scales_reference(cfg, layers) if cfg.precision == "int8" else None
         n_ev = max(1, min(args.cpu_events // 4, batch.n_events))
         for _ in range(min(args.warmup, 1)):
             run_oracle_sample(cfg, batch, layers, 1, scales)

@@ -303,6 +303,21 @@ typedef struct {
 
 etx_status etx_triplet_tracks(etx_handle h, int32_t min_hits, etx_stream stream, etx_triplet_tracks_output* out);
 
+/* INT8 calibration (sec. 7.4: the quantised model is "calibrated" on a sample of events; DESIGN.md
+ * R21): the activation scales an INT8 blob needs, one per quantised Linear (K >= 16, not the d -> 1
+ * heads) in blob order.  Runs the whole fp32 path S0..S5 (and, if the blob carries triplet classifiers, the triplet
+ * stage) over the given calibration batch on a handle created with precision ETX_FP32, keeps on the device the running
+ * max |x| of every such Linear's input tensor (rows that exist only; max is order-free, so the result is reproducible),
+ * and returns s_x = max|x| / 127 (true fp32 division; 1.0 if the maximum is 0) in h_scales [*n_scales].  The blob of
+ * the INT8 handle is then the same weights followed by these scales (datagen/weights.py: header word 9 = their count).
+ *   d_xyz, d_plane, h_event_offsets, n_events   a batch, as for etx_run
+ *   h_scales [capacity]  host, written on ETX_OK; NULL: only *n_scales (the count the model needs) is returned
+ * Synchronises `stream`.  ETX_ERR_UNSUPPORTED on a handle that is not ETX_FP32; ETX_ERR_CAPACITY if capacity is too
+ * small, or if the blob has triplet classifiers and max_triplets is 0 or was exceeded by the batch.  The first call
+ * allocates one small device array through the handle's allocator. */
+etx_status etx_calibrate(etx_handle h, const float* d_xyz, const int32_t* d_plane, const int32_t* h_event_offsets,
+                         int32_t n_events, etx_stream stream, float* h_scales, int32_t capacity, int32_t* n_scales);
+
 etx_status etx_destroy(etx_handle h);
 
 /* Device bytes held by the handle (workspace + converted weights), as requested from the allocator. */

@@ -115,6 +115,8 @@ def load_library():
     L.etx_triplet_components.argtypes = [vp, vp, C.POINTER(EtxTripletComponents)]
     L.etx_triplet_tracks.restype = C.c_int
     L.etx_triplet_tracks.argtypes = [vp, C.c_int32, vp, C.POINTER(EtxTripletTracks)]
+    L.etx_calibrate.restype = C.c_int
+    L.etx_calibrate.argtypes = [vp, vp, vp, i32p, C.c_int32, vp, f32p, C.c_int32, i32p]
     L.etx_input_status.restype = C.c_int
     L.etx_input_status.argtypes = [vp]
     L.etx_tracks.restype = C.c_int
@@ -370,6 +372,18 @@ class Etx:
         return dict(n_tracks=T, n_listed_hits=H, overflow=ovf,
                     track_offsets=self._copy_out(out.d_track_offsets, 4 * (Tl + 1), torch.int32),
                     track_hits=self._copy_out(out.d_track_hits, 4 * Hl, torch.int32))
+
+    def calibrate(self, d_xyz, d_plane, event_offsets):
+        """etx_calibrate on the current stream (an ETX_FP32 handle): the INT8 activation scales, one per quantised Linear
+        in blob order, as a numpy float32 array -- what datagen.pack_blob(cfg, layers, scales) appends to the blob."""
+        import numpy as np
+        eo, eop, B = self._offsets(event_offsets)
+        n = C.c_int32(0)
+        self._check(self._L.etx_calibrate(self._h, None, None, eop, B, self._stream(), None, 0, C.byref(n)), "etx_calibrate")
+        scales = np.zeros(int(n.value), np.float32)
+        self._check(self._L.etx_calibrate(self._h, C.c_void_p(d_xyz.data_ptr()), C.c_void_p(d_plane.data_ptr()), eop, B, self._stream(),
+                                          scales.ctypes.data_as(C.POINTER(C.c_float)), int(n.value), C.byref(n)), "etx_calibrate")
+        return scales
 
     def workspace_bytes(self) -> int:
         return int(self._L.etx_workspace_bytes(self._h))

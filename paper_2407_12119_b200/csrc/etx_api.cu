@@ -549,6 +549,55 @@ etx_status etx_triplet_components(etx_handle c, etx_stream stream, etx_triplet_c
   return ETX_OK;
 }
 
+etx_status etx_calibrate(etx_handle c, const float* d_xyz, const int32_t* d_plane, const int32_t* h_event_offsets, int32_t n_events,
+                         etx_stream stream, float* h_scales, int32_t capacity, int32_t* n_scales) {
+  if (!c) return ETX_ERR_ARG;
+  if (!n_scales) return fail(c, ETX_ERR_ARG, "etx_calibrate: null n_scales");
+  int nq = 0;
+  for (auto& l : c->layers) nq += l.tensor;
+  *n_scales = nq;
+  if (!h_scales) return ETX_OK;                              // query: how many scales the model needs
+  if (capacity < nq) return fail(c, ETX_ERR_CAPACITY, "etx_calibrate: h_scales is too small (see *n_scales)");
+  if (c->precision != ETX_FP32)
+    return fail(c, ETX_ERR_UNSUPPORTED, "etx_calibrate records the fp32 forward: create the handle with precision ETX_FP32");
+  if (c->slot_unwaited[0] || c->slot_unwaited[1])
+    return fail(c, ETX_ERR_ARG, "a submission of etx_submit_host has not been waited for yet (etx_wait_host)");
+  if (c->i_trip >= 0 && c->hp.max_triplets <= 0)
+    return fail(c, ETX_ERR_CAPACITY, "etx_calibrate: the blob carries triplet classifiers; set max_triplets so that their inputs can be recorded");
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  const size_t nl = c->layers.size();
+  std::vector<float> amax(nl, 0.0f);
+  try {
+    if (!c->absmax) c->absmax = dev_alloc<float>(c, nl);      // through the handle's allocator; adds to etx_workspace_bytes
+    ETX_CUDA(cudaMemsetAsync(c->absmax, 0, nl * sizeof(float), s));
+    c->calibrating = true;
+    etx_output o;
+    etx_status st = run_impl(c, d_xyz, d_plane, h_event_offsets, n_events, s, nullptr, &o);
+    if (st == ETX_OK && c->i_trip >= 0) {
+      launch_triplet_build(c, c->last_n_hits, s);
+      for (int k = 0; k < 3; ++k) launch_triplet_classifier(c, k, s);
+      ETX_CUDA(cudaMemcpyAsync(c->h_trip_total, c->trip_total, 3 * sizeof(int32_t), cudaMemcpyDeviceToHost, s));
+    }
+    c->calibrating = false;
+    if (st != ETX_OK) return st;
+    ETX_CUDA(cudaMemcpyAsync(amax.data(), c->absmax, nl * sizeof(float), cudaMemcpyDeviceToHost, s));
+    ETX_CUDA(cudaStreamSynchronize(s));
+    ETX_CUDA(cudaGetLastError());
+  } catch (const CudaFail& f) {
+    c->calibrating = false;
+    return fail(c, ETX_ERR_CUDA, std::string(f.what) + ": " + cudaGetErrorString(f.err));
+  }
+  if (etx_input_status(c) != ETX_OK) return ETX_ERR_INPUT_ORDER;
+  if (c->i_trip >= 0)
+    for (int k = 0; k < 3; ++k)
+      if (c->h_trip_total[k] > c->hp.max_triplets)
+        return fail(c, ETX_ERR_CAPACITY, "etx_calibrate: more triplets than max_triplets; the triplet classifiers saw only a part of their inputs");
+  int q = 0;
+  for (auto& l : c->layers)
+    if (l.tensor) { const float a = amax[l.index]; h_scales[q++] = a > 0.0f ? a / 127.0f : 1.0f; }
+  return ETX_OK;
+}
+
 etx_status etx_triplet_tracks(etx_handle c, int32_t min_hits, etx_stream stream, etx_triplet_tracks_output* out) {
   if (!c) return ETX_ERR_ARG;
   if (!out || min_hits < 1) return fail(c, ETX_ERR_ARG, "etx_triplet_tracks: null output or min_hits < 1");

@@ -57,6 +57,7 @@ struct GnnArgs {
   int8_t* hq_out = nullptr;
   float hq_inv_sx = 1.0f;
   const int8_t* hq_in = nullptr;
+  float* absmax = nullptr;   // etx_calibrate (FFMA kernels, fp32 mode): running max |x| per layer in blob order, or nullptr
 };
 
 struct EmbArgs {
@@ -67,6 +68,7 @@ struct EmbArgs {
   int n_rows;
   int32_t* tap;
   int tap_layer;
+  float* absmax = nullptr;    // etx_calibrate: running max |x| per layer (blob order), or nullptr
 };
 
 struct HostLayer {
@@ -147,6 +149,8 @@ struct etx_ctx {
   int32_t* tap = nullptr;
   size_t tap_bytes = 0;
   int tap_layer = -1;
+  float* absmax = nullptr;                // [layers] etx_calibrate: max |x| of every Linear's input (device)
+  bool calibrating = false;
   // host side
   int32_t* h_event_off = nullptr;         // pinned staging [max_events + 1]
   int32_t* h_n_edges = nullptr;           // pinned mirror

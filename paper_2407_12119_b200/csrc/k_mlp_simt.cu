@@ -55,6 +55,18 @@ __device__ __forceinline__ float to_operand(float v, float inv_sx_next) {
   return v;
 }
 
+// INT8 calibration (etx_calibrate; sec. 7.4, R21): max |x| over the existing rows of a
+// Linear's input tile.  Called by all threads of the CTA once the tile is complete; max is order-free, and non-negative
+// floats order like their bit patterns, so one integer atomicMax per warp keeps the running maximum.
+template <int NT>
+__device__ __forceinline__ void tile_absmax(float* slot, const float* X, int ld, int K, int rows) {
+  float mx = 0.0f;
+  for (int i = threadIdx.x; i < rows * K; i += NT) mx = fmaxf(mx, fabsf(X[(i / K) * ld + i % K]));
+#pragma unroll
+  for (int o = 16; o; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+  if ((threadIdx.x & 31) == 0 && mx > 0.0f) atomicMax(reinterpret_cast<int*>(slot), __float_as_int(mx));
+}
+
 // ---- one dense layer over a tile of R rows held in shared memory -----------------------------------------
 // 256 threads; thread (rg, cg) owns the TM rows rg, rg + RG, rg + 2 RG, ... x 4 consecutive output columns (rows
 // interleaved, so the two row groups of a warp read neighbouring rows of X: different banks whatever TM is).
@@ -142,6 +154,8 @@ __global__ void __launch_bounds__(kMlpThreads) embed_simt_kernel(EmbArgs a) {
     __syncthreads();
     input_layer3<MODE, R>(F, a.layers[0], a.layers[1].inv_sx, A, LD);
     __syncthreads();
+    const int rows_here = min(R, a.n_rows - row0);
+    if (a.absmax) tile_absmax<kMlpThreads>(a.absmax + a.layers[1].index, A, LD, a.layers[1].K, rows_here);
     float* cur = A; float* nxt = B;
     for (int l = 1; l < H; ++l) {
       const LayerP L = a.layers[l];
@@ -158,6 +172,7 @@ __global__ void __launch_bounds__(kMlpThreads) embed_simt_kernel(EmbArgs a) {
       });
       __syncthreads();
       float* t = cur; cur = nxt; nxt = t;
+      if (a.absmax) tile_absmax<kMlpThreads>(a.absmax + a.layers[l + 1].index, cur, LD, a.layers[l + 1].K, rows_here);
     }
     // output layer D -> 4, linear, fp32 result (R20: the embedding output is not rounded)
     {
@@ -229,6 +244,7 @@ __global__ void __launch_bounds__(kGnnThreads) gnn_mlp_simt_kernel(GnnArgs a) {
       // layer 0 (K = 3) writes its output (the layer-1 operand) into X, then Y is free again
       input_layer3<MODE, R, kGnnThreads>(Y, L0, L1.inv_sx, X, LDX);
       __syncthreads();
+      if (a.absmax) tile_absmax<kGnnThreads>(a.absmax + L1.index, X, LDX, D, min(R, n_rows - row0));
     } else {
       const int K0 = L0.K;                               // 2D (paper's edge encoder) or 3D
       const int c4n = K0 / 4, seg4 = D / 4;
@@ -265,6 +281,7 @@ __global__ void __launch_bounds__(kGnnThreads) gnn_mlp_simt_kernel(GnnArgs a) {
         }
       }
       __syncthreads();
+      if (a.absmax) tile_absmax<kGnnThreads>(a.absmax + L0.index, X, LDX, K0, min(R, n_rows - row0));
       // layer 0: K0 -> D, ReLU, operand conversion for layer 1
       int32_t* tap0 = (a.tap && a.tap_layer == L0.index) ? a.tap : nullptr;
       dense_tile<D, R, kGnnThreads>(X, LDX, K0, W0s, [&](int r, int c, const float* acc) {
@@ -277,6 +294,7 @@ __global__ void __launch_bounds__(kGnnThreads) gnn_mlp_simt_kernel(GnnArgs a) {
           for (int j = 0; j < 4; ++j) tap0[(size_t)(row0 + r) * D + c + j] = (int32_t)acc[j];
       });
       __syncthreads();
+      if (a.absmax) tile_absmax<kGnnThreads>(a.absmax + L1.index, Y, LDY, D, min(R, n_rows - row0));
     }
     const bool hidden_in_x = (KIND == kNodeEnc || (KIND == kEdgeEnc && a.edge_enc_input == 0));
     const float* HID = hidden_in_x ? X : Y;
@@ -435,6 +453,7 @@ void fill_gnn_args(etx_ctx* c, int kind, int iter, int n_hits, bool do_head, Gnn
   a.edge_enc_input = c->hp.edge_enc_input;
   a.tap = c->tap_layer >= 0 ? c->tap : nullptr;
   a.tap_layer = c->tap_layer;
+  a.absmax = c->calibrating ? c->absmax : nullptr;
 }
 
 void launch_gnn_mlp_simt(etx_ctx* c, int kind, int iter, int n_hits, bool do_head, cudaStream_t s) {
@@ -465,6 +484,7 @@ void launch_embed_simt(etx_ctx* c, int n_hits, cudaStream_t s) {
   for (int l = 0; l < a.n_layers; ++l) a.layers[l] = c->layers[c->i_emb0 + l].dev;
   a.feat = c->feat_emb; a.emb = c->emb; a.n_rows = n_hits;
   a.tap = c->tap_layer >= 0 ? c->tap : nullptr; a.tap_layer = c->tap_layer;
+  a.absmax = c->calibrating ? c->absmax : nullptr;
   const int D = c->hp.emb_hidden;
 #define ETX_EMB(MODE)                                   \
   if (D == 64) emb_launch<MODE, 64>(c, a, s);           \
@@ -503,6 +523,7 @@ struct TripArgs {
   const int32_t* n_ptr;         // device count of this kind
   int cap;
   float* logit; float* score;
+  float* absmax;                // calibration: running max |x| per layer (blob order), or nullptr
 };
 
 template <int MODE, typename ST, int D>
@@ -526,6 +547,7 @@ __global__ void __launch_bounds__(kMlpThreads) triplet_cls_simt_kernel(TripArgs 
       *reinterpret_cast<float4*>(X + r * LDX + c4 * 4) = v;
     }
     __syncthreads();
+    if (a.absmax) tile_absmax<kMlpThreads>(a.absmax + L0.index, X, LDX, 2 * D, min(R, n_rows - row0));
     dense_tile<D, R>(X, LDX, 2 * D, L0.Wt, [&](int r, int c, const float* acc) {
       float4 sc = __ldg(reinterpret_cast<const float4*>(L0.scale + c)), bi = __ldg(reinterpret_cast<const float4*>(L0.bias + c));
       float y[4] = {__fmaf_rn(acc[0], sc.x, bi.x), __fmaf_rn(acc[1], sc.y, bi.y), __fmaf_rn(acc[2], sc.z, bi.z), __fmaf_rn(acc[3], sc.w, bi.w)};
@@ -568,6 +590,7 @@ void launch_triplet_classifier(etx_ctx* c, int kind, cudaStream_t s) {
   a.first = c->trip_first + kind * cap; a.second = c->trip_second + kind * cap;
   a.n_ptr = c->trip_total + kind; a.cap = c->hp.max_triplets;
   a.logit = c->trip_logit + kind * cap; a.score = c->trip_score + kind * cap;
+  a.absmax = c->calibrating ? c->absmax : nullptr;
 #define ETX_TRIP(MODE, ST) { if (c->hp.gnn_latent == 32) trip_launch<MODE, ST, 32>(c, a, s); else trip_launch<MODE, ST, 64>(c, a, s); }
   if (c->precision == ETX_FP32) ETX_TRIP(kModeF32, float)
   else if (c->precision == ETX_BF16) ETX_TRIP(kModeBf16, __nv_bfloat16)

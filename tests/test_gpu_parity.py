@@ -575,6 +575,41 @@ def test_submit_host_pipelined_matches_run_host(precision):
     ctx.destroy()
 
 
+# ================================================================================== INT8 calibration in the product
+@pytest.mark.parametrize("name,triplets", [("cfg1", 0), ("cfg0", 1), ("cfg5", 0)])
+def test_calibrate_scales_equal_the_oracle_bit_for_bit(name, triplets):
+    # etx_calibrate (R21): the fp32 FFMA engine is bit-exact against the oracle's fp32 forward and a
+    # maximum does not depend on the order it is taken in, so the 16-event calibration batch must give the oracle's
+    # activation scales to the bit -- the oracle checks the product's calibration instead of supplying it.
+    import paper_2407_12119_b200 as etx
+    cfg = datagen.get_config(name).replace(precision="fp32", triplets=triplets)
+    cal = datagen.generate_batch(datagen.get_config("cfg1"), n_events=datagen.configs.CALIBRATION_EVENTS, seed=datagen.configs.CALIBRATION_SEED)
+    W = datagen.make_weights(cfg, "parity")
+    blob = datagen.pack_blob(cfg, W)
+    want = oracle.calibrate_int8(blob, cal.xyz, cal.plane, cal.event_offsets, cfg.k, cfg.window, cfg.d2_max, cfg.threshold)
+    ctx = make_ctx(cfg, blob, cal, max_triplets=8_000_000 if triplets else 0)
+    got = ctx.calibrate(dev(cal.xyz), dev(cal.plane), cal.event_offsets)
+    assert got.size == want.size == datagen.weights.n_act_scales(cfg) and got.size >= 10
+    assert np.array_equal(got.view(np.uint32), want.view(np.uint32)), np.flatnonzero(got != want)
+    assert (got > 0).all() and not np.all(got == 1.0)
+    # a second call on the same handle starts from zero again, and an ordinary run afterwards is unaffected
+    small = cal.slice_events(0, 3)
+    got2 = ctx.calibrate(dev(small.xyz), dev(small.plane), small.event_offsets)
+    want2 = oracle.calibrate_int8(blob, small.xyz, small.plane, small.event_offsets, cfg.k, cfg.window, cfg.d2_max, cfg.threshold)
+    assert np.array_equal(got2.view(np.uint32), want2.view(np.uint32)) and (got2 <= got).all()
+    g = run_gpu(ctx, small, debug=False)
+    assert g["n_edges"] > 0
+    ctx.destroy()
+    # the scales make a valid INT8 blob; a bf16 handle cannot calibrate
+    cfg8 = cfg.replace(precision="int8")
+    ctx8 = make_ctx(cfg8, datagen.pack_blob(cfg8, W, got), small, max_triplets=8_000_000 if triplets else 0)
+    assert run_gpu(ctx8, small, debug=False)["n_edges"] > 0      # (with a radius cut the quantised embedding moves a few edges)
+    with pytest.raises(etx.EtxError) as ei:
+        ctx8.calibrate(dev(small.xyz), dev(small.plane), small.event_offsets)
+    assert ei.value.status == -6
+    ctx8.destroy()
+
+
 # ================================================================================== tcgen05 engine (bf16 / int8)
 def _int8_blob(cfg, b, W):
     scales = oracle.calibrate_int8(datagen.pack_blob(cfg, W), b.xyz, b.plane, b.event_offsets, cfg.k, cfg.window)
