@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the ETX4VELO hot path (S0..S5) on synthetic VELO-shaped events.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config cfg2] [--engine auto|simt]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config cfg2] [--engine auto|simt] [--streams S]
     python bench.py --impl reference ...        # the CPU oracle on a bounded sample of the same workload
 
 One "step" = one pass of the whole hot path over one batch (BASELINE.json configs[2]: 500 events at
@@ -29,9 +29,10 @@ sys.path.insert(0, ROOT)
 import datagen  # noqa: E402
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel (S4e edge network): the mean over the
-# six launches of one pass (five write e back, the last does not) from the `ncu --set full` capture summarised in
-# profiles/r2_launches_cfg2.md, per workload; bench.py cannot run ncu itself.
-NCU_TRAFFIC_BYTES = {("cfg2", 500): 2.5139e9}
+# six launches of one pass (five write e back, the last does not), from the ncu pass over this very command summarised
+# in profiles/r3_launches_cfg2.md (15,061.8 MB / 6; round 2's --set full capture gave 2.5139e9), per workload; bench.py
+# cannot run ncu itself.
+NCU_TRAFFIC_BYTES = {("cfg2", 500): 2.5103e9}
 METRIC = "events_per_s"
 UNIT = "events/s"
 DTYPE = {"fp32": "f32", "bf16": "bf16", "int8": "int8"}
@@ -412,7 +413,7 @@ def main():
     else:
         dom_bytes = wide
     rate = lambda work: work / (dom_ms * 1e-3) / dom_div if dom_ms > 0 else None
-    hbm_note = ("S4e moves its bytes once (ncu traffic / compulsory bytes = 0.98 at cfg2); what holds it below the copy peak is on chip: "
+    hbm_note = ("S4e moves its bytes once (ncu traffic / compulsory bytes = 0.98 at cfg2, 1.07 on the 8(d) count); what holds it below the copy peak is on chip: "
                 "shared-memory bandwidth and the cp.async gather of h[src], h[dst] (profiles/r2_s4e_ablation.md)")
     roofline = {"kernel": "edge network MLP (S4e), one launch per message-passing step", "bound": dom_bound,
                 "achieved": rate(dom_bytes), "peak": dom_peak, "unit": dom_unit,
@@ -424,7 +425,7 @@ def main():
                                "count": "algorithmic + src / dst (8 E) + h once per node (N d b) + logit and score writes"}
                               if dom_bound == "hbm" else None,
                 "traffic": NCU_TRAFFIC_BYTES.get((cfg.name, cfg.n_events)) if n_str == 1 and args.engine == "auto" else None,
-                "traffic_source": ("recorded: ncu --set full capture of this kernel at this workload (profiles/r2_launches_cfg2.md); "
+                "traffic_source": ("recorded: ncu dram__bytes_read.sum + dram__bytes_write.sum of this kernel at this workload (profiles/r3_launches_cfg2.md); "
                                    "bench.py cannot run ncu") if (cfg.name, cfg.n_events) in NCU_TRAFFIC_BYTES
                                   else "no ncu capture recorded for this workload",
                 "note": hbm_note if dom_bound == "hbm" else "fp32 mode runs the networks on the FFMA pipe in the oracle's pinned order (DESIGN.md R4)",
