@@ -167,7 +167,11 @@ etx_status etx_run_host(etx_handle h, const float* h_xyz, const int32_t* h_plane
  * slot has its own device score buffer).  *h_n_edges (plain host int32) receives E and is valid after etx_wait_host.
  * While a submission has not been waited for, etx_run / etx_run_host / etx_dbg_run on the same handle return
  * ETX_ERR_ARG (they would overwrite its results).  The h_* input arrays and
- * h_event_offsets must stay valid until the submission has completed (h_event_offsets: until the call returns). */
+ * h_event_offsets must stay valid until the submission has completed (h_event_offsets: until the call returns).
+ * A submission slot is released by etx_wait_host only: submitting i + 2 before waiting for i returns ETX_ERR_ARG and
+ * leaves the two submissions in flight untouched.  The first etx_submit_host on a handle allocates a second input
+ * staging set and score buffer through the handle's allocator (etx_workspace_bytes grows by 16 max_hits + 4 k max_hits
+ * bytes); a first call that fails half-way is completed by the next one. */
 etx_status etx_submit_host(etx_handle h, const float* h_xyz, const int32_t* h_plane,
                            const int32_t* h_event_offsets, int32_t n_events, etx_stream stream,
                            float* h_edge_score, int32_t* h_edge_src, int32_t* h_edge_dst,
